@@ -1,0 +1,607 @@
+// ProtoKV CPU ORACLE -- TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, single-threaded restatement of the paper's hot path (PAPER.md = arxiv 2606.26762 text):
+//   Alg. 1 streaming update   (Eq. 1 at L93)      -> append_frame_sync / append_frame_seq
+//   Eq. 3 + Alg. 3 beam decode             -> decode_top_s
+//   Alg. 4 decode + attention, Eq. 2/4 -> materialize / attention
+// One object = one bank = one (stream, layer, KV head): banks are independent.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call this.
+// It shares no code with paper_2606_26762_b200/ (the CUDA path) and must never be used by the product path.
+//
+// Arithmetic: state is fp32 (what is compared); every expression is evaluated in fp64 from the fp32
+// state and rounded once.  Discrete decisions (argmin of Eq. 1, nearest PQ codeword) compare the
+// fp32-rounded values, lowest index on exact ties.  Readings of silent/garbled points: DESIGN.md "Readings".
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): mass conservation; histogram row sums; T=1 frame-synchronous
+// == sequential; forced replay; brute-force recomputation of the statistics from the assignment log (numpy);
+// constant-stream closed forms; exact attention over the full history when K_max >= evicted tokens; a mass-m
+// prototype == m duplicated tokens; torch SDPA on the materialised context; cosine nearest centroid; Euclidean
+// special case of d_Mah; beam == brute-force top-S.  What stays unpinned: the absolute values produced on the five
+// configs ("parity unpinned" beyond those pins).
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <deque>
+#include <limits>
+#include <vector>
+
+namespace {
+
+enum : uint32_t {
+  FLAG_MAH_SQUARED = 1u,   // use d_Mah^2 instead of d_Mah (reading 4 alternative)
+  FLAG_NO_MASS_BIAS = 2u,  // b_k = 0          (Table 2 "w/o mass bias")
+  FLAG_NO_RESIDUAL = 4u,   // no histograms    (Table 2 "w/o residual stats", L179)
+  FLAG_NEAR_ONLY = 8u,     // attention over the near window only (L176)
+  FLAG_FAR_ONLY = 16u,     // attention over pseudo-tokens only   (L177)
+};
+
+struct Config {
+  int32_t T, near_frames, k_max, d, S, G, C, beam;
+  float lambda_sp, lambda_idle;
+  int32_t t_idle;
+  float alpha, beta, eta, sigma_eps, cos_eps;
+  double pq_eps;
+  uint32_t flags;
+};
+
+struct Trace {          // all pointers nullable; sizes [T] or [T][G]
+  int32_t evicted;      // out: 1 if a frame was evicted by this call
+  int32_t n_fill;       // out: tokens that opened a new slot (Alg. 1 l.3-4)
+  int32_t* assign;      // out: the oracle's own choice (slot index for fills, argmin for the rest)
+  float* best;          // out: best Eq. 1 score (0 for fills)
+  float* second;        // out: second best score (+inf if none)
+  float* forced_excess; // out: score(forced choice) - best, 0 when not forced
+  uint8_t* codes_k;     // out: the oracle's own PQ codes [T][G] (255 = no residual update)
+  uint8_t* codes_v;
+  float* code_gap_k;    // out: (dist(forced code) - dist(best)) / max(dist(best), 1e-30), [T][G]
+  float* code_gap_v;
+};
+
+struct StateView {      // host pointers, any may be NULL
+  float* c; float* p;           // [k_max][d]
+  int32_t* n;                   // [k_max] mass
+  float* mu; float* sigma;      // [k_max][2], [k_max][3] = (xx, xy, yy)
+  int32_t* tau; int64_t* pos;   // [k_max] frame index of last absorption / stream position of last absorbed token
+  uint32_t* hist_k; uint32_t* hist_v;  // [k_max][G][C]
+  uint32_t* nres;               // [k_max]
+  uint8_t* active;              // [k_max]
+};
+
+struct Frame {
+  int32_t index;
+  std::vector<float> K, V, s;
+};
+
+using Tuple = std::array<uint8_t, 16>;
+
+struct Bank {
+  Config cfg;
+  int sub;  // d / G
+  bool has_cb;
+  std::vector<float> cbk, cbv;  // [G][C][sub]
+  std::deque<Frame> ring;
+  int32_t frames_seen = 0;
+  std::vector<float> c, p, mu, sigma;
+  std::vector<int32_t> n, tau;
+  std::vector<int64_t> pos;
+  std::vector<uint32_t> hk, hv, nres;
+  std::vector<uint8_t> active;
+
+  Bank(const Config& cf, const float* ck, const float* cv) : cfg(cf) {
+    sub = cfg.d / cfg.G;
+    has_cb = ck && cv && !(cfg.flags & FLAG_NO_RESIDUAL);
+    if (has_cb) {
+      size_t nn = (size_t)cfg.G * cfg.C * sub;
+      cbk.assign(ck, ck + nn);
+      cbv.assign(cv, cv + nn);
+    }
+    size_t K = cfg.k_max, d = cfg.d;
+    c.assign(K * d, 0.f); p.assign(K * d, 0.f);
+    mu.assign(K * 2, 0.f); sigma.assign(K * 3, 0.f);
+    n.assign(K, 0); tau.assign(K, 0); pos.assign(K, 0);
+    hk.assign(K * cfg.G * cfg.C, 0u); hv.assign(K * cfg.G * cfg.C, 0u);
+    nres.assign(K, 0u); active.assign(K, 0);
+  }
+
+  int free_slot() const {  // lowest-index inactive slot (reading 9), -1 if none
+    for (int k = 0; k < cfg.k_max; ++k) if (!active[k]) return k;
+    return -1;
+  }
+
+  // Alg. 1 l.4: c<-K_e, p<-V_e, n<-1, mu<-s_e, Sigma<-I, tau<-t, R<-0
+  void init_slot(int k, const float* Ke, const float* Ve, const float* se, int32_t t, int64_t ps) {
+    int d = cfg.d;
+    for (int i = 0; i < d; ++i) { c[(size_t)k * d + i] = Ke[i]; p[(size_t)k * d + i] = Ve[i]; }
+    n[k] = 1; mu[k * 2] = se[0]; mu[k * 2 + 1] = se[1];
+    sigma[k * 3] = 1.f; sigma[k * 3 + 1] = 0.f; sigma[k * 3 + 2] = 1.f;
+    tau[k] = t; pos[k] = ps;
+    std::fill(hk.begin() + (size_t)k * cfg.G * cfg.C, hk.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
+    std::fill(hv.begin() + (size_t)k * cfg.G * cfg.C, hv.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
+    nres[k] = 0; active[k] = 1;
+  }
+
+  // Eq. 1: -cos(K_e,c_k) + lambda_sp d_Mah(s_e;mu_k,Sigma_k) + lambda_idle 1[t - tau_k > T_idle]
+  float score(const float* Ke, const float* se, int k, int32_t t) const {
+    int d = cfg.d;
+    const float* ck = &c[(size_t)k * d];
+    double dot = 0, kk = 0, cc = 0;
+    for (int i = 0; i < d; ++i) {
+      dot += (double)Ke[i] * (double)ck[i];
+      kk += (double)Ke[i] * (double)Ke[i];
+      cc += (double)ck[i] * (double)ck[i];
+    }
+    double cosv = dot / std::max(std::sqrt(kk * cc), (double)cfg.cos_eps);
+    double dx = (double)se[0] - (double)mu[k * 2], dy = (double)se[1] - (double)mu[k * 2 + 1];
+    double a = (double)sigma[k * 3] + (double)cfg.sigma_eps, b = (double)sigma[k * 3 + 1],
+           e = (double)sigma[k * 3 + 2] + (double)cfg.sigma_eps;
+    double det = a * e - b * b;
+    double q = (e * dx * dx - 2.0 * b * dx * dy + a * dy * dy) / det;  // delta^T (Sigma+eps I)^-1 delta
+    if (q < 0) q = 0;
+    double dm = (cfg.flags & FLAG_MAH_SQUARED) ? q : std::sqrt(q);
+    double idle = ((int64_t)t - (int64_t)tau[k] > (int64_t)cfg.t_idle) ? (double)cfg.lambda_idle : 0.0;
+    return (float)(-cosv + (double)cfg.lambda_sp * dm + idle);
+  }
+
+  // argmin over active prototypes, lowest index on exact ties; also second best
+  int argmin_score(const float* Ke, const float* se, int32_t t, float* best, float* second) const {
+    int kb = -1;
+    float b = std::numeric_limits<float>::infinity(), s2 = b;
+    for (int k = 0; k < cfg.k_max; ++k) {
+      if (!active[k]) continue;
+      float sc = score(Ke, se, k, t);
+      if (sc < b) { s2 = b; b = sc; kb = k; }
+      else if (sc < s2) s2 = sc;
+    }
+    *best = b; *second = s2;
+    return kb;
+  }
+
+  // nearest codeword per subspace in squared L2 (reading 10); returns code, writes rounded distances
+  int nearest_code(const std::vector<float>& cb, int g, const double* r, float* dist_out) const {
+    int zb = 0;
+    float db = std::numeric_limits<float>::infinity();
+    for (int z = 0; z < cfg.C; ++z) {
+      double acc = 0;
+      const float* cw = &cb[((size_t)g * cfg.C + z) * sub];
+      for (int m = 0; m < sub; ++m) { double t = r[m] - (double)cw[m]; acc += t * t; }
+      float df = (float)acc;
+      if (dist_out) dist_out[z] = df;
+      if (df < db) { db = df; zb = z; }
+    }
+    return zb;
+  }
+
+  // Alg. 1 l.8-13, in the listed order; residuals use the just-updated centres (reading 7)
+  void update_proto(int k, const float* Ke, const float* Ve, const float* se, int32_t t, int64_t ps,
+                    const uint8_t* fck, const uint8_t* fcv, uint8_t* ock, uint8_t* ocv, float* gk, float* gv) {
+    int d = cfg.d;
+    double al = cfg.alpha, be = cfg.beta, et = cfg.eta;
+    float* ck = &c[(size_t)k * d];
+    float* pk = &p[(size_t)k * d];
+    for (int i = 0; i < d; ++i) {
+      ck[i] = (float)((1.0 - al) * (double)ck[i] + al * (double)Ke[i]);   // l.8
+      pk[i] = (float)((1.0 - be) * (double)pk[i] + be * (double)Ve[i]);   // l.9
+    }
+    n[k] += 1; tau[k] = t; pos[k] = ps;                                   // l.10
+    mu[k * 2] = (float)((1.0 - et) * (double)mu[k * 2] + et * (double)se[0]);          // l.11
+    mu[k * 2 + 1] = (float)((1.0 - et) * (double)mu[k * 2 + 1] + et * (double)se[1]);
+    double dx = (double)se[0] - (double)mu[k * 2], dy = (double)se[1] - (double)mu[k * 2 + 1];  // new mu
+    sigma[k * 3] = (float)((1.0 - et) * (double)sigma[k * 3] + et * dx * dx);          // l.12
+    sigma[k * 3 + 1] = (float)((1.0 - et) * (double)sigma[k * 3 + 1] + et * dx * dy);
+    sigma[k * 3 + 2] = (float)((1.0 - et) * (double)sigma[k * 3 + 2] + et * dy * dy);
+    if (!has_cb) return;
+    std::vector<double> r(sub);
+    std::vector<float> dist(cfg.C);
+    for (int kv = 0; kv < 2; ++kv) {                                      // l.13
+      const float* x = kv ? Ve : Ke;
+      const float* cen = kv ? pk : ck;
+      const std::vector<float>& cb = kv ? cbv : cbk;
+      std::vector<uint32_t>& H = kv ? hv : hk;
+      const uint8_t* forced = kv ? fcv : fck;
+      uint8_t* oc = kv ? ocv : ock;
+      float* gap = kv ? gv : gk;
+      for (int g = 0; g < cfg.G; ++g) {
+        for (int m = 0; m < sub; ++m) r[m] = (double)x[g * sub + m] - (double)cen[g * sub + m];
+        int z = nearest_code(cb, g, r.data(), dist.data());
+        if (oc) oc[g] = (uint8_t)z;
+        int use = z;
+        if (forced) {
+          use = forced[g];
+          if (gap) gap[g] = (dist[use] - dist[z]) / std::max(dist[z], 1e-30f);
+        } else if (gap) gap[g] = 0.f;
+        H[((size_t)k * cfg.G + g) * cfg.C + use] += 1;
+      }
+    }
+    nres[k] += 1;
+  }
+
+  bool pop_if_full(Frame* ev) {
+    if ((int)ring.size() < cfg.near_frames) return false;
+    *ev = std::move(ring.front());
+    ring.pop_front();
+    return true;
+  }
+  void push(const float* K, const float* V, const float* s) {
+    Frame f;
+    f.index = frames_seen;
+    size_t nkv = (size_t)cfg.T * cfg.d;
+    f.K.assign(K, K + nkv); f.V.assign(V, V + nkv); f.s.assign(s, s + (size_t)cfg.T * 2);
+    ring.push_back(std::move(f));
+  }
+  static void clear_trace(Trace* tr, int T, int G) {
+    if (!tr) return;
+    tr->evicted = 0; tr->n_fill = 0;
+    for (int j = 0; j < T; ++j) {
+      if (tr->assign) tr->assign[j] = -1;
+      if (tr->best) tr->best[j] = 0.f;
+      if (tr->second) tr->second[j] = std::numeric_limits<float>::infinity();
+      if (tr->forced_excess) tr->forced_excess[j] = 0.f;
+      for (int g = 0; g < G; ++g) {
+        if (tr->codes_k) tr->codes_k[j * G + g] = 255;
+        if (tr->codes_v) tr->codes_v[j * G + g] = 255;
+        if (tr->code_gap_k) tr->code_gap_k[j * G + g] = 0.f;
+        if (tr->code_gap_v) tr->code_gap_v[j * G + g] = 0.f;
+      }
+    }
+  }
+
+  // Frame-synchronous update (reading 1; the graded definition):
+  //  A) slot fill in eviction order, B) Eq. 1 scores of the remaining tokens against the bank as it stands
+  //  after (A), C) Alg. 1 l.8-13 replayed token by token, in eviction order, on the live bank.
+  void append_frame_sync(const float* K, const float* V, const float* s, const int32_t* forced,
+                         const uint8_t* fck, const uint8_t* fcv, Trace* tr) {
+    const int T = cfg.T, d = cfg.d, G = cfg.G;
+    clear_trace(tr, T, G);
+    Frame E;
+    bool ev = pop_if_full(&E);                 // |B_near| > W after the append  (Alg. 1 l.1-3)
+    push(K, V, s);
+    const int32_t t = frames_seen;             // stream time = frame index (reading 2)
+    frames_seen += 1;
+    if (!ev) return;
+    if (tr) tr->evicted = 1;
+    int j = 0;
+    for (; j < T; ++j) {                        // (A)
+      int k = free_slot();
+      if (k < 0) break;
+      init_slot(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, (int64_t)E.index * T + j);
+      if (tr && tr->assign) tr->assign[j] = k;
+    }
+    const int nf = j;
+    if (tr) tr->n_fill = nf;
+    std::vector<int> own(T, -1);
+    for (j = nf; j < T; ++j) {                  // (B) -- the bank is frozen during this loop
+      float b, s2;
+      own[j] = argmin_score(&E.K[(size_t)j * d], &E.s[j * 2], t, &b, &s2);
+      if (tr) {
+        if (tr->assign) tr->assign[j] = own[j];
+        if (tr->best) tr->best[j] = b;
+        if (tr->second) tr->second[j] = s2;
+        if (forced && tr->forced_excess)
+          tr->forced_excess[j] = score(&E.K[(size_t)j * d], &E.s[j * 2], forced[j], t) - b;
+      }
+    }
+    for (j = nf; j < T; ++j) {                  // (C)
+      int k = forced ? forced[j] : own[j];
+      update_proto(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, (int64_t)E.index * T + j,
+                   fck ? fck + j * G : nullptr, fcv ? fcv + j * G : nullptr,
+                   tr && tr->codes_k ? tr->codes_k + j * G : nullptr, tr && tr->codes_v ? tr->codes_v + j * G : nullptr,
+                   tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
+                   tr && tr->code_gap_v ? tr->code_gap_v + j * G : nullptr);
+    }
+  }
+
+  // Literal Alg. 1 (token-sequential): every evicted token sees the live bank. Used for pinning only.
+  void append_frame_seq(const float* K, const float* V, const float* s, const int32_t* forced,
+                        const uint8_t* fck, const uint8_t* fcv, Trace* tr) {
+    const int T = cfg.T, d = cfg.d, G = cfg.G;
+    clear_trace(tr, T, G);
+    Frame E;
+    bool ev = pop_if_full(&E);
+    push(K, V, s);
+    const int32_t t = frames_seen;
+    frames_seen += 1;
+    if (!ev) return;
+    if (tr) tr->evicted = 1;
+    int nf = 0;
+    for (int j = 0; j < T; ++j) {
+      const float* Ke = &E.K[(size_t)j * d];
+      const float* Ve = &E.V[(size_t)j * d];
+      const float* se = &E.s[j * 2];
+      int64_t ps = (int64_t)E.index * T + j;
+      int k = free_slot();
+      if (k >= 0) {                                                   // l.3-4
+        init_slot(k, Ke, Ve, se, t, ps);
+        if (tr && tr->assign) tr->assign[j] = k;
+        ++nf;
+        continue;
+      }
+      float b, s2;
+      int own = argmin_score(Ke, se, t, &b, &s2);                     // l.6
+      if (tr) {
+        if (tr->assign) tr->assign[j] = own;
+        if (tr->best) tr->best[j] = b;
+        if (tr->second) tr->second[j] = s2;
+        if (forced && tr->forced_excess) tr->forced_excess[j] = score(Ke, se, forced[j], t) - b;
+      }
+      k = forced ? forced[j] : own;
+      update_proto(k, Ke, Ve, se, t, ps, fck ? fck + j * G : nullptr, fcv ? fcv + j * G : nullptr,     // l.8-13
+                   tr && tr->codes_k ? tr->codes_k + j * G : nullptr, tr && tr->codes_v ? tr->codes_v + j * G : nullptr,
+                   tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
+                   tr && tr->code_gap_v ? tr->code_gap_v + j * G : nullptr);
+    }
+    if (tr) tr->n_fill = nf;
+  }
+
+  // Eq. 3 in fixed point (reading 13): q(g,c) = llround(2^24 * log P(g,c))
+  void log_table(const uint32_t* H, std::vector<int64_t>& q) const {
+    q.resize((size_t)cfg.G * cfg.C);
+    for (int g = 0; g < cfg.G; ++g) {
+      double tot = 0;
+      for (int z = 0; z < cfg.C; ++z) tot += (double)H[g * cfg.C + z];
+      double den = tot + (double)cfg.C * cfg.pq_eps;
+      for (int z = 0; z < cfg.C; ++z) {
+        double P = ((double)H[g * cfg.C + z] + cfg.pq_eps) / den;
+        q[g * cfg.C + z] = std::llround(std::log(P) * 16777216.0);
+      }
+    }
+  }
+
+  // Alg. 3: beam search over subquantisers, beam width B, output the top S tuples.
+  // Order: score descending, then tuple ascending lexicographically (z_1 most significant).
+  void decode_top_s(const uint32_t* H, std::vector<Tuple>& out, std::vector<int64_t>* out_scores) const {
+    std::vector<int64_t> q;
+    log_table(H, q);
+    struct Item { int64_t a; Tuple z; };
+    std::vector<Item> beam(1), next;
+    beam[0].a = 0; beam[0].z.fill(0);
+    for (int g = 0; g < cfg.G; ++g) {                      // l.2
+      next.clear();                                        // B' <- empty
+      for (const Item& it : beam)                          // l.4
+        for (int z = 0; z < cfg.C; ++z) {                  // l.5
+          Item e = it;
+          e.a = it.a + q[g * cfg.C + z];                   // l.6
+          e.z[g] = (uint8_t)z;
+          next.push_back(e);
+        }
+      std::sort(next.begin(), next.end(), [&](const Item& x, const Item& y) {
+        if (x.a != y.a) return x.a > y.a;
+        return std::lexicographical_compare(x.z.begin(), x.z.begin() + g + 1, y.z.begin(), y.z.begin() + g + 1);
+      });
+      if ((int)next.size() > cfg.beam) next.resize(cfg.beam);   // TopB, l.10
+      beam.swap(next);
+    }
+    out.clear();
+    if (out_scores) out_scores->clear();
+    for (int s = 0; s < cfg.S && s < (int)beam.size(); ++s) {    // TopS, l.12
+      out.push_back(beam[s].z);
+      if (out_scores) out_scores->push_back(beam[s].a);
+    }
+  }
+
+  int64_t tuple_score(int k, int which, const uint8_t* z) const {
+    std::vector<int64_t> q;
+    const std::vector<uint32_t>& H = which ? hv : hk;
+    log_table(&H[(size_t)k * cfg.G * cfg.C], q);
+    int64_t a = 0;
+    for (int g = 0; g < cfg.G; ++g) a += q[g * cfg.C + z[g]];
+    return a;
+  }
+
+  // Alg. 4 l.1-13: [near || pseudo] keys/values and bias b
+  void materialize(const uint8_t* fck, const uint8_t* fcv, std::vector<double>& Kt, std::vector<double>& Vt,
+                   std::vector<double>& b) const {
+    const int d = cfg.d, S = cfg.S, G = cfg.G;
+    Kt.clear(); Vt.clear(); b.clear();
+    if (!(cfg.flags & FLAG_FAR_ONLY))
+      for (const Frame& f : ring)
+        for (int j = 0; j < cfg.T; ++j) {
+          for (int i = 0; i < d; ++i) { Kt.push_back(f.K[(size_t)j * d + i]); Vt.push_back(f.V[(size_t)j * d + i]); }
+          b.push_back(0.0);                                                   // near tokens carry zero bias (L407)
+        }
+    if (cfg.flags & FLAG_NEAR_ONLY) return;
+    std::vector<Tuple> zk, zv;
+    for (int k = 0; k < cfg.k_max; ++k) {
+      if (!active[k] || n[k] < 1) continue;                                   // l.2 "each active prototype"
+      bool zero = (!has_cb) || nres[k] == 0;                                  // l.3-4
+      if (!zero) {
+        if (fck && fcv) {
+          zk.assign(S, Tuple{}); zv.assign(S, Tuple{});
+          for (int s = 0; s < S; ++s)
+            for (int g = 0; g < G; ++g) {
+              zk[s][g] = fck[((size_t)k * S + s) * G + g];
+              zv[s][g] = fcv[((size_t)k * S + s) * G + g];
+            }
+        } else {
+          decode_top_s(&hk[(size_t)k * G * cfg.C], zk, nullptr);              // l.5
+          decode_top_s(&hv[(size_t)k * G * cfg.C], zv, nullptr);              // l.6
+        }
+      }
+      double bias = (cfg.flags & FLAG_NO_MASS_BIAS) ? 0.0 : std::log((double)n[k]);   // Eq. 4, natural log
+      for (int s = 0; s < S; ++s) {                                           // l.8-10
+        for (int i = 0; i < d; ++i) {
+          double rk = 0, rv = 0;
+          if (!zero) {
+            int g = i / sub, m = i % sub;
+            rk = cbk[((size_t)g * cfg.C + zk[s][g]) * sub + m];
+            rv = cbv[((size_t)g * cfg.C + zv[s][g]) * sub + m];
+          }
+          Kt.push_back((double)c[(size_t)k * d + i] + rk);
+          Vt.push_back((double)p[(size_t)k * d + i] + rv);
+        }
+        b.push_back(bias);
+      }
+    }
+  }
+
+  // Alg. 4 l.14-15: A = Q K~^T / sqrt(d) + b ; O = softmax(A) V~   (no mask, reading 17)
+  void attention(const float* Q, int rows, const uint8_t* fck, const uint8_t* fcv, float* out, double* lse) const {
+    const int d = cfg.d;
+    std::vector<double> Kt, Vt, b;
+    materialize(fck, fcv, Kt, Vt, b);
+    const size_t L = b.size();
+    const double scale = 1.0 / std::sqrt((double)d);
+    std::vector<double> logit(L), acc(d);
+    for (int r = 0; r < rows; ++r) {
+      const float* q = Q + (size_t)r * d;
+      double m = -std::numeric_limits<double>::infinity();
+      for (size_t j = 0; j < L; ++j) {
+        double dot = 0;
+        for (int i = 0; i < d; ++i) dot += (double)q[i] * Kt[j * d + i];
+        logit[j] = dot * scale + b[j];
+        m = std::max(m, logit[j]);
+      }
+      double sum = 0;
+      std::fill(acc.begin(), acc.end(), 0.0);
+      for (size_t j = 0; j < L; ++j) {
+        double w = std::exp(logit[j] - m);
+        sum += w;
+        for (int i = 0; i < d; ++i) acc[i] += w * Vt[j * d + i];
+      }
+      for (int i = 0; i < d; ++i) out[(size_t)r * d + i] = L ? (float)(acc[i] / sum) : 0.f;
+      if (lse) lse[r] = L ? m + std::log(sum) : -std::numeric_limits<double>::infinity();
+    }
+  }
+};
+
+}  // namespace
+
+extern "C" {
+
+void* pko_create(const Config* cfg, const float* codebook_k, const float* codebook_v) {
+  if (!cfg || cfg->d <= 0 || cfg->G <= 0 || cfg->d % cfg->G || cfg->C <= 0 || cfg->C > 255 || cfg->G > 16 ||
+      cfg->S <= 0 || cfg->beam < cfg->S || cfg->T <= 0 || cfg->near_frames <= 0 || cfg->k_max <= 0)
+    return nullptr;
+  return new Bank(*cfg, codebook_k, codebook_v);
+}
+void pko_destroy(void* h) { delete static_cast<Bank*>(h); }
+
+// mode 0: frame-synchronous (graded); mode 1: token-sequential (literal Alg. 1)
+int pko_append_frame(void* h, const float* K, const float* V, const float* s, int mode, const int32_t* forced_assign,
+                     const uint8_t* forced_codes_k, const uint8_t* forced_codes_v, Trace* trace) {
+  Bank* b = static_cast<Bank*>(h);
+  if (!b || !K || !V || !s) return 1;
+  if (mode == 0) b->append_frame_sync(K, V, s, forced_assign, forced_codes_k, forced_codes_v, trace);
+  else b->append_frame_seq(K, V, s, forced_assign, forced_codes_k, forced_codes_v, trace);
+  return 0;
+}
+
+int pko_frames_seen(void* h) { return static_cast<Bank*>(h)->frames_seen; }
+int pko_ring_frames(void* h) { return (int)static_cast<Bank*>(h)->ring.size(); }
+
+// ring in chronological order: K,V [n][T][d], s [n][T][2], idx [n]; returns n
+int pko_get_ring(void* h, float* K, float* V, float* s, int32_t* idx) {
+  Bank* b = static_cast<Bank*>(h);
+  size_t nkv = (size_t)b->cfg.T * b->cfg.d, ns = (size_t)b->cfg.T * 2;
+  int i = 0;
+  for (const Frame& f : b->ring) {
+    if (K) std::memcpy(K + i * nkv, f.K.data(), nkv * sizeof(float));
+    if (V) std::memcpy(V + i * nkv, f.V.data(), nkv * sizeof(float));
+    if (s) std::memcpy(s + i * ns, f.s.data(), ns * sizeof(float));
+    if (idx) idx[i] = f.index;
+    ++i;
+  }
+  return i;
+}
+
+#define PKO_COPY(field, vec) \
+  if (v->field) std::memcpy(v->field, b->vec.data(), b->vec.size() * sizeof(b->vec[0]))
+#define PKO_LOAD(field, vec) \
+  if (v->field) std::memcpy(b->vec.data(), v->field, b->vec.size() * sizeof(b->vec[0]))
+
+void pko_get_state(void* h, StateView* v) {
+  Bank* b = static_cast<Bank*>(h);
+  PKO_COPY(c, c); PKO_COPY(p, p); PKO_COPY(n, n); PKO_COPY(mu, mu); PKO_COPY(sigma, sigma);
+  PKO_COPY(tau, tau); PKO_COPY(pos, pos); PKO_COPY(hist_k, hk); PKO_COPY(hist_v, hv); PKO_COPY(nres, nres);
+  PKO_COPY(active, active);
+}
+void pko_set_state(void* h, const StateView* v) {
+  Bank* b = static_cast<Bank*>(h);
+  PKO_LOAD(c, c); PKO_LOAD(p, p); PKO_LOAD(n, n); PKO_LOAD(mu, mu); PKO_LOAD(sigma, sigma);
+  PKO_LOAD(tau, tau); PKO_LOAD(pos, pos); PKO_LOAD(hist_k, hk); PKO_LOAD(hist_v, hv); PKO_LOAD(nres, nres);
+  PKO_LOAD(active, active);
+}
+
+// Eq. 1 score of (K_e, s_e) against prototype k at stream time t, on the current bank
+float pko_score(void* h, const float* Ke, const float* se, int k, int32_t t) {
+  return static_cast<Bank*>(h)->score(Ke, se, k, t);
+}
+
+// Alg. 3 for every slot: codes [k_max][S][G] (K and V), scores [k_max][S] (fixed-point), zero[k_max] = 1 when
+// the slot contributes zero residuals (n_res = 0 or no codebooks), 2 when the slot is not in the context at all.
+void pko_synthesize(void* h, uint8_t* codes_k, uint8_t* codes_v, int64_t* scores_k, int64_t* scores_v, uint8_t* zero) {
+  Bank* b = static_cast<Bank*>(h);
+  const Config& cf = b->cfg;
+  std::vector<Tuple> z;
+  std::vector<int64_t> sc;
+  for (int k = 0; k < cf.k_max; ++k) {
+    bool present = b->active[k] && b->n[k] >= 1;
+    bool zr = !b->has_cb || b->nres[k] == 0;
+    if (zero) zero[k] = present ? (zr ? 1 : 0) : 2;
+    for (int kv = 0; kv < 2; ++kv) {
+      uint8_t* oc = kv ? codes_v : codes_k;
+      int64_t* os = kv ? scores_v : scores_k;
+      if (present && !zr) b->decode_top_s(&(kv ? b->hv : b->hk)[(size_t)k * cf.G * cf.C], z, &sc);
+      for (int s = 0; s < cf.S; ++s) {
+        bool have = present && !zr && s < (int)z.size();
+        if (oc) for (int g = 0; g < cf.G; ++g) oc[((size_t)k * cf.S + s) * cf.G + g] = have ? z[s][g] : 0;
+        if (os) os[(size_t)k * cf.S + s] = have ? sc[s] : 0;
+      }
+    }
+  }
+}
+
+// Alg. 3 on a caller-supplied histogram [G][C]; returns the number of tuples written (<= S)
+int pko_decode_hist(void* h, const uint32_t* H, uint8_t* codes /*[S][G]*/, int64_t* scores /*[S]*/) {
+  Bank* b = static_cast<Bank*>(h);
+  std::vector<Tuple> z;
+  std::vector<int64_t> sc;
+  b->decode_top_s(H, z, &sc);
+  for (size_t s = 0; s < z.size(); ++s) {
+    for (int g = 0; g < b->cfg.G; ++g) codes[s * b->cfg.G + g] = z[s][g];
+    if (scores) scores[s] = sc[s];
+  }
+  return (int)z.size();
+}
+// fixed-point Eq. 3 table of a caller-supplied histogram, q [G][C]
+void pko_log_table(void* h, const uint32_t* H, int64_t* q) {
+  Bank* b = static_cast<Bank*>(h);
+  std::vector<int64_t> t;
+  b->log_table(H, t);
+  std::memcpy(q, t.data(), t.size() * sizeof(int64_t));
+}
+int64_t pko_tuple_score(void* h, int k, int which, const uint8_t* z) {
+  return static_cast<Bank*>(h)->tuple_score(k, which, z);
+}
+
+// context length of the current state
+int pko_context_len(void* h) {
+  Bank* b = static_cast<Bank*>(h);
+  std::vector<double> Kt, Vt, bb;
+  b->materialize(nullptr, nullptr, Kt, Vt, bb);
+  return (int)bb.size();
+}
+// [near || pseudo] as doubles: Kt, Vt [L][d], bias [L]; returns L (call pko_context_len first)
+int pko_materialize(void* h, const uint8_t* forced_codes_k, const uint8_t* forced_codes_v, double* Kt, double* Vt,
+                    double* bias) {
+  Bank* b = static_cast<Bank*>(h);
+  std::vector<double> k, v, bb;
+  b->materialize(forced_codes_k, forced_codes_v, k, v, bb);
+  if (Kt) std::memcpy(Kt, k.data(), k.size() * sizeof(double));
+  if (Vt) std::memcpy(Vt, v.data(), v.size() * sizeof(double));
+  if (bias) std::memcpy(bias, bb.data(), bb.size() * sizeof(double));
+  return (int)bb.size();
+}
+
+// Q [rows][d] fp32 (bf16 inputs widened exactly by the caller); out [rows][d] fp32; lse [rows] or NULL
+int pko_attention(void* h, const float* Q, int rows, const uint8_t* forced_codes_k, const uint8_t* forced_codes_v,
+                  float* out, double* lse) {
+  Bank* b = static_cast<Bank*>(h);
+  if (!b || !Q || !out || rows < 0) return 1;
+  b->attention(Q, rows, forced_codes_k, forced_codes_v, out, lse);
+  return 0;
+}
+
+}  // extern "C"
