@@ -1,0 +1,179 @@
+/*
+ * protokv.h -- C ABI of the B200-native (sm_100a) ProtoKV two-tier KV memory hot path.
+ *
+ * Paper: arxiv 2606.26762 ("PAPER.md" below = the extracted text of that paper).  One *bank* is the memory
+ * of one (stream, layer, KV head): an exact near-window ring buffer B_near of the last W = near_frames * T
+ * visual tokens and a fixed-capacity far prototype bank B_far = {Pi_k}, k < K_max,
+ * Pi_k = (c_k, p_k, n_k, R_k, mu_k, Sigma_k, tau_k).  Banks are independent
+ * (PAPER.md:L312); one state object holds n_streams * n_layers * n_kv_heads of them and every call processes
+ * all of them in batched kernel launches.
+ *
+ * Everything runs in hand-written CUDA kernels on the caller's stream.  There is no CPU fallback: on a machine
+ * without an sm_100 device protokv_create fails with PROTOKV_EUNSUPPORTED.
+ *
+ * Conventions
+ *   - "device"/"host" says where a pointer must live.  Tensor arguments are caller-owned and contiguous.
+ *   - Calls enqueue work on cfg.cuda_stream and return without synchronising unless stated otherwise.
+ *     Arguments must stay valid until the stream has passed the call's work.
+ *   - Every function returns a protokv_status (0 = OK) unless stated otherwise; argument, shape and capability
+ *     errors are detected before any launch and leave the state unchanged.  protokv_last_error() returns a
+ *     thread-local message for the last failing call.  Nothing throws or aborts across this boundary.
+ *   - A state is not thread-safe; distinct states are independent.
+ *
+ * Layouts (row-major, last index fastest), bank = (stream * n_layers + layer) * n_kv_heads + kv_head:
+ *   K, V      [n_streams][n_layers][T][n_kv_heads][head_dim]     dtype cfg.dtype
+ *   grid_pos  [n_streams][T][2]  fp32 normalised (x, y) of each token's cell in its frame
+ *   Q, out    [n_streams][n_layers][n_query_tokens][n_q_heads][head_dim]   dtype cfg.dtype
+ *   query head h reads the bank of KV head h / (n_q_heads / n_kv_heads)    (GQA)
+ *   codebooks [n_streams][n_layers][n_kv_heads][G][C][head_dim / G]  fp32
+ */
+#ifndef PROTOKV_H_
+#define PROTOKV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct protokv_state protokv_state; /* opaque; owned by the library until protokv_destroy */
+
+typedef enum {
+  PROTOKV_OK = 0,
+  PROTOKV_EINVAL = 1,       /* NULL pointer, bad shape, bad struct_size, index out of range */
+  PROTOKV_EUNSUPPORTED = 2, /* valid request this build cannot run (head_dim, C > 16, no sm_100 device, ...) */
+  PROTOKV_ENOMEM = 3,       /* workspace too small */
+  PROTOKV_ECUDA = 4,        /* a CUDA call failed; text in protokv_last_error() */
+  PROTOKV_ESTATE = 5        /* call not valid in the current state (e.g. trace before any eviction) */
+} protokv_status;
+
+typedef enum { PROTOKV_F32 = 0, PROTOKV_BF16 = 1 } protokv_dtype;
+
+/* cfg.flags */
+enum {
+  PROTOKV_MAH_SQUARED = 1u,  /* use d_Mah^2 in Eq. 1 (alternative reading of PAPER.md:L93)              */
+  PROTOKV_NO_MASS_BIAS = 2u, /* b_k = 0              (Table 2 "w/o mass bias", L180)            */
+  PROTOKV_NO_RESIDUAL = 4u,  /* never update histograms => zero residuals (Table 2)               */
+  PROTOKV_NEAR_ONLY = 8u,    /* attention over the near window only (L176)                              */
+  PROTOKV_FAR_ONLY = 16u,    /* attention over pseudo-tokens only   (L177)                              */
+  PROTOKV_FORCE_SIMT = 32u   /* use the fp32 SIMT kernels even where a tcgen05 kernel exists (cross-check) */
+};
+
+typedef struct {
+  uint32_t struct_size;   /* = sizeof(protokv_config); ABI versioning */
+  int32_t n_streams, n_layers, n_q_heads, n_kv_heads, head_dim; /* head_dim in {64, 128}; n_q % n_kv == 0 */
+  int32_t dtype;          /* protokv_dtype of K, V, Q, out */
+  int32_t tokens_per_frame; /* T  */
+  int32_t near_frames;    /* W_f: the near window holds W_f whole frames, W = W_f * T tokens */
+  int32_t k_max;          /* prototype capacity per bank */
+  int32_t n_query_tokens; /* N_q of protokv_query_attention */
+  int32_t S, G, C, beam;  /* Table 5: 8, 8, 16, 32.  S <= 8, G <= 8, C <= 16, C^G >= S, beam >= S */
+  float lambda_sp, lambda_idle; /* Eq. 1 weights: 0.1, 0.01 */
+  int32_t t_idle;         /* T_idle in frames: 120 */
+  float alpha, beta, eta; /* EMA rates of c, p and (mu, Sigma): 0.05 */
+  float sigma_eps;        /* added to the diagonal of Sigma_k before inversion (reading 4): 1e-4 */
+  float cos_eps;          /* lower bound of |K||c| in the cosine (reading 6): 1e-12 */
+  double pq_eps;          /* epsilon of Eq. 3 (value not given in the paper): 1e-6 */
+  uint32_t flags;
+  const float *codebook_k, *codebook_v; /* device; copied at create.  NULL => no residual statistics */
+  void *workspace;        /* device memory from the caller, >= protokv_workspace_bytes(cfg), 256-byte aligned */
+  size_t workspace_bytes;
+  void *cuda_stream;      /* cudaStream_t of the caller (NULL = legacy default stream) */
+} protokv_config;
+
+/* Bytes of device workspace a state with this configuration needs; 0 if the configuration is invalid
+ * (protokv_last_error() says why).  Pointer fields of cfg are ignored.  Host-only, no CUDA call. */
+size_t protokv_workspace_bytes(const protokv_config *cfg);
+
+/* Builds the state inside cfg->workspace (zeroed asynchronously on the stream).  NULL on failure. */
+protokv_state *protokv_create(const protokv_config *cfg);
+
+/* Releases host-side resources.  The workspace stays the caller's.  NULL is a no-op. */
+void protokv_destroy(protokv_state *st);
+
+/*
+ * Alg. 1 for one frame of every bank, frame-synchronous reading (reading 1):
+ * the frame is appended to the ring; if the ring was full its oldest frame (T tokens, in stored order) is
+ * evicted and absorbed:  (A) while free slots remain each evicted token opens the lowest free slot (l.3-4, L83);
+ * (B) the others are assigned by Eq. 1 (L93) against the bank as it stands after (A), lowest index on ties;
+ * (C) Alg. 1 l.8-13 is replayed token by token in eviction order (EMA centres, mass, recency, spatial mean and
+ * covariance, PQ residual histograms of the just-updated centres).  Alg. 1 l.15 (maintenance) is not run.
+ * K, V, grid_pos: device.
+ */
+int protokv_append_frame(protokv_state *st, const void *K, const void *V, const float *grid_pos);
+
+/*
+ * Alg. 4: for every active prototype decode the top-S residual modes of H^K and H^V by
+ * Alg. 3 / Eq. 3 (zero residuals when n_res = 0), then O = softmax(Q K~^T / sqrt(d) + b) V~ over
+ * [near window || pseudo-tokens], b = log n_k on pseudo-tokens (Eq. 2/4) and 0 on near tokens; no mask.
+ * Pseudo-tokens are built on chip and never written to HBM.  Q, out: device.  Does not modify the memory.
+ */
+int protokv_query_attention(protokv_state *st, const void *Q, void *out);
+
+/* The same two calls with HOST buffers (pinned memory recommended): inputs are copied to the device and, for
+ * the query, the result copied back, on the state's stream.  append returns without synchronising; the query
+ * variant synchronises the stream before returning so `out` is ready. */
+int protokv_append_frame_host(protokv_state *st, const void *K, const void *V, const float *grid_pos);
+int protokv_query_attention_host(protokv_state *st, const void *Q, void *out);
+
+/* Thread-local description of the last error returned on this thread ("" if none). */
+const char *protokv_last_error(void);
+
+/* ------------------------------------------------------------------------------------------------------ */
+/* Parity / debug surface (not on the timed path).                                                          */
+/* ------------------------------------------------------------------------------------------------------ */
+
+/* Attention for n_q query tokens (<= cfg.n_query_tokens) of layers [layer_begin, layer_begin + layer_count):
+ * Q, out [n_streams][layer_count][n_q][n_q_heads][head_dim] device; lse (optional, device)
+ * [n_streams][layer_count][n_q][n_q_heads] fp32 natural-log-sum-exp of the logits.  run_synthesis = 0 reuses
+ * the codes of the previous synthesis (or of protokv_import_codes). */
+int protokv_query_attention_ex(protokv_state *st, const void *Q, int32_t n_q, int32_t layer_begin,
+                               int32_t layer_count, void *out, float *lse, int32_t run_synthesis);
+
+/* Alg. 3 for every bank without the attention (timing / parity of the synthesis kernel alone). */
+int protokv_synthesize(protokv_state *st);
+
+/* Host views of one bank; NULL members are skipped.  Both calls synchronise the stream. */
+typedef struct {
+  float *c, *p;                 /* [k_max][head_dim] key / value centres                                  */
+  int32_t *n;                   /* [k_max] mass                                                           */
+  float *mu, *sigma;            /* [k_max][2]; [k_max][3] = (xx, xy, yy)                                  */
+  int32_t *tau;                 /* [k_max] frame index of the last absorption (idle test)                 */
+  int64_t *pos;                 /* [k_max] stream position of the last absorbed token (RoPE anchor, L126) */
+  uint32_t *hist_k, *hist_v;    /* [k_max][G][C]                                                          */
+  uint32_t *nres;               /* [k_max]                                                                */
+  uint8_t *active;              /* [k_max]                                                                */
+} protokv_bank_view;
+int protokv_export_state(protokv_state *st, int32_t bank, const protokv_bank_view *host_dst);
+int protokv_import_state(protokv_state *st, int32_t bank, const protokv_bank_view *host_src);
+
+/* Near window of one bank in chronological order, as fp32 on the host: K, V [n][T][head_dim], s [n][T][2],
+ * frame_index [n]; *n_frames receives n (<= near_frames).  NULL members are skipped.  Synchronises. */
+int protokv_export_ring(protokv_state *st, int32_t bank, float *K, float *V, float *s, int32_t *frame_index,
+                        int32_t *n_frames);
+
+/* Result of the last synthesis for one bank, on the host: codes [k_max][S][G] (one code per byte) and
+ * kind [k_max] (0 = decoded modes, 1 = zero residuals, 2 = slot not in the context).  Synchronises. */
+int protokv_export_codes(protokv_state *st, int32_t bank, uint8_t *codes_k, uint8_t *codes_v, uint8_t *kind);
+int protokv_import_codes(protokv_state *st, int32_t bank, const uint8_t *codes_k, const uint8_t *codes_v);
+
+/* What the last append_frame decided, all banks, on the host: assign [banks][T] (slot index; -1 if no frame
+ * was evicted), best [banks][T] (Eq. 1 score of the choice; 0 for slot fills), codes_k/v [banks][T][G]
+ * (255 = no residual update); *n_fill = tokens per bank that opened a new slot; *evicted_frame = index of the
+ * evicted frame or -1.  NULL members are skipped.  Synchronises. */
+int protokv_last_frame_trace(protokv_state *st, int32_t *assign, float *best, uint8_t *codes_k,
+                             uint8_t *codes_v, int32_t *n_fill, int32_t *evicted_frame);
+
+/* Counters: frames appended so far; kernels launched by this state since create (bench's gpu_launches). */
+int64_t protokv_frames_seen(const protokv_state *st);
+int64_t protokv_kernel_launches(const protokv_state *st);
+
+/* Names the kernel variant each stage uses for this state ("simt" / "tcgen05"), for reports.
+ * stage: 0 = assignment, 1 = attention.  Returns a static string, never NULL. */
+const char *protokv_stage_impl(const protokv_state *st, int32_t stage);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PROTOKV_H_ */

@@ -1,0 +1,149 @@
+// Internal definitions shared by the ProtoKV CUDA kernels and the C-ABI host code (not part of the ABI).
+// Layout of the device state is documented in DESIGN.md "Data layout in HBM".
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/protokv.h"
+
+namespace pkv {
+
+constexpr int kMaxS = 8, kMaxG = 8, kMaxC = 16;
+constexpr int kCbPad = 16;  // floats of padding after each subspace's [C][sub] block in shared memory
+
+// Shapes, fixed at create.
+struct Dims {
+  int B;       // banks = NS * L * Hkv
+  int NS, L, Hq, Hkv, group;
+  int d, sub;  // head_dim, d / G
+  int T, Wf;   // tokens per frame, near frames (= ring slots; frame f lives in slot f % Wf)
+  int K;       // k_max
+  int S, G, C;
+  int Nq;
+  int bf16;    // 1: K/V/Q/out are bf16, 0: fp32
+};
+
+struct Hyper {
+  float lambda_sp, lambda_idle;
+  int t_idle;
+  float alpha, beta, eta, sigma_eps, cos_eps;
+  double pq_eps;
+  uint32_t flags;
+};
+
+// Per-prototype scoring record (Eq. 1 terms that do not depend on the token), 32 bytes.
+//   invc = 1/|c_k|;  (mux, muy) = mu_k;  (u, v, w) = lambda-scaled inverse Cholesky factor of Sigma_k + eps I:
+//   lambda_sp * d_Mah = sqrt((dx u)^2 + (dy v - dx w)^2);  tau = frame index of the last absorption.
+struct __align__(16) ScoreRec {
+  float invc, mux, muy, u;
+  float v, w;
+  int tau;
+  int pad;
+};
+
+// Device pointers into the workspace.
+struct Dev {
+  // near window
+  void* ringK;   // [B][Wf][T][d] elt
+  void* ringV;
+  float* ringS;  // [NS][Wf][T][2]
+  // far bank
+  float* c;      // [B][K][d]
+  float* p;
+  __nv_bfloat16* c_hi;  // [B][K][d] bf16 shadows (bf16 mode): c = c_hi + c_lo + O(2^-17 |c|)
+  __nv_bfloat16* c_lo;
+  int* n;        // [B][K]
+  float* mu;     // [B][K][2]
+  float* sigma;  // [B][K][3]
+  int* tau;      // [B][K]
+  long long* pos;  // [B][K]
+  uint32_t* nres;  // [B][K]
+  ScoreRec* rec;   // [B][K]
+  float* logn;     // [B][K]  log n_k (Eq. 4 bias)
+  uint32_t* hist;  // [B][K][2][G][C]
+  float* cbk;      // [B][G][C][sub]  (NULL when the state has no residual statistics)
+  float* cbv;
+  // synthesis result
+  uint32_t* codesK;  // [B][K][S], code of subspace g in bits [4g, 4g+4)
+  uint32_t* codesV;
+  uint8_t* kind;     // [B][K] 0 decoded, 1 zero residual, 2 absent
+  // per-frame scratch / trace
+  int* assign;       // [B][T]
+  float* best;       // [B][T]
+  uint8_t* tcodeK;   // [B][T][G]
+  uint8_t* tcodeV;
+  // attention scratch
+  float* part;   // [rows_total][nsplit][d + 2]
+  // host-variant staging
+  void* stageK; void* stageV; float* stageS; void* stageQ; void* stageO;
+};
+
+__host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+template <typename T> __device__ __forceinline__ float to_f32(T x);
+template <> __device__ __forceinline__ float to_f32<float>(float x) { return x; }
+template <> __device__ __forceinline__ float to_f32<__nv_bfloat16>(__nv_bfloat16 x) { return __bfloat162float(x); }
+template <typename T> __device__ __forceinline__ T from_f32(float x);
+template <> __device__ __forceinline__ float from_f32<float>(float x) { return x; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float x) { return __float2bfloat16_rn(x); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Load VEC consecutive elements starting at ptr[i0] as floats (VEC in {2, 4}; 4-/8-/16-byte aligned accesses).
+template <typename T, int VEC> __device__ __forceinline__ void load_vec(const T* ptr, float (&out)[VEC]);
+template <> __device__ __forceinline__ void load_vec<float, 4>(const float* ptr, float (&o)[4]) {
+  float4 v = *reinterpret_cast<const float4*>(ptr); o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+template <> __device__ __forceinline__ void load_vec<float, 2>(const float* ptr, float (&o)[2]) {
+  float2 v = *reinterpret_cast<const float2*>(ptr); o[0] = v.x; o[1] = v.y;
+}
+template <> __device__ __forceinline__ void load_vec<__nv_bfloat16, 4>(const __nv_bfloat16* ptr, float (&o)[4]) {
+  uint2 v = *reinterpret_cast<const uint2*>(ptr);
+  o[0] = __uint_as_float(v.x << 16); o[1] = __uint_as_float(v.x & 0xffff0000u);
+  o[2] = __uint_as_float(v.y << 16); o[3] = __uint_as_float(v.y & 0xffff0000u);
+}
+template <> __device__ __forceinline__ void load_vec<__nv_bfloat16, 2>(const __nv_bfloat16* ptr, float (&o)[2]) {
+  uint32_t v = *reinterpret_cast<const uint32_t*>(ptr);
+  o[0] = __uint_as_float(v << 16); o[1] = __uint_as_float(v & 0xffff0000u);
+}
+
+// ---- launchers implemented in the .cu files (all asynchronous on `stream`) -------------------------------
+struct FrameArgs {
+  int t;         // stream time of this step = index of the appended frame (reading 2)
+  int slot;      // ring slot of the appended frame = slot of the evicted frame (f % Wf)
+  int evicted;   // 1 if a frame leaves the window in this step
+  int ev_frame;  // index of the evicted frame
+  int n_act0;    // active prototypes before this step's slot fill
+  int n_fill;    // evicted tokens that open a new slot (Alg. 1 l.3-4)
+  int n_act;     // active prototypes after the fill = what Eq. 1 scans
+};
+
+// Every launcher returns the number of kernels it launched (0 if there was nothing to do).
+int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const void* Kin, const void* Vin,
+                       const float* grid_pos, cudaStream_t s);
+int launch_fill(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
+int launch_score_simt(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
+int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s);
+int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, cudaStream_t s);
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s);
+
+struct AttnArgs {
+  const void* Q; void* out; float* lse;
+  int n_q, layer_begin, layer_count;
+  int n_near;          // near-window tokens currently held (frames held * T): ring rows [0, n_near) of each bank
+  int n_act;
+  int nsplit;
+};
+int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
+int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
+
+// tcgen05 paths (bf16, d = 128)
+bool tc_assign_supported(const Dims& D, const Hyper& H);
+int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
+
+}  // namespace pkv

@@ -1,0 +1,490 @@
+// C ABI of the ProtoKV hot path (include/protokv.h): host-side state, workspace carving, argument checks and
+// kernel sequencing.  No arithmetic of the method happens here; every step runs in the kernels of
+// update_kernels.cu / query_kernels.cu / tc_*.cu.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace pkv;
+
+struct protokv_state {
+  protokv_config cfg;
+  Dims D;
+  Hyper H;
+  Dev V;
+  cudaStream_t stream;
+  int sm_count;
+  int64_t frames;     // frames appended so far = stream time of the next frame
+  int n_act;          // active prototypes per bank (identical in every bank: slot fill is data-independent)
+  int64_t launches;
+  int last_ev_frame;  // index of the frame evicted by the last append, -1 if none
+  int last_n_fill;
+  bool codes_valid;   // codes/kind describe the current histograms
+  bool use_tc_assign;
+  int nsplit;
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define PKV_CUDA(call)                                                                       \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess) return fail(PROTOKV_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+static bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
+
+// Validates everything that does not need a device.  Returns PROTOKV_OK or sets the error text.
+static int validate(const protokv_config* c) {
+  if (!c) return fail(PROTOKV_EINVAL, "cfg is NULL");
+  if (c->struct_size != sizeof(protokv_config))
+    return fail(PROTOKV_EINVAL, "struct_size %u != %zu", c->struct_size, sizeof(protokv_config));
+  if (c->n_streams < 1 || c->n_layers < 1 || c->n_q_heads < 1 || c->n_kv_heads < 1 || c->tokens_per_frame < 1 ||
+      c->near_frames < 1 || c->k_max < 1 || c->n_query_tokens < 1)
+    return fail(PROTOKV_EINVAL, "shape fields must be >= 1");
+  if (c->n_q_heads % c->n_kv_heads) return fail(PROTOKV_EINVAL, "n_q_heads %% n_kv_heads != 0");
+  if (c->dtype != PROTOKV_F32 && c->dtype != PROTOKV_BF16) return fail(PROTOKV_EINVAL, "unknown dtype");
+  if (c->head_dim != 64 && c->head_dim != 128) return fail(PROTOKV_EUNSUPPORTED, "head_dim must be 64 or 128");
+  if (c->S < 1 || c->G < 1 || c->C < 1 || c->beam < c->S) return fail(PROTOKV_EINVAL, "need S,G,C >= 1, beam >= S");
+  if (c->S > kMaxS || c->C > kMaxC || c->G > kMaxG || !is_pow2(c->G))
+    return fail(PROTOKV_EUNSUPPORTED, "need S <= 8, C <= 16, G in {1,2,4,8}");
+  if (c->head_dim % c->G) return fail(PROTOKV_EINVAL, "head_dim %% G != 0");
+  {
+    double tuples = 1;
+    for (int g = 0; g < c->G; ++g) tuples *= c->C;
+    if (tuples < c->S) return fail(PROTOKV_EINVAL, "C^G < S");
+  }
+  if (c->tokens_per_frame > 4096) return fail(PROTOKV_EUNSUPPORTED, "tokens_per_frame > 4096");
+  if (c->k_max >= (1 << 20)) return fail(PROTOKV_EUNSUPPORTED, "k_max >= 2^20");
+  if (!(c->alpha >= 0.f && c->alpha <= 1.f && c->beta >= 0.f && c->beta <= 1.f && c->eta >= 0.f && c->eta <= 1.f))
+    return fail(PROTOKV_EINVAL, "alpha, beta, eta must lie in [0, 1]");
+  if (!(c->sigma_eps >= 0.f) || !(c->cos_eps > 0.f) || !(c->pq_eps > 0.0))
+    return fail(PROTOKV_EINVAL, "need sigma_eps >= 0, cos_eps > 0, pq_eps > 0");
+  if ((c->flags & PROTOKV_NEAR_ONLY) && (c->flags & PROTOKV_FAR_ONLY))
+    return fail(PROTOKV_EINVAL, "NEAR_ONLY and FAR_ONLY are exclusive");
+  return PROTOKV_OK;
+}
+
+static void fill_dims(const protokv_config* c, Dims* D, Hyper* H) {
+  D->NS = c->n_streams; D->L = c->n_layers; D->Hq = c->n_q_heads; D->Hkv = c->n_kv_heads;
+  D->group = c->n_q_heads / c->n_kv_heads;
+  D->B = c->n_streams * c->n_layers * c->n_kv_heads;
+  D->d = c->head_dim; D->sub = c->head_dim / c->G;
+  D->T = c->tokens_per_frame; D->Wf = c->near_frames; D->K = c->k_max;
+  D->S = c->S; D->G = c->G; D->C = c->C; D->Nq = c->n_query_tokens;
+  D->bf16 = c->dtype == PROTOKV_BF16;
+  H->lambda_sp = c->lambda_sp; H->lambda_idle = c->lambda_idle; H->t_idle = c->t_idle;
+  H->alpha = c->alpha; H->beta = c->beta; H->eta = c->eta;
+  H->sigma_eps = c->sigma_eps; H->cos_eps = c->cos_eps; H->pq_eps = c->pq_eps; H->flags = c->flags;
+}
+
+// Lays the state out in the workspace (base may be NULL to only measure).  Every array is 256-byte aligned.
+static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> void* {
+    off = align_up(off, 256);
+    void* p = base ? base + off : nullptr;
+    off += bytes;
+    return p;
+  };
+  const size_t elt = D.bf16 ? 2 : 4;
+  const size_t BK = (size_t)D.B * D.K, BT = (size_t)D.B * D.T;
+  const size_t ring = (size_t)D.B * D.Wf * D.T * D.d * elt;
+  Dev v{};
+  v.ringK = take(ring); v.ringV = take(ring);
+  v.ringS = (float*)take((size_t)D.NS * D.Wf * D.T * 2 * 4);
+  v.c = (float*)take(BK * D.d * 4); v.p = (float*)take(BK * D.d * 4);
+  if (D.bf16) {
+    v.c_hi = (__nv_bfloat16*)take(BK * D.d * 2);
+    v.c_lo = (__nv_bfloat16*)take(BK * D.d * 2);
+  }
+  v.n = (int*)take(BK * 4); v.mu = (float*)take(BK * 8); v.sigma = (float*)take(BK * 12);
+  v.tau = (int*)take(BK * 4); v.pos = (long long*)take(BK * 8); v.nres = (uint32_t*)take(BK * 4);
+  v.rec = (ScoreRec*)take(BK * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
+  v.hist = (uint32_t*)take(BK * 2 * D.G * D.C * 4);
+  if (has_cb) {
+    v.cbk = (float*)take((size_t)D.B * D.G * D.C * D.sub * 4);
+    v.cbv = (float*)take((size_t)D.B * D.G * D.C * D.sub * 4);
+  }
+  v.codesK = (uint32_t*)take(BK * D.S * 4); v.codesV = (uint32_t*)take(BK * D.S * 4);
+  v.kind = (uint8_t*)take(BK);
+  v.assign = (int*)take(BT * 4); v.best = (float*)take(BT * 4);
+  v.tcodeK = (uint8_t*)take(BT * D.G); v.tcodeV = (uint8_t*)take(BT * D.G);
+  const size_t rows = (size_t)D.B * D.Nq * D.group;
+  v.part = (float*)take(rows * nsplit * (D.d + 2) * 4);
+  const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * elt;
+  const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * elt;
+  v.stageK = take(frame); v.stageV = take(frame);
+  v.stageS = (float*)take((size_t)D.NS * D.T * 2 * 4);
+  v.stageQ = take(qbytes); v.stageO = take(qbytes);
+  if (V) *V = v;
+  return align_up(off, 256);
+}
+
+// nsplit must be known without a device for protokv_workspace_bytes: size for the B200's 148 SMs.
+static int plan_nsplit(const Dims& D) { return attention_simt_splits(D, 148); }
+
+extern "C" {
+
+const char* protokv_last_error(void) { return g_err; }
+
+size_t protokv_workspace_bytes(const protokv_config* cfg) {
+  if (validate(cfg) != PROTOKV_OK) return 0;
+  Dims D; Hyper H;
+  fill_dims(cfg, &D, &H);
+  const bool has_cb = !(cfg->flags & PROTOKV_NO_RESIDUAL);   // sized as if codebooks were given
+  return carve(D, has_cb, plan_nsplit(D), nullptr, nullptr);
+}
+
+protokv_state* protokv_create(const protokv_config* cfg) {
+  g_err[0] = 0;
+  if (validate(cfg) != PROTOKV_OK) return nullptr;
+  if (!cfg->workspace) { fail(PROTOKV_EINVAL, "workspace is NULL"); return nullptr; }
+  if ((uintptr_t)cfg->workspace % 256) { fail(PROTOKV_EINVAL, "workspace must be 256-byte aligned"); return nullptr; }
+  if ((cfg->codebook_k == nullptr) != (cfg->codebook_v == nullptr)) {
+    fail(PROTOKV_EINVAL, "codebook_k and codebook_v must both be given or both be NULL");
+    return nullptr;
+  }
+  int dev = 0, major = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+    cudaGetLastError();
+    fail(PROTOKV_EUNSUPPORTED, "no CUDA device: this library has no CPU fallback");
+    return nullptr;
+  }
+  if (major != 10) { fail(PROTOKV_EUNSUPPORTED, "device is sm_%d0, this build is sm_100a only", major); return nullptr; }
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+
+  protokv_state* st = new (std::nothrow) protokv_state();
+  if (!st) { fail(PROTOKV_ENOMEM, "host allocation failed"); return nullptr; }
+  st->cfg = *cfg;
+  fill_dims(cfg, &st->D, &st->H);
+  st->stream = (cudaStream_t)cfg->cuda_stream;
+  st->sm_count = sms;
+  st->nsplit = plan_nsplit(st->D);
+  const bool has_cb = cfg->codebook_k && !(cfg->flags & PROTOKV_NO_RESIDUAL);
+  const size_t need = carve(st->D, has_cb, st->nsplit, (char*)cfg->workspace, &st->V);
+  if (need > cfg->workspace_bytes) {
+    fail(PROTOKV_ENOMEM, "workspace too small: need %zu bytes, got %zu", need, cfg->workspace_bytes);
+    delete st;
+    return nullptr;
+  }
+  cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, st->stream);
+  if (e == cudaSuccess && has_cb) {
+    const size_t cb = (size_t)st->D.B * st->D.G * st->D.C * st->D.sub * 4;
+    e = cudaMemcpyAsync(st->V.cbk, cfg->codebook_k, cb, cudaMemcpyDeviceToDevice, st->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st->V.cbv, cfg->codebook_v, cb, cudaMemcpyDeviceToDevice, st->stream);
+  }
+  if (e != cudaSuccess) {
+    fail(PROTOKV_ECUDA, "state initialisation: %s", cudaGetErrorString(e));
+    delete st;
+    return nullptr;
+  }
+  st->frames = 0; st->n_act = 0; st->launches = 0; st->last_ev_frame = -1; st->last_n_fill = 0;
+  st->codes_valid = false;
+  st->use_tc_assign = !(cfg->flags & PROTOKV_FORCE_SIMT) && tc_assign_supported(st->D, st->H);
+  return st;
+}
+
+void protokv_destroy(protokv_state* st) { delete st; }
+
+int protokv_append_frame(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
+  if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
+  const Dims& D = st->D;
+  FrameArgs F{};
+  F.t = (int)st->frames;
+  F.slot = (int)(st->frames % D.Wf);
+  F.evicted = st->frames >= D.Wf;
+  F.ev_frame = F.evicted ? (int)(st->frames - D.Wf) : -1;
+  F.n_act0 = st->n_act;
+  F.n_fill = F.evicted ? (D.K - st->n_act < D.T ? D.K - st->n_act : D.T) : 0;
+  F.n_act = st->n_act + F.n_fill;
+  int nl = 0;
+  if (F.evicted) {
+    nl += launch_fill(D, st->H, st->V, F, st->stream);                                  // U2
+    if (D.T - F.n_fill > 0) {
+      nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->stream)        // U3
+                              : launch_score_simt(D, st->H, st->V, F, st->stream);
+      nl += launch_update(D, st->H, st->V, F, st->sm_count, st->stream);                // U4-U6
+    }
+  }
+  nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                    // U1 (overwrites the slot)
+  PKV_CUDA(cudaGetLastError());
+  st->launches += nl;
+  st->n_act = F.n_act;
+  st->last_ev_frame = F.ev_frame;
+  st->last_n_fill = F.n_fill;
+  if (F.evicted) st->codes_valid = false;
+  st->frames += 1;
+  return PROTOKV_OK;
+}
+
+int protokv_synthesize(protokv_state* st) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->stream);
+  PKV_CUDA(cudaGetLastError());
+  st->codes_valid = true;
+  return PROTOKV_OK;
+}
+
+int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, int32_t layer_begin,
+                               int32_t layer_count, void* out, float* lse, int32_t run_synthesis) {
+  if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
+  const Dims& D = st->D;
+  if (n_q < 1 || n_q > D.Nq) return fail(PROTOKV_EINVAL, "n_q %d outside [1, %d]", n_q, D.Nq);
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > D.L)
+    return fail(PROTOKV_EINVAL, "layer range [%d, %d) outside [0, %d)", layer_begin, layer_begin + layer_count, D.L);
+  const bool far = !(st->H.flags & PROTOKV_NEAR_ONLY);
+  if (far) {
+    if (run_synthesis) {
+      const int rc = protokv_synthesize(st);
+      if (rc != PROTOKV_OK) return rc;
+    } else if (!st->codes_valid) {
+      return fail(PROTOKV_ESTATE, "run_synthesis = 0 but no synthesis result is valid for the current state");
+    }
+  }
+  AttnArgs A{};
+  A.Q = Q; A.out = out; A.lse = lse;
+  A.n_q = n_q; A.layer_begin = layer_begin; A.layer_count = layer_count;
+  const int64_t held = st->frames < D.Wf ? st->frames : D.Wf;
+  A.n_near = (int)(held * D.T);
+  A.n_act = st->n_act;
+  A.nsplit = st->nsplit;
+  st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
+  PKV_CUDA(cudaGetLastError());
+  return PROTOKV_OK;
+}
+
+int protokv_query_attention(protokv_state* st, const void* Q, void* out) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  return protokv_query_attention_ex(st, Q, st->D.Nq, 0, st->D.L, out, nullptr, 1);
+}
+
+int protokv_append_frame_host(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
+  if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
+  const Dims& D = st->D;
+  const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * (D.bf16 ? 2 : 4);
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageK, K, frame, cudaMemcpyHostToDevice, st->stream));
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageV, V, frame, cudaMemcpyHostToDevice, st->stream));
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageS, grid_pos, (size_t)D.NS * D.T * 8, cudaMemcpyHostToDevice, st->stream));
+  return protokv_append_frame(st, st->V.stageK, st->V.stageV, st->V.stageS);
+}
+
+int protokv_query_attention_host(protokv_state* st, const void* Q, void* out) {
+  if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
+  const Dims& D = st->D;
+  const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * (D.bf16 ? 2 : 4);
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageQ, Q, qbytes, cudaMemcpyHostToDevice, st->stream));
+  const int rc = protokv_query_attention(st, st->V.stageQ, st->V.stageO);
+  if (rc != PROTOKV_OK) return rc;
+  PKV_CUDA(cudaMemcpyAsync(out, st->V.stageO, qbytes, cudaMemcpyDeviceToHost, st->stream));
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  return PROTOKV_OK;
+}
+
+int64_t protokv_frames_seen(const protokv_state* st) { return st ? st->frames : -1; }
+int64_t protokv_kernel_launches(const protokv_state* st) { return st ? st->launches : -1; }
+
+const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
+  if (!st) return "none";
+  if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
+  if (stage == 1) return "simt";
+  return "none";
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------
+// Parity / debug surface (not on the timed path): host views of the state.  All of these synchronise.
+// ---------------------------------------------------------------------------------------------------------
+static int check_bank(const protokv_state* st, int32_t bank) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  if (bank < 0 || bank >= st->D.B) return fail(PROTOKV_EINVAL, "bank %d outside [0, %d)", bank, st->D.B);
+  return PROTOKV_OK;
+}
+
+static inline float bf16_to_f32(uint16_t h) {
+  uint32_t u = (uint32_t)h << 16;
+  float f;
+  memcpy(&f, &u, 4);
+  return f;
+}
+
+extern "C" {
+
+int protokv_export_state(protokv_state* st, int32_t bank, const protokv_bank_view* v) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!v) return fail(PROTOKV_EINVAL, "NULL view");
+  const Dims& D = st->D;
+  const Dev& V = st->V;
+  const size_t K = D.K, o = (size_t)bank * K;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  if (v->c) PKV_CUDA(cudaMemcpy(v->c, V.c + o * D.d, K * D.d * 4, cudaMemcpyDeviceToHost));
+  if (v->p) PKV_CUDA(cudaMemcpy(v->p, V.p + o * D.d, K * D.d * 4, cudaMemcpyDeviceToHost));
+  if (v->n) PKV_CUDA(cudaMemcpy(v->n, V.n + o, K * 4, cudaMemcpyDeviceToHost));
+  if (v->mu) PKV_CUDA(cudaMemcpy(v->mu, V.mu + o * 2, K * 8, cudaMemcpyDeviceToHost));
+  if (v->sigma) PKV_CUDA(cudaMemcpy(v->sigma, V.sigma + o * 3, K * 12, cudaMemcpyDeviceToHost));
+  if (v->tau) PKV_CUDA(cudaMemcpy(v->tau, V.tau + o, K * 4, cudaMemcpyDeviceToHost));
+  if (v->pos) PKV_CUDA(cudaMemcpy(v->pos, V.pos + o, K * 8, cudaMemcpyDeviceToHost));
+  if (v->nres) PKV_CUDA(cudaMemcpy(v->nres, V.nres + o, K * 4, cudaMemcpyDeviceToHost));
+  const size_t gc = (size_t)D.G * D.C * 4;
+  if (v->hist_k) PKV_CUDA(cudaMemcpy2D(v->hist_k, gc, V.hist + o * 2 * D.G * D.C, 2 * gc, gc, K, cudaMemcpyDeviceToHost));
+  if (v->hist_v)
+    PKV_CUDA(cudaMemcpy2D(v->hist_v, gc, V.hist + o * 2 * D.G * D.C + D.G * D.C, 2 * gc, gc, K, cudaMemcpyDeviceToHost));
+  if (v->active)
+    for (int k = 0; k < D.K; ++k) v->active[k] = k < st->n_act ? 1 : 0;
+  return PROTOKV_OK;
+}
+
+int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_view* v) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!v) return fail(PROTOKV_EINVAL, "NULL view");
+  const Dims& D = st->D;
+  const Dev& V = st->V;
+  const size_t K = D.K, o = (size_t)bank * K;
+  if (v->active) {   // the active set must be the prefix this state already has (slot fill is data-independent)
+    int na = 0;
+    while (na < D.K && v->active[na]) ++na;
+    for (int k = na; k < D.K; ++k)
+      if (v->active[k]) return fail(PROTOKV_EINVAL, "active set is not a prefix");
+    if (na != st->n_act) return fail(PROTOKV_EINVAL, "imported active count %d != state's %d", na, st->n_act);
+  }
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  if (v->c) PKV_CUDA(cudaMemcpy(V.c + o * D.d, v->c, K * D.d * 4, cudaMemcpyHostToDevice));
+  if (v->p) PKV_CUDA(cudaMemcpy(V.p + o * D.d, v->p, K * D.d * 4, cudaMemcpyHostToDevice));
+  if (v->n) PKV_CUDA(cudaMemcpy(V.n + o, v->n, K * 4, cudaMemcpyHostToDevice));
+  if (v->mu) PKV_CUDA(cudaMemcpy(V.mu + o * 2, v->mu, K * 8, cudaMemcpyHostToDevice));
+  if (v->sigma) PKV_CUDA(cudaMemcpy(V.sigma + o * 3, v->sigma, K * 12, cudaMemcpyHostToDevice));
+  if (v->tau) PKV_CUDA(cudaMemcpy(V.tau + o, v->tau, K * 4, cudaMemcpyHostToDevice));
+  if (v->pos) PKV_CUDA(cudaMemcpy(V.pos + o, v->pos, K * 8, cudaMemcpyHostToDevice));
+  if (v->nres) PKV_CUDA(cudaMemcpy(V.nres + o, v->nres, K * 4, cudaMemcpyHostToDevice));
+  const size_t gc = (size_t)D.G * D.C * 4;
+  if (v->hist_k) PKV_CUDA(cudaMemcpy2D(V.hist + o * 2 * D.G * D.C, 2 * gc, v->hist_k, gc, gc, K, cudaMemcpyHostToDevice));
+  if (v->hist_v)
+    PKV_CUDA(cudaMemcpy2D(V.hist + o * 2 * D.G * D.C + D.G * D.C, 2 * gc, v->hist_v, gc, gc, K, cudaMemcpyHostToDevice));
+  st->launches += launch_refresh_derived(D, st->H, V, bank, st->stream);
+  PKV_CUDA(cudaGetLastError());
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  st->codes_valid = false;
+  return PROTOKV_OK;
+}
+
+int protokv_export_ring(protokv_state* st, int32_t bank, float* K, float* Vv, float* s, int32_t* frame_index,
+                        int32_t* n_frames) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  const Dims& D = st->D;
+  const int held = (int)(st->frames < D.Wf ? st->frames : D.Wf);
+  if (n_frames) *n_frames = held;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  const size_t fe = (size_t)D.T * D.d, elt = D.bf16 ? 2 : 4;
+  const int stream_idx = bank / (D.L * D.Hkv);
+  std::vector<unsigned char> tmp(fe * elt);
+  for (int i = 0; i < held; ++i) {
+    const int64_t f = st->frames - held + i;
+    const int slot = (int)(f % D.Wf);
+    if (frame_index) frame_index[i] = (int32_t)f;
+    for (int kv = 0; kv < 2; ++kv) {
+      float* dst = kv ? Vv : K;
+      if (!dst) continue;
+      const char* src = (const char*)(kv ? st->V.ringV : st->V.ringK) + (((size_t)bank * D.Wf + slot) * fe) * elt;
+      if (D.bf16) {
+        PKV_CUDA(cudaMemcpy(tmp.data(), src, fe * 2, cudaMemcpyDeviceToHost));
+        const uint16_t* h = (const uint16_t*)tmp.data();
+        for (size_t e = 0; e < fe; ++e) dst[i * fe + e] = bf16_to_f32(h[e]);
+      } else {
+        PKV_CUDA(cudaMemcpy(dst + i * fe, src, fe * 4, cudaMemcpyDeviceToHost));
+      }
+    }
+    if (s)
+      PKV_CUDA(cudaMemcpy(s + (size_t)i * D.T * 2, st->V.ringS + ((size_t)stream_idx * D.Wf + slot) * D.T * 2,
+                          (size_t)D.T * 8, cudaMemcpyDeviceToHost));
+  }
+  return PROTOKV_OK;
+}
+
+int protokv_export_codes(protokv_state* st, int32_t bank, uint8_t* codes_k, uint8_t* codes_v, uint8_t* kind) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!st->codes_valid) return fail(PROTOKV_ESTATE, "no synthesis result for the current state");
+  const Dims& D = st->D;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  std::vector<uint32_t> tmp((size_t)D.K * D.S);
+  for (int kv = 0; kv < 2; ++kv) {
+    uint8_t* dst = kv ? codes_v : codes_k;
+    if (!dst) continue;
+    PKV_CUDA(cudaMemcpy(tmp.data(), (kv ? st->V.codesV : st->V.codesK) + (size_t)bank * D.K * D.S, tmp.size() * 4,
+                        cudaMemcpyDeviceToHost));
+    for (size_t e = 0; e < tmp.size(); ++e)
+      for (int g = 0; g < D.G; ++g) dst[e * D.G + g] = (uint8_t)((tmp[e] >> (4 * g)) & 15u);
+  }
+  if (kind) PKV_CUDA(cudaMemcpy(kind, st->V.kind + (size_t)bank * D.K, D.K, cudaMemcpyDeviceToHost));
+  return PROTOKV_OK;
+}
+
+int protokv_import_codes(protokv_state* st, int32_t bank, const uint8_t* codes_k, const uint8_t* codes_v) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!st->codes_valid) return fail(PROTOKV_ESTATE, "run protokv_synthesize first (kind[] comes from it)");
+  const Dims& D = st->D;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  std::vector<uint32_t> tmp((size_t)D.K * D.S);
+  for (int kv = 0; kv < 2; ++kv) {
+    const uint8_t* src = kv ? codes_v : codes_k;
+    if (!src) continue;
+    for (size_t e = 0; e < tmp.size(); ++e) {
+      uint32_t w = 0;
+      for (int g = 0; g < D.G; ++g) {
+        if (src[e * D.G + g] >= D.C) return fail(PROTOKV_EINVAL, "code out of range");
+        w |= (uint32_t)src[e * D.G + g] << (4 * g);
+      }
+      tmp[e] = w;
+    }
+    PKV_CUDA(cudaMemcpy((kv ? st->V.codesV : st->V.codesK) + (size_t)bank * D.K * D.S, tmp.data(), tmp.size() * 4,
+                        cudaMemcpyHostToDevice));
+  }
+  return PROTOKV_OK;
+}
+
+int protokv_last_frame_trace(protokv_state* st, int32_t* assign, float* best, uint8_t* codes_k, uint8_t* codes_v,
+                             int32_t* n_fill, int32_t* evicted_frame) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  if (st->frames == 0) return fail(PROTOKV_ESTATE, "no frame appended yet");
+  const Dims& D = st->D;
+  if (n_fill) *n_fill = st->last_n_fill;
+  if (evicted_frame) *evicted_frame = st->last_ev_frame;
+  const size_t BT = (size_t)D.B * D.T;
+  if (st->last_ev_frame < 0) {
+    if (assign) for (size_t i = 0; i < BT; ++i) assign[i] = -1;
+    if (best) memset(best, 0, BT * 4);
+    if (codes_k) memset(codes_k, 255, BT * D.G);
+    if (codes_v) memset(codes_v, 255, BT * D.G);
+    return PROTOKV_OK;
+  }
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  if (assign) PKV_CUDA(cudaMemcpy(assign, st->V.assign, BT * 4, cudaMemcpyDeviceToHost));
+  if (best) PKV_CUDA(cudaMemcpy(best, st->V.best, BT * 4, cudaMemcpyDeviceToHost));
+  if (st->V.cbk) {
+    if (codes_k) PKV_CUDA(cudaMemcpy(codes_k, st->V.tcodeK, BT * D.G, cudaMemcpyDeviceToHost));
+    if (codes_v) PKV_CUDA(cudaMemcpy(codes_v, st->V.tcodeV, BT * D.G, cudaMemcpyDeviceToHost));
+  } else {
+    if (codes_k) memset(codes_k, 255, BT * D.G);
+    if (codes_v) memset(codes_v, 255, BT * D.G);
+  }
+  return PROTOKV_OK;
+}
+
+}  // extern "C"

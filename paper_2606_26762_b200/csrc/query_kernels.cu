@@ -1,0 +1,316 @@
+// ProtoKV query-time path (Alg. 3, Eq. 3, Alg. 4, Eq. 2/4 L130/L405):
+// pseudo-token synthesis (top-S residual modes per prototype) and the fp32 SIMT fused attention over
+// [near window || pseudo-tokens] with the log-mass bias inside the online softmax.  Pseudo-tokens are built in
+// registers from (c_k, p_k, codes, codebooks) and never written to HBM.  See DESIGN.md "Kernels".
+#include "common.cuh"
+
+namespace pkv {
+
+// ---------------------------------------------------------------------------------------------------------
+// Q1 synthesis.  One thread per (bank, prototype, K|V).
+//
+// Scores are the fixed-point log-probabilities of Eq. 3, q(g,z) = llround(2^24 log((H[g,z]+eps)/(sum+C eps)))
+// (reading 13), tuples are ordered by (sum of q descending, tuple ascending lexicographically, z_1 most
+// significant).  Beam search with width >= S over additive per-subspace scores under that total order returns
+// exactly the global top-S, so this kernel keeps S partial tuples per step, and of the S x S products of the
+// (sorted) beam with the (sorted) top-S codes of the next subspace only the staircase i*j <= S can survive:
+// an entry (i, j) is preceded by every (i', j') <= (i, j).
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kSynThreads = 128;
+
+__global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act) {
+  const long long idx = (long long)blockIdx.x * kSynThreads + threadIdx.x;
+  const long long total = (long long)D.B * D.K * 2;
+  if (idx >= total) return;
+  const int kv = (int)(idx & 1);
+  const size_t pk = (size_t)(idx >> 1);
+  const int k = (int)(pk % D.K);
+  const bool has_cb = V.cbk != nullptr;
+  const bool present = k < n_act && V.n[pk] >= 1;
+  const bool zero = !has_cb || V.nres[pk] == 0;
+  uint32_t* codes = (kv ? V.codesV : V.codesK) + pk * D.S;
+  if (kv == 0) V.kind[pk] = present ? (zero ? 1 : 0) : 2;
+  if (!present || zero) {
+    for (int s = 0; s < D.S; ++s) codes[s] = 0u;
+    return;
+  }
+  const uint32_t* Hrow = V.hist + (pk * 2 + kv) * D.G * D.C;
+  const int S = D.S, C = D.C, G = D.G;
+  const int m = C < S ? C : S;
+  long long bc[kMaxS];       // beam cost = -sum q (>= 0), ascending
+  uint32_t bt[kMaxS];        // beam tuple, z_1 in the most significant nibble
+  int nb = 1;
+  bc[0] = 0; bt[0] = 0u;
+  for (int g = 0; g < G; ++g) {
+    uint32_t h[kMaxC];
+    long long q[kMaxC];
+    double tot = 0.0;
+    for (int z = 0; z < C; ++z) { h[z] = Hrow[g * C + z]; tot += (double)h[z]; }
+    const double den = tot + (double)C * H.pq_eps;
+    for (int z = 0; z < C; ++z) {
+      int same = -1;
+      for (int y = 0; y < z; ++y) if (h[y] == h[z]) { same = y; break; }
+      if (same >= 0) q[z] = q[same];
+      else {
+        const double P = ((double)h[z] + H.pq_eps) / den;
+        q[z] = -llround(log(P) * 16777216.0);   // cost = -q
+      }
+    }
+    // top-m codes by (cost ascending, z ascending)
+    long long tq[kMaxS];
+    int tz[kMaxS];
+    uint32_t taken = 0u;
+    for (int i = 0; i < m; ++i) {
+      int bz = -1;
+      long long bq = 0;
+      for (int z = 0; z < C; ++z)
+        if (!((taken >> z) & 1u) && (bz < 0 || q[z] < bq)) { bz = z; bq = q[z]; }
+      taken |= 1u << bz;
+      tq[i] = bq; tz[i] = bz;
+    }
+    // staircase candidates -> new beam (insertion sort by (cost, tuple))
+    long long nc[kMaxS];
+    uint32_t nt[kMaxS];
+    int cnt = 0;
+    for (int i = 0; i < nb; ++i) {
+      for (int j = 0; j < m && (i + 1) * (j + 1) <= S; ++j) {
+        const long long cost = bc[i] + tq[j];
+        const uint32_t tup = (bt[i] << 4) | (uint32_t)tz[j];
+        int pos = cnt;
+        while (pos > 0 && (nc[pos - 1] > cost || (nc[pos - 1] == cost && nt[pos - 1] > tup))) --pos;
+        if (pos >= S) continue;
+        const int last = cnt < S ? cnt : S - 1;
+        for (int e = last; e > pos; --e) { nc[e] = nc[e - 1]; nt[e] = nt[e - 1]; }
+        nc[pos] = cost; nt[pos] = tup;
+        if (cnt < S) ++cnt;
+      }
+    }
+    nb = cnt;
+    for (int i = 0; i < nb; ++i) { bc[i] = nc[i]; bt[i] = nt[i]; }
+  }
+  for (int s = 0; s < S; ++s) {
+    uint32_t packed = 0u;
+    if (s < nb)
+      for (int g = 0; g < G; ++g) packed |= ((bt[s] >> (4 * (G - 1 - g))) & 15u) << (4 * g);
+    codes[s] = packed;
+  }
+}
+
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s) {
+  const long long total = (long long)D.B * D.K * 2;
+  synthesis_kernel<<<(unsigned)((total + kSynThreads - 1) / kSynThreads), kSynThreads, 0, s>>>(D, H, V, n_act);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Q2 fused attention, fp32 SIMT variant (Alg. 4 l.8-15; Eq. 4).  One warp per query row (query token x query
+// head), DH/32 dims per lane, split over the context (flash-decoding style) with a combine kernel.
+// Context element e < n_near is ring row e of the bank; e >= n_near is pseudo-token (k, s) of prototype
+// k = (e - n_near) / S:  k~ = c_k + concat_g CK_g[zK(k,s,g)],  v~ = p_k + concat_g CV_g[zV(k,s,g)],  bias log n_k.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kAttWarps = 4;
+
+struct Softmax1 {   // running (max, sum) of one row; acc lives in the caller
+  float m, l;
+};
+
+template <int VEC>
+__device__ __forceinline__ void online_update(Softmax1& st, float (&acc)[VEC], float logit, const float (&v)[VEC]) {
+  if (logit > st.m) {
+    const float sc = __expf(st.m - logit);   // exp(-inf) = 0 on the first element
+    st.l = fmaf(st.l, sc, 1.f);
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) acc[i] = fmaf(acc[i], sc, v[i]);
+    st.m = logit;
+  } else {
+    const float w = __expf(logit - st.m);
+    st.l += w;
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) acc[i] = fmaf(w, v[i], acc[i]);
+  }
+}
+
+template <typename T, int DH>
+__global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
+  constexpr int VEC = DH / 32;
+  extern __shared__ __align__(16) float cb_s[];
+  const int gstride = D.C * D.sub + kCbPad;
+  float* cbk_s = cb_s;
+  float* cbv_s = cb_s + D.G * gstride;
+
+  const int R = A.n_q * D.group;
+  const int rgroups = (R + kAttWarps - 1) / kAttWarps;
+  const int bsel = blockIdx.x / rgroups, rg = blockIdx.x % rgroups;
+  const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
+  const int b = (st * D.L + A.layer_begin + ll) * D.Hkv + hd;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool has_cb = V.cbk != nullptr;
+  if (has_cb) {
+    const int per_g = D.C * D.sub;
+    for (int e = tid; e < D.G * per_g; e += kAttWarps * 32) {
+      const int g = e / per_g, r = e % per_g;
+      cbk_s[g * gstride + r] = V.cbk[(size_t)b * D.G * per_g + e];
+      cbv_s[g * gstride + r] = V.cbv[(size_t)b * D.G * per_g + e];
+    }
+  }
+  __syncthreads();
+  const int row = rg * kAttWarps + warp;
+  if (row >= R) return;
+  const int qi = row / D.group, h = hd * D.group + row % D.group;
+  const size_t qoff = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + h) * DH;
+  float q[VEC];
+  load_vec<T, VEC>((const T*)A.Q + qoff + lane * VEC, q);
+  const float scale = 1.0f / sqrtf((float)DH);
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) q[v] *= scale;
+
+  const int near_cnt = (H.flags & PROTOKV_FAR_ONLY) ? 0 : A.n_near;
+  const int ps_cnt = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : A.n_act * D.S;
+  const int Lc = near_cnt + ps_cnt;
+  const int chunk = (Lc + A.nsplit - 1) / A.nsplit;
+  const int lo = blockIdx.y * chunk, hi = min(Lc, lo + chunk);
+  Softmax1 sm{-INFINITY, 0.f};
+  float acc[VEC];
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
+
+  // near-window tokens
+  const T* rK = (const T*)V.ringK + (size_t)b * D.Wf * D.T * DH;
+  const T* rV = (const T*)V.ringV + (size_t)b * D.Wf * D.T * DH;
+  int e = lo;
+  const int near_hi = min(hi, near_cnt);
+  for (; e + 4 <= near_hi; e += 4) {
+    float kk[4][VEC], vv[4][VEC], dot[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      load_vec<T, VEC>(rK + (size_t)(e + u) * DH + lane * VEC, kk[u]);
+      load_vec<T, VEC>(rV + (size_t)(e + u) * DH + lane * VEC, vv[u]);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      dot[u] = 0.f;
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) dot[u] = fmaf(q[v], kk[u][v], dot[u]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) dot[u] += __shfl_xor_sync(0xffffffffu, dot[u], o);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) online_update<VEC>(sm, acc, dot[u], vv[u]);
+  }
+  for (; e < near_hi; ++e) {
+    float kk[VEC], vv[VEC];
+    load_vec<T, VEC>(rK + (size_t)e * DH + lane * VEC, kk);
+    load_vec<T, VEC>(rV + (size_t)e * DH + lane * VEC, vv);
+    float dot = 0.f;
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], kk[v], dot);
+    dot = warp_sum(dot);
+    online_update<VEC>(sm, acc, dot, vv);
+  }
+  // pseudo-tokens
+  if (hi > near_cnt) {
+    const int p_lo = max(lo, near_cnt) - near_cnt, p_hi = hi - near_cnt;
+    const int LPS = 32 / D.G, g = lane / LPS, li = lane % LPS;
+    const bool use_bias = !(H.flags & PROTOKV_NO_MASS_BIAS);
+    for (int k = p_lo / D.S; k * D.S < p_hi; ++k) {
+      const size_t pk = (size_t)b * D.K + k;
+      const int kind = V.kind[pk];
+      if (kind == 2) continue;
+      const int s_lo = max(p_lo - k * D.S, 0), s_hi = min(p_hi - k * D.S, D.S);
+      float c[VEC], p[VEC];
+      load_vec<float, VEC>(V.c + pk * DH + lane * VEC, c);
+      load_vec<float, VEC>(V.p + pk * DH + lane * VEC, p);
+      const float bias = use_bias ? V.logn[pk] : 0.f;
+      if (kind == 1) {             // zero residuals: S identical pseudo-tokens (Alg. 4 l.3-4)
+        float dot = 0.f;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], c[v], dot);
+        dot = warp_sum(dot) + bias;
+        for (int s = s_lo; s < s_hi; ++s) online_update<VEC>(sm, acc, dot, p);
+        continue;
+      }
+      for (int s = s_lo; s < s_hi; ++s) {
+        const uint32_t zk = (V.codesK[pk * D.S + s] >> (4 * g)) & 15u;
+        const uint32_t zv = (V.codesV[pk * D.S + s] >> (4 * g)) & 15u;
+        float rk[VEC], rv[VEC];
+        load_vec<float, VEC>(cbk_s + g * gstride + zk * D.sub + li * VEC, rk);
+        load_vec<float, VEC>(cbv_s + g * gstride + zv * D.sub + li * VEC, rv);
+        float dot = 0.f;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { dot = fmaf(q[v], c[v] + rk[v], dot); rv[v] += p[v]; }
+        dot = warp_sum(dot) + bias;
+        online_update<VEC>(sm, acc, dot, rv);
+      }
+    }
+  }
+  float* part = V.part + (((size_t)bsel * R + row) * A.nsplit + blockIdx.y) * (DH + 2);
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) part[lane * VEC + v] = acc[v];
+  if (lane == 0) { part[DH] = sm.m; part[DH + 1] = sm.l; }
+}
+
+template <typename T, int DH>
+__global__ void __launch_bounds__(128) attention_combine_kernel(Dims D, Dev V, AttnArgs A, int rows_total) {
+  constexpr int VEC = DH / 32;
+  const int gr = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (gr >= rows_total) return;
+  const int R = A.n_q * D.group;
+  const int bsel = gr / R, row = gr % R;
+  const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
+  const int qi = row / D.group, h = hd * D.group + row % D.group;
+  const float* part = V.part + (size_t)gr * A.nsplit * (DH + 2);
+  float M = -INFINITY;
+  for (int sp = 0; sp < A.nsplit; ++sp) M = fmaxf(M, part[sp * (DH + 2) + DH]);
+  float l = 0.f, acc[VEC];
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
+  if (M > -INFINITY) {
+    for (int sp = 0; sp < A.nsplit; ++sp) {
+      const float* ps = part + sp * (DH + 2);
+      const float w = __expf(ps[DH] - M);   // exp(-inf) = 0 for empty splits
+      l = fmaf(ps[DH + 1], w, l);
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) acc[v] = fmaf(ps[lane * VEC + v], w, acc[v]);
+    }
+  }
+  const float inv = l > 0.f ? 1.f / l : 0.f;
+  const size_t ooff = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + h);
+  T* out = (T*)A.out + ooff * DH + lane * VEC;
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) out[v] = from_f32<T>(acc[v] * inv);
+  if (A.lse && lane == 0) A.lse[ooff] = l > 0.f ? M + logf(l) : -INFINITY;
+}
+
+int attention_simt_splits(const Dims& D, int sm_count) {
+  const int R = D.Nq * D.group;
+  const long long ctas = (long long)D.B * ((R + kAttWarps - 1) / kAttWarps);
+  long long ns = (4LL * sm_count + ctas - 1) / ctas;
+  if (ns < 1) ns = 1;
+  if (ns > 64) ns = 64;
+  return (int)ns;
+}
+
+template <typename T, int DH>
+static int attention_simt_launch(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s) {
+  const int R = A.n_q * D.group;
+  const int nb = D.NS * A.layer_count * D.Hkv;
+  const int rgroups = (R + kAttWarps - 1) / kAttWarps;
+  const size_t sm = V.cbk ? 2 * (size_t)D.G * (D.C * D.sub + kCbPad) * 4 : 0;
+  dim3 grid(nb * rgroups, A.nsplit);
+  attention_simt_kernel<T, DH><<<grid, kAttWarps * 32, sm, s>>>(D, H, V, A);
+  const int rows_total = nb * R;
+  attention_combine_kernel<T, DH><<<(rows_total + 3) / 4, 128, 0, s>>>(D, V, A, rows_total);
+  return 2;
+}
+
+int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s) {
+  if (D.bf16) return D.d == 128 ? attention_simt_launch<__nv_bfloat16, 128>(D, H, V, A, s)
+                                : attention_simt_launch<__nv_bfloat16, 64>(D, H, V, A, s);
+  return D.d == 128 ? attention_simt_launch<float, 128>(D, H, V, A, s)
+                    : attention_simt_launch<float, 64>(D, H, V, A, s);
+}
+
+}  // namespace pkv

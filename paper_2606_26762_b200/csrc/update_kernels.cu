@@ -1,0 +1,458 @@
+// ProtoKV per-frame far-memory update (Alg. 1): ring append, slot fill, Eq. 1 scoring (fp32
+// SIMT variant), segmenting and the segmented prototype update with PQ residual histograms.
+// See DESIGN.md "Kernels".  All launchers are asynchronous on the caller's stream.
+#include "common.cuh"
+
+namespace pkv {
+
+// Token-independent part of Eq. 1 for one prototype.  Sigma + eps I = R R^T (Cholesky),
+// d_Mah^2 = |R^-1 delta|^2 = (dx/r11)^2 + ((dy - r21 dx/r11)/r22)^2.  Evaluated in fp64 from the fp32 state.
+__device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, float sxx, float sxy, float syy, int tau,
+                                             const Hyper& H) {
+  ScoreRec r;
+  r.invc = cc > 0.f ? (float)(1.0 / sqrt((double)cc)) : 0.f;
+  r.mux = mux; r.muy = muy;
+  double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
+  double r11 = sqrt(a);
+  double r21 = b / r11;
+  double t = e - r21 * r21;
+  double r22 = sqrt(t > 0.0 ? t : 0.0);
+  // lambda_sp * d_Mah = sqrt(q) with factors scaled by lambda_sp; for MAH_SQUARED scale by sqrt(lambda_sp).
+  double lam = (H.flags & PROTOKV_MAH_SQUARED) ? sqrt((double)H.lambda_sp) : (double)H.lambda_sp;
+  r.u = (float)(lam / r11);
+  r.v = (float)(lam / r22);
+  r.w = (float)(lam * r21 / (r11 * r22));
+  r.tau = tau;
+  r.pad = 0;
+  return r;
+}
+
+__device__ __forceinline__ void split_bf16(float x, __nv_bfloat16& hi, __nv_bfloat16& lo) {
+  hi = __float2bfloat16_rn(x);
+  lo = __float2bfloat16_rn(x - __bfloat162float(hi));
+}
+
+template <int VEC>
+__device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const float (&c)[VEC]) {
+  if (!V.c_hi) return;
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) {
+    __nv_bfloat16 hi, lo;
+    split_bf16(c[v], hi, lo);
+    V.c_hi[off + v] = hi; V.c_lo[off + v] = lo;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// U1 ring append (Alg. 1 l.1): frame f goes to slot f % Wf, transposed from the model-native
+// [stream][layer][T][Hkv][d] to the bank-major ring [bank][Wf][T][d].  16-byte vectors, one per thread.
+// grid.y = 0: K, 1: V.  The first threads of grid.y == 0 also copy grid_pos.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slot, const uint4* __restrict__ Kin,
+                                                          const uint4* __restrict__ Vin,
+                                                          const float* __restrict__ grid_pos, int vpr) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t total = (size_t)D.B * D.T * vpr;
+  if (blockIdx.y == 0 && idx < (size_t)D.NS * D.T * 2) {
+    const int st = (int)(idx / (D.T * 2)), e = (int)(idx % (D.T * 2));
+    V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[idx];
+  }
+  if (idx >= total) return;
+  const int v = (int)(idx % vpr);
+  const int j = (int)((idx / vpr) % D.T);
+  const int b = (int)(idx / ((size_t)vpr * D.T));
+  const int hd = b % D.Hkv, sl = b / D.Hkv;  // sl = stream * L + layer
+  const size_t src = (((size_t)sl * D.T + j) * D.Hkv + hd) * vpr + v;
+  const size_t dst = (((size_t)b * D.Wf + slot) * D.T + j) * vpr + v;
+  const uint4* in = blockIdx.y ? Vin : Kin;
+  uint4* out = (uint4*)(blockIdx.y ? V.ringV : V.ringK);
+  out[dst] = in[src];
+}
+
+int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const void* Kin, const void* Vin,
+                       const float* grid_pos, cudaStream_t s) {
+  const int vpr = D.d * (D.bf16 ? 2 : 4) / 16;
+  const size_t total = (size_t)D.B * D.T * vpr;
+  dim3 grid((unsigned)((total + 255) / 256), 2);
+  ring_append_kernel<<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// U2 slot fill (Alg. 1 l.3-4; L83): evicted token j < n_fill opens slot n_act0 + j.
+// One warp per (token, bank).
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
+  const int j = blockIdx.x, b = blockIdx.y, lane = threadIdx.x;
+  const int k = F.n_act0 + j;
+  const int st = b / (D.L * D.Hkv);
+  const T* Ke = (const T*)V.ringK + (((size_t)b * D.Wf + F.slot) * D.T + j) * D.d;
+  const T* Ve = (const T*)V.ringV + (((size_t)b * D.Wf + F.slot) * D.T + j) * D.d;
+  const size_t pk = (size_t)b * D.K + k;
+  float cc = 0.f;
+  for (int i = lane; i < D.d; i += 32) {
+    float kf = to_f32(Ke[i]), vf = to_f32(Ve[i]);
+    V.c[pk * D.d + i] = kf;
+    V.p[pk * D.d + i] = vf;
+    if (V.c_hi) {
+      __nv_bfloat16 hi, lo;
+      split_bf16(kf, hi, lo);
+      V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
+    }
+    cc += kf * kf;
+  }
+  cc = warp_sum(cc);
+  const int ghc = 2 * D.G * D.C;
+  for (int i = lane; i < ghc; i += 32) V.hist[pk * ghc + i] = 0u;
+  if (lane == 0) {
+    const float* se = V.ringS + (((size_t)st * D.Wf + F.slot) * D.T + j) * 2;
+    V.n[pk] = 1;
+    V.mu[pk * 2] = se[0]; V.mu[pk * 2 + 1] = se[1];
+    V.sigma[pk * 3] = 1.f; V.sigma[pk * 3 + 1] = 0.f; V.sigma[pk * 3 + 2] = 1.f;
+    V.tau[pk] = F.t;
+    V.pos[pk] = (long long)F.ev_frame * D.T + j;
+    V.nres[pk] = 0u;
+    V.rec[pk] = make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H);
+    V.logn[pk] = 0.f;
+    V.assign[(size_t)b * D.T + j] = k;
+    V.best[(size_t)b * D.T + j] = 0.f;
+  }
+  for (int g = lane; g < D.G; g += 32) {
+    V.tcodeK[((size_t)b * D.T + j) * D.G + g] = 255;
+    V.tcodeV[((size_t)b * D.T + j) * D.G + g] = 255;
+  }
+}
+
+int launch_fill(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s) {
+  if (F.n_fill <= 0) return 0;
+  dim3 grid(F.n_fill, D.B);
+  if (D.bf16) fill_kernel<__nv_bfloat16><<<grid, 32, 0, s>>>(D, H, V, F);
+  else fill_kernel<float><<<grid, 32, 0, s>>>(D, H, V, F);
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// U3 assignment, fp32 SIMT variant (Eq. 1; Alg. 1 l.6).  Used for fp32 inputs and as the
+// cross-check of the tcgen05 kernel.  CTA = (bank, tile of 32 tokens); 256 threads = 32 tokens x 8 prototype
+// lanes; prototypes are staged through shared memory 64 at a time.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kScoreTok = 32, kScoreKc = 64, kScoreThreads = 256;
+
+template <typename T, int DH>
+__global__ void __launch_bounds__(kScoreThreads) score_simt_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
+  extern __shared__ float smem[];
+  float* tokT = smem;                          // [DH][32]   token tile, transposed
+  float* cs = tokT + DH * kScoreTok;           // [64][DH]   centre chunk
+  ScoreRec* recs = (ScoreRec*)(cs + kScoreKc * DH);  // [64]
+  float* bestv = (float*)(recs + kScoreKc);    // [8][32]
+  int* besti = (int*)(bestv + 8 * kScoreTok);  // [8][32]
+
+  const int b = blockIdx.y, j0 = F.n_fill + blockIdx.x * kScoreTok;
+  const int tid = threadIdx.x, tl = tid & 31, kg = tid >> 5;
+  const int st = b / (D.L * D.Hkv);
+  const T* Ke = (const T*)V.ringK + ((size_t)b * D.Wf + F.slot) * D.T * DH;
+  // token tile -> smem (transposed), zero beyond T
+  for (int e = tid; e < kScoreTok * DH; e += kScoreThreads) {
+    int tt = e / DH, i = e % DH;
+    int j = j0 + tt;
+    tokT[i * kScoreTok + tt] = j < D.T ? to_f32(Ke[(size_t)j * DH + i]) : 0.f;
+  }
+  __syncthreads();
+  const int j = j0 + tl;
+  float kk = 0.f;
+  for (int i = 0; i < DH; ++i) { float x = tokT[i * kScoreTok + tl]; kk = fmaf(x, x, kk); }
+  const float invk = kk > 0.f ? rsqrtf(kk) : 0.f;
+  const float inv_cap = 1.f / H.cos_eps;       // cos = dot / max(|K||c|, cos_eps)  (reading 6)
+  float sx = 0.f, sy = 0.f;
+  if (j < D.T) {
+    const float* se = V.ringS + (((size_t)st * D.Wf + F.slot) * D.T + j) * 2;
+    sx = se[0]; sy = se[1];
+  }
+  float best = INFINITY;
+  int bidx = 0x7fffffff;
+  const bool squared = H.flags & PROTOKV_MAH_SQUARED;
+  for (int k0 = 0; k0 < F.n_act; k0 += kScoreKc) {
+    __syncthreads();
+    const int nk = min(kScoreKc, F.n_act - k0);
+    const float4* src = (const float4*)(V.c + ((size_t)b * D.K + k0) * DH);
+    for (int e = tid; e < nk * DH / 4; e += kScoreThreads) ((float4*)cs)[e] = src[e];
+    if (tid < nk) recs[tid] = V.rec[(size_t)b * D.K + k0 + tid];
+    __syncthreads();
+    float acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = 0.f;
+    for (int i = 0; i < DH; i += 4) {
+      float x0 = tokT[(i + 0) * kScoreTok + tl], x1 = tokT[(i + 1) * kScoreTok + tl];
+      float x2 = tokT[(i + 2) * kScoreTok + tl], x3 = tokT[(i + 3) * kScoreTok + tl];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        float4 cv = *(const float4*)(cs + (kg * 8 + q) * DH + i);
+        acc[q] = fmaf(x0, cv.x, acc[q]); acc[q] = fmaf(x1, cv.y, acc[q]);
+        acc[q] = fmaf(x2, cv.z, acc[q]); acc[q] = fmaf(x3, cv.w, acc[q]);
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const int kl = kg * 8 + q;
+      if (kl < nk) {
+        const ScoreRec r = recs[kl];
+        float dx = sx - r.mux, dy = sy - r.muy;
+        float y1 = dx * r.u, y2 = fmaf(dy, r.v, -(dx * r.w));
+        float qq = fmaf(y1, y1, y2 * y2);
+        float sp = squared ? qq : sqrtf(qq);
+        float idle = (F.t - r.tau > H.t_idle) ? H.lambda_idle : 0.f;
+        float inv = fminf(r.invc * invk, inv_cap);
+        float sc = fmaf(-acc[q], inv, sp + idle);
+        if (sc < best) { best = sc; bidx = k0 + kl; }   // increasing k within a thread: lowest index on ties
+      }
+    }
+  }
+  bestv[kg * kScoreTok + tl] = best;
+  besti[kg * kScoreTok + tl] = bidx;
+  __syncthreads();
+  if (kg == 0 && j < D.T) {
+#pragma unroll
+    for (int q = 1; q < 8; ++q) {
+      float v = bestv[q * kScoreTok + tl];
+      int ix = besti[q * kScoreTok + tl];
+      if (v < best || (v == best && ix < bidx)) { best = v; bidx = ix; }
+    }
+    V.assign[(size_t)b * D.T + j] = bidx;
+    V.best[(size_t)b * D.T + j] = best;
+  }
+}
+
+static size_t score_simt_smem(int dh) {
+  return (size_t)(dh * kScoreTok + kScoreKc * dh) * 4 + kScoreKc * sizeof(ScoreRec) + 8 * kScoreTok * 8;
+}
+
+template <typename T, int DH>
+static void score_simt_launch(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, dim3 grid,
+                              cudaStream_t s) {
+  const size_t sm = score_simt_smem(DH);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(score_simt_kernel<T, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    attr_done = true;
+  }
+  score_simt_kernel<T, DH><<<grid, kScoreThreads, sm, s>>>(D, H, V, F);
+}
+
+int launch_score_simt(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s) {
+  const int ntok = D.T - F.n_fill;
+  if (ntok <= 0) return 0;
+  dim3 grid((ntok + kScoreTok - 1) / kScoreTok, D.B);
+  if (D.bf16) {
+    if (D.d == 128) score_simt_launch<__nv_bfloat16, 128>(D, H, V, F, grid, s);
+    else score_simt_launch<__nv_bfloat16, 64>(D, H, V, F, grid, s);
+  } else {
+    if (D.d == 128) score_simt_launch<float, 128>(D, H, V, F, grid, s);
+    else score_simt_launch<float, 64>(D, H, V, F, grid, s);
+  }
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// U4 segmenting + U5 prototype update + U6 residual histograms (Alg. 1 l.8-13).
+//
+// CTA = (chunk, bank).  Every CTA of a bank sorts the bank's (k*, j) keys in shared memory (bitonic; stable in
+// eviction order because j is the low part of the key), so that segments = runs of equal k*.  Warps then take
+// segment heads round-robin over all CTAs of the bank; one warp owns one prototype: it holds c_k and p_k in
+// registers (DH/32 dims per lane) and replays Alg. 1 l.8-13 over its tokens in eviction order.
+//
+// Arithmetic: the EMA / mean / covariance recurrences are evaluated like the definition reads, in fp64 from the
+// fp32 state with one rounding back to fp32 per step (a handful of DFMA-class ops per token and dimension);
+// the PQ distances |r_g - C_g[z]|^2 are fp32, reduced over the 32/G lanes that share a subspace.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kUpdThreads = 256, kUpdWarps = kUpdThreads / 32;
+
+__device__ __forceinline__ float ema_step(double one_minus, double rate, float state, float x) {
+  // (1 - a) * state + a * x with every product and the sum rounded separately (no contraction), then to fp32
+  return (float)__dadd_rn(__dmul_rn(one_minus, (double)state), __dmul_rn(rate, (double)x));
+}
+
+template <typename T, int DH>
+__global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, Dev V, FrameArgs F, int P) {
+  constexpr int VEC = DH / 32;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint32_t* keys = (uint32_t*)smem_raw;                      // [P]
+  float* cbk_s = (float*)(keys + P);                         // [G][C*sub + pad]
+  const int gstride = D.C * D.sub + kCbPad;
+  float* cbv_s = cbk_s + D.G * gstride;
+
+  const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int ntok = D.T - F.n_fill;
+  const bool has_cb = V.cbk != nullptr;
+  for (int i = tid; i < P; i += kUpdThreads) {
+    const int j = F.n_fill + i;
+    keys[i] = i < ntok ? (((uint32_t)V.assign[(size_t)b * D.T + j] << 12) | (uint32_t)j) : 0xffffffffu;
+  }
+  if (has_cb) {
+    const int per_g = D.C * D.sub;
+    for (int e = tid; e < D.G * per_g; e += kUpdThreads) {
+      const int g = e / per_g, r = e % per_g;
+      cbk_s[g * gstride + r] = V.cbk[(size_t)b * D.G * per_g + e];
+      cbv_s[g * gstride + r] = V.cbv[(size_t)b * D.G * per_g + e];
+    }
+  }
+  __syncthreads();
+  for (int size = 2; size <= P; size <<= 1) {
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = tid; i < P / 2; i += kUpdThreads) {
+        const int lo = 2 * i - (i & (stride - 1)), hi = lo + stride;
+        const bool up = (lo & size) == 0;
+        const uint32_t a = keys[lo], c = keys[hi];
+        if ((a > c) == up) { keys[lo] = c; keys[hi] = a; }
+      }
+      __syncthreads();
+    }
+  }
+
+  const int st = b / (D.L * D.Hkv);
+  const T* ringK = (const T*)V.ringK + ((size_t)b * D.Wf + F.slot) * D.T * DH;
+  const T* ringV = (const T*)V.ringV + ((size_t)b * D.Wf + F.slot) * D.T * DH;
+  const float* ringS = V.ringS + ((size_t)st * D.Wf + F.slot) * D.T * 2;
+  const double al = (double)H.alpha, be = (double)H.beta, et = (double)H.eta;
+  const double oma = 1.0 - al, omb = 1.0 - be, ome = 1.0 - et;
+  const int LPS = 32 / D.G;                       // lanes per PQ subspace
+  const int g = lane / LPS, li = lane % LPS;
+
+  for (int i = blockIdx.x * kUpdWarps + warp; i < ntok; i += gridDim.x * kUpdWarps) {
+    const uint32_t key = keys[i];
+    const int k = (int)(key >> 12);
+    if (i > 0 && (int)(keys[i - 1] >> 12) == k) continue;   // not a segment head
+    const size_t pk = (size_t)b * D.K + k;
+    float c[VEC], p[VEC];
+    load_vec<float, VEC>(V.c + pk * DH + lane * VEC, c);
+    load_vec<float, VEC>(V.p + pk * DH + lane * VEC, p);
+    float mu0 = V.mu[pk * 2], mu1 = V.mu[pk * 2 + 1];
+    float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
+    int n = V.n[pk];
+    int m = 0, jlast = 0;
+    for (int ii = i; ii < ntok && (int)(keys[ii] >> 12) == k; ++ii) {
+      const int j = (int)(keys[ii] & 0xfffu);
+      float ke[VEC], ve[VEC];
+      load_vec<T, VEC>(ringK + (size_t)j * DH + lane * VEC, ke);
+      load_vec<T, VEC>(ringV + (size_t)j * DH + lane * VEC, ve);
+      const float s0 = ringS[j * 2], s1 = ringS[j * 2 + 1];
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) {
+        c[v] = ema_step(oma, al, c[v], ke[v]);                       // l.8
+        p[v] = ema_step(omb, be, p[v], ve[v]);                       // l.9
+      }
+      n += 1; ++m; jlast = j;                                        // l.10
+      mu0 = ema_step(ome, et, mu0, s0);                              // l.11
+      mu1 = ema_step(ome, et, mu1, s1);
+      const double dx = (double)s0 - (double)mu0, dy = (double)s1 - (double)mu1;   // new mu
+      const double edx = __dmul_rn(et, dx), edy = __dmul_rn(et, dy);
+      sxx = (float)__dadd_rn(__dmul_rn(ome, (double)sxx), __dmul_rn(edx, dx));     // l.12
+      sxy = (float)__dadd_rn(__dmul_rn(ome, (double)sxy), __dmul_rn(edx, dy));
+      syy = (float)__dadd_rn(__dmul_rn(ome, (double)syy), __dmul_rn(edy, dy));
+      if (has_cb) {                                                  // l.13, residual of the updated centres
+#pragma unroll
+        for (int kv = 0; kv < 2; ++kv) {
+          const float* cb = (kv ? cbv_s : cbk_s) + g * gstride + li * VEC;
+          float r[VEC];
+#pragma unroll
+          for (int v = 0; v < VEC; ++v) r[v] = kv ? ve[v] - p[v] : ke[v] - c[v];
+          float bestd = INFINITY;
+          int bz = 0;
+          for (int z = 0; z < D.C; ++z) {
+            float cw[VEC];
+            load_vec<float, VEC>(cb + z * D.sub, cw);
+            float dist = 0.f;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) { const float t = r[v] - cw[v]; dist = fmaf(t, t, dist); }
+            for (int o = LPS >> 1; o > 0; o >>= 1) dist += __shfl_xor_sync(0xffffffffu, dist, o);
+            if (dist < bestd) { bestd = dist; bz = z; }              // lowest z on ties
+          }
+          if (li == 0) {
+            atomicAdd(V.hist + ((pk * 2 + kv) * D.G + g) * D.C + bz, 1u);
+            (kv ? V.tcodeV : V.tcodeK)[((size_t)b * D.T + j) * D.G + g] = (uint8_t)bz;
+          }
+        }
+      }
+    }
+    // write back the prototype and everything derived from it
+    if (VEC == 4) {
+      *(float4*)(V.c + pk * DH + lane * 4) = make_float4(c[0], c[1], c[2], c[VEC - 1]);
+      *(float4*)(V.p + pk * DH + lane * 4) = make_float4(p[0], p[1], p[2], p[VEC - 1]);
+    } else {
+      *(float2*)(V.c + pk * DH + lane * 2) = make_float2(c[0], c[1]);
+      *(float2*)(V.p + pk * DH + lane * 2) = make_float2(p[0], p[1]);
+    }
+    store_shadows<VEC>(V, pk * DH + lane * VEC, c);
+    float cc = 0.f;
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) cc = fmaf(c[v], c[v], cc);
+    cc = warp_sum(cc);
+    if (lane == 0) {
+      V.n[pk] = n;
+      V.tau[pk] = F.t;
+      V.pos[pk] = (long long)F.ev_frame * D.T + jlast;
+      V.mu[pk * 2] = mu0; V.mu[pk * 2 + 1] = mu1;
+      V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
+      if (has_cb) V.nres[pk] += (uint32_t)m;
+      V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
+      V.logn[pk] = (float)log((double)n);
+    }
+  }
+}
+
+static int next_pow2(int x) { int p = 2; while (p < x) p <<= 1; return p; }
+
+int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s) {
+  const int ntok = D.T - F.n_fill;
+  if (ntok <= 0) return 0;
+  const int P = next_pow2(ntok);
+  int nchunk = (2 * sm_count + D.B - 1) / D.B;
+  nchunk = nchunk < 1 ? 1 : nchunk;
+  const int max_chunk = (ntok + kUpdWarps - 1) / kUpdWarps;
+  if (nchunk > max_chunk) nchunk = max_chunk;
+  if (nchunk > 32) nchunk = 32;
+  const size_t sm = (size_t)P * 4 + 2 * (size_t)D.G * (D.C * D.sub + kCbPad) * 4;
+  dim3 grid(nchunk, D.B);
+  if (D.bf16) {
+    if (D.d == 128) update_kernel<__nv_bfloat16, 128><<<grid, kUpdThreads, sm, s>>>(D, H, V, F, P);
+    else update_kernel<__nv_bfloat16, 64><<<grid, kUpdThreads, sm, s>>>(D, H, V, F, P);
+  } else {
+    if (D.d == 128) update_kernel<float, 128><<<grid, kUpdThreads, sm, s>>>(D, H, V, F, P);
+    else update_kernel<float, 64><<<grid, kUpdThreads, sm, s>>>(D, H, V, F, P);
+  }
+  return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Derived per-prototype data (scoring record, log-mass, bf16 shadows) recomputed from the primary state of one
+// bank -- used after protokv_import_state.  One warp per prototype.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
+  const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (k >= D.K) return;
+  const size_t pk = (size_t)b * D.K + k;
+  float cc = 0.f;
+  for (int i = lane; i < D.d; i += 32) {
+    const float x = V.c[pk * D.d + i];
+    cc = fmaf(x, x, cc);
+    if (V.c_hi) {
+      __nv_bfloat16 hi, lo;
+      split_bf16(x, hi, lo);
+      V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
+    }
+  }
+  cc = warp_sum(cc);
+  if (lane == 0) {
+    V.rec[pk] = make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
+                         V.sigma[pk * 3 + 2], V.tau[pk], H);
+    const int n = V.n[pk];
+    V.logn[pk] = n >= 1 ? (float)log((double)n) : 0.f;
+  }
+}
+
+int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, cudaStream_t s) {
+  refresh_derived_kernel<<<(D.K + 7) / 8, 256, 0, s>>>(D, H, V, bank);
+  return 1;
+}
+
+}  // namespace pkv

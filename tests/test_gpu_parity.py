@@ -1,0 +1,232 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Protocol: teacher-forced streams -- after every frame the GPU's decisions (assignment,
+PQ codes) are checked against the oracle's own, under north_star's gap rule, and the oracle then follows the GPU's
+decisions so that one accepted near-tie cannot cascade; statistics are compared field by field; synthesis codes
+and attention outputs are compared at the query.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+from gpu_helpers import (make_gpu, make_oracles, run_stream, compare_ring, compare_codes, compare_attention,
+                         compare_state, new_stats)
+from oracle import FLAG_NEAR_ONLY, FLAG_FAR_ONLY, FLAG_NO_MASS_BIAS, FLAG_MAH_SQUARED
+from paper_2606_26762_b200 import ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT
+
+pytestmark = pytest.mark.gpu
+
+
+def _query_and_check(spec, gpu, oracles, query_index=0, **kw):
+    flips = compare_codes(gpu, oracles, spec.G)
+    Q = gen.queries(spec, query_index)
+    worst = compare_attention(spec, gpu, oracles, Q, run_synthesis=False, **kw)
+    return flips, worst
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 1 (BASELINE.json configs[0]): the whole 64-frame stream, every frame, every field, then the query
+# ---------------------------------------------------------------------------------------------------------
+def test_c1_full_stream():
+    spec = gen.spec_for("c1")
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [0])
+    stats = run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=1)
+    assert stats["scored"] == (spec.n_frames - spec.near_frames) * spec.T - spec.k_max
+    compare_ring(gpu, oracles)
+    st = gpu.export_state(0)
+    assert int(st["n"].sum()) == (spec.n_frames - spec.near_frames) * spec.T      # mass conservation
+    _query_and_check(spec, gpu, oracles)
+    # end to end without forced codes
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=True)
+    assert gpu.frames_seen == spec.n_frames and gpu.kernel_launches > 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 2 shape (bf16, GQA 28/4, d=128, T=196 -> ragged tiles), all 4 banks, first frames incl. the fill phase
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_c2_shape_short_stream(force_simt):
+    spec = gen.spec_for("c2", n_frames=30)
+    gpu = make_gpu(spec, flags=FORCE_SIMT if force_simt else 0)
+    oracles = make_oracles(spec, range(spec.n_banks))
+    stats = run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=7)
+    assert stats["scored"] > 0
+    compare_ring(gpu, oracles)
+    _query_and_check(spec, gpu, oracles)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 1), run_synthesis=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 3 shape: several layers in one state; attention of a layer subset and of fewer query tokens
+# ---------------------------------------------------------------------------------------------------------
+def test_c3_shape_layers_subset():
+    spec = gen.spec_for("c3", n_layers=3, n_frames=26, k_max=512)
+    gpu = make_gpu(spec)
+    banks = [0, 5, 11]     # (layer 0, head 0), (layer 1, head 1), (layer 2, head 3)
+    oracles = make_oracles(spec, banks)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=13)
+    compare_codes(gpu, oracles, spec.G)
+    Q = gen.queries(spec, 0)
+    compare_attention(spec, gpu, oracles, Q, run_synthesis=False)
+    # layers [1, 3), 5 query tokens
+    Qs = Q[:, 1:3, :5].contiguous()
+    compare_attention(spec, gpu, oracles, Qs, layer_begin=1, run_synthesis=False)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 5 shape: 2 streams x 8 KV heads, T = 576, K_max = 2048, N_q = 64 (256 rows per bank)
+# ---------------------------------------------------------------------------------------------------------
+def test_c5_shape_multi_stream():
+    spec = gen.spec_for("c5", n_streams=2, n_frames=14)
+    gpu = make_gpu(spec)
+    banks = [0, 7, 9]
+    oracles = make_oracles(spec, banks)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=7)
+    compare_ring(gpu, oracles)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False, rows_sample=range(0, 256, 5))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 4 cells (small ends of the sweep): K_max 256 with W_f 4, and a bank larger than the stream ever fills
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k_max,near", [(256, 4), (4096, 4)])
+def test_c4_cells(k_max, near):
+    spec = gen.spec_for(f"c4_k{k_max}_w{near}", n_frames=14)
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [0, 3])
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=7)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False, rows_sample=range(0, 224, 3))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# degenerate cases of the method
+# ---------------------------------------------------------------------------------------------------------
+def test_empty_and_near_only_states():
+    spec = gen.spec_for("c1")
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [0])
+    Q = gen.queries(spec, 0)
+    # no frame yet: empty context -> zeros, lse = -inf
+    out, lse = gpu.query_attention_ex(Q.to(gpu.device), return_lse=True)
+    assert (out == 0).all() and torch.isinf(lse).all()
+    # fewer frames than the window holds: nothing evicted, attention = plain attention over the partial window
+    run_stream(spec, gpu, oracles, 3, check_state_every=1)
+    assert gpu.last_frame_trace()["evicted_frame"] == -1
+    compare_attention(spec, gpu, oracles, Q, run_synthesis=True)
+    # exactly the first eviction
+    run_stream(spec, gpu, oracles, 2, check_state_every=1, first_frame=3)
+    compare_attention(spec, gpu, oracles, Q, run_synthesis=True)
+
+
+@pytest.mark.parametrize("gflag,oflag", [(NEAR_ONLY, FLAG_NEAR_ONLY), (FAR_ONLY, FLAG_FAR_ONLY),
+                                         (NO_MASS_BIAS, FLAG_NO_MASS_BIAS), (MAH_SQUARED, FLAG_MAH_SQUARED)])
+def test_ablation_flags(gflag, oflag):
+    spec = gen.spec_for("c1", n_frames=24)
+    gpu = make_gpu(spec, flags=gflag)
+    oracles = make_oracles(spec, [0], flags=oflag)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=4)
+    if gflag != NEAR_ONLY:
+        compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=True)
+
+
+def test_no_codebooks_zero_residuals():
+    spec = gen.spec_for("c1", n_frames=20)
+    gpu = make_gpu(spec, with_codebooks=False)
+    oracles = make_oracles(spec, [0], with_codebooks=False)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=4, with_codebooks=False)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=True)
+
+
+def test_small_pq_and_single_mode():
+    # G = 2, C = 4, S = 3: C^G = 16 >= S; exercises ragged code tables and S < 8
+    spec = gen.spec_for("c1", n_frames=30, G=2, C=4)
+    gpu = make_gpu(spec, S=3, beam=3)
+    oracles = make_oracles(spec, [0], S=3, beam=3)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=5)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False)
+
+
+def test_ragged_frame_size_and_bf16_d64():
+    spec = dataclasses.replace(gen.spec_for("c1"), name="ragged", dtype="bf16", grid_h=5, grid_w=7, k_max=50,
+                               n_q_heads=6, n_kv_heads=2, n_frames=20, n_query_tokens=3)
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [0, 1])
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=5)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# boundary behaviour: host variants, state import/export, errors
+# ---------------------------------------------------------------------------------------------------------
+def test_host_variants_match_device_calls():
+    spec = gen.spec_for("c1", n_frames=12)
+    a, b = make_gpu(spec), make_gpu(spec)
+    s = gen.grid_positions(spec)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        a.append_frame(K.cuda(), V.cuda(), s.cuda())
+        b.append_frame_host(K.pin_memory(), V.pin_memory(), s.pin_memory())
+    Q = gen.queries(spec, 0)
+    oa = a.query_attention(Q.cuda()).cpu()
+    ob = torch.empty_like(Q).pin_memory()
+    b.query_attention_host(Q.pin_memory(), ob)
+    assert torch.equal(oa, ob)
+    for f in ("c", "p", "n", "hist_k", "hist_v", "mu", "sigma"):
+        assert np.array_equal(a.export_state(0)[f], b.export_state(0)[f])
+
+
+def test_import_state_round_trip():
+    spec = gen.spec_for("c1", n_frames=16)
+    a, b = make_gpu(spec), make_gpu(spec)
+    s = gen.grid_positions(spec).cuda()
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        a.append_frame(K.cuda(), V.cuda(), s)
+        b.append_frame(K.cuda(), V.cuda(), s)
+    st = a.export_state(0)
+    st2 = {k: v.copy() for k, v in st.items()}
+    st2["c"][:] *= 0.5
+    b.import_state(0, **st2)
+    got = b.export_state(0)
+    assert np.array_equal(got["c"], st2["c"]) and np.array_equal(got["hist_k"], st["hist_k"])
+    b.import_state(0, **st)
+    K, V = gen.frame_kv(spec, spec.n_frames)
+    a.append_frame(K.cuda(), V.cuda(), s)
+    b.append_frame(K.cuda(), V.cuda(), s)
+    ta, tb = a.last_frame_trace(), b.last_frame_trace()
+    assert np.array_equal(ta["assign"], tb["assign"]) and np.array_equal(ta["best"], tb["best"])
+    for f in ("c", "p", "n", "hist_k", "mu", "sigma"):
+        assert np.array_equal(a.export_state(0)[f], b.export_state(0)[f])
+
+
+def test_errors_leave_state_unchanged():
+    spec = gen.spec_for("c1")
+    gpu = make_gpu(spec)
+    K, V = gen.frame_kv(spec, 0)
+    s = gen.grid_positions(spec)
+    with pytest.raises(ProtoKVError):
+        gpu.append_frame(K.cuda()[..., :32].contiguous(), V.cuda(), s.cuda())      # wrong size
+    with pytest.raises(ProtoKVError):
+        gpu.append_frame(K, V, s)                                                  # host tensors
+    assert gpu.frames_seen == 0
+    Q = gen.queries(spec, 0).cuda()
+    with pytest.raises(ProtoKVError) as ei:
+        gpu.query_attention_ex(Q[:, :, :4].contiguous(), n_q=4, layer_begin=1)     # layer range
+    assert ei.value.code == 1
+    with pytest.raises(ProtoKVError) as ei:
+        gpu.export_state(7)
+    assert ei.value.code == 1
+    with pytest.raises(ProtoKVError) as ei:
+        make_gpu(dataclasses.replace(spec, head_dim=96))
+    with pytest.raises(ProtoKVError):
+        gpu.export_codes(0)                                                        # nothing synthesised yet
