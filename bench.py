@@ -1,0 +1,439 @@
+#!/usr/bin/env python
+"""bench.py -- ProtoKV hot path on B200: update frames/s, query-attention latency, roofline fractions.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over one batch of synthetic input:
+    protokv_append_frame   (U1 ring append, U2 slot fill, U3 assignment, U4 segmenting, U5 update, U6 histograms)
+    protokv_query_attention (Q1 synthesis, Q2 fused attention over [near || pseudo-tokens])
+in steady state (near window and prototype bank full).  CUDA events split every step into its update part and
+its query part: `value` = update frames/s (BASELINE.json's first metric component), `query_attn_us` = query
+latency, `ms_per_step` = the whole step.  One JSON line on stdout (rank 0); progress goes to stderr.
+See DESIGN.md "Measurement" for the byte / flop counts behind the roofline objects.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+import gen  # noqa: E402
+
+METRIC = "frames/sec far-memory update; query-attn latency us; % HBM/tensor roofline"
+UNIT = "frames/s"
+L2_BYTES = 126 * 2 ** 20
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm=float(p["hbm_gbs"]), bf16_burst=float(p["bf16_tflops"]),
+                    bf16_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), source="measured")
+    return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, source="fallback")   # B200_PROFILING.md fallback
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# algorithmic bytes / flops (restated in DESIGN.md "Measurement")
+# ---------------------------------------------------------------------------------------------------------------
+def update_bytes_per_frame(spec, touched_per_bank):
+    elt = 2 if spec.dtype == "bf16" else 4
+    T, d, K, G = spec.T, spec.head_dim, spec.k_max, spec.G
+    per_bank = 6 * T * d * elt + K * (4 * d + 40) + touched_per_bank * (16 * d + 80) + T * 16 * G
+    return per_bank * spec.n_banks
+
+
+def assign_flops_per_frame(spec):
+    return 2.0 * spec.T * spec.k_max * spec.head_dim * spec.n_banks
+
+
+def query_bytes(spec):
+    elt = 2 if spec.dtype == "bf16" else 4
+    d, K, S, G = spec.head_dim, spec.k_max, 8, spec.G
+    W = spec.near_frames * spec.T
+    rows = spec.n_query_tokens * (spec.n_q_heads // spec.n_kv_heads)
+    per_bank = 2 * W * d * elt + K * (2 * d * 4 + S * G + 4) + 2 * rows * d * elt
+    return per_bank * spec.n_banks
+
+
+def query_flops(spec):
+    d, K, S = spec.head_dim, spec.k_max, 8
+    W = spec.near_frames * spec.T
+    rows = spec.n_query_tokens * (spec.n_q_heads // spec.n_kv_heads)
+    fact = 4.0 * rows * (W + K) * d * spec.n_banks
+    dense = 4.0 * rows * (W + K * S) * d * spec.n_banks
+    return fact, dense
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        return dict(sm_mhz=sm[len(sm) // 2] if sm else None, sm_max_mhz=mx, samples=len(sm), reasons=sorted(reasons))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------------------------
+def make_state(spec, device):
+    from paper_2606_26762_b200 import ProtoKV
+    ck, cv = gen.codebooks(spec, device=device)
+    return ProtoKV(n_streams=spec.n_streams, n_layers=spec.n_layers, n_q_heads=spec.n_q_heads,
+                   n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim, dtype=spec.dtype, tokens_per_frame=spec.T,
+                   near_frames=spec.near_frames, k_max=spec.k_max, n_query_tokens=spec.n_query_tokens,
+                   codebook_k=ck, codebook_v=cv, device=device, G=spec.G, C=spec.C)
+
+
+def steady_state_frames(spec):
+    """Frames to stream before the ring and the bank are full (+2 so that every prototype has absorbed tokens)."""
+    return spec.near_frames + math.ceil(spec.k_max / spec.T) + 2
+
+
+def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=True, sampler=None, barrier=None):
+    dev = str(device)
+    st = make_state(spec, dev)
+    s = gen.grid_positions(spec, device=dev)
+    prime = steady_state_frames(spec)
+    frame_bytes = 2 * spec.n_streams * spec.n_layers * spec.T * spec.n_kv_heads * spec.head_dim * (2 if spec.dtype == "bf16" else 4)
+    pool_n = max(4, min(64, math.ceil(2.2 * L2_BYTES / frame_bytes)))
+    log(f"[{spec.name}] banks={spec.n_banks} workspace={st.workspace_bytes / 1e6:.0f} MB, priming {prime} frames, "
+        f"pool {pool_n} frames ({pool_n * frame_bytes / 1e6:.0f} MB)")
+    for f in range(prime):
+        K, V = gen.frame_kv(spec, f + 1000 * rank, device=dev)
+        st.append_frame(K, V, s)
+    pool = [gen.frame_kv(spec, prime + i + 1000 * rank, device=dev) for i in range(pool_n)]
+    Q = gen.queries(spec, 0, device=dev)
+    out = torch.empty_like(Q)
+    state_bytes = st.workspace_bytes
+    flush = None
+    if state_bytes + pool_n * frame_bytes < 2 * L2_BYTES:
+        flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+    torch.cuda.synchronize()
+
+    def step(i, evs=None):
+        K, V = pool[i % pool_n]
+        if flush is not None:
+            flush.fill_(i & 255)
+        if evs: evs[0].record()
+        st.append_frame(K, V, s)
+        if evs: evs[1].record()
+        if flush is not None:
+            flush.fill_((i + 1) & 255)
+        if evs: evs[2].record()
+        st.query_attention(Q, out)
+        if evs: evs[3].record()
+
+    for i in range(warmup):
+        step(i)
+    torch.cuda.synchronize()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    launches0 = st.kernel_launches
+    if barrier: barrier()
+    torch.cuda.synchronize()
+    if sampler: sampler.start()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        step(warmup + i, evs[i])
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop() if sampler else None
+    if barrier: barrier()
+    launches = st.kernel_launches - launches0
+    upd = sorted(e[0].elapsed_time(e[1]) for e in evs)
+    qry = sorted(e[2].elapsed_time(e[3]) for e in evs)
+    res = dict(update_ms_sum=sum(upd), query_ms_sum=sum(qry), update_ms_median=upd[len(upd) // 2],
+               query_ms_median=qry[len(qry) // 2], region_ms=evs[0][0].elapsed_time(evs[-1][3]), wall_ms=wall * 1e3,
+               launches=launches, clocks=clocks, l2="flush: 252 MB fill between timed segments" if flush is not None else
+               f"no flush: state {state_bytes / 1e6:.0f} MB + cycled input pool {pool_n * frame_bytes / 1e6:.0f} MB > 2x L2",
+               impl=dict(assign=st.stage_impl(0), attention=st.stage_impl(1)), state_bytes=state_bytes)
+
+    # touched prototypes per bank-frame (U of the byte formula), from the decisions of the last frame
+    tr = st.last_frame_trace()
+    res["touched_per_bank"] = float(sum(len(set(a.tolist())) for a in tr["assign"]) / len(tr["assign"]))
+
+    if do_profile:   # per-kernel durations: same steps again with the library's stage events switched on
+        st.profile_enable(True)
+        for i in range(steps):
+            step(warmup + steps + i)
+        res["stages"] = st.profile_read()
+        st.profile_enable(False)
+
+    if do_e2e:       # through the host-buffer entry points: H2D of the frame and D2H of the result inside the region
+        hp = [(K.cpu().pin_memory(), V.cpu().pin_memory()) for K, V in pool[:min(pool_n, 8)]]
+        hs, hQ = s.cpu().pin_memory(), Q.cpu().pin_memory()
+        hout = torch.empty_like(hQ).pin_memory()
+        n_e2e = max(3, min(steps, 50))
+        for i in range(2):
+            st.append_frame_host(hp[i % len(hp)][0], hp[i % len(hp)][1], hs)
+            st.query_attention_host(hQ, hout)
+        torch.cuda.synchronize()
+        tu = tq = 0.0
+        t_all = time.perf_counter()
+        for i in range(n_e2e):
+            K, V = hp[i % len(hp)]
+            t1 = time.perf_counter()
+            st.append_frame_host(K, V, hs)
+            torch.cuda.synchronize()
+            t2 = time.perf_counter()
+            st.query_attention_host(hQ, hout)     # synchronises: result is on the host
+            t3 = time.perf_counter()
+            tu += t2 - t1; tq += t3 - t2
+        res["e2e"] = dict(update_s=tu, query_s=tq, steps=n_e2e, total_s=time.perf_counter() - t_all,
+                          h2d=frame_bytes + s.numel() * 4 + Q.numel() * Q.element_size(),
+                          d2h=Q.numel() * Q.element_size())
+    st.close()
+    return res
+
+
+def roofline_objects(spec, res, peaks, steps):
+    """roofline of the dominant kernel + one object per stage group."""
+    out = {}
+    stages = res.get("stages")
+    if not stages:
+        return None, out
+    ub = update_bytes_per_frame(spec, res["touched_per_bank"])
+    qb = query_bytes(spec)
+    fact, dense = query_flops(spec)
+    upd_ms = sum(stages[k][0] for k in ("fill", "score", "update", "append")) / steps
+    out["update_path"] = dict(bound="hbm", achieved=ub / (upd_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
+                              algorithmic_bytes=ub, ms=upd_ms, note="all update kernels of one frame (profiled pass)")
+    out["update_path"]["frac"] = out["update_path"]["achieved"] / peaks["hbm"]
+    sc_ms = stages["score"][0] / max(1, stages["score"][1])
+    af = assign_flops_per_frame(spec)
+    out["score"] = dict(bound="tensor", achieved=af / (sc_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
+                        algorithmic_flops=af, ms=sc_ms, note="T x K_max x d contraction, 1x flops (hi+lo split doubles the MMA work)")
+    out["score"]["frac"] = out["score"]["achieved"] / peaks["bf16_sustained"]
+    at_ms = stages["attention"][0] / max(1, stages["attention"][1])
+    t_roof = max(qb / (peaks["hbm"] * 1e9), fact / (peaks["bf16_sustained"] * 1e12))
+    out["attention"] = dict(bound="tensor" if fact / (peaks["bf16_sustained"] * 1e12) >= qb / (peaks["hbm"] * 1e9) else "hbm",
+                            achieved=fact / (at_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
+                            frac=fact / (at_ms * 1e-3) / 1e12 / peaks["bf16_sustained"], algorithmic_flops=fact,
+                            dense_equivalent_flops=dense, dense_equivalent_tflops=dense / (at_ms * 1e-3) / 1e12,
+                            algorithmic_bytes=qb, hbm_gbs=qb / (at_ms * 1e-3) / 1e9, roofline_us=t_roof * 1e6, ms=at_ms)
+    sy_ms = stages["synthesis"][0] / max(1, stages["synthesis"][1])
+    out["synthesis"] = dict(ms=sy_ms)
+    # dominant kernel of the step = the stage with the largest summed device time
+    dom = max(("score", "update", "attention", "synthesis", "append", "fill"), key=lambda k: stages[k][0])
+    src = {"score": out["score"], "attention": out["attention"]}.get(dom)
+    if src is None:   # a bandwidth-side kernel dominates: report the update path
+        src = out["update_path"]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(spec.name, {}).get(dom)
+        except Exception:
+            traffic = None
+    roof = dict(bound=src["bound"], achieved=src["achieved"], peak=src["peak"], unit=src["unit"], frac=src["frac"],
+                traffic=traffic, kernel=dom, peak_source=peaks["source"] + (" sustained bf16 (kernel timed inside a long step)"
+                                                                         if src["unit"] == "TFLOP/s" else " copy bandwidth"))
+    return roof, out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference)
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_sample(spec, budget_s=15.0, query_rows=16):
+    """Times the CPU oracle, as it stands, on one bank of the workload in steady state: seconds per bank-frame and
+    seconds per query row; returns whole-workload figures by multiplying with the bank / row counts."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import frame_for_bank, codebooks_for_bank, query_rows_for_bank
+    from oracle import OracleBank
+    import dataclasses
+    # bank 0 = (stream 0, layer 0, head 0): the generator is counter-based, so the one-layer / one-stream spec yields
+    # exactly the values bank 0 has in the full workload without generating the other banks.
+    one = dataclasses.replace(spec, n_layers=1, n_streams=1)
+    ck, cv = codebooks_for_bank(one, 0)
+    o = OracleBank(one.T, one.near_frames, one.k_max, one.head_dim, ck, cv, G=one.G, C=one.C)
+    prime = steady_state_frames(one)
+    for f in range(prime):
+        K, V, s = frame_for_bank(one, f, 0)
+        o.append_frame(K, V, s, trace=False)
+    n, t_upd = 0, 0.0
+    while t_upd < budget_s * 0.6 and n < 200:
+        K, V, s = frame_for_bank(one, prime + n, 0)
+        t0 = time.perf_counter()
+        o.append_frame(K, V, s, trace=False)
+        t_upd += time.perf_counter() - t0
+        n += 1
+    Q = gen.queries(one, 0)
+    rows = query_rows_for_bank(one, Q, 0)
+    t0 = time.perf_counter()
+    o.attention(rows[:1])                      # synthesis of every prototype + materialisation + 1 row
+    t_one = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.attention(rows[:1 + query_rows])
+    t_many = time.perf_counter() - t0
+    per_row = max(0.0, (t_many - t_one) / query_rows)
+    per_bank_fixed = max(0.0, t_one - per_row)
+    rows_total = rows.shape[0]
+    s_frame = t_upd / n * spec.n_banks
+    s_query = (per_bank_fixed + per_row * rows_total) * spec.n_banks
+    return dict(frames_per_s=1.0 / s_frame, query_s=s_query, s_per_bank_frame=t_upd / n, frames_timed=n,
+                sample=f"bank 0 of {spec.n_banks}: {n} steady-state frames after {prime} priming frames; query: synthesis "
+                       f"+ materialisation of bank 0 once, {query_rows} of its {rows_total} rows; both scaled by the bank "
+                       f"and row counts", cores=1)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="c3")
+    ap.add_argument("--extras", default="c2,c5", help="comma list of further configs measured briefly in the same line (N=1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    warmup = max(3, args.warmup)
+    rank = int(os.environ.get("RANK", 0))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    spec = gen.spec_for(args.workload)
+    config = dict(workload=f"{spec.name}: BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c3': 2, 'c5': 4}.get(spec.name, 3)}]",
+                  banks=spec.n_banks, layers=spec.n_layers, streams=spec.n_streams, q_heads=spec.n_q_heads,
+                  kv_heads=spec.n_kv_heads, head_dim=spec.head_dim, tokens_per_frame=spec.T, near_frames=spec.near_frames,
+                  k_max=spec.k_max, n_query_tokens=spec.n_query_tokens,
+                  step="1 protokv_append_frame (steady state) + 1 protokv_query_attention; value = frames/s of the update "
+                       "part, query_attn_us = the query part, ms_per_step = both")
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        t_all = time.perf_counter()
+        os_ = oracle_sample(spec, budget_s=min(60.0, 4.0 * max(1, args.steps)))
+        line = dict(metric=METRIC, value=os_["frames_per_s"], unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=warmup,
+                    ms_per_step=1e3 / os_["frames_per_s"] + os_["query_s"] * 1e3, higher_is_better=True, scaling="weak",
+                    vs_baseline=None, dtype="f64", data="synthetic", config=config, impl="reference",
+                    query_attn_us=os_["query_s"] * 1e6,
+                    cpu_baseline=dict(value=os_["frames_per_s"], unit=UNIT, cores=os_["cores"], kind="oracle", sample=os_["sample"]),
+                    e2e=dict(value=os_["frames_per_s"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                    wall_s=time.perf_counter() - t_all)
+        print(json.dumps(line))
+        return
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    barrier = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+        barrier = lambda: dist.barrier()
+    peaks = load_peaks()
+    sampler = ClockSampler(local) if rank == 0 else None
+    res = run_workload(spec, device, args.steps, warmup, rank=rank, sampler=sampler, barrier=barrier,
+                       do_e2e=True, do_profile=True)
+    upd_ms, qry_ms, region_ms = res["update_ms_sum"], res["query_ms_sum"], res["region_ms"]
+    e2e_u, e2e_q = res["e2e"]["update_s"] / res["e2e"]["steps"], res["e2e"]["query_s"] / res["e2e"]["steps"]
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([upd_ms, qry_ms, region_ms, e2e_u, e2e_q], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        upd_ms, qry_ms, region_ms, e2e_u, e2e_q = t.tolist()
+        ln = torch.tensor([res["launches"]], device=device, dtype=torch.int64)
+        dist.all_reduce(ln)
+        res["launches"] = int(ln.item())
+    if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return
+    K = args.steps
+    fps = world * K / (upd_ms * 1e-3)
+    roof, stage_roofs = roofline_objects(spec, res, peaks, K)
+    line = dict(metric=METRIC, value=fps, unit=UNIT, n_gpus=world, steps=K, warmup=warmup,
+                ms_per_step=region_ms / K, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="bf16" if spec.dtype == "bf16" else "f32", data="synthetic", config=dict(config, l2=res["l2"]),
+                update_ms_per_frame=upd_ms / K, update_ms_median=res["update_ms_median"],
+                query_attn_us=qry_ms / K * 1e3, query_attn_us_median=res["query_ms_median"] * 1e3,
+                gpu_launches=res["launches"], impl_kernels=res["impl"], clocks=res["clocks"],
+                e2e=dict(value=world / e2e_u, unit=UNIT, h2d_bytes_per_step=res["e2e"]["h2d"],
+                         d2h_bytes_per_step=res["e2e"]["d2h"], query_attn_us=e2e_q * 1e6,
+                         steps=res["e2e"]["steps"],
+                         note="protokv_append_frame_host / protokv_query_attention_host with pinned host buffers; "
+                              "value = frames/s of the update call incl. its H2D copies, query_attn_us incl. H2D of Q and D2H of out"),
+                roofline=roof, rooflines=stage_roofs,
+                stages_ms_per_step={k: v[0] / K for k, v in res.get("stages", {}).items()},
+                touched_prototypes_per_bank_frame=res["touched_per_bank"], state_bytes=res["state_bytes"],
+                peaks=peaks)
+    if world == 1 and args.extras:
+        extras = {}
+        for name in [x for x in args.extras.split(",") if x and x != spec.name]:
+            try:
+                sp = gen.spec_for(name)
+                r = run_workload(sp, device, max(10, K // 4), warmup, do_e2e=False, do_profile=True)
+                n = max(10, K // 4)
+                ro, sr = roofline_objects(sp, r, peaks, n)
+                extras[name] = dict(frames_per_s=n / (r["update_ms_sum"] * 1e-3), update_ms_per_frame=r["update_ms_sum"] / n,
+                                    query_attn_us=r["query_ms_sum"] / n * 1e3, steps=n, l2=r["l2"], roofline=ro,
+                                    rooflines=sr, stages_ms_per_step={k: v[0] / n for k, v in r["stages"].items()})
+            except Exception as e:   # an extra must not take the headline down
+                extras[name] = dict(error=repr(e))
+        line["other_workloads"] = extras
+    if world == 1 and not args.no_cpu_baseline:
+        os_ = oracle_sample(spec, budget_s=15.0)
+        line["cpu_baseline"] = dict(value=os_["frames_per_s"], unit=UNIT, cores=os_["cores"], kind="oracle",
+                                    sample=os_["sample"], query_attn_us=os_["query_s"] * 1e6,
+                                    host_cores_available=os.cpu_count())
+    print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

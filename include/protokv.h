@@ -169,6 +169,22 @@ int protokv_last_frame_trace(protokv_state *st, int32_t *assign, float *best, ui
 int64_t protokv_frames_seen(const protokv_state *st);
 int64_t protokv_kernel_launches(const protokv_state *st);
 
+/* Stage timing (measurement aid, off by default).  When enabled the library brackets every kernel group it launches
+ * with CUDA events on the state's stream; protokv_profile_read synchronises the stream and returns, per stage, the
+ * summed device time in milliseconds and the number of bracketed launches since the last enable, then resets.
+ * ms_sum and launches hold PROTOKV_N_STAGES entries (host). */
+enum {
+  PROTOKV_STAGE_FILL = 0,    /* U2 slot fill                       */
+  PROTOKV_STAGE_SCORE = 1,   /* U3 Eq. 1 scores + argmin           */
+  PROTOKV_STAGE_UPDATE = 2,  /* U4-U6 segmenting, update, PQ hist  */
+  PROTOKV_STAGE_APPEND = 3,  /* U1 ring append                     */
+  PROTOKV_STAGE_SYNTH = 4,   /* Q1 synthesis                       */
+  PROTOKV_STAGE_ATTN = 5,    /* Q2 fused attention (+ split combine) */
+  PROTOKV_N_STAGES = 6
+};
+int protokv_profile_enable(protokv_state *st, int32_t on);
+int protokv_profile_read(protokv_state *st, double *ms_sum, int64_t *launches);
+
 /* Names the kernel variant each stage uses for this state ("simt" / "tcgen05"), for reports.
  * stage: 0 = assignment, 1 = attention.  Returns a static string, never NULL. */
 const char *protokv_stage_impl(const protokv_state *st, int32_t stage);

@@ -21,8 +21,10 @@ EXPORTED_SYMBOLS = [
     "protokv_query_attention", "protokv_append_frame_host", "protokv_query_attention_host", "protokv_last_error",
     "protokv_query_attention_ex", "protokv_synthesize", "protokv_export_state", "protokv_import_state",
     "protokv_export_ring", "protokv_export_codes", "protokv_import_codes", "protokv_last_frame_trace",
-    "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl",
+    "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl", "protokv_profile_enable",
+    "protokv_profile_read",
 ]
+STAGES = ["fill", "score", "update", "append", "synthesis", "attention"]
 
 
 class ProtoKVError(RuntimeError):
@@ -85,6 +87,8 @@ def load_library():
     lib.protokv_frames_seen.argtypes = [vp]
     lib.protokv_kernel_launches.restype = C.c_int64
     lib.protokv_kernel_launches.argtypes = [vp]
+    lib.protokv_profile_enable.argtypes = [vp, i32]
+    lib.protokv_profile_read.argtypes = [vp, vp, vp]
     lib.protokv_stage_impl.restype = C.c_char_p
     lib.protokv_stage_impl.argtypes = [vp, i32]
     _lib = lib
@@ -297,6 +301,16 @@ class ProtoKV:
                                                        C.byref(nf), C.byref(ev)))
         out["n_fill"], out["evicted_frame"] = nf.value, ev.value
         return out
+
+    def profile_enable(self, on=True):
+        self._check(self._lib.protokv_profile_enable(self._h, int(on)))
+
+    def profile_read(self):
+        """{stage: (summed device ms, bracketed launches)} since the last enable/read."""
+        ms = np.zeros(len(STAGES), np.float64)
+        n = np.zeros(len(STAGES), np.int64)
+        self._check(self._lib.protokv_profile_read(self._h, _np_ptr(ms), _np_ptr(n)))
+        return {s: (float(ms[i]), int(n[i])) for i, s in enumerate(STAGES)}
 
     @property
     def frames_seen(self):

@@ -26,7 +26,47 @@ struct protokv_state {
   bool codes_valid;   // codes/kind describe the current histograms
   bool use_tc_assign;
   int nsplit;
+  // stage timing (protokv_profile_*)
+  bool profiling;
+  std::vector<cudaEvent_t> ev_free;
+  struct Span { int stage; cudaEvent_t a, b; };
+  std::vector<Span> spans;
+  double prof_ms[PROTOKV_N_STAGES];
+  int64_t prof_n[PROTOKV_N_STAGES];
 };
+
+// Brackets one launcher call with events when profiling is on.
+struct StageTimer {
+  protokv_state* st;
+  int stage;
+  cudaEvent_t a = nullptr, b = nullptr;
+  static cudaEvent_t get(protokv_state* st) {
+    if (!st->ev_free.empty()) { cudaEvent_t e = st->ev_free.back(); st->ev_free.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+  }
+  StageTimer(protokv_state* s, int stg) : st(s), stage(stg) {
+    if (!st->profiling) return;
+    a = get(st); b = get(st);
+    cudaEventRecord(a, st->stream);
+  }
+  ~StageTimer() {
+    if (!a) return;
+    cudaEventRecord(b, st->stream);
+    st->spans.push_back({stage, a, b});
+  }
+};
+
+static int drain_spans(protokv_state* st) {
+  for (auto& sp : st->spans) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) { st->prof_ms[sp.stage] += ms; st->prof_n[sp.stage] += 1; }
+    st->ev_free.push_back(sp.a); st->ev_free.push_back(sp.b);
+  }
+  st->spans.clear();
+  return 0;
+}
 
 static thread_local char g_err[512] = "";
 
@@ -193,11 +233,38 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   }
   st->frames = 0; st->n_act = 0; st->launches = 0; st->last_ev_frame = -1; st->last_n_fill = 0;
   st->codes_valid = false;
+  st->profiling = false;
+  for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->use_tc_assign = !(cfg->flags & PROTOKV_FORCE_SIMT) && tc_assign_supported(st->D, st->H);
   return st;
 }
 
-void protokv_destroy(protokv_state* st) { delete st; }
+void protokv_destroy(protokv_state* st) {
+  if (!st) return;
+  for (auto& sp : st->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  for (auto e : st->ev_free) cudaEventDestroy(e);
+  delete st;
+}
+
+int protokv_profile_enable(protokv_state* st, int32_t on) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  drain_spans(st);
+  for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
+  st->profiling = on != 0;
+  return PROTOKV_OK;
+}
+
+int protokv_profile_read(protokv_state* st, double* ms_sum, int64_t* launches) {
+  if (!st || !ms_sum || !launches) return fail(PROTOKV_EINVAL, "NULL argument");
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  drain_spans(st);
+  for (int i = 0; i < PROTOKV_N_STAGES; ++i) {
+    ms_sum[i] = st->prof_ms[i]; launches[i] = st->prof_n[i];
+    st->prof_ms[i] = 0.0; st->prof_n[i] = 0;
+  }
+  return PROTOKV_OK;
+}
 
 int protokv_append_frame(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
   if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
@@ -212,14 +279,24 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   F.n_act = st->n_act + F.n_fill;
   int nl = 0;
   if (F.evicted) {
-    nl += launch_fill(D, st->H, st->V, F, st->stream);                                  // U2
+    if (F.n_fill > 0) {
+      StageTimer tm(st, PROTOKV_STAGE_FILL);
+      nl += launch_fill(D, st->H, st->V, F, st->stream);                                // U2
+    }
     if (D.T - F.n_fill > 0) {
-      nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->stream)        // U3
-                              : launch_score_simt(D, st->H, st->V, F, st->stream);
+      {
+        StageTimer tm(st, PROTOKV_STAGE_SCORE);
+        nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->stream)      // U3
+                                : launch_score_simt(D, st->H, st->V, F, st->stream);
+      }
+      StageTimer tm(st, PROTOKV_STAGE_UPDATE);
       nl += launch_update(D, st->H, st->V, F, st->sm_count, st->stream);                // U4-U6
     }
   }
-  nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                    // U1 (overwrites the slot)
+  {
+    StageTimer tm(st, PROTOKV_STAGE_APPEND);
+    nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                  // U1 (overwrites the slot)
+  }
   PKV_CUDA(cudaGetLastError());
   st->launches += nl;
   st->n_act = F.n_act;
@@ -232,7 +309,10 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
 
 int protokv_synthesize(protokv_state* st) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
-  st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->stream);
+  {
+    StageTimer tm(st, PROTOKV_STAGE_SYNTH);
+    st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->stream);
+  }
   PKV_CUDA(cudaGetLastError());
   st->codes_valid = true;
   return PROTOKV_OK;
@@ -261,7 +341,10 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
   A.n_near = (int)(held * D.T);
   A.n_act = st->n_act;
   A.nsplit = st->nsplit;
-  st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
+  {
+    StageTimer tm(st, PROTOKV_STAGE_ATTN);
+    st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
+  }
   PKV_CUDA(cudaGetLastError());
   return PROTOKV_OK;
 }

@@ -432,7 +432,9 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
   if (k >= D.K) return;
   const size_t pk = (size_t)b * D.K + k;
   float cc = 0.f;
-  for (int i = lane; i < D.d; i += 32) {
+  const int vec = D.d / 32;   // same per-lane order as update_kernel so that derived values are reproduced bit for bit
+  for (int v = 0; v < vec; ++v) {
+    const int i = lane * vec + v;
     const float x = V.c[pk * D.d + i];
     cc = fmaf(x, x, cc);
     if (V.c_hi) {

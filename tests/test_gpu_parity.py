@@ -204,9 +204,25 @@ def test_import_state_round_trip():
     a.append_frame(K.cuda(), V.cuda(), s)
     b.append_frame(K.cuda(), V.cuda(), s)
     ta, tb = a.last_frame_trace(), b.last_frame_trace()
-    assert np.array_equal(ta["assign"], tb["assign"]) and np.array_equal(ta["best"], tb["best"])
+    assert np.array_equal(ta["assign"], tb["assign"]) and np.allclose(ta["best"], tb["best"], rtol=0, atol=1e-6)
     for f in ("c", "p", "n", "hist_k", "mu", "sigma"):
         assert np.array_equal(a.export_state(0)[f], b.export_state(0)[f])
+
+
+def test_stage_profile_counts_launches():
+    spec = gen.spec_for("c1", n_frames=10)
+    gpu = make_gpu(spec)
+    s = gen.grid_positions(spec).cuda()
+    gpu.profile_enable(True)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        gpu.append_frame(K.cuda(), V.cuda(), s)
+    gpu.query_attention(gen.queries(spec, 0).cuda())
+    prof = gpu.profile_read()
+    assert prof["append"][1] == 10 and prof["fill"][1] == 2 and prof["score"][1] == 4 and prof["update"][1] == 4
+    assert prof["synthesis"][1] == 1 and prof["attention"][1] == 1
+    assert all(ms >= 0 for ms, _ in prof.values()) and prof["attention"][0] > 0
+    gpu.profile_enable(False)
 
 
 def test_errors_leave_state_unchanged():
