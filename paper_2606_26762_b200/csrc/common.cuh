@@ -1,6 +1,7 @@
 // Internal definitions shared by the ProtoKV CUDA kernels and the C-ABI host code (not part of the ABI).
 // Layout of the device state is documented in DESIGN.md "Data layout in HBM".
 #pragma once
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -142,8 +143,15 @@ struct AttnArgs {
 int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
 
-// tcgen05 paths (bf16, d = 128)
+// tcgen05 paths (bf16, d = 128).  The TMA tensor maps are built once per state.
+struct TcMaps {
+  CUtensorMap ringK, ringV;   // [B*Wf*T][128] bf16, box {64 cols, 128 rows}, 128-byte swizzle
+  CUtensorMap c_hi, c_lo;     // [B*K][128] bf16, same box
+  bool ok;
+};
 bool tc_assign_supported(const Dims& D, const Hyper& H);
-int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
+bool tc_build_maps(const Dims& D, const Dev& V, TcMaps* maps);
+int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, const TcMaps& maps,
+                    cudaStream_t s);
 
 }  // namespace pkv

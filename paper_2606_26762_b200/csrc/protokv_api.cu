@@ -25,6 +25,7 @@ struct protokv_state {
   int last_n_fill;
   bool codes_valid;   // codes/kind describe the current histograms
   bool use_tc_assign;
+  TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
   bool profiling;
@@ -235,7 +236,9 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->codes_valid = false;
   st->profiling = false;
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
-  st->use_tc_assign = !(cfg->flags & PROTOKV_FORCE_SIMT) && tc_assign_supported(st->D, st->H);
+  st->maps.ok = false;
+  st->use_tc_assign = !(cfg->flags & PROTOKV_FORCE_SIMT) && tc_assign_supported(st->D, st->H) &&
+                      tc_build_maps(st->D, st->V, &st->maps);
   return st;
 }
 
@@ -286,7 +289,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
     if (D.T - F.n_fill > 0) {
       {
         StageTimer tm(st, PROTOKV_STAGE_SCORE);
-        nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->stream)      // U3
+        nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->maps, st->stream)      // U3
                                 : launch_score_simt(D, st->H, st->V, F, st->stream);
       }
       StageTimer tm(st, PROTOKV_STAGE_UPDATE);
