@@ -153,5 +153,11 @@ bool tc_assign_supported(const Dims& D, const Hyper& H);
 bool tc_build_maps(const Dims& D, const Dev& V, TcMaps* maps);
 int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, const TcMaps& maps,
                     cudaStream_t s);
+bool tc_attention_supported(const Dims& D);
+size_t tc_attention_part_bytes(const Dims& D);   // partial-result buffer the tcgen05 attention needs at most
+bool tc_attention_prepare();                     // one-time function attributes; false if the device refuses them
+// Returns the number of kernels launched, or -1 if the Q tensor map could not be encoded.
+int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, const TcMaps& maps,
+                        int sm_count, cudaStream_t s);
 
 }  // namespace pkv

@@ -25,6 +25,7 @@ struct protokv_state {
   int last_n_fill;
   bool codes_valid;   // codes/kind describe the current histograms
   bool use_tc_assign;
+  bool use_tc_attn;
   TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
@@ -164,7 +165,9 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   v.assign = (int*)take(BT * 4); v.best = (float*)take(BT * 4);
   v.tcodeK = (uint8_t*)take(BT * D.G); v.tcodeV = (uint8_t*)take(BT * D.G);
   const size_t rows = (size_t)D.B * D.Nq * D.group;
-  v.part = (float*)take(rows * nsplit * (D.d + 2) * 4);
+  size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
+  if (tc_attention_supported(D) && tc_attention_part_bytes(D) > part_bytes) part_bytes = tc_attention_part_bytes(D);
+  v.part = (float*)take(part_bytes);
   const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * elt;
   const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * elt;
   v.stageK = take(frame); v.stageV = take(frame);
@@ -237,8 +240,10 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->profiling = false;
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->maps.ok = false;
-  st->use_tc_assign = !(cfg->flags & PROTOKV_FORCE_SIMT) && tc_assign_supported(st->D, st->H) &&
-                      tc_build_maps(st->D, st->V, &st->maps);
+  const bool want_tc = !(cfg->flags & PROTOKV_FORCE_SIMT);
+  if (want_tc && (tc_assign_supported(st->D, st->H) || tc_attention_supported(st->D))) tc_build_maps(st->D, st->V, &st->maps);
+  st->use_tc_assign = want_tc && tc_assign_supported(st->D, st->H) && st->maps.ok;
+  st->use_tc_attn = want_tc && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
   return st;
 }
 
@@ -346,7 +351,13 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
   A.nsplit = st->nsplit;
   {
     StageTimer tm(st, PROTOKV_STAGE_ATTN);
-    st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
+    if (st->use_tc_attn && (uintptr_t)Q % 16 == 0 && (uintptr_t)out % 8 == 0) {
+      const int nl = launch_attention_tc(D, st->H, st->V, A, st->maps, st->sm_count, st->stream);
+      if (nl < 0) return fail(PROTOKV_ECUDA, "cuTensorMapEncodeTiled failed for Q");
+      st->launches += nl;
+    } else {
+      st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
+    }
   }
   PKV_CUDA(cudaGetLastError());
   return PROTOKV_OK;
@@ -385,7 +396,7 @@ int64_t protokv_kernel_launches(const protokv_state* st) { return st ? st->launc
 const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
   if (!st) return "none";
   if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
-  if (stage == 1) return "simt";
+  if (stage == 1) return st->use_tc_attn ? "tcgen05" : "simt";
   return "none";
 }
 

@@ -1,0 +1,649 @@
+// Q2 fused attention on the 5th-gen tensor cores (bf16, d = 128, S = 8, G = 8, C = 16): Alg. 4 l.8-15 / Eq. 4
+// as a flash-style kernel over [near window || pseudo-tokens].
+//
+//   near tiles    128 ring rows of K and V, loaded by TMA (128-byte swizzle)
+//   pseudo tiles  16 prototypes x S = 128 pseudo-tokens k~ = c_k + concat_g CK_g[zK(k,s,g)], v~ = p_k + concat_g CV_g[zV]
+//                 (Alg. 4 l.5-9) built in shared memory by the producer warps from the fp32 centres, the 4-bit codes
+//                 of the synthesis step and the codebooks held in shared memory -- pseudo-tokens never exist in HBM
+//   S = Q K~^T    tcgen05.mma, Q tile (M = 128 query rows) and K~ tile from shared memory, fp32 accumulator in TMEM
+//   softmax       one thread per query row drains S with tcgen05.ld, adds the log-mass bias log n_k (Eq. 2/4, 0 on
+//                 near tokens), exponentiates against a lazily updated reference maximum, writes P as bf16 back into
+//                 the columns S occupied (tcgen05.st)
+//   O += P V~     tcgen05.mma with A = P from TMEM, B = V~ tile (MN-major) from shared memory
+//
+// One CTA works on two M tiles of a bank (256 query rows = n_q x GQA group) in ping-pong, so the tensor pipe runs the
+// MMAs of one tile while the softmax warps of the other drain theirs.  The grid is persistent: the (item, tile) space
+// -- item = (bank, block of <= 256 query rows) -- is cut into gridDim.x equal contiguous spans, so a CTA's span may
+// cover the tail of one item and the head of the next; every (item, span) piece writes an unnormalised partial
+// (O, m, l) and attention_tc_combine_kernel merges the pieces of an item.
+//
+// Warp roles (13 warps): 0 = MMA issuer + TMEM owner; 1-4 = producers (TMA for Q and near tiles, builders of the
+// pseudo tiles); 5-8 = softmax of M tile 0; 9-12 = softmax of M tile 1.
+#include "common.cuh"
+#include "tc_common.cuh"
+
+namespace pkv {
+
+using namespace tc;
+
+constexpr int kAtThreads = 416;
+constexpr int kAtCols = 128;            // context columns per tile
+constexpr int kAtProto = 16;            // prototypes per pseudo tile (x S = 8)
+constexpr int kAtRows = 256;            // query rows per item (two M tiles)
+constexpr uint32_t kAtHalf = 128 * 128; // one [128 rows][64 bf16] swizzled box = 16 KB
+constexpr int kAtBiasRing = 4;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kRescaleGap = 8.f;      // P may reach 2^8 before the reference maximum is moved
+
+struct AtSmem {   // byte offsets from a 1024-byte aligned base
+  static constexpr uint32_t Q = 0;                          // 2 d-halves x [256 rows][128 B]
+  static constexpr uint32_t K = Q + 4 * kAtHalf;            // 2 stages x (2 d-halves x 16 KB)
+  static constexpr uint32_t V = K + 4 * kAtHalf;            // 2 stages x (2 d-halves x 16 KB)
+  static constexpr uint32_t CBK = V + 4 * kAtHalf;          // [G][C][16] fp32
+  static constexpr uint32_t CBV = CBK + 8192;
+  static constexpr uint32_t Bias = CBV + 8192;              // [ring][16] fp32, log2 domain
+  static constexpr uint32_t Bar = Bias + kAtBiasRing * kAtProto * 4;
+  static constexpr uint32_t Total = Bar + 256;
+};
+
+// Partition of the tile space shared by the kernel, the combine kernel and the host.
+struct AtPlan {
+  int items;        // (bank selection, row block) pairs
+  int nrb;          // row blocks per bank
+  int tb;           // query tokens per row block (tb * group <= 256)
+  int nt_near;      // near tiles per item
+  int nt_ps;        // pseudo tiles per item
+  int ntile;        // nt_near + nt_ps
+  int grid;
+  int nsplit;       // max pieces per item (partial buffer stride)
+  long long ttot;   // items * ntile
+};
+
+__host__ __device__ inline long long at_span_begin(const AtPlan& P, int cta) { return ((long long)cta * P.ttot) / P.grid; }
+// CTA whose span contains global tile x.
+__host__ __device__ inline int at_cta_of(const AtPlan& P, long long x) {
+  return (int)(((x + 1) * P.grid + P.ttot - 1) / P.ttot - 1);
+}
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+
+struct AtArgs {
+  const void* Q;   // unused by the kernel (the tensor map addresses it); kept for the combine kernel's layout maths
+  int n_q, layer_begin, layer_count;
+  int n_near, n_act;
+  int use_bias;
+};
+
+// One contiguous piece of an item inside this CTA's span.
+struct AtSeg {
+  int item, t0, t1;       // tiles [t0, t1) of the item
+  int b;                  // bank
+  int st, ll, hd, rb;     // stream, layer (relative to layer_begin), KV head, row block
+  int R;                  // valid query rows of the block (<= 256)
+  int ntm;                // M tiles in use (1 or 2)
+  int piece;              // index of this piece among the item's pieces
+};
+
+__device__ __forceinline__ AtSeg at_segment(const AtPlan& P, const Dims& D, const AtArgs& A, long long g, long long g1) {
+  AtSeg s;
+  s.item = (int)(g / P.ntile);
+  s.t0 = (int)(g - (long long)s.item * P.ntile);
+  const long long room = g1 - g;
+  s.t1 = (int)((long long)(P.ntile - s.t0) < room ? P.ntile : s.t0 + room);
+  const int bsel = s.item / P.nrb;
+  s.rb = s.item % P.nrb;
+  s.hd = bsel % D.Hkv;
+  s.ll = (bsel / D.Hkv) % A.layer_count;
+  s.st = bsel / (D.Hkv * A.layer_count);
+  s.b = (s.st * D.L + A.layer_begin + s.ll) * D.Hkv + s.hd;
+  const int tok0 = s.rb * P.tb;
+  const int ntok = min(P.tb, A.n_q - tok0);
+  s.R = ntok * D.group;
+  s.ntm = s.R > 128 ? 2 : 1;
+  s.piece = (int)blockIdx.x - at_cta_of(P, (long long)s.item * P.ntile);
+  return s;
+}
+
+// x'_i = S_i * sc2 + bm[i / 8]  (log2 domain, relative to the reference maximum); returns max_i x'_i of the row.
+template <bool RAGGED>
+__device__ __forceinline__ float at_row_max(uint32_t s_addr, float sc2, const float (&bm)[16], int nvalid) {
+  float mx = -INFINITY;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    uint32_t a[32];
+    tmem_ld_32x32(s_addr + c * 32, a);
+    tmem_ld_wait();
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      float x = fmaf(__uint_as_float(a[i]), sc2, bm[(c * 32 + i) >> 3]);
+      if (RAGGED && c * 32 + i >= nvalid) x = -INFINITY;
+      mx = fmaxf(mx, x);
+    }
+  }
+  return mx;
+}
+
+// One pass over the S tile of this row: P = exp2(x') packed to bf16 pairs, row sum and row max of x'.
+template <bool RAGGED>
+__device__ __forceinline__ void at_row_pass(uint32_t s_addr, float sc2, const float (&bm)[16], int nvalid,
+                                            uint32_t (&pk)[64], float& lsum, float& mx) {
+  float l0 = 0.f, l1 = 0.f, m0 = -INFINITY, m1 = -INFINITY;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    uint32_t a[32];
+    tmem_ld_32x32(s_addr + c * 32, a);
+    tmem_ld_wait();
+#pragma unroll
+    for (int i = 0; i < 32; i += 2) {
+      float x0 = fmaf(__uint_as_float(a[i]), sc2, bm[(c * 32 + i) >> 3]);
+      float x1 = fmaf(__uint_as_float(a[i + 1]), sc2, bm[(c * 32 + i) >> 3]);
+      if (RAGGED) {
+        if (c * 32 + i >= nvalid) x0 = -INFINITY;
+        if (c * 32 + i + 1 >= nvalid) x1 = -INFINITY;
+      }
+      m0 = fmaxf(m0, x0); m1 = fmaxf(m1, x1);
+      const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+      l0 += p0; l1 += p1;
+      pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+    }
+  }
+  lsum = l0 + l1;
+  mx = fmaxf(m0, m1);
+}
+
+struct AtBars {
+  uint64_t *q_full, *q_empty, *k_full, *k_empty, *v_full, *v_empty, *s_full, *p_full, *pv_done, *o_empty;
+  __device__ explicit AtBars(uint64_t* b)
+      : q_full(b), q_empty(b + 1), k_full(b + 2), k_empty(b + 4), v_full(b + 6), v_empty(b + 8), s_full(b + 10),
+        p_full(b + 12), pv_done(b + 14), o_empty(b + 16) {}
+};
+
+// ---- warp 0: MMA issuer -------------------------------------------------------------------------------------
+__device__ __forceinline__ void at_issue_s(uint32_t tmem_base, uint32_t q_addr, uint32_t k_addr, int w) {
+  constexpr uint32_t idesc = idesc_bf16(128, 128, 0, 0);
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {
+      const uint64_t ad = desc_kmajor_sw128(q_addr + half * 2 * kAtHalf + w * kAtHalf + kk * 32);
+      const uint64_t bd = desc_kmajor_sw128(k_addr + half * kAtHalf + kk * 32);
+      umma_bf16(tmem_base + w * 128, ad, bd, idesc, (half | kk) != 0);
+    }
+  }
+}
+__device__ __forceinline__ void at_issue_pv(uint32_t tmem_base, uint32_t v_addr, int w, bool acc) {
+  constexpr uint32_t idesc = idesc_bf16(128, 128, 0, 1);   // B = V~ tile, MN-major (d contiguous)
+#pragma unroll
+  for (int kk = 0; kk < 8; ++kk) {                         // 16 context columns (= MMA K) per instruction
+    const uint64_t bd = desc_mnmajor_sw128(v_addr + kk * 2048, kAtHalf);
+    umma_bf16_ts(tmem_base + 256 + w * 128, tmem_base + w * 128 + kk * 8, bd, idesc, acc || kk != 0);
+  }
+}
+
+__device__ void at_mma_role(unsigned char* sm, const AtBars& B, uint32_t tmem_base, const Dims& D, const AtArgs& A,
+                            const AtPlan& P) {
+  const uint32_t q_addr = smem_u32(sm + AtSmem::Q), k_addr = smem_u32(sm + AtSmem::K), v_addr = smem_u32(sm + AtSmem::V);
+  uint32_t kc = 0, vc = 0, ic = 0, pc[2] = {0, 0}, oc[2] = {0, 0};
+  const long long g1 = at_span_begin(P, blockIdx.x + 1);
+  for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
+    const AtSeg sg = at_segment(P, D, A, g, g1);
+    const int n = sg.t1 - sg.t0;
+    g += n;
+    mbar_wait(B.q_full, ic & 1);
+    mbar_wait(B.k_full + (kc & 1), (kc >> 1) & 1);
+    tc_fence_after_sync();
+    for (int w = 0; w < sg.ntm; ++w) {
+      at_issue_s(tmem_base, q_addr, k_addr + (kc & 1) * 2 * kAtHalf, w);
+      umma_commit(B.s_full + w);
+    }
+    umma_commit(B.k_empty + (kc & 1));
+    ++kc;
+    for (int jj = 0; jj < n; ++jj) {
+      const bool more = jj + 1 < n;
+      const uint32_t sv = vc & 1;
+      mbar_wait(B.v_full + sv, (vc >> 1) & 1);
+      for (int w = 0; w < sg.ntm; ++w) {
+        mbar_wait(B.p_full + w, pc[w] & 1);
+        ++pc[w];
+        if (jj == 0) {             // the first PV of an item overwrites O: the previous item's epilogue must have read it
+          mbar_wait(B.o_empty + w, (oc[w] & 1) ^ 1);
+          ++oc[w];
+        }
+        tc_fence_after_sync();
+        at_issue_pv(tmem_base, v_addr + sv * 2 * kAtHalf, w, jj > 0);
+        umma_commit(B.pv_done + w);
+        if (more) {
+          if (w == 0) {
+            mbar_wait(B.k_full + (kc & 1), (kc >> 1) & 1);
+            tc_fence_after_sync();
+          }
+          at_issue_s(tmem_base, q_addr, k_addr + (kc & 1) * 2 * kAtHalf, w);   // after PV_w: P_w aliases S_w
+          umma_commit(B.s_full + w);
+        }
+      }
+      umma_commit(B.v_empty + sv);
+      ++vc;
+      if (more) {
+        umma_commit(B.k_empty + (kc & 1));
+        ++kc;
+      }
+    }
+    umma_commit(B.q_empty);
+    ++ic;
+  }
+}
+
+// ---- warps 1-4: producers -------------------------------------------------------------------------------------
+// Per-thread operands of a pseudo tile: thread (kk, ch) owns the 16-byte chunk ch (8 dims of subspace ch / 2) of
+// prototypes kk and kk + 8 of the tile, for all S pseudo-tokens of each.
+struct AtProtoRegs {
+  float x[2][8];        // centre chunk (c_k or p_k)
+  uint32_t code[2][8];  // packed codes of the S modes (subspace g in bits [4g, 4g+4))
+  bool zero[2];         // zero residual (Alg. 4 l.3-4) or absent prototype
+};
+
+__device__ __forceinline__ void at_load_proto(AtProtoRegs& r, const float* centres, const uint32_t* codes,
+                                              const uint8_t* kind, size_t pk0, int k0, int n_act, int kk, int ch) {
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const int k = k0 + kk + 8 * u;
+    const size_t pk = pk0 + kk + 8 * u;
+    const int kd = k < n_act ? kind[pk] : 2;
+    r.zero[u] = kd != 0;
+    if (kd != 2) {
+      const float4 a = *reinterpret_cast<const float4*>(centres + pk * 128 + ch * 8);
+      const float4 b = *reinterpret_cast<const float4*>(centres + pk * 128 + ch * 8 + 4);
+      r.x[u][0] = a.x; r.x[u][1] = a.y; r.x[u][2] = a.z; r.x[u][3] = a.w;
+      r.x[u][4] = b.x; r.x[u][5] = b.y; r.x[u][6] = b.z; r.x[u][7] = b.w;
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) r.x[u][i] = 0.f;
+    }
+    if (kd == 0) {
+      const uint4 a = *reinterpret_cast<const uint4*>(codes + pk * 8);
+      const uint4 b = *reinterpret_cast<const uint4*>(codes + pk * 8 + 4);
+      r.code[u][0] = a.x; r.code[u][1] = a.y; r.code[u][2] = a.z; r.code[u][3] = a.w;
+      r.code[u][4] = b.x; r.code[u][5] = b.y; r.code[u][6] = b.z; r.code[u][7] = b.w;
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) r.code[u][i] = 0u;
+    }
+  }
+}
+
+// Writes rows (kl * 8 + s) of the tile (K-major, 128-byte swizzle, two d-halves) for this thread's two prototypes.
+__device__ __forceinline__ void at_build_tile(unsigned char* tile, const float* cb, const AtProtoRegs& r, int kk, int ch) {
+  const int g = ch >> 1;
+  const float* cbg = cb + g * 256 + (ch & 1) * 8;          // [C][16] block of subspace g, this chunk's 8 dims
+  unsigned char* base = tile + (ch >> 3) * kAtHalf;
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+#pragma unroll
+    for (int s = 0; s < 8; ++s) {
+      float o[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) o[i] = r.x[u][i];
+      if (!r.zero[u]) {
+        const uint32_t z = (r.code[u][s] >> (4 * g)) & 15u;
+        const float4 a = *reinterpret_cast<const float4*>(cbg + z * 16);
+        const float4 b = *reinterpret_cast<const float4*>(cbg + z * 16 + 4);
+        o[0] += a.x; o[1] += a.y; o[2] += a.z; o[3] += a.w;
+        o[4] += b.x; o[5] += b.y; o[6] += b.z; o[7] += b.w;
+      }
+      const int row = (kk + 8 * u) * 8 + s;                // row & 7 == s
+      const uint4 w = make_uint4(pack_bf16(o[0], o[1]), pack_bf16(o[2], o[3]), pack_bf16(o[4], o[5]), pack_bf16(o[6], o[7]));
+      *reinterpret_cast<uint4*>(base + row * 128 + (((ch & 7) ^ s) << 4)) = w;
+    }
+  }
+}
+
+__device__ void at_producer_role(unsigned char* sm, const AtBars& B, const CUtensorMap* tmQ, const CUtensorMap* tmRK,
+                                 const CUtensorMap* tmRV, const Dims& D, const Dev& V, const AtArgs& A, const AtPlan& P,
+                                 int ptid) {
+  const int kk = ptid >> 4, ch = ptid & 15;
+  float* cbk_s = reinterpret_cast<float*>(sm + AtSmem::CBK);
+  float* cbv_s = reinterpret_cast<float*>(sm + AtSmem::CBV);
+  float* bias_s = reinterpret_cast<float*>(sm + AtSmem::Bias);
+  const uint32_t qbytes = 256u * (uint32_t)D.group * (uint32_t)P.tb;   // two boxes {64 bf16, group, tb}
+  uint32_t tcnt = 0, ic = 0;
+  int cur_bank = -1;
+  const long long g1 = at_span_begin(P, blockIdx.x + 1);
+  for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
+    const AtSeg sg = at_segment(P, D, A, g, g1);
+    g += sg.t1 - sg.t0;
+    if (ptid == 0) {
+      mbar_wait(B.q_empty, (ic & 1) ^ 1);
+      mbar_arrive_expect_tx(B.q_full, qbytes);
+      const int tok = (sg.st * A.layer_count + sg.ll) * A.n_q + sg.rb * P.tb;
+      tma_load_3d(sm + AtSmem::Q, tmQ, 0, sg.hd * D.group, tok, B.q_full);
+      tma_load_3d(sm + AtSmem::Q + 2 * kAtHalf, tmQ, 64, sg.hd * D.group, tok, B.q_full);
+    }
+    ++ic;
+    if (sg.b != cur_bank && sg.t1 > P.nt_near && V.cbk) {    // codebooks of this bank (only the builders read them)
+      const float4* srck = reinterpret_cast<const float4*>(V.cbk + (size_t)sg.b * 2048);
+      const float4* srcv = reinterpret_cast<const float4*>(V.cbv + (size_t)sg.b * 2048);
+      for (int e = ptid; e < 512; e += 128) {
+        reinterpret_cast<float4*>(cbk_s)[e] = srck[e];
+        reinterpret_cast<float4*>(cbv_s)[e] = srcv[e];
+      }
+      cur_bank = sg.b;
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+    }
+    for (int j = sg.t0; j < sg.t1; ++j, ++tcnt) {
+      const uint32_t stg = tcnt & 1, par = ((tcnt >> 1) & 1) ^ 1;
+      unsigned char* ks = sm + AtSmem::K + stg * 2 * kAtHalf;
+      unsigned char* vs = sm + AtSmem::V + stg * 2 * kAtHalf;
+      if (j < P.nt_near) {
+        // every producer thread observes every phase of the empty barriers (a parity wait is only meaningful for a
+        // waiter that is at most one phase behind); thread 0 alone issues the copies
+        const int row0 = sg.b * D.Wf * D.T + j * kAtCols;
+        mbar_wait(B.k_empty + stg, par);
+        if (ptid == 0) {
+          mbar_arrive_expect_tx(B.k_full + stg, 2 * kAtHalf);
+          tma_load_2d(ks, tmRK, 0, row0, B.k_full + stg);
+          tma_load_2d(ks + kAtHalf, tmRK, 64, row0, B.k_full + stg);
+        }
+        mbar_wait(B.v_empty + stg, par);
+        if (ptid == 0) {
+          mbar_arrive_expect_tx(B.v_full + stg, 2 * kAtHalf);
+          tma_load_2d(vs, tmRV, 0, row0, B.v_full + stg);
+          tma_load_2d(vs + kAtHalf, tmRV, 64, row0, B.v_full + stg);
+        }
+      } else {
+        const int k0 = (j - P.nt_near) * kAtProto;
+        const size_t pk0 = (size_t)sg.b * D.K + k0;
+        AtProtoRegs rk, rv;
+        at_load_proto(rk, V.c, V.codesK, V.kind, pk0, k0, A.n_act, kk, ch);
+        at_load_proto(rv, V.p, V.codesV, V.kind, pk0, k0, A.n_act, kk, ch);
+        if (ptid < kAtProto) {
+          const int k = k0 + ptid;
+          float bias = -INFINITY;
+          if (k < A.n_act && V.kind[pk0 + ptid] != 2) bias = A.use_bias ? V.logn[pk0 + ptid] * kLog2e : 0.f;
+          bias_s[(tcnt & (kAtBiasRing - 1)) * kAtProto + ptid] = bias;
+        }
+        mbar_wait(B.k_empty + stg, par);
+        at_build_tile(ks, cbk_s, rk, kk, ch);
+        fence_proxy_async_smem();
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (ptid == 0) mbar_arrive(B.k_full + stg);
+        mbar_wait(B.v_empty + stg, par);
+        at_build_tile(vs, cbv_s, rv, kk, ch);
+        fence_proxy_async_smem();
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (ptid == 0) mbar_arrive(B.v_full + stg);
+      }
+    }
+  }
+  if (ptid == 0 && ic > 0) mbar_wait(B.q_empty, (ic & 1) ^ 1);   // every MMA of this CTA has completed
+}
+
+// ---- warps 5-12: softmax (thread = query row of M tile w) -----------------------------------------------------
+constexpr int kPartStride = 132;   // floats per partial row: O[128], m (natural log units), l, 2 pad (16-byte rows)
+
+__device__ void at_softmax_role(unsigned char* sm, const AtBars& B, uint32_t tmem_base, const Dims& D, const AtArgs& A,
+                                const AtPlan& P, float* part, int w, int q, int lane) {
+  const int row = q * 32 + lane;
+  const uint32_t lane_off = (uint32_t)(q * 32) << 16;
+  const uint32_t s_addr = tmem_base + lane_off + w * 128;
+  const uint32_t o_addr = tmem_base + lane_off + 256 + w * 128;
+  const float sc2 = kLog2e * rsqrtf(128.f);
+  const float* bias_s = reinterpret_cast<const float*>(sm + AtSmem::Bias);
+  uint32_t cnt = 0, gt = 0;     // tiles this warpgroup has finished; tiles the CTA has been through
+  const long long g1 = at_span_begin(P, blockIdx.x + 1);
+  for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
+    const AtSeg sg = at_segment(P, D, A, g, g1);
+    const int n = sg.t1 - sg.t0;
+    g += n;
+    if (w >= sg.ntm) { gt += n; continue; }
+    float m_ref = 0.f, l_run = 0.f;
+    for (int jj = 0; jj < n; ++jj, ++cnt, ++gt) {
+      const int j = sg.t0 + jj;
+      const bool pseudo = j >= P.nt_near;
+      const int nvalid = pseudo ? kAtCols : min(kAtCols, A.n_near - j * kAtCols);
+      mbar_wait(B.s_full + w, cnt & 1);
+      tc_fence_after_sync();
+      float bm[16];
+      auto load_bm = [&](float m) {
+        if (pseudo) {
+          const float4* bp = reinterpret_cast<const float4*>(bias_s + (gt & (kAtBiasRing - 1)) * kAtProto);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float4 v = bp[i];
+            bm[4 * i] = v.x - m; bm[4 * i + 1] = v.y - m; bm[4 * i + 2] = v.z - m; bm[4 * i + 3] = v.w - m;
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) bm[i] = -m;
+        }
+      };
+      if (jj == 0) {              // first tile of the piece: the reference maximum is this tile's row maximum
+        load_bm(0.f);
+        const float mx = nvalid < kAtCols ? at_row_max<true>(s_addr, sc2, bm, nvalid)
+                                          : at_row_max<false>(s_addr, sc2, bm, nvalid);
+        m_ref = mx == -INFINITY ? 0.f : mx;
+      }
+      load_bm(m_ref);
+      uint32_t pk[64];
+      float lsum, mx;
+      for (;;) {
+        if (nvalid < kAtCols) at_row_pass<true>(s_addr, sc2, bm, nvalid, pk, lsum, mx);
+        else at_row_pass<false>(s_addr, sc2, bm, nvalid, pk, lsum, mx);
+        if (!__any_sync(0xffffffffu, mx > kRescaleGap)) break;
+        // some row of this warp ran past its reference maximum: move it and rescale l and O (rare)
+        float alpha = 1.f;
+        if (mx > 0.f) {
+          alpha = ex2_approx(-mx);
+          m_ref += mx;
+          l_run *= alpha;
+#pragma unroll
+          for (int i = 0; i < 16; ++i) bm[i] -= mx;
+        }
+        if (jj > 0) {
+          mbar_wait(B.pv_done + w, (cnt - 1) & 1);
+          tc_fence_after_sync();
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            uint32_t o[32];
+            tmem_ld_32x32(o_addr + c * 32, o);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st_32x32(o_addr + c * 32, o);
+          }
+          tmem_st_wait();
+        }
+      }
+      l_run += lsum;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_st_32x16<64>(s_addr + c * 16, pk, c * 16);
+      tmem_st_wait();
+      tc_fence_before_sync();
+      mbar_arrive(B.p_full + w);
+    }
+    // partial result of this piece: unnormalised O, reference maximum, row sum
+    mbar_wait(B.pv_done + w, (cnt - 1) & 1);
+    tc_fence_after_sync();
+    const int r = w * 128 + row;
+    float* dst = part + (((size_t)sg.item * P.nsplit + sg.piece) * kAtRows + r) * kPartStride;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      uint32_t o[32];
+      tmem_ld_32x32(o_addr + c * 32, o);
+      tmem_ld_wait();
+      if (r < sg.R) {
+#pragma unroll
+        for (int i = 0; i < 32; i += 4)
+          *reinterpret_cast<uint4*>(dst + c * 32 + i) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
+      }
+    }
+    if (r < sg.R) *reinterpret_cast<float2*>(dst + 128) = make_float2(m_ref * kLn2, l_run);
+    tc_fence_before_sync();
+    mbar_arrive(B.o_empty + w);
+  }
+}
+
+__global__ void __launch_bounds__(kAtThreads, 1)
+attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmRK,
+                    const __grid_constant__ CUtensorMap tmRV, Dims D, Dev V, AtArgs A, AtPlan P, float* part) {
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* sm = (unsigned char*)(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + AtSmem::Bar);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 18);
+  const AtBars B(bars);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&tmQ); prefetch_tmap(&tmRK); prefetch_tmap(&tmRV);
+    mbar_init(B.q_full, 1); mbar_init(B.q_empty, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(B.k_full + i, 1); mbar_init(B.k_empty + i, 1);
+      mbar_init(B.v_full + i, 1); mbar_init(B.v_empty + i, 1);
+      mbar_init(B.s_full + i, 1); mbar_init(B.p_full + i, 128);
+      mbar_init(B.pv_done + i, 1); mbar_init(B.o_empty + i, 128);
+    }
+    fence_barrier_init();
+  }
+  // rows of the Q staging area that no Q box ever writes must hold finite values
+  for (uint32_t e = threadIdx.x; e < 4 * kAtHalf / 16; e += kAtThreads)
+    reinterpret_cast<uint4*>(sm + AtSmem::Q)[e] = make_uint4(0u, 0u, 0u, 0u);
+  fence_proxy_async_smem();
+  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) at_mma_role(sm, B, tmem_base, D, A, P);
+  } else if (warp < 5) {
+    at_producer_role(sm, B, &tmQ, &tmRK, &tmRV, D, V, A, P, (int)threadIdx.x - 32);
+  } else {
+    at_softmax_role(sm, B, tmem_base, D, A, P, part, (warp - 5) >> 2, warp & 3, lane);
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 0) {
+    __syncwarp();
+    tc_fence_after_sync();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+// Merges the pieces of every item: one warp per output row, 4 dims per lane.
+__global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArgs A, AtPlan P, const float* part,
+                                                                   __nv_bfloat16* out, float* lse, int rows_total) {
+  const int gr = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (gr >= rows_total) return;
+  const int Rb = A.n_q * D.group;
+  const int bsel = gr / Rb, rr = gr % Rb;
+  const int qi = rr / D.group, hh = rr % D.group;
+  const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
+  const int rb = qi / P.tb;
+  const int rin = (qi - rb * P.tb) * D.group + hh;
+  const int item = bsel * P.nrb + rb;
+  int np = 0, cf = 0;
+  if (P.ntile > 0) {
+    cf = at_cta_of(P, (long long)item * P.ntile);
+    np = at_cta_of(P, (long long)(item + 1) * P.ntile - 1) - cf + 1;
+  }
+  const float* base = part + ((size_t)item * P.nsplit * kAtRows + rin) * kPartStride;
+  const size_t pstride = (size_t)kAtRows * kPartStride;
+  float M = -INFINITY;
+  for (int sp = 0; sp < np; ++sp) {
+    const float2 ml = *reinterpret_cast<const float2*>(base + sp * pstride + 128);
+    if (ml.y > 0.f) M = fmaxf(M, ml.x);
+  }
+  float l = 0.f;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int sp = 0; sp < np; ++sp) {
+    const float* ps = base + sp * pstride;
+    const float2 ml = *reinterpret_cast<const float2*>(ps + 128);
+    if (!(ml.y > 0.f)) continue;
+    const float wgt = __expf(ml.x - M);
+    const float4 v = *reinterpret_cast<const float4*>(ps + lane * 4);
+    l = fmaf(ml.y, wgt, l);
+    acc.x = fmaf(v.x, wgt, acc.x); acc.y = fmaf(v.y, wgt, acc.y);
+    acc.z = fmaf(v.z, wgt, acc.z); acc.w = fmaf(v.w, wgt, acc.w);
+  }
+  const float inv = l > 0.f ? 1.f / l : 0.f;
+  const size_t ooff = (((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh;
+  uint2 o;
+  o.x = pack_bf16(acc.x * inv, acc.y * inv);
+  o.y = pack_bf16(acc.z * inv, acc.w * inv);
+  *reinterpret_cast<uint2*>(out + ooff * 128 + lane * 4) = o;
+  if (lse && lane == 0) lse[ooff] = l > 0.f ? M + logf(l) : -INFINITY;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+bool tc_attention_supported(const Dims& D) {
+  return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && D.group <= kAtRows;
+}
+
+static int at_rows_tb(const Dims& D, int n_q) {
+  const int tb = kAtRows / D.group;
+  return n_q < tb ? n_q : tb;
+}
+
+size_t tc_attention_part_bytes(const Dims& D) {
+  // a call with I items on G <= 148 CTAs writes at most G + 2 I pieces (every item has <= ceil(G / I) + 1 of them)
+  const int tb = at_rows_tb(D, D.Nq);
+  const size_t items = (size_t)D.NS * D.L * D.Hkv * ((D.Nq + tb - 1) / tb);
+  return (148 + 2 * items) * kAtRows * kPartStride * sizeof(float);
+}
+
+bool tc_attention_prepare() {
+  const cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)AtSmem::Total + 1024);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return true;
+}
+
+int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, const TcMaps& maps,
+                        int sm_count, cudaStream_t s) {
+  AtArgs a{};
+  a.Q = A.Q; a.n_q = A.n_q; a.layer_begin = A.layer_begin; a.layer_count = A.layer_count;
+  a.n_near = (H.flags & PROTOKV_FAR_ONLY) ? 0 : A.n_near;
+  a.n_act = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : A.n_act;
+  a.use_bias = !(H.flags & PROTOKV_NO_MASS_BIAS);
+  AtPlan P{};
+  P.tb = at_rows_tb(D, A.n_q);
+  P.nrb = (A.n_q + P.tb - 1) / P.tb;
+  P.items = D.NS * A.layer_count * D.Hkv * P.nrb;
+  P.nt_near = (a.n_near + kAtCols - 1) / kAtCols;
+  P.nt_ps = (a.n_act + kAtProto - 1) / kAtProto;
+  P.ntile = P.nt_near + P.nt_ps;
+  P.ttot = (long long)P.items * P.ntile;
+  int grid = sm_count < 148 ? sm_count : 148;
+  if ((long long)grid > P.ttot) grid = (int)P.ttot;
+  P.grid = grid > 0 ? grid : 1;
+  P.nsplit = 1;
+  int launched = 0;
+  if (P.ttot > 0) {
+    for (int i = 0; i < P.items; ++i) {
+      const int np = at_cta_of(P, (long long)(i + 1) * P.ntile - 1) - at_cta_of(P, (long long)i * P.ntile) + 1;
+      if (np > P.nsplit) P.nsplit = np;
+    }
+    CUtensorMap tmQ;
+    const uint64_t ntok = (uint64_t)D.NS * A.layer_count * A.n_q;
+    if (!make_tmap_3d_bf16(&tmQ, A.Q, 128, (uint64_t)D.Hq, ntok, 64, (uint32_t)D.group, (uint32_t)P.tb)) return -1;
+    attention_tc_kernel<<<P.grid, kAtThreads, AtSmem::Total + 1024, s>>>(tmQ, maps.ringK, maps.ringV, D, V, a, P, V.part);
+    ++launched;
+  }
+  const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
+  attention_tc_combine_kernel<<<(rows_total + 3) / 4, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+  return launched + 1;
+}
+
+}  // namespace pkv
