@@ -7,16 +7,53 @@
 namespace pkv {
 
 // ---------------------------------------------------------------------------------------------------------
-// Q1 synthesis.  One thread per (bank, prototype, K|V).
+// Q1 synthesis.  One thread per (bank, prototype, K|V); everything lives in registers (fully unrolled sorting
+// networks, no dynamically indexed arrays).
 //
 // Scores are the fixed-point log-probabilities of Eq. 3, q(g,z) = llround(2^24 log((H[g,z]+eps)/(sum+C eps)))
 // (reading 13), tuples are ordered by (sum of q descending, tuple ascending lexicographically, z_1 most
 // significant).  Beam search with width >= S over additive per-subspace scores under that total order returns
-// exactly the global top-S, so this kernel keeps S partial tuples per step, and of the S x S products of the
-// (sorted) beam with the (sorted) top-S codes of the next subspace only the staircase i*j <= S can survive:
-// an entry (i, j) is preceded by every (i', j') <= (i, j).
+// exactly the global top-S, so this kernel keeps the 8 best partial tuples per step.  Of the products of the sorted
+// beam with the sorted codes of the next subspace only the staircase (i+1)(j+1) <= 8 can survive (an entry (i, j)
+// is preceded by every (i', j') <= (i, j)): 20 candidates, which arrive as five sorted runs
+//   R0 = beam[0] + code[0..7],  R1 = beam[1] + code[0..3],  R2 = beam[2] + code[0..1],  R3 = beam[3] + code[0..1],
+//   R4 = beam[4..7] + code[0]
+// and are reduced to the 8 best by bitonic merges.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSynThreads = 128;
+constexpr long long kSynInf = 1LL << 58;
+
+struct SynCand {
+  long long c;   // cost = -sum q  (>= 0), smaller is better
+  uint32_t t;    // tuple, z_1 in the most significant used nibble; smaller is better on equal cost
+};
+
+__device__ __forceinline__ void syn_ce(SynCand& a, SynCand& b) {   // afterwards a <= b
+  const bool sw = b.c < a.c || (b.c == a.c && b.t < a.t);
+  const long long c0 = sw ? b.c : a.c, c1 = sw ? a.c : b.c;
+  const uint32_t t0 = sw ? b.t : a.t, t1 = sw ? a.t : b.t;
+  a.c = c0; a.t = t0; b.c = c1; b.t = t1;
+}
+__device__ __forceinline__ SynCand syn_min(const SynCand& a, const SynCand& b) {
+  const bool sw = b.c < a.c || (b.c == a.c && b.t < a.t);
+  return sw ? b : a;
+}
+template <int N>
+__device__ __forceinline__ void syn_bitonic_merge(SynCand (&x)[N]) {   // bitonic input -> ascending
+#pragma unroll
+  for (int j = N >> 1; j > 0; j >>= 1) {
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+      if ((i & j) == 0) syn_ce(x[i], x[i | j]);
+  }
+}
+__device__ __forceinline__ SynCand syn_add(const SynCand& b, long long cost, uint32_t z) {
+  SynCand r;
+  r.c = b.c + cost;
+  r.c = r.c < kSynInf ? r.c : kSynInf;
+  r.t = (b.t << 4) | z;
+  return r;
+}
 
 __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act) {
   const long long idx = (long long)blockIdx.x * kSynThreads + threadIdx.x;
@@ -35,64 +72,83 @@ __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H,
     return;
   }
   const uint32_t* Hrow = V.hist + (pk * 2 + kv) * D.G * D.C;
-  const int S = D.S, C = D.C, G = D.G;
-  const int m = C < S ? C : S;
-  long long bc[kMaxS];       // beam cost = -sum q (>= 0), ascending
-  uint32_t bt[kMaxS];        // beam tuple, z_1 in the most significant nibble
-  int nb = 1;
-  bc[0] = 0; bt[0] = 0u;
+  const int C = D.C, G = D.G;
+  SynCand beam[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { beam[i].c = kSynInf; beam[i].t = 0xffffffffu; }
+  beam[0].c = 0; beam[0].t = 0u;
   for (int g = 0; g < G; ++g) {
-    uint32_t h[kMaxC];
-    long long q[kMaxC];
+    // keys of the C codes: (count + 1) in the high bits, 15 - z in the low nibble; 0 = no such code
+    uint32_t key[16];
     double tot = 0.0;
-    for (int z = 0; z < C; ++z) { h[z] = Hrow[g * C + z]; tot += (double)h[z]; }
+#pragma unroll
+    for (int z = 0; z < 16; ++z) {
+      key[z] = 0u;
+      if (z < C) {
+        const uint32_t h = Hrow[g * C + z];
+        tot += (double)h;
+        key[z] = ((h + 1u) << 4) | (uint32_t)(15 - z);
+      }
+    }
     const double den = tot + (double)C * H.pq_eps;
-    for (int z = 0; z < C; ++z) {
-      int same = -1;
-      for (int y = 0; y < z; ++y) if (h[y] == h[z]) { same = y; break; }
-      if (same >= 0) q[z] = q[same];
+    // descending bitonic sort of the 16 keys (the best 8 are needed, sorted)
+#pragma unroll
+    for (int kk = 2; kk <= 16; kk <<= 1) {
+#pragma unroll
+      for (int j = kk >> 1; j > 0; j >>= 1) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const int l = i ^ j;
+          if (l > i) {
+            const uint32_t lo = min(key[i], key[l]), hi = max(key[i], key[l]);
+            const bool desc = (i & kk) == 0;
+            key[i] = desc ? hi : lo; key[l] = desc ? lo : hi;
+          }
+        }
+      }
+    }
+    long long cost[8];
+    uint32_t zc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      zc[i] = 15u - (key[i] & 15u);
+      if (key[i] == 0u) cost[i] = kSynInf;
+      else if (i > 0 && (key[i] >> 4) == (key[i - 1] >> 4)) cost[i] = cost[i - 1];
       else {
-        const double P = ((double)h[z] + H.pq_eps) / den;
-        q[z] = -llround(log(P) * 16777216.0);   // cost = -q
+        const double P = ((double)((key[i] >> 4) - 1u) + H.pq_eps) / den;
+        cost[i] = -llround(log(P) * 16777216.0);
       }
     }
-    // top-m codes by (cost ascending, z ascending)
-    long long tq[kMaxS];
-    int tz[kMaxS];
-    uint32_t taken = 0u;
-    for (int i = 0; i < m; ++i) {
-      int bz = -1;
-      long long bq = 0;
-      for (int z = 0; z < C; ++z)
-        if (!((taken >> z) & 1u) && (bz < 0 || q[z] < bq)) { bz = z; bq = q[z]; }
-      taken |= 1u << bz;
-      tq[i] = bq; tz[i] = bz;
-    }
-    // staircase candidates -> new beam (insertion sort by (cost, tuple))
-    long long nc[kMaxS];
-    uint32_t nt[kMaxS];
-    int cnt = 0;
-    for (int i = 0; i < nb; ++i) {
-      for (int j = 0; j < m && (i + 1) * (j + 1) <= S; ++j) {
-        const long long cost = bc[i] + tq[j];
-        const uint32_t tup = (bt[i] << 4) | (uint32_t)tz[j];
-        int pos = cnt;
-        while (pos > 0 && (nc[pos - 1] > cost || (nc[pos - 1] == cost && nt[pos - 1] > tup))) --pos;
-        if (pos >= S) continue;
-        const int last = cnt < S ? cnt : S - 1;
-        for (int e = last; e > pos; --e) { nc[e] = nc[e - 1]; nt[e] = nt[e - 1]; }
-        nc[pos] = cost; nt[pos] = tup;
-        if (cnt < S) ++cnt;
-      }
-    }
-    nb = cnt;
-    for (int i = 0; i < nb; ++i) { bc[i] = nc[i]; bt[i] = nt[i]; }
+    SynCand a[8], b[8], c4[4];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = syn_add(beam[0], cost[j], zc[j]);                 // R0, ascending
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = syn_add(beam[1], cost[j], zc[j]);                 // R1
+#pragma unroll
+    for (int i = 0; i < 4; ++i) b[7 - i] = syn_add(beam[4 + i], cost[0], zc[0]);         // R4 reversed: [R1, rev R4] is bitonic
+    syn_bitonic_merge<8>(b);
+#pragma unroll
+    for (int j = 0; j < 2; ++j) c4[j] = syn_add(beam[2], cost[j], zc[j]);                // R2
+#pragma unroll
+    for (int j = 0; j < 2; ++j) c4[3 - j] = syn_add(beam[3], cost[j], zc[j]);            // R3 reversed
+    syn_bitonic_merge<4>(c4);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = syn_min(a[i], b[7 - i]);                          // 8 best of R0 u R1 u R4, bitonic
+    syn_bitonic_merge<8>(a);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) a[4 + i] = syn_min(a[4 + i], c4[3 - i]);                 // 8 best of all 20, bitonic
+    syn_bitonic_merge<8>(a);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) beam[i] = a[i];
   }
-  for (int s = 0; s < S; ++s) {
-    uint32_t packed = 0u;
-    if (s < nb)
-      for (int g = 0; g < G; ++g) packed |= ((bt[s] >> (4 * (G - 1 - g))) & 15u) << (4 * g);
-    codes[s] = packed;
+#pragma unroll
+  for (int s = 0; s < 8; ++s) {
+    if (s < D.S) {
+      uint32_t packed = 0u;
+      if (beam[s].c < kSynInf)
+        for (int g = 0; g < G; ++g) packed |= ((beam[s].t >> (4 * (G - 1 - g))) & 15u) << (4 * g);
+      codes[s] = packed;
+    }
   }
 }
 
