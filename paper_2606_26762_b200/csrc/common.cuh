@@ -35,12 +35,13 @@ struct Hyper {
 
 // Per-prototype scoring record (Eq. 1 terms that do not depend on the token), 32 bytes.
 //   invc = 1/|c_k|;  (mux, muy) = mu_k;  (u, v, w) = lambda-scaled inverse Cholesky factor of Sigma_k + eps I:
-//   lambda_sp * d_Mah = sqrt((dx u)^2 + (dy v - dx w)^2);  tau = frame index of the last absorption.
+//   lambda_sp * d_Mah = sqrt((dx u)^2 + (dy v - dx w)^2);  tau = frame index of the last absorption (tauf = the same
+//   as a float, exact below 2^24 frames: the tcgen05 epilogue evaluates the idle test with one saturating add).
+//   Field order = the two broadcast loads of the tcgen05 epilogue: {mux, muy, u, w} and {v, tauf}.
 struct __align__(16) ScoreRec {
-  float invc, mux, muy, u;
-  float v, w;
+  float mux, muy, u, w;
+  float v, tauf, invc;
   int tau;
-  int pad;
 };
 
 // Device pointers into the workspace.
@@ -49,6 +50,7 @@ struct Dev {
   void* ringK;   // [B][Wf][T][d] elt
   void* ringV;
   float* ringS;  // [NS][Wf][T][2]
+  float* ringN;  // [B][Wf][T]  |K_j|^2 of the ring rows (written by the append; the tcgen05 assignment scales by |K_j|)
   // far bank
   float* c;      // [B][K][d]
   float* p;
@@ -72,6 +74,8 @@ struct Dev {
   // per-frame scratch / trace
   int* assign;       // [B][T]
   float* best;       // [B][T]
+  unsigned long long* akey;  // [B][T] packed (orderable(|K_j| * score) << 32 | k): atomicMin target of the tcgen05
+                             // assignment; all-ones between frames (reset by the append kernel)
   uint8_t* tcodeK;   // [B][T][G]
   uint8_t* tcodeV;
   // attention scratch
@@ -122,6 +126,7 @@ struct FrameArgs {
   int n_act0;    // active prototypes before this step's slot fill
   int n_fill;    // evicted tokens that open a new slot (Alg. 1 l.3-4)
   int n_act;     // active prototypes after the fill = what Eq. 1 scans
+  int keys;      // 1: the assignment of this frame is in Dev::akey (tcgen05 path), 0: in Dev::assign / best (SIMT)
 };
 
 // Every launcher returns the number of kernels it launched (0 if there was nothing to do).
@@ -152,7 +157,7 @@ struct TcMaps {
 bool tc_assign_supported(const Dims& D, const Hyper& H);
 bool tc_build_maps(const Dims& D, const Dev& V, TcMaps* maps);
 int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, const TcMaps& maps,
-                    cudaStream_t s);
+                    int sm_count, cudaStream_t s);
 bool tc_attention_supported(const Dims& D);
 size_t tc_attention_part_bytes(const Dims& D);   // partial-result buffer the tcgen05 attention needs at most
 bool tc_attention_prepare();                     // one-time function attributes; false if the device refuses them

@@ -147,6 +147,7 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   Dev v{};
   v.ringK = take(ring); v.ringV = take(ring);
   v.ringS = (float*)take((size_t)D.NS * D.Wf * D.T * 2 * 4);
+  v.ringN = (float*)take((size_t)D.B * D.Wf * D.T * 4);
   v.c = (float*)take(BK * D.d * 4); v.p = (float*)take(BK * D.d * 4);
   if (D.bf16) {
     v.c_hi = (__nv_bfloat16*)take(BK * D.d * 2);
@@ -163,6 +164,7 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   v.codesK = (uint32_t*)take(BK * D.S * 4); v.codesV = (uint32_t*)take(BK * D.S * 4);
   v.kind = (uint8_t*)take(BK);
   v.assign = (int*)take(BT * 4); v.best = (float*)take(BT * 4);
+  v.akey = (unsigned long long*)take(BT * 8);
   v.tcodeK = (uint8_t*)take(BT * D.G); v.tcodeV = (uint8_t*)take(BT * D.G);
   const size_t rows = (size_t)D.B * D.Nq * D.group;
   size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
@@ -225,6 +227,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
     return nullptr;
   }
   cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, st->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(st->V.akey, 0xff, (size_t)st->D.B * st->D.T * 8, st->stream);
   if (e == cudaSuccess && has_cb) {
     const size_t cb = (size_t)st->D.B * st->D.G * st->D.C * st->D.sub * 4;
     e = cudaMemcpyAsync(st->V.cbk, cfg->codebook_k, cb, cudaMemcpyDeviceToDevice, st->stream);
@@ -285,6 +288,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   F.n_act0 = st->n_act;
   F.n_fill = F.evicted ? (D.K - st->n_act < D.T ? D.K - st->n_act : D.T) : 0;
   F.n_act = st->n_act + F.n_fill;
+  F.keys = st->use_tc_assign ? 1 : 0;
   int nl = 0;
   if (F.evicted) {
     if (F.n_fill > 0) {
@@ -294,7 +298,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
     if (D.T - F.n_fill > 0) {
       {
         StageTimer tm(st, PROTOKV_STAGE_SCORE);
-        nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->maps, st->stream)      // U3
+        nl += st->use_tc_assign ? launch_score_tc(D, st->H, st->V, F, st->maps, st->sm_count, st->stream)      // U3
                                 : launch_score_simt(D, st->H, st->V, F, st->stream);
       }
       StageTimer tm(st, PROTOKV_STAGE_UPDATE);

@@ -1,15 +1,21 @@
 // U3 assignment on the 5th-gen tensor cores (bf16 inputs, d = 128): the tokens x prototypes x head_dim contraction of
-// Eq. 1 as tcgen05.mma tiles fed by TMA, with the rest of Eq. 1 (cosine normalisation, Mahalanobis
-// spatial term, idle penalty) and the argmin fused into the epilogue that drains TMEM.  See DESIGN.md "Kernels".
+// Eq. 1 as tcgen05.mma tiles fed by TMA, with the rest of Eq. 1 (Mahalanobis spatial term, idle
+// penalty) and the argmin fused into the epilogue that drains TMEM.  See DESIGN.md "Kernels".
 //
-// Exactness: the evicted keys are bf16 already; the fp32 centres are split c = c_hi + c_lo (two bf16 terms, kept as
-// shadows by the update kernel), and both products accumulate into the same fp32 TMEM tile, so the dot product
-// carries ~2^-17 relative error of |c| instead of bf16's 2^-9 -- below north_star's 1e-5 gap rule.
+// Exactness: the evicted keys are bf16 already; the fp32 centres are normalised and split c/|c| = hi + lo (two bf16
+// terms, kept as shadows by the update kernel); both products accumulate into the same fp32 TMEM tile, so the
+// accumulator is |K_j| cos(K_j, c_k) with ~2^-17 relative error instead of bf16's 2^-9 -- below north_star's 1e-5 gap
+// rule.  The epilogue minimises |K_j| * score = |K_j| (lambda_sp d_Mah + lambda_idle [idle]) - acc, which has the same
+// argmin as Eq. 1 (|K_j| > 0 is constant along a row) and needs no per-column normalisation.
 //
-// CTA = (token tile of 128, bank); 6 warps: warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer,
-// warps 2-5 = epilogue (one TMEM lane quarter each; thread <-> token row).  Prototypes stream through shared
-// memory in chunks of 128 (hi and lo, 64 KB per stage, 2 stages); accumulators are double-buffered in TMEM
-// (2 x 128 columns) so the MMAs of chunk i+1 overlap the epilogue of chunk i.
+// Persistent kernel, one CTA per SM.  Work unit = (bank, pair of 128-token M tiles, chunk of 64 prototypes); the unit
+// list is cut into gridDim.x contiguous spans, so consecutive units of a CTA share the token tiles (A operand, loaded
+// once per (bank, pair)).  18 warps: warp 0 = TMA producer, warp 1 = TMEM owner + MMA issuer, warps 2-17 = epilogue in
+// two groups of 8 (group = unit parity; warp = (M tile, TMEM lane quarter); thread <-> token row).  Prototype chunks
+// (hi and lo, 32 KB) and their Eq. 1 records (2 KB) stream through 4-stage rings; accumulators rotate through
+// 4 x 128 TMEM columns, so the MMAs run up to 4 units ahead of the epilogue.  Each thread keeps the running argmin of
+// its row over the units it sees and merges it into akey[bank][token] with a 64-bit atomicMin on
+// (orderable(score) << 32 | k): lowest score first, lowest index on ties, whatever CTA / group saw the chunk.
 #include "common.cuh"
 #include "tc_common.cuh"
 
@@ -17,54 +23,106 @@ namespace pkv {
 
 using namespace tc;
 
-constexpr int kTcM = 128;        // tokens per CTA tile (UMMA M)
-constexpr int kTcN = 128;        // prototypes per chunk (UMMA N)
-constexpr int kTcStages = 2;
-constexpr int kTcThreads = 192;
-constexpr uint32_t kHalfTile = 128 * 64 * 2;           // one [128 rows][64 bf16] swizzled box = 16 KB
-constexpr uint32_t kStageBytes = 4 * kHalfTile;        // c_hi (2 K-halves) + c_lo (2 K-halves)
+constexpr int kUN = 64;                                  // prototypes per unit (UMMA N)
+constexpr int kRing = 4;                                 // B stages = rec slots = TMEM buffers
+constexpr int kAsThreads = 18 * 32;
+constexpr uint32_t kAHalf = 128 * 128;                   // [128 rows][64 bf16] swizzled box = 16 KB
+constexpr uint32_t kBHalf = kUN * 128;                   // [64 rows][64 bf16] = 8 KB
+constexpr uint32_t kBStage = 4 * kBHalf;                 // hi (2 K-halves) + lo (2 K-halves) = 32 KB
+constexpr uint32_t kRecBytes = kUN * sizeof(ScoreRec);   // 2 KB
 
-struct __align__(16) EpiRec {   // transformed ScoreRec, 32 bytes: two LDS.128 per prototype column
-  float ninvc, mux, muy, u;
-  float v, w, idle, pad;
+struct AsSmem {   // byte offsets from a 1024-byte aligned base
+  static constexpr uint32_t A = 0;                                  // 2 tiles x 2 K-halves x 16 KB
+  static constexpr uint32_t Bst = A + 4 * kAHalf;                   // kRing x 32 KB
+  static constexpr uint32_t Rec = Bst + kRing * kBStage;            // kRing x 2 KB
+  static constexpr uint32_t Bar = Rec + kRing * kRecBytes;
+  static constexpr uint32_t Total = Bar + 256;
 };
 
-struct TcAssignSmem {
-  // offsets from a 1024-byte aligned base
-  static constexpr uint32_t A = 0;                                   // 2 x 16 KB token tile (K-halves)
-  static constexpr uint32_t Bst = A + 2 * kHalfTile;                 // stages x 64 KB
-  static constexpr uint32_t Rec = Bst + kTcStages * kStageBytes;     // 2 x 128 x 32 B
-  static constexpr uint32_t Bar = Rec + 2 * kTcN * sizeof(EpiRec);   // barriers
-  static constexpr uint32_t Total = Bar + 128;
+struct AsPlan {
+  int NP;        // token-tile pairs per bank
+  int NC;        // prototype chunks per bank
+  int units;     // B * NP * NC
+  int ntok;      // scored tokens per bank (T - n_fill)
 };
 
-__global__ void __launch_bounds__(kTcThreads, 1)
+struct AsUnit { int b, mp, nc, akey, ntiles; };
+
+__device__ __forceinline__ AsUnit as_unit(const AsPlan& P, int u) {
+  AsUnit x;
+  x.nc = u % P.NC;
+  x.akey = u / P.NC;
+  x.mp = x.akey % P.NP;
+  x.b = x.akey / P.NP;
+  x.ntiles = (P.ntok - x.mp * 256) > 128 ? 2 : 1;
+  return x;
+}
+
+__device__ __forceinline__ uint32_t orderable(float f) {
+  const uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+// One row's scan over the (up to) 64 accumulator columns of a unit: rest of Eq. 1 + running argmin.
+template <bool SQUARED, bool RAGGED>
+__device__ __forceinline__ void as_scan(uint32_t taddr, const float4* rc, int ncol, float sx, float sy, float nk,
+                                        float thr, float lam_idle, float& ub, int& ucol) {
+#pragma unroll
+  for (int c0 = 0; c0 < kUN; c0 += 32) {
+    if (!RAGGED || c0 < ncol) {
+      uint32_t acc[32];
+      tmem_ld_32x32(taddr + c0, acc);
+      tmem_ld_wait();
+#pragma unroll
+      for (int c = 0; c < 32; ++c) {
+        const float4 r0 = rc[(c0 + c) * 2];            // mux, muy, u, w
+        const float2 r1 = *reinterpret_cast<const float2*>(&rc[(c0 + c) * 2 + 1]);   // v, tauf
+        const float dx = sx - r0.x, dy = sy - r0.y;
+        const float y1 = dx * r0.z;
+        const float y2 = fmaf(dy, r1.x, -(dx * r0.w));
+        const float qq = fmaf(y1, y1, y2 * y2);
+        float sp;
+        if (SQUARED) sp = qq;
+        else asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sp) : "f"(qq));
+        const float ee = fmaf(lam_idle, __saturatef(thr - r1.y), sp);
+        float sc = fmaf(nk, ee, -__uint_as_float(acc[c]));
+        if (RAGGED && c0 + c >= ncol) sc = INFINITY;
+        if (sc < ub) { ub = sc; ucol = c0 + c; }       // increasing k: lowest index on ties
+      }
+    }
+  }
+}
+
+template <bool SQUARED>
+__global__ void __launch_bounds__(kAsThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmChi,
-                const __grid_constant__ CUtensorMap tmClo, Dims D, Hyper H, Dev V, FrameArgs F) {
+                const __grid_constant__ CUtensorMap tmClo, Dims D, Hyper H, Dev V, FrameArgs F, AsPlan P) {
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* sm = (unsigned char*)(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
-  uint64_t* bars = (uint64_t*)(sm + TcAssignSmem::Bar);
+  uint64_t* bars = (uint64_t*)(sm + AsSmem::Bar);
   uint64_t* a_full = bars + 0;
-  uint64_t* full = bars + 1;                  // [stages]
-  uint64_t* empty = full + kTcStages;         // [stages]
-  uint64_t* tfull = empty + kTcStages;        // [2]
-  uint64_t* tempty = tfull + 2;               // [2]
-  uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
-  EpiRec* recs = (EpiRec*)(sm + TcAssignSmem::Rec);
+  uint64_t* a_empty = bars + 1;
+  uint64_t* b_full = bars + 2;                 // [kRing]
+  uint64_t* b_empty = b_full + kRing;
+  uint64_t* r_full = b_empty + kRing;
+  uint64_t* t_full = r_full + kRing;
+  uint64_t* t_empty = t_full + kRing;
+  uint32_t* tmem_slot = (uint32_t*)(t_empty + kRing);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int b = blockIdx.y;
-  const int j0 = F.n_fill + blockIdx.x * kTcM;          // first token of this tile
-  const int nchunks = (F.n_act + kTcN - 1) / kTcN;
+  const int u0 = (int)(((long long)blockIdx.x * P.units) / gridDim.x);
+  const int u1 = (int)(((long long)(blockIdx.x + 1) * P.units) / gridDim.x);
 
   if (threadIdx.x == 0) {
     prefetch_tmap(&tmK); prefetch_tmap(&tmChi); prefetch_tmap(&tmClo);
-    mbar_init(a_full, 1);
-    for (int s = 0; s < kTcStages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 128); }
+    mbar_init(a_full, 1); mbar_init(a_empty, 1);
+    for (int s = 0; s < kRing; ++s) {
+      mbar_init(b_full + s, 1); mbar_init(b_empty + s, 1); mbar_init(r_full + s, 1);
+      mbar_init(t_full + s, 1); mbar_init(t_empty + s, 8);
+    }
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(tmem_slot, 256);
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
@@ -73,141 +131,128 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
   if (warp == 0) {
     // ===== TMA producer =====
     if (lane == 0) {
-      const int row0 = (b * D.Wf + F.slot) * D.T + j0;
-      mbar_arrive_expect_tx(a_full, 2 * kHalfTile);
-      tma_load_2d(sm + TcAssignSmem::A, &tmK, 0, row0, a_full);
-      tma_load_2d(sm + TcAssignSmem::A + kHalfTile, &tmK, 64, row0, a_full);
-      for (int c = 0; c < nchunks; ++c) {
-        const int s = c % kTcStages, ph = (c / kTcStages) & 1;
-        mbar_wait(empty + s, ph ^ 1);
-        unsigned char* dst = sm + TcAssignSmem::Bst + s * kStageBytes;
-        const int prow = b * D.K + c * kTcN;
-        mbar_arrive_expect_tx(full + s, kStageBytes);
-        tma_load_2d(dst, &tmChi, 0, prow, full + s);
-        tma_load_2d(dst + kHalfTile, &tmChi, 64, prow, full + s);
-        tma_load_2d(dst + 2 * kHalfTile, &tmClo, 0, prow, full + s);
-        tma_load_2d(dst + 3 * kHalfTile, &tmClo, 64, prow, full + s);
+      int prev = -1, acnt = 0;
+      for (int u = u0; u < u1; ++u) {
+        const AsUnit x = as_unit(P, u);
+        const int i = u - u0, s = i % kRing;
+        const uint32_t par = ((i / kRing) & 1) ^ 1;
+        if (x.akey != prev) {
+          mbar_wait(a_empty, (acnt & 1) ^ 1);
+          const int row0 = (x.b * D.Wf + F.slot) * D.T + F.n_fill + x.mp * 256;
+          mbar_arrive_expect_tx(a_full, (uint32_t)x.ntiles * 2 * kAHalf);
+          for (int t = 0; t < x.ntiles; ++t) {
+            tma_load_2d(sm + AsSmem::A + (t * 2) * kAHalf, &tmK, 0, row0 + t * 128, a_full);
+            tma_load_2d(sm + AsSmem::A + (t * 2 + 1) * kAHalf, &tmK, 64, row0 + t * 128, a_full);
+          }
+          prev = x.akey; ++acnt;
+        }
+        const int prow = x.b * D.K + x.nc * kUN;
+        unsigned char* dst = sm + AsSmem::Bst + s * kBStage;
+        mbar_wait(b_empty + s, par);
+        mbar_arrive_expect_tx(b_full + s, kBStage);
+        tma_load_2d(dst, &tmChi, 0, prow, b_full + s);
+        tma_load_2d(dst + kBHalf, &tmChi, 64, prow, b_full + s);
+        tma_load_2d(dst + 2 * kBHalf, &tmClo, 0, prow, b_full + s);
+        tma_load_2d(dst + 3 * kBHalf, &tmClo, 64, prow, b_full + s);
+        mbar_wait(t_empty + s, par);                 // the epilogue of unit i - kRing has read this record slot
+        const int nrec = min(kUN, D.K - x.nc * kUN);
+        mbar_arrive_expect_tx(r_full + s, (uint32_t)nrec * sizeof(ScoreRec));
+        bulk_load_1d(sm + AsSmem::Rec + s * kRecBytes, V.rec + (size_t)prow, (uint32_t)nrec * sizeof(ScoreRec), r_full + s);
       }
     }
   } else if (warp == 1) {
     // ===== MMA issuer =====
     if (lane == 0) {
-      constexpr uint32_t idesc = idesc_bf16(kTcM, kTcN, 0, 0);
-      const uint32_t a_addr = smem_u32(sm + TcAssignSmem::A);
-      mbar_wait(a_full, 0);
-      for (int c = 0; c < nchunks; ++c) {
-        const int s = c % kTcStages, ph = (c / kTcStages) & 1;
-        const int buf = c & 1, bph = (c >> 1) & 1;
-        mbar_wait(tempty + buf, bph ^ 1);
-        mbar_wait(full + s, ph);
+      constexpr uint32_t idesc = idesc_bf16(128, kUN, 0, 0);
+      const uint32_t a_addr = smem_u32(sm + AsSmem::A);
+      int prev = -1, acnt = 0;
+      for (int u = u0; u < u1; ++u) {
+        const AsUnit x = as_unit(P, u);
+        const int i = u - u0, s = i % kRing;
+        const uint32_t par = (i / kRing) & 1;
+        if (x.akey != prev) { mbar_wait(a_full, acnt & 1); prev = x.akey; ++acnt; }
+        mbar_wait(t_empty + s, par ^ 1);
+        mbar_wait(b_full + s, par);
         tc_fence_after_sync();
-        const uint32_t b_addr = smem_u32(sm + TcAssignSmem::Bst + s * kStageBytes);
-        const uint32_t d_tmem = tmem_base + buf * kTcN;
-        bool acc = false;
+        const uint32_t b_addr = smem_u32(sm + AsSmem::Bst + s * kBStage);
+        for (int t = 0; t < x.ntiles; ++t) {
+          const uint32_t d_tmem = tmem_base + s * 128 + t * kUN;
+          bool acc = false;
 #pragma unroll
-        for (int part = 0; part < 2; ++part) {        // c_hi, c_lo
+          for (int part = 0; part < 2; ++part) {        // hi, lo
 #pragma unroll
-          for (int half = 0; half < 2; ++half) {      // d 0..63, 64..127
+            for (int half = 0; half < 2; ++half) {      // d 0..63, 64..127
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {          // 4 x K=16 inside the 128-byte swizzle atom
-              const uint64_t ad = desc_kmajor_sw128(a_addr + half * kHalfTile + kk * 32);
-              const uint64_t bd = desc_kmajor_sw128(b_addr + (part * 2 + half) * kHalfTile + kk * 32);
-              umma_bf16(d_tmem, ad, bd, idesc, acc);
-              acc = true;
+              for (int kk = 0; kk < 4; ++kk) {          // 4 x K=16 inside the 128-byte swizzle atom
+                const uint64_t ad = desc_kmajor_sw128(a_addr + (t * 2 + half) * kAHalf + kk * 32);
+                const uint64_t bd = desc_kmajor_sw128(b_addr + (part * 2 + half) * kBHalf + kk * 32);
+                umma_bf16(d_tmem, ad, bd, idesc, acc);
+                acc = true;
+              }
             }
           }
         }
-        umma_commit(empty + s);       // smem stage reusable once these MMAs have read it
-        umma_commit(tfull + buf);     // accumulator complete
+        umma_commit(b_empty + s);       // smem stage reusable once these MMAs have read it
+        umma_commit(t_full + s);        // accumulators complete
+        if (u + 1 == u1 || (u + 1) / P.NC != x.akey) umma_commit(a_empty);   // last unit on these token tiles
       }
     }
   } else {
-    // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
-    const int q = warp & 3;
-    const int row = q * 32 + lane;                 // token row in the tile = TMEM lane
-    const int et = (warp - 2) * 32 + lane;         // 0..127 index among the epilogue threads (rec staging)
-    const int j = j0 + row;
-    const int st = b / (D.L * D.Hkv);
-    float sx = 0.f, sy = 0.f;
-    if (j < D.T) {
-      const float* se = V.ringS + (((size_t)st * D.Wf + F.slot) * D.T + j) * 2;
-      sx = se[0]; sy = se[1];
-    }
-    auto load_rec = [&](int c) -> EpiRec {
-      EpiRec e{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-      const int k = c * kTcN + et;
-      if (c < nchunks && k < F.n_act) {
-        const ScoreRec r = V.rec[(size_t)b * D.K + k];
-        e.ninvc = -r.invc; e.mux = r.mux; e.muy = r.muy; e.u = r.u; e.v = r.v; e.w = r.w;
-        e.idle = (F.t - r.tau > H.t_idle) ? H.lambda_idle : 0.f;
-      }
-      return e;
+    // ===== epilogue: 16 warps; group = unit parity, tile = M tile of the pair, q = TMEM lane quarter =====
+    const int e = warp - 2;
+    const int grp = e >> 3, tile = (e >> 2) & 1, q = warp & 3;
+    const int row = tile * 128 + q * 32 + lane;             // token row within the pair
+    const float thr = (float)(F.t - H.t_idle);               // idle <=> tau < t - T_idle  (Eq. 1, reading 2)
+    const float lam_idle = H.lambda_idle;
+    float sx = 0.f, sy = 0.f, nk = 1.f, best = INFINITY;
+    int bidx = 0x7fffffff, j = -1, cur_b = 0, prev = -1;
+    bool valid = false;
+    auto flush = [&]() {
+      if (valid && best < INFINITY)
+        atomicMin(V.akey + (size_t)cur_b * D.T + j, ((unsigned long long)orderable(best) << 32) | (uint32_t)bidx);
     };
-    EpiRec next = load_rec(0);
-    // |K_j|^2 from the swizzled A tile: row r, 16-byte chunk c lives at r*128 + ((c ^ (r & 7)) << 4) in each K-half
-    mbar_wait(a_full, 0);
-    float kk2 = 0.f;
-#pragma unroll
-    for (int half = 0; half < 2; ++half) {
-      const unsigned char* base = sm + TcAssignSmem::A + half * kHalfTile + row * 128;
-#pragma unroll
-      for (int ch = 0; ch < 8; ++ch) {
-        const uint4 w = *(const uint4*)(base + ((ch ^ (row & 7)) << 4));
-        const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const float lo = __uint_as_float(ww[e] << 16), hi = __uint_as_float(ww[e] & 0xffff0000u);
-          kk2 = fmaf(lo, lo, kk2); kk2 = fmaf(hi, hi, kk2);
+    for (int u = u0 + grp; u < u1; u += 2) {
+      const AsUnit x = as_unit(P, u);
+      const int i = u - u0, s = i % kRing;
+      const uint32_t par = (i / kRing) & 1;
+      if (x.akey != prev) {
+        flush();
+        prev = x.akey; cur_b = x.b;
+        j = F.n_fill + x.mp * 256 + row;
+        valid = j < D.T;
+        best = INFINITY; bidx = 0x7fffffff;
+        if (valid) {
+          const int st = x.b / (D.L * D.Hkv);
+          const float2 se = *reinterpret_cast<const float2*>(V.ringS + (((size_t)st * D.Wf + F.slot) * D.T + j) * 2);
+          sx = se.x; sy = se.y;
+          const float kk = V.ringN[((size_t)x.b * D.Wf + F.slot) * D.T + j];
+          nk = kk > 0.f ? sqrtf(kk) : 1.f;                   // |K_j| = 0: acc = 0 and Eq. 1 reduces to its other terms
         }
       }
-    }
-    const float invk = kk2 > 0.f ? rsqrtf(kk2) : 0.f;
-    const float ninv_cap = -1.f / H.cos_eps;       // cos = dot / max(|K||c|, cos_eps)  (reading 6)
-    const bool squared = H.flags & PROTOKV_MAH_SQUARED;
-    float best = INFINITY;
-    int bidx = 0x7fffffff;
-    for (int c = 0; c < nchunks; ++c) {
-      const int buf = c & 1, bph = (c >> 1) & 1;
-      recs[buf * kTcN + et] = next;
-      next = load_rec(c + 1);
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      mbar_wait(tfull + buf, bph);
+      mbar_wait(r_full + s, par);
+      mbar_wait(t_full + s, par);
       tc_fence_after_sync();
-      const int nk = min(kTcN, F.n_act - c * kTcN);
-      const EpiRec* rc = recs + buf * kTcN;
-      for (int col0 = 0; col0 < nk; col0 += 32) {
-        uint32_t acc[32];
-        tmem_ld_32x32(tmem_base + ((uint32_t)(q * 32) << 16) + buf * kTcN + col0, acc);
-        tmem_ld_wait();
-        const int lim = min(32, nk - col0);
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          if (i < lim) {
-            const float4 r0 = *(const float4*)&rc[col0 + i].ninvc;
-            const float4 r1 = *(const float4*)&rc[col0 + i].v;
-            const float dx = sx - r0.y, dy = sy - r0.z;
-            const float y1 = dx * r0.w, y2 = fmaf(dy, r1.x, -(dx * r1.y));
-            const float qq = fmaf(y1, y1, y2 * y2);
-            const float sp = squared ? qq : sqrtf(qq);
-            const float ninv = fmaxf(r0.x * invk, ninv_cap);
-            const float sc = fmaf(__uint_as_float(acc[i]), ninv, sp + r1.z);
-            if (sc < best) { best = sc; bidx = c * kTcN + col0 + i; }   // increasing k: lowest index on ties
-          }
-        }
+      if (__any_sync(0xffffffffu, valid)) {
+        const int ncol = min(kUN, F.n_act - x.nc * kUN);
+        const float4* rc = reinterpret_cast<const float4*>(sm + AsSmem::Rec + s * kRecBytes);
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + s * 128 + tile * kUN;
+        float ub = INFINITY;
+        int ucol = 0;
+        if (ncol == kUN) as_scan<SQUARED, false>(taddr, rc, ncol, sx, sy, nk, thr, lam_idle, ub, ucol);
+        else as_scan<SQUARED, true>(taddr, rc, ncol, sx, sy, nk, thr, lam_idle, ub, ucol);
+        if (ub < best) { best = ub; bidx = x.nc * kUN + ucol; }
       }
       tc_fence_before_sync();
-      mbar_arrive(tempty + buf);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(t_empty + s);
     }
-    if (j < D.T) {
-      V.assign[(size_t)b * D.T + j] = bidx;
-      V.best[(size_t)b * D.T + j] = best;
-    }
+    flush();
   }
   tc_fence_before_sync();
   __syncthreads();
   if (warp == 1) {
     tc_fence_after_sync();
-    tmem_dealloc(tmem_base, 256);
+    tmem_dealloc(tmem_base, 512);
   }
 }
 
@@ -274,22 +319,31 @@ bool tc_build_maps(const Dims& D, const Dev& V, TcMaps* maps) {
   const uint64_t ring_rows = (uint64_t)D.B * D.Wf * D.T, bank_rows = (uint64_t)D.B * D.K;
   maps->ok = make_tmap_2d_bf16(&maps->ringK, V.ringK, ring_rows, 128, 128, 64) &&
              make_tmap_2d_bf16(&maps->ringV, V.ringV, ring_rows, 128, 128, 64) &&
-             make_tmap_2d_bf16(&maps->c_hi, V.c_hi, bank_rows, 128, 128, 64) &&
-             make_tmap_2d_bf16(&maps->c_lo, V.c_lo, bank_rows, 128, 128, 64);
+             make_tmap_2d_bf16(&maps->c_hi, V.c_hi, bank_rows, 128, kUN, 64) &&
+             make_tmap_2d_bf16(&maps->c_lo, V.c_lo, bank_rows, 128, kUN, 64);
   if (maps->ok) {
-    const cudaError_t e = cudaFuncSetAttribute(score_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                               (int)TcAssignSmem::Total + 1024);
+    cudaError_t e = cudaFuncSetAttribute(score_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)AsSmem::Total + 1024);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(score_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AsSmem::Total + 1024);
     if (e != cudaSuccess) { cudaGetLastError(); maps->ok = false; }
   }
   return maps->ok;
 }
 
 int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, const TcMaps& maps,
-                    cudaStream_t s) {
-  const int ntok = D.T - F.n_fill;
-  if (ntok <= 0) return 0;
-  dim3 grid((ntok + kTcM - 1) / kTcM, D.B);
-  score_tc_kernel<<<grid, kTcThreads, TcAssignSmem::Total + 1024, s>>>(maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F);
+                    int sm_count, cudaStream_t s) {
+  AsPlan P{};
+  P.ntok = D.T - F.n_fill;
+  if (P.ntok <= 0 || F.n_act <= 0) return 0;
+  P.NP = (P.ntok + 255) / 256;
+  P.NC = (F.n_act + kUN - 1) / kUN;
+  P.units = D.B * P.NP * P.NC;
+  const int grid = P.units < sm_count ? P.units : sm_count;
+  if (H.flags & PROTOKV_MAH_SQUARED)
+    score_tc_kernel<true><<<grid, kAsThreads, AsSmem::Total + 1024, s>>>(maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
+  else
+    score_tc_kernel<false><<<grid, kAsThreads, AsSmem::Total + 1024, s>>>(maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
   return 1;
 }
 

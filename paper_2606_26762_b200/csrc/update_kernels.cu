@@ -7,10 +7,11 @@ namespace pkv {
 
 // Token-independent part of Eq. 1 for one prototype.  Sigma + eps I = R R^T (Cholesky),
 // d_Mah^2 = |R^-1 delta|^2 = (dx/r11)^2 + ((dy - r21 dx/r11)/r22)^2.  Evaluated in fp64 from the fp32 state.
+__device__ __forceinline__ float inv_norm(float cc);
 __device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, float sxx, float sxy, float syy, int tau,
                                              const Hyper& H) {
   ScoreRec r;
-  r.invc = cc > 0.f ? (float)(1.0 / sqrt((double)cc)) : 0.f;
+  r.invc = inv_norm(cc);
   r.mux = mux; r.muy = muy;
   double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
   double r11 = sqrt(a);
@@ -23,7 +24,7 @@ __device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, flo
   r.v = (float)(lam / r22);
   r.w = (float)(lam * r21 / (r11 * r22));
   r.tau = tau;
-  r.pad = 0;
+  r.tauf = (float)tau;
   return r;
 }
 
@@ -32,14 +33,22 @@ __device__ __forceinline__ void split_bf16(float x, __nv_bfloat16& hi, __nv_bflo
   lo = __float2bfloat16_rn(x - __bfloat162float(hi));
 }
 
+__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)(1.0 / sqrt((double)cc)) : 0.f; }
+
+// bf16 shadows of the NORMALISED key centre c / |c| = hi + lo (+ O(2^-17)): the tcgen05 assignment contracts the
+// evicted keys with these, so its accumulator is |K_j| cos(K_j, c_k) and Eq. 1 needs no per-column scale.
 template <int VEC>
-__device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const float (&c)[VEC]) {
+__device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const float (&c)[VEC], float invc) {
   if (!V.c_hi) return;
+  __nv_bfloat16 hi[VEC], lo[VEC];
 #pragma unroll
-  for (int v = 0; v < VEC; ++v) {
-    __nv_bfloat16 hi, lo;
-    split_bf16(c[v], hi, lo);
-    V.c_hi[off + v] = hi; V.c_lo[off + v] = lo;
+  for (int v = 0; v < VEC; ++v) split_bf16(c[v] * invc, hi[v], lo[v]);
+  if (VEC == 4) {
+    *reinterpret_cast<uint2*>(V.c_hi + off) = *reinterpret_cast<const uint2*>(hi);
+    *reinterpret_cast<uint2*>(V.c_lo + off) = *reinterpret_cast<const uint2*>(lo);
+  } else {
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) { V.c_hi[off + v] = hi[v]; V.c_lo[off + v] = lo[v]; }
   }
 }
 
@@ -48,25 +57,47 @@ __device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const fl
 // [stream][layer][T][Hkv][d] to the bank-major ring [bank][Wf][T][d].  16-byte vectors, one per thread.
 // grid.y = 0: K, 1: V.  The first threads of grid.y == 0 also copy grid_pos.
 // ---------------------------------------------------------------------------------------------------------
+template <bool BF16>
 __global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slot, const uint4* __restrict__ Kin,
                                                           const uint4* __restrict__ Vin,
                                                           const float* __restrict__ grid_pos, int vpr) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   const size_t total = (size_t)D.B * D.T * vpr;
-  if (blockIdx.y == 0 && idx < (size_t)D.NS * D.T * 2) {
-    const int st = (int)(idx / (D.T * 2)), e = (int)(idx % (D.T * 2));
-    V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[idx];
+  if (blockIdx.y == 0) {
+    if (idx < (size_t)D.NS * D.T * 2) {
+      const int st = (int)(idx / (D.T * 2)), e = (int)(idx % (D.T * 2));
+      V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[idx];
+    }
+    if (idx < (size_t)D.B * D.T) V.akey[idx] = ~0ull;      // next frame's assignment keys (see tc_assign.cu)
   }
-  if (idx >= total) return;
-  const int v = (int)(idx % vpr);
-  const int j = (int)((idx / vpr) % D.T);
-  const int b = (int)(idx / ((size_t)vpr * D.T));
+  const bool valid = idx < total;                          // total is a multiple of vpr: whole rows are valid or not
+  const size_t id = valid ? idx : 0;
+  const int v = (int)(id % vpr);
+  const int j = (int)((id / vpr) % D.T);
+  const int b = (int)(id / ((size_t)vpr * D.T));
   const int hd = b % D.Hkv, sl = b / D.Hkv;  // sl = stream * L + layer
   const size_t src = (((size_t)sl * D.T + j) * D.Hkv + hd) * vpr + v;
-  const size_t dst = (((size_t)b * D.Wf + slot) * D.T + j) * vpr + v;
+  const size_t row = ((size_t)b * D.Wf + slot) * D.T + j;
   const uint4* in = blockIdx.y ? Vin : Kin;
   uint4* out = (uint4*)(blockIdx.y ? V.ringV : V.ringK);
-  out[dst] = in[src];
+  const uint4 w = in[src];
+  if (valid) out[row * vpr + v] = w;
+  if (blockIdx.y == 0) {                                   // |K_j|^2, reduced over the vpr lanes that hold the row
+    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+    float kk = 0.f;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      if (BF16) {
+        const float lo = __uint_as_float(ww[e] << 16), hi = __uint_as_float(ww[e] & 0xffff0000u);
+        kk = fmaf(lo, lo, kk); kk = fmaf(hi, hi, kk);
+      } else {
+        const float x = __uint_as_float(ww[e]);
+        kk = fmaf(x, x, kk);
+      }
+    }
+    for (int o = vpr >> 1; o > 0; o >>= 1) kk += __shfl_xor_sync(0xffffffffu, kk, o);
+    if (valid && v == 0) V.ringN[row] = kk;
+  }
 }
 
 int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const void* Kin, const void* Vin,
@@ -74,7 +105,8 @@ int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const vo
   const int vpr = D.d * (D.bf16 ? 2 : 4) / 16;
   const size_t total = (size_t)D.B * D.T * vpr;
   dim3 grid((unsigned)((total + 255) / 256), 2);
-  ring_append_kernel<<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
+  if (D.bf16) ring_append_kernel<true><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
+  else ring_append_kernel<false><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
   return 1;
 }
 
@@ -95,14 +127,17 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     float kf = to_f32(Ke[i]), vf = to_f32(Ve[i]);
     V.c[pk * D.d + i] = kf;
     V.p[pk * D.d + i] = vf;
-    if (V.c_hi) {
-      __nv_bfloat16 hi, lo;
-      split_bf16(kf, hi, lo);
-      V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
-    }
     cc += kf * kf;
   }
   cc = warp_sum(cc);
+  if (V.c_hi) {
+    const float invc = inv_norm(cc);
+    for (int i = lane; i < D.d; i += 32) {
+      __nv_bfloat16 hi, lo;
+      split_bf16(to_f32(Ke[i]) * invc, hi, lo);
+      V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
+    }
+  }
   const int ghc = 2 * D.G * D.C;
   for (int i = lane; i < ghc; i += 32) V.hist[pk * ghc + i] = 0u;
   if (lane == 0) {
@@ -286,7 +321,25 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
   const bool has_cb = V.cbk != nullptr;
   for (int i = tid; i < P; i += kUpdThreads) {
     const int j = F.n_fill + i;
-    keys[i] = i < ntok ? (((uint32_t)V.assign[(size_t)b * D.T + j] << 12) | (uint32_t)j) : 0xffffffffu;
+    uint32_t key = 0xffffffffu;
+    if (i < ntok) {
+      int a;
+      if (F.keys) {   // tcgen05 assignment: (orderable(|K_j| * score) << 32 | k), see tc_assign.cu
+        const unsigned long long ak = V.akey[(size_t)b * D.T + j];
+        a = (int)(uint32_t)ak;
+        if (blockIdx.x == 0) {
+          const uint32_t o = (uint32_t)(ak >> 32);
+          const float sc = __uint_as_float((o & 0x80000000u) ? (o ^ 0x80000000u) : ~o);
+          const float kk = V.ringN[((size_t)b * D.Wf + F.slot) * D.T + j];
+          V.assign[(size_t)b * D.T + j] = a;
+          V.best[(size_t)b * D.T + j] = kk > 0.f ? sc / sqrtf(kk) : sc;
+        }
+      } else {
+        a = V.assign[(size_t)b * D.T + j];
+      }
+      key = ((uint32_t)a << 12) | (uint32_t)j;
+    }
+    keys[i] = key;
   }
   if (has_cb) {
     const int per_g = D.C * D.sub;
@@ -382,11 +435,11 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       *(float2*)(V.c + pk * DH + lane * 2) = make_float2(c[0], c[1]);
       *(float2*)(V.p + pk * DH + lane * 2) = make_float2(p[0], p[1]);
     }
-    store_shadows<VEC>(V, pk * DH + lane * VEC, c);
     float cc = 0.f;
 #pragma unroll
     for (int v = 0; v < VEC; ++v) cc = fmaf(c[v], c[v], cc);
     cc = warp_sum(cc);
+    store_shadows<VEC>(V, pk * DH + lane * VEC, c, inv_norm(cc));
     if (lane == 0) {
       V.n[pk] = n;
       V.tau[pk] = F.t;
@@ -434,16 +487,19 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
   float cc = 0.f;
   const int vec = D.d / 32;   // same per-lane order as update_kernel so that derived values are reproduced bit for bit
   for (int v = 0; v < vec; ++v) {
-    const int i = lane * vec + v;
-    const float x = V.c[pk * D.d + i];
+    const float x = V.c[pk * D.d + lane * vec + v];
     cc = fmaf(x, x, cc);
-    if (V.c_hi) {
+  }
+  cc = warp_sum(cc);
+  if (V.c_hi) {
+    const float invc = inv_norm(cc);
+    for (int v = 0; v < vec; ++v) {
+      const int i = lane * vec + v;
       __nv_bfloat16 hi, lo;
-      split_bf16(x, hi, lo);
+      split_bf16(V.c[pk * D.d + i] * invc, hi, lo);
       V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
     }
   }
-  cc = warp_sum(cc);
   if (lane == 0) {
     V.rec[pk] = make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
                          V.sigma[pk * 3 + 2], V.tau[pk], H);
