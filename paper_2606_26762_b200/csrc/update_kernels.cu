@@ -13,16 +13,16 @@ __device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, flo
   ScoreRec r;
   r.invc = inv_norm(cc);
   r.mux = mux; r.muy = muy;
-  double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
-  double r11 = sqrt(a);
-  double r21 = b / r11;
-  double t = e - r21 * r21;
-  double r22 = sqrt(t > 0.0 ? t : 0.0);
+  const double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
+  const double i11 = rsqrt(a);                 // 1 / r11
+  const double r21 = b * i11;
+  const double t = e - r21 * r21;              // r22^2
+  const double i22 = t > 0.0 ? rsqrt(t) : (double)INFINITY;
   // lambda_sp * d_Mah = sqrt(q) with factors scaled by lambda_sp; for MAH_SQUARED scale by sqrt(lambda_sp).
-  double lam = (H.flags & PROTOKV_MAH_SQUARED) ? sqrt((double)H.lambda_sp) : (double)H.lambda_sp;
-  r.u = (float)(lam / r11);
-  r.v = (float)(lam / r22);
-  r.w = (float)(lam * r21 / (r11 * r22));
+  const double lam = (H.flags & PROTOKV_MAH_SQUARED) ? sqrt((double)H.lambda_sp) : (double)H.lambda_sp;
+  r.u = (float)(lam * i11);
+  r.v = (float)(lam * i22);
+  r.w = (float)(lam * r21 * i11 * i22);
   r.tau = tau;
   r.tauf = (float)tau;
   return r;
@@ -33,7 +33,7 @@ __device__ __forceinline__ void split_bf16(float x, __nv_bfloat16& hi, __nv_bflo
   lo = __float2bfloat16_rn(x - __bfloat162float(hi));
 }
 
-__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)(1.0 / sqrt((double)cc)) : 0.f; }
+__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)rsqrt((double)cc) : 0.f; }
 
 // bf16 shadows of the NORMALISED key centre c / |c| = hi + lo (+ O(2^-17)): the tcgen05 assignment contracts the
 // evicted keys with these, so its accumulator is |K_j| cos(K_j, c_k) and Eq. 1 needs no per-column scale.
@@ -453,11 +453,236 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// U4-U6, specialised for the production shape (head_dim 128, G = 8, C = 16; bf16 or fp32 tokens).
+//
+// CTA = (split, bank), 8 warps.  Every CTA of a bank orders the bank's (k*, j) keys by rank counting (key distinct,
+// rank = number of smaller keys: T^2 broadcast compares instead of a bitonic network), marks segment heads, scans
+// them into a segment table, and the warps of all CTAs of the bank take segments round-robin.  A warp owns one
+// prototype (4 dims per lane, so the 4 lanes [4g, 4g+4) hold PQ subspace g) and replays Alg. 1 l.8-13 over its tokens
+// in eviction order with the next token's K/V prefetched.  PQ search: the residual is exchanged through a per-warp
+// shared scratch so that every lane holds its subspace's 16 dims, lane (g, li) evaluates codewords li, li+4, li+8,
+// li+12 in full (no shuffles inside the distance), and a 2-step lexicographic (distance, code) min over the 4 lanes
+// picks the codeword.  Codebooks sit in shared memory as [g][q][z] float4 with a 4-unit pad per g: the 8 lanes of a
+// quarter warp then read 8 distinct 16-byte bank groups.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kUfThreads = 256, kUfWarps = kUfThreads / 32;
+constexpr int kCbG = 68;   // float4 units per subspace block: 4 q x 16 z + 4 pad
+
+__device__ __forceinline__ void pq_pick(const float4* __restrict__ cb4, const float4* __restrict__ rsc, int g, int li,
+                                        int& code) {
+  float4 r[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) r[q] = rsc[g * 4 + q];
+  float bestd = INFINITY;
+  int bz = 0;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const int z = li + 4 * t;
+    float dist = 0.f;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const float4 cw = cb4[g * kCbG + q * 16 + z];
+      float e;
+      e = r[q].x - cw.x; dist = fmaf(e, e, dist);
+      e = r[q].y - cw.y; dist = fmaf(e, e, dist);
+      e = r[q].z - cw.z; dist = fmaf(e, e, dist);
+      e = r[q].w - cw.w; dist = fmaf(e, e, dist);
+    }
+    if (dist < bestd) { bestd = dist; bz = z; }           // increasing z within the lane: lowest z on ties
+  }
+#pragma unroll
+  for (int o = 1; o <= 2; o <<= 1) {
+    const float od = __shfl_xor_sync(0xffffffffu, bestd, o);
+    const int oz = __shfl_xor_sync(0xffffffffu, bz, o);
+    if (od < bestd || (od == bestd && oz < bz)) { bestd = od; bz = oz; }
+  }
+  code = bz;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hyper H, Dev V, FrameArgs F, int Tpad) {
+  constexpr int DH = 128;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* cbk4 = (float4*)smem_raw;                           // [8][68]
+  float4* cbv4 = cbk4 + 8 * kCbG;
+  float4* scratch = cbv4 + 8 * kCbG;                          // [warps][2][32]
+  uint32_t* keys = (uint32_t*)(scratch + kUfWarps * 64);      // [Tpad]
+  uint32_t* sorted = keys + Tpad;                             // [Tpad]
+  int* segstart = (int*)(sorted + Tpad);                      // [Tpad + 1]
+  __shared__ int wtot[kUfWarps];
+  __shared__ int nseg_s;
+
+  const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int ntok = D.T - F.n_fill;
+  const bool has_cb = V.cbk != nullptr;
+  const size_t bt = (size_t)b * D.T;
+  const size_t rrow = ((size_t)b * D.Wf + F.slot) * D.T;      // ring row of evicted token 0
+  for (int i = tid; i < ntok; i += kUfThreads) {
+    const int j = F.n_fill + i;
+    int a;
+    if (F.keys) {   // tcgen05 assignment: (orderable(|K_j| * score) << 32 | k), see tc_assign.cu
+      const unsigned long long ak = V.akey[bt + j];
+      a = (int)(uint32_t)ak;
+      if (blockIdx.x == 0) {
+        const uint32_t o = (uint32_t)(ak >> 32);
+        const float sc = __uint_as_float((o & 0x80000000u) ? (o ^ 0x80000000u) : ~o);
+        const float kk = V.ringN[rrow + j];
+        V.assign[bt + j] = a;
+        V.best[bt + j] = kk > 0.f ? sc / sqrtf(kk) : sc;
+      }
+    } else {
+      a = V.assign[bt + j];
+    }
+    keys[i] = ((uint32_t)a << 12) | (uint32_t)j;
+  }
+  if (has_cb) {
+    const float4* sk = (const float4*)(V.cbk + (size_t)b * 2048);
+    const float4* sv = (const float4*)(V.cbv + (size_t)b * 2048);
+    for (int e = tid; e < 512; e += kUfThreads) {             // e = (g * 16 + z) * 4 + q
+      const int q = e & 3, z = (e >> 2) & 15, g = e >> 6;
+      cbk4[g * kCbG + q * 16 + z] = sk[e];
+      cbv4[g * kCbG + q * 16 + z] = sv[e];
+    }
+  }
+  __syncthreads();
+  // ---- U4: rank counting sort, segment heads, segment table ----
+  for (int i = tid; i < ntok; i += kUfThreads) {
+    const uint32_t my = keys[i];
+    int r = 0;
+    int i2 = 0;
+    for (; i2 + 4 <= ntok; i2 += 4) {
+      const uint4 kq = *(const uint4*)(keys + i2);
+      r += (kq.x < my) + (kq.y < my) + (kq.z < my) + (kq.w < my);
+    }
+    for (; i2 < ntok; ++i2) r += keys[i2] < my;
+    sorted[r] = my;
+  }
+  __syncthreads();
+  int base = 0;
+  for (int r0 = 0; r0 < ntok; r0 += kUfThreads) {
+    const int r = r0 + tid;
+    const bool head = r < ntok && (r == 0 || (sorted[r] >> 12) != (sorted[r - 1] >> 12));
+    const uint32_t bal = __ballot_sync(0xffffffffu, head);
+    if (lane == 0) wtot[warp] = __popc(bal);
+    __syncthreads();
+    int off = base, tot = 0;
+#pragma unroll
+    for (int w = 0; w < kUfWarps; ++w) { const int c = wtot[w]; if (w < warp) off += c; tot += c; }
+    if (head) segstart[off + __popc(bal & ((1u << lane) - 1u))] = r;
+    base += tot;
+    __syncthreads();
+  }
+  if (tid == 0) { segstart[base] = ntok; nseg_s = base; }
+  __syncthreads();
+  const int nseg = nseg_s;
+
+  // ---- U5 / U6 ----
+  const int st = b / (D.L * D.Hkv);
+  const T* ringK = (const T*)V.ringK + rrow * DH;
+  const T* ringV = (const T*)V.ringV + rrow * DH;
+  const float* ringS = V.ringS + ((size_t)st * D.Wf + F.slot) * D.T * 2;
+  const double al = (double)H.alpha, be = (double)H.beta, et = (double)H.eta;
+  const double oma = 1.0 - al, omb = 1.0 - be, ome = 1.0 - et;
+  const int g = lane >> 2, li = lane & 3;
+  float4* rsc = scratch + warp * 64;
+
+  for (int seg = blockIdx.x * kUfWarps + warp; seg < nseg; seg += gridDim.x * kUfWarps) {
+    const int r0 = segstart[seg], r1 = segstart[seg + 1];
+    const int k = (int)(sorted[r0] >> 12);
+    const size_t pk = (size_t)b * D.K + k;
+    float c[4], p[4];
+    load_vec<float, 4>(V.c + pk * DH + lane * 4, c);
+    load_vec<float, 4>(V.p + pk * DH + lane * 4, p);
+    const float2 mu2 = *(const float2*)(V.mu + pk * 2);
+    float mu0 = mu2.x, mu1 = mu2.y;
+    float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
+    int jn = (int)(sorted[r0] & 0xfffu);
+    float ken[4], ven[4];
+    load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
+    load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
+    float2 sn = *(const float2*)(ringS + jn * 2);
+    int j = jn;
+    for (int r = r0; r < r1; ++r) {
+      j = jn;
+      float ke[4], ve[4];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { ke[v] = ken[v]; ve[v] = ven[v]; }
+      const float s0 = sn.x, s1 = sn.y;
+      if (r + 1 < r1) {                                              // prefetch the next token of the segment
+        jn = (int)(sorted[r + 1] & 0xfffu);
+        load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
+        load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
+        sn = *(const float2*)(ringS + jn * 2);
+      }
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        c[v] = ema_step(oma, al, c[v], ke[v]);                       // l.8
+        p[v] = ema_step(omb, be, p[v], ve[v]);                       // l.9
+      }
+      mu0 = ema_step(ome, et, mu0, s0);                              // l.11
+      mu1 = ema_step(ome, et, mu1, s1);
+      const double dx = (double)s0 - (double)mu0, dy = (double)s1 - (double)mu1;   // new mu
+      const double edx = __dmul_rn(et, dx), edy = __dmul_rn(et, dy);
+      sxx = (float)__dadd_rn(__dmul_rn(ome, (double)sxx), __dmul_rn(edx, dx));     // l.12
+      sxy = (float)__dadd_rn(__dmul_rn(ome, (double)sxy), __dmul_rn(edx, dy));
+      syy = (float)__dadd_rn(__dmul_rn(ome, (double)syy), __dmul_rn(edy, dy));
+      if (has_cb) {                                                  // l.13, residual of the updated centres
+        __syncwarp();
+        rsc[lane] = make_float4(ke[0] - c[0], ke[1] - c[1], ke[2] - c[2], ke[3] - c[3]);
+        rsc[32 + lane] = make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
+        __syncwarp();
+        int zk, zv;
+        pq_pick(cbk4, rsc, g, li, zk);
+        pq_pick(cbv4, rsc + 32, g, li, zv);
+        if (li == 0) {
+          atomicAdd(V.hist + ((pk * 2 + 0) * 8 + g) * 16 + zk, 1u);
+          atomicAdd(V.hist + ((pk * 2 + 1) * 8 + g) * 16 + zv, 1u);
+          V.tcodeK[(bt + j) * 8 + g] = (uint8_t)zk;
+          V.tcodeV[(bt + j) * 8 + g] = (uint8_t)zv;
+        }
+      }
+    }
+    // write back the prototype and everything derived from it
+    *(float4*)(V.c + pk * DH + lane * 4) = make_float4(c[0], c[1], c[2], c[3]);
+    *(float4*)(V.p + pk * DH + lane * 4) = make_float4(p[0], p[1], p[2], p[3]);
+    float cc = 0.f;
+#pragma unroll
+    for (int v = 0; v < 4; ++v) cc = fmaf(c[v], c[v], cc);
+    cc = warp_sum(cc);
+    store_shadows<4>(V, pk * DH + lane * 4, c, inv_norm(cc));
+    if (lane == 0) {
+      const int m = r1 - r0;
+      const int n = V.n[pk] + m;                                     // l.10
+      V.n[pk] = n;
+      V.tau[pk] = F.t;
+      V.pos[pk] = (long long)F.ev_frame * D.T + j;
+      *(float2*)(V.mu + pk * 2) = make_float2(mu0, mu1);
+      V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
+      if (has_cb) V.nres[pk] += (uint32_t)m;
+      V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
+      V.logn[pk] = logf((float)n);
+    }
+  }
+}
+
 static int next_pow2(int x) { int p = 2; while (p < x) p <<= 1; return p; }
 
 int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s) {
   const int ntok = D.T - F.n_fill;
   if (ntok <= 0) return 0;
+  if (D.d == 128 && D.G == 8 && D.C == 16) {
+    const int Tpad = (ntok + 3) / 4 * 4;
+    const size_t sm = (size_t)(2 * 8 * kCbG + kUfWarps * 64) * 16 + (size_t)(3 * Tpad + 1) * 4;
+    int nsplit = 4 * sm_count / D.B;
+    const int max_split = (ntok + 2 * kUfWarps - 1) / (2 * kUfWarps);
+    if (nsplit > max_split) nsplit = max_split;
+    if (nsplit < 1) nsplit = 1;
+    dim3 grid(nsplit, D.B);
+    if (D.bf16) update_fast_kernel<__nv_bfloat16><<<grid, kUfThreads, sm, s>>>(D, H, V, F, Tpad);
+    else update_fast_kernel<float><<<grid, kUfThreads, sm, s>>>(D, H, V, F, Tpad);
+    return 1;
+  }
   const int P = next_pow2(ntok);
   int nchunk = (2 * sm_count + D.B - 1) / D.B;
   nchunk = nchunk < 1 ? 1 : nchunk;
@@ -504,7 +729,7 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
     V.rec[pk] = make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
                          V.sigma[pk * 3 + 2], V.tau[pk], H);
     const int n = V.n[pk];
-    V.logn[pk] = n >= 1 ? (float)log((double)n) : 0.f;
+    V.logn[pk] = n >= 1 ? logf((float)n) : 0.f;
   }
 }
 
