@@ -24,7 +24,8 @@ namespace pkv {
 using namespace tc;
 
 constexpr int kUN = 64;                                  // prototypes per unit (UMMA N)
-constexpr int kRing = 4;                                 // B stages = rec slots = TMEM buffers
+constexpr int kRing = 4;                                 // B stages = TMEM buffers
+constexpr int kRecRing = 8;                              // record slots (deeper: a slot is held until the epilogue is done)
 constexpr int kAsThreads = 18 * 32;
 constexpr uint32_t kAHalf = 128 * 128;                   // [128 rows][64 bf16] swizzled box = 16 KB
 constexpr uint32_t kBHalf = kUN * 128;                   // [64 rows][64 bf16] = 8 KB
@@ -34,8 +35,8 @@ constexpr uint32_t kRecBytes = kUN * sizeof(ScoreRec);   // 2 KB
 struct AsSmem {   // byte offsets from a 1024-byte aligned base
   static constexpr uint32_t A = 0;                                  // 2 tiles x 2 K-halves x 16 KB
   static constexpr uint32_t Bst = A + 4 * kAHalf;                   // kRing x 32 KB
-  static constexpr uint32_t Rec = Bst + kRing * kBStage;            // kRing x 2 KB
-  static constexpr uint32_t Bar = Rec + kRing * kRecBytes;
+  static constexpr uint32_t Rec = Bst + kRing * kBStage;            // kRecRing x 2 KB
+  static constexpr uint32_t Bar = Rec + kRecRing * kRecBytes;
   static constexpr uint32_t Total = Bar + 256;
 };
 
@@ -65,7 +66,7 @@ __device__ __forceinline__ uint32_t orderable(float f) {
 
 // One row's scan over the (up to) 64 accumulator columns of a unit: rest of Eq. 1 + running argmin.
 template <bool SQUARED, bool RAGGED>
-__device__ __forceinline__ void as_scan(uint32_t taddr, const float4* rc, int ncol, float sx, float sy, float nk,
+__device__ __forceinline__ void as_scan(uint32_t taddr, uint32_t rc, int ncol, float sx, float sy, float nk,
                                         float thr, float lam_idle, float& ub, int& ucol) {
 #pragma unroll
   for (int c0 = 0; c0 < kUN; c0 += 32) {
@@ -75,8 +76,11 @@ __device__ __forceinline__ void as_scan(uint32_t taddr, const float4* rc, int nc
       tmem_ld_wait();
 #pragma unroll
       for (int c = 0; c < 32; ++c) {
-        const float4 r0 = rc[(c0 + c) * 2];            // mux, muy, u, w
-        const float2 r1 = *reinterpret_cast<const float2*>(&rc[(c0 + c) * 2 + 1]);   // v, tauf
+        float4 r0;                                     // mux, muy, u, w
+        float2 r1;                                     // v, tauf
+        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w)
+                     : "r"(rc + (c0 + c) * 32) : "memory");
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r1.x), "=f"(r1.y) : "r"(rc + (c0 + c) * 32 + 16) : "memory");
         const float dx = sx - r0.x, dy = sy - r0.y;
         const float y1 = dx * r0.z;
         const float y2 = fmaf(dy, r1.x, -(dx * r0.w));
@@ -104,10 +108,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
   uint64_t* a_empty = bars + 1;
   uint64_t* b_full = bars + 2;                 // [kRing]
   uint64_t* b_empty = b_full + kRing;
-  uint64_t* r_full = b_empty + kRing;
-  uint64_t* t_full = r_full + kRing;
+  uint64_t* t_full = b_empty + kRing;
   uint64_t* t_empty = t_full + kRing;
-  uint32_t* tmem_slot = (uint32_t*)(t_empty + kRing);
+  uint64_t* r_full = t_empty + kRing;          // [kRecRing]
+  uint64_t* r_empty = r_full + kRecRing;
+  uint32_t* tmem_slot = (uint32_t*)(r_empty + kRecRing);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int u0 = (int)(((long long)blockIdx.x * P.units) / gridDim.x);
@@ -117,9 +122,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
     prefetch_tmap(&tmK); prefetch_tmap(&tmChi); prefetch_tmap(&tmClo);
     mbar_init(a_full, 1); mbar_init(a_empty, 1);
     for (int s = 0; s < kRing; ++s) {
-      mbar_init(b_full + s, 1); mbar_init(b_empty + s, 1); mbar_init(r_full + s, 1);
+      mbar_init(b_full + s, 1); mbar_init(b_empty + s, 1);
       mbar_init(t_full + s, 1); mbar_init(t_empty + s, 8);
     }
+    for (int s = 0; s < kRecRing; ++s) { mbar_init(r_full + s, 1); mbar_init(r_empty + s, 8); }
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -154,48 +160,53 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
         tma_load_2d(dst + kBHalf, &tmChi, 64, prow, b_full + s);
         tma_load_2d(dst + 2 * kBHalf, &tmClo, 0, prow, b_full + s);
         tma_load_2d(dst + 3 * kBHalf, &tmClo, 64, prow, b_full + s);
-        mbar_wait(t_empty + s, par);                 // the epilogue of unit i - kRing has read this record slot
+        const int rs = i % kRecRing;
+        mbar_wait(r_empty + rs, ((i / kRecRing) & 1) ^ 1);   // the epilogue of unit i - kRecRing has read this slot
         const int nrec = min(kUN, D.K - x.nc * kUN);
-        mbar_arrive_expect_tx(r_full + s, (uint32_t)nrec * sizeof(ScoreRec));
-        bulk_load_1d(sm + AsSmem::Rec + s * kRecBytes, V.rec + (size_t)prow, (uint32_t)nrec * sizeof(ScoreRec), r_full + s);
+        mbar_arrive_expect_tx(r_full + rs, (uint32_t)nrec * sizeof(ScoreRec));
+        bulk_load_1d(sm + AsSmem::Rec + rs * kRecBytes, V.rec + (size_t)prow, (uint32_t)nrec * sizeof(ScoreRec), r_full + rs);
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer =====
-    if (lane == 0) {
-      constexpr uint32_t idesc = idesc_bf16(128, kUN, 0, 0);
-      const uint32_t a_addr = smem_u32(sm + AsSmem::A);
-      int prev = -1, acnt = 0;
-      for (int u = u0; u < u1; ++u) {
-        const AsUnit x = as_unit(P, u);
-        const int i = u - u0, s = i % kRing;
-        const uint32_t par = (i / kRing) & 1;
-        if (x.akey != prev) { mbar_wait(a_full, acnt & 1); prev = x.akey; ++acnt; }
-        mbar_wait(t_empty + s, par ^ 1);
-        mbar_wait(b_full + s, par);
-        tc_fence_after_sync();
-        const uint32_t b_addr = smem_u32(sm + AsSmem::Bst + s * kBStage);
-        for (int t = 0; t < x.ntiles; ++t) {
+    // ===== MMA issuer: the whole warp walks the unit list (uniform control flow), one elected lane issues =====
+    constexpr uint32_t idesc = idesc_bf16(128, kUN, 0, 0);
+    const uint64_t a_desc0 = desc_kmajor_sw128(smem_u32(sm + AsSmem::A));
+    const uint64_t b_desc0 = desc_kmajor_sw128(smem_u32(sm + AsSmem::Bst));
+    int nc = u0 % P.NC, akey = u0 / P.NC, acnt = 0;
+    bool fresh = true;                               // first unit on this (bank, pair): wait for its token tiles
+    for (int u = u0; u < u1; ++u) {
+      const int i = u - u0, s = i % kRing;
+      const uint32_t par = (i / kRing) & 1;
+      const int ntiles = (P.ntok - (akey % P.NP) * 256) > 128 ? 2 : 1;
+      if (fresh) { mbar_wait(a_full, acnt & 1); ++acnt; fresh = false; }
+      mbar_wait(t_empty + s, par ^ 1);
+      mbar_wait(b_full + s, par);
+      tc_fence_after_sync();
+      const bool last = (nc + 1 == P.NC) || (u + 1 == u1);
+      if (elect_one_sync()) {
+        const uint64_t bs = b_desc0 + (uint64_t)(s * (kBStage >> 4));
+        for (int t = 0; t < ntiles; ++t) {
           const uint32_t d_tmem = tmem_base + s * 128 + t * kUN;
-          bool acc = false;
+          const uint64_t at = a_desc0 + (uint64_t)(t * (2 * kAHalf >> 4));
 #pragma unroll
           for (int part = 0; part < 2; ++part) {        // hi, lo
 #pragma unroll
             for (int half = 0; half < 2; ++half) {      // d 0..63, 64..127
 #pragma unroll
               for (int kk = 0; kk < 4; ++kk) {          // 4 x K=16 inside the 128-byte swizzle atom
-                const uint64_t ad = desc_kmajor_sw128(a_addr + (t * 2 + half) * kAHalf + kk * 32);
-                const uint64_t bd = desc_kmajor_sw128(b_addr + (part * 2 + half) * kBHalf + kk * 32);
-                umma_bf16(d_tmem, ad, bd, idesc, acc);
-                acc = true;
+                const uint64_t ad = at + (uint64_t)((half * kAHalf + kk * 32) >> 4);
+                const uint64_t bd = bs + (uint64_t)(((part * 2 + half) * kBHalf + kk * 32) >> 4);
+                umma_bf16(d_tmem, ad, bd, idesc, (part | half | kk) != 0);
               }
             }
           }
         }
         umma_commit(b_empty + s);       // smem stage reusable once these MMAs have read it
         umma_commit(t_full + s);        // accumulators complete
-        if (u + 1 == u1 || (u + 1) / P.NC != x.akey) umma_commit(a_empty);   // last unit on these token tiles
+        if (last) umma_commit(a_empty); // last unit on these token tiles
       }
+      __syncwarp();
+      if (++nc == P.NC) { nc = 0; ++akey; fresh = true; }
     }
   } else {
     // ===== epilogue: 16 warps; group = unit parity, tile = M tile of the pair, q = TMEM lane quarter =====
@@ -229,12 +240,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
           nk = kk > 0.f ? sqrtf(kk) : 1.f;                   // |K_j| = 0: acc = 0 and Eq. 1 reduces to its other terms
         }
       }
-      mbar_wait(r_full + s, par);
+      const int rs = i % kRecRing;
+      mbar_wait(r_full + rs, (i / kRecRing) & 1);
       mbar_wait(t_full + s, par);
       tc_fence_after_sync();
       if (__any_sync(0xffffffffu, valid)) {
         const int ncol = min(kUN, F.n_act - x.nc * kUN);
-        const float4* rc = reinterpret_cast<const float4*>(sm + AsSmem::Rec + s * kRecBytes);
+        const uint32_t rc = smem_u32(sm + AsSmem::Rec + rs * kRecBytes);
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + s * 128 + tile * kUN;
         float ub = INFINITY;
         int ucol = 0;
@@ -244,7 +256,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
       }
       tc_fence_before_sync();
       __syncwarp();
-      if (lane == 0) mbar_arrive(t_empty + s);
+      if (lane == 0) { mbar_arrive(t_empty + s); mbar_arrive(r_empty + rs); }
     }
     flush();
   }
