@@ -71,6 +71,10 @@ struct Dev {
   uint32_t* codesK;  // [B][K][S], code of subspace g in bits [4g, 4g+4)
   uint32_t* codesV;
   uint8_t* kind;     // [B][K] 0 decoded, 1 zero residual, 2 absent
+  // dirty[pk] = id of the synthesis epoch in which the prototype's histograms / mass last changed (0 = never).  The
+  // host counts epochs (one per synthesis); the synthesis of epoch e re-decodes exactly the prototypes stamped e and
+  // leaves the codes of the others, which are still valid, alone.  Plain stores, no atomics, nothing to clear.
+  uint32_t* dirty;       // [B][K]
   // per-frame scratch / trace
   int* assign;       // [B][T]
   float* best;       // [B][T]
@@ -126,6 +130,7 @@ struct FrameArgs {
   int n_act0;    // active prototypes before this step's slot fill
   int n_fill;    // evicted tokens that open a new slot (Alg. 1 l.3-4)
   int n_act;     // active prototypes after the fill = what Eq. 1 scans
+  int epoch;     // id of the current synthesis epoch (>= 1), see Dev::dirty
   int keys;      // 1: the assignment of this frame is in Dev::akey (tcgen05 path), 0: in Dev::assign / best (SIMT)
 };
 
@@ -135,8 +140,12 @@ int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const vo
 int launch_fill(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
 int launch_score_simt(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
 int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s);
-int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, cudaStream_t s);
-int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s);
+int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s);
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s);
+
+__device__ __forceinline__ void mark_dirty(const Dims& D, const Dev& V, int b, int k, int epoch) {
+  V.dirty[(size_t)b * D.K + k] = (uint32_t)epoch;
+}
 
 struct AttnArgs {
   const void* Q; void* out; float* lse;

@@ -24,6 +24,7 @@ struct protokv_state {
   int last_ev_frame;  // index of the frame evicted by the last append, -1 if none
   int last_n_fill;
   bool codes_valid;   // codes/kind describe the current histograms
+  int epoch;          // synthesis epoch (see Dev::dirty_cnt)
   bool use_tc_assign;
   bool use_tc_attn;
   TcMaps maps;
@@ -109,7 +110,7 @@ static int validate(const protokv_config* c) {
     if (tuples < c->S) return fail(PROTOKV_EINVAL, "C^G < S");
   }
   if (c->tokens_per_frame > 4096) return fail(PROTOKV_EUNSUPPORTED, "tokens_per_frame > 4096");
-  if (c->k_max >= (1 << 20)) return fail(PROTOKV_EUNSUPPORTED, "k_max >= 2^20");
+  if (c->k_max > 16384) return fail(PROTOKV_EUNSUPPORTED, "k_max > 16384");
   if (!(c->alpha >= 0.f && c->alpha <= 1.f && c->beta >= 0.f && c->beta <= 1.f && c->eta >= 0.f && c->eta <= 1.f))
     return fail(PROTOKV_EINVAL, "alpha, beta, eta must lie in [0, 1]");
   if (!(c->sigma_eps >= 0.f) || !(c->cos_eps > 0.f) || !(c->pq_eps > 0.0))
@@ -163,6 +164,7 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   }
   v.codesK = (uint32_t*)take(BK * D.S * 4); v.codesV = (uint32_t*)take(BK * D.S * 4);
   v.kind = (uint8_t*)take(BK);
+  v.dirty = (uint32_t*)take(BK * 4);
   v.assign = (int*)take(BT * 4); v.best = (float*)take(BT * 4);
   v.akey = (unsigned long long*)take(BT * 8);
   v.tcodeK = (uint8_t*)take(BT * D.G); v.tcodeV = (uint8_t*)take(BT * D.G);
@@ -228,6 +230,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   }
   cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, st->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(st->V.akey, 0xff, (size_t)st->D.B * st->D.T * 8, st->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(st->V.kind, 2, (size_t)st->D.B * st->D.K, st->stream);   // every slot absent
   if (e == cudaSuccess && has_cb) {
     const size_t cb = (size_t)st->D.B * st->D.G * st->D.C * st->D.sub * 4;
     e = cudaMemcpyAsync(st->V.cbk, cfg->codebook_k, cb, cudaMemcpyDeviceToDevice, st->stream);
@@ -240,6 +243,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   }
   st->frames = 0; st->n_act = 0; st->launches = 0; st->last_ev_frame = -1; st->last_n_fill = 0;
   st->codes_valid = false;
+  st->epoch = 1;
   st->profiling = false;
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->maps.ok = false;
@@ -289,6 +293,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   F.n_fill = F.evicted ? (D.K - st->n_act < D.T ? D.K - st->n_act : D.T) : 0;
   F.n_act = st->n_act + F.n_fill;
   F.keys = st->use_tc_assign ? 1 : 0;
+  F.epoch = st->epoch;
   int nl = 0;
   if (F.evicted) {
     if (F.n_fill > 0) {
@@ -323,9 +328,10 @@ int protokv_synthesize(protokv_state* st) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
   {
     StageTimer tm(st, PROTOKV_STAGE_SYNTH);
-    st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->stream);
+    st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->sm_count, st->stream);
   }
   PKV_CUDA(cudaGetLastError());
+  st->epoch += 1;
   st->codes_valid = true;
   return PROTOKV_OK;
 }
@@ -340,8 +346,10 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
   const bool far = !(st->H.flags & PROTOKV_NEAR_ONLY);
   if (far) {
     if (run_synthesis) {
-      const int rc = protokv_synthesize(st);
-      if (rc != PROTOKV_OK) return rc;
+      if (!st->codes_valid) {       // nothing changed since the last synthesis otherwise
+        const int rc = protokv_synthesize(st);
+        if (rc != PROTOKV_OK) return rc;
+      }
     } else if (!st->codes_valid) {
       return fail(PROTOKV_ESTATE, "run_synthesis = 0 but no synthesis result is valid for the current state");
     }
@@ -476,7 +484,7 @@ int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   if (v->hist_k) PKV_CUDA(cudaMemcpy2D(V.hist + o * 2 * D.G * D.C, 2 * gc, v->hist_k, gc, gc, K, cudaMemcpyHostToDevice));
   if (v->hist_v)
     PKV_CUDA(cudaMemcpy2D(V.hist + o * 2 * D.G * D.C + D.G * D.C, 2 * gc, v->hist_v, gc, gc, K, cudaMemcpyHostToDevice));
-  st->launches += launch_refresh_derived(D, st->H, V, bank, st->stream);
+  st->launches += launch_refresh_derived(D, st->H, V, bank, st->epoch, st->stream);
   PKV_CUDA(cudaGetLastError());
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   st->codes_valid = false;

@@ -55,12 +55,36 @@ __device__ __forceinline__ SynCand syn_add(const SynCand& b, long long cost, uin
   return r;
 }
 
-__global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act) {
-  const long long idx = (long long)blockIdx.x * kSynThreads + threadIdx.x;
-  const long long total = (long long)D.B * D.K * 2;
-  if (idx >= total) return;
-  const int kv = (int)(idx & 1);
-  const size_t pk = (size_t)(idx >> 1);
+// Work list: the prototypes stamped with the current epoch (Dev::dirty); the codes of the others are still valid.
+// Every block of a bank compacts the bank's stamps into the same list in shared memory (ballot + prefix), then the
+// blocks share the list entries by index.
+__device__ void synthesize_one(const Dims& D, const Hyper& H, const Dev& V, int n_act, size_t pk, int kv);
+
+__global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act, int epoch) {
+  extern __shared__ uint16_t syn_list[];      // [K]
+  __shared__ int wcnt[kSynThreads / 32];
+  const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t* flags = V.dirty + (size_t)b * D.K;
+  int base = 0;
+  for (int k0 = 0; k0 < D.K; k0 += kSynThreads) {
+    const int k = k0 + tid;
+    const bool hit = k < D.K && flags[k] == (uint32_t)epoch;
+    const uint32_t bal = __ballot_sync(0xffffffffu, hit);
+    if (lane == 0) wcnt[warp] = __popc(bal);
+    __syncthreads();
+    int off = base, tot = 0;
+#pragma unroll
+    for (int w = 0; w < kSynThreads / 32; ++w) { const int c = wcnt[w]; if (w < warp) off += c; tot += c; }
+    if (hit) syn_list[off + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)k;
+    base += tot;
+    __syncthreads();
+  }
+  const int cnt = base;
+  for (int idx = blockIdx.x * kSynThreads + tid; idx < 2 * cnt; idx += gridDim.x * kSynThreads)
+    synthesize_one(D, H, V, n_act, (size_t)b * D.K + syn_list[idx >> 1], idx & 1);
+}
+
+__device__ void synthesize_one(const Dims& D, const Hyper& H, const Dev& V, int n_act, size_t pk, int kv) {
   const int k = (int)(pk % D.K);
   const bool has_cb = V.cbk != nullptr;
   const bool present = k < n_act && V.n[pk] >= 1;
@@ -152,9 +176,13 @@ __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H,
   }
 }
 
-int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s) {
-  const long long total = (long long)D.B * D.K * 2;
-  synthesis_kernel<<<(unsigned)((total + kSynThreads - 1) / kSynThreads), kSynThreads, 0, s>>>(D, H, V, n_act);
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s) {
+  // grid-stride over each bank's work list; its length is only known on the device
+  int per_bank = (2 * D.K + kSynThreads - 1) / kSynThreads;
+  const int cap = (6 * sm_count + D.B - 1) / D.B;
+  if (per_bank > cap) per_bank = cap;
+  if (per_bank < 1) per_bank = 1;
+  synthesis_kernel<<<dim3(per_bank, D.B), kSynThreads, (size_t)D.K * 2, s>>>(D, H, V, n_act, epoch);
   return 1;
 }
 

@@ -150,6 +150,7 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     V.nres[pk] = 0u;
     V.rec[pk] = make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H);
     V.logn[pk] = 0.f;
+    mark_dirty(D, V, b, k, F.epoch);
     V.assign[(size_t)b * D.T + j] = k;
     V.best[(size_t)b * D.T + j] = 0.f;
   }
@@ -448,7 +449,8 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] += (uint32_t)m;
       V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
-      V.logn[pk] = (float)log((double)n);
+      V.logn[pk] = logf((float)n);
+      mark_dirty(D, V, b, k, F.epoch);
     }
   }
 }
@@ -662,6 +664,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       if (has_cb) V.nres[pk] += (uint32_t)m;
       V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
       V.logn[pk] = logf((float)n);
+      mark_dirty(D, V, b, k, F.epoch);
     }
   }
 }
@@ -705,7 +708,7 @@ int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& 
 // Derived per-prototype data (scoring record, log-mass, bf16 shadows) recomputed from the primary state of one
 // bank -- used after protokv_import_state.  One warp per prototype.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
+__global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b, int epoch) {
   const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (k >= D.K) return;
   const size_t pk = (size_t)b * D.K + k;
@@ -730,11 +733,12 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b) {
                          V.sigma[pk * 3 + 2], V.tau[pk], H);
     const int n = V.n[pk];
     V.logn[pk] = n >= 1 ? logf((float)n) : 0.f;
+    mark_dirty(D, V, b, k, epoch);
   }
 }
 
-int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, cudaStream_t s) {
-  refresh_derived_kernel<<<(D.K + 7) / 8, 256, 0, s>>>(D, H, V, bank);
+int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s) {
+  refresh_derived_kernel<<<(D.K + 7) / 8, 256, 0, s>>>(D, H, V, bank, epoch);
   return 1;
 }
 
