@@ -259,12 +259,17 @@ def roofline_objects(spec, res, peaks, steps):
                         algorithmic_flops=af, ms=sc_ms, note="T x K_max x d contraction, 1x flops (hi+lo split doubles the MMA work)")
     out["score"]["frac"] = out["score"]["achieved"] / peaks["bf16_sustained"]
     at_ms = stages["attention"][0] / max(1, stages["attention"][1])
-    t_roof = max(qb / (peaks["hbm"] * 1e9), fact / (peaks["bf16_sustained"] * 1e12))
-    out["attention"] = dict(bound="tensor" if fact / (peaks["bf16_sustained"] * 1e12) >= qb / (peaks["hbm"] * 1e9) else "hbm",
-                            achieved=fact / (at_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
-                            frac=fact / (at_ms * 1e-3) / 1e12 / peaks["bf16_sustained"], algorithmic_flops=fact,
-                            dense_equivalent_flops=dense, dense_equivalent_tflops=dense / (at_ms * 1e-3) / 1e12,
-                            algorithmic_bytes=qb, hbm_gbs=qb / (at_ms * 1e-3) / 1e9, roofline_us=t_roof * 1e6, ms=at_ms)
+    # The kernel issues the dense contraction 4 rows L_context d on the tensor pipe (the "factorised"
+    # count of SURVEY 8(d) is not reachable -- its per-(row, pseudo-token) code gathers are themselves G*C = d wide), so
+    # `achieved` is dense-equivalent TFLOP/s = tensor-pipe utilisation; the stricter factorised figures ride along.
+    t_dense = max(qb / (peaks["hbm"] * 1e9), dense / (peaks["bf16_sustained"] * 1e12))
+    t_fact = max(qb / (peaks["hbm"] * 1e9), fact / (peaks["bf16_sustained"] * 1e12))
+    out["attention"] = dict(bound="tensor", achieved=dense / (at_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
+                            frac=dense / (at_ms * 1e-3) / 1e12 / peaks["bf16_sustained"], algorithmic_flops=dense,
+                            factorised_flops=fact, factorised_tflops=fact / (at_ms * 1e-3) / 1e12,
+                            algorithmic_bytes=qb, hbm_gbs=qb / (at_ms * 1e-3) / 1e9, hbm_frac=qb / (at_ms * 1e-3) / 1e9 / peaks["hbm"],
+                            roofline_us=t_dense * 1e6, frac_of_roofline_time=t_dense * 1e3 / at_ms,
+                            factorised_roofline_us=t_fact * 1e6, frac_of_factorised_roofline_time=t_fact * 1e3 / at_ms, ms=at_ms)
     sy_ms = stages["synthesis"][0] / max(1, stages["synthesis"][1])
     out["synthesis"] = dict(ms=sy_ms)
     # dominant kernel of the step = the stage with the largest summed device time
@@ -383,9 +388,8 @@ def main():
     e2e_u, e2e_q = res["e2e"]["update_s"] / res["e2e"]["steps"], res["e2e"]["query_s"] / res["e2e"]["steps"]
     if world > 1:
         import torch.distributed as dist
-        t = torch.tensor([upd_ms, qry_ms, region_ms, e2e_u, e2e_q], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        upd_ms, qry_ms, region_ms, e2e_u, e2e_q = t.tolist()
+        from paper_2606_26762_b200 import sharding
+        upd_ms, qry_ms, region_ms, e2e_u, e2e_q = sharding.max_over_ranks([upd_ms, qry_ms, region_ms, e2e_u, e2e_q], device=device)
         ln = torch.tensor([res["launches"]], device=device, dtype=torch.int64)
         dist.all_reduce(ln)
         res["launches"] = int(ln.item())
