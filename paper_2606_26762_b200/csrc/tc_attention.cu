@@ -3,12 +3,13 @@
 //
 //   near tiles    128 ring rows of K and V, loaded by TMA (128-byte swizzle)
 //   pseudo tiles  16 prototypes x S = 128 pseudo-tokens k~ = c_k + concat_g CK_g[zK(k,s,g)], v~ = p_k + concat_g CV_g[zV]
-//                 (Alg. 4 l.5-9) built in shared memory by the producer warps from the fp32 centres, the 4-bit codes
-//                 of the synthesis step and the codebooks held in shared memory -- pseudo-tokens never exist in HBM
+//                 (Alg. 4 l.5-9) built in shared memory by the builder warpgroup: the tile's centres, codes, kinds and
+//                 log-masses arrive in a staging buffer by bulk copies issued one tile ahead, the codebooks sit in
+//                 shared memory as bf16 -- pseudo-tokens never exist in HBM
 //   S = Q K~^T    tcgen05.mma, Q tile (M = 128 query rows) and K~ tile from shared memory, fp32 accumulator in TMEM
-//   softmax       one thread per query row drains S with tcgen05.ld, adds the log-mass bias log n_k (Eq. 2/4, 0 on
-//                 near tokens), exponentiates against a lazily updated reference maximum, writes P as bf16 back into
-//                 the columns S occupied (tcgen05.st)
+//   softmax       one thread per query row drains S with tcgen05.ld (double-buffered 32-column chunks), adds the
+//                 log-mass bias log n_k (Eq. 2/4, 0 on near tokens), exponentiates against a lazily updated reference
+//                 maximum (packed f32x2 arithmetic), writes P as bf16 back into the columns S occupied (tcgen05.st)
 //   O += P V~     tcgen05.mma with A = P from TMEM, B = V~ tile (MN-major) from shared memory
 //
 // One CTA works on two M tiles of a bank (256 query rows = n_q x GQA group) in ping-pong, so the tensor pipe runs the
@@ -17,8 +18,11 @@
 // cover the tail of one item and the head of the next; every (item, span) piece writes an unnormalised partial
 // (O, m, l) and attention_tc_combine_kernel merges the pieces of an item.
 //
-// Warp roles (13 warps): 0 = MMA issuer + TMEM owner; 1-4 = producers (TMA for Q and near tiles, builders of the
-// pseudo tiles); 5-8 = softmax of M tile 0; 9-12 = softmax of M tile 1.
+// Warp roles (16 warps, warpgroup-aligned so that setmaxnreg can move registers to the softmax threads):
+//   warps 0-3 / 4-7   softmax of M tile 0 / 1 (warp % 4 = TMEM lane quarter)
+//   warps 8-11        builders of the pseudo tiles
+//   warp 12           MMA issuer + TMEM owner;  warp 13: loader (TMA for Q and near tiles, bulk copies into the staging
+//                     buffer);  warps 14-15 idle
 #include "common.cuh"
 #include "tc_common.cuh"
 
@@ -26,7 +30,7 @@ namespace pkv {
 
 using namespace tc;
 
-constexpr int kAtThreads = 416;
+constexpr int kAtThreads = 512;
 constexpr int kAtCols = 128;            // context columns per tile
 constexpr int kAtProto = 16;            // prototypes per pseudo tile (x S = 8)
 constexpr int kAtRows = 256;            // query rows per item (two M tiles)
@@ -34,18 +38,26 @@ constexpr uint32_t kAtHalf = 128 * 128; // one [128 rows][64 bf16] swizzled box 
 constexpr int kAtBiasRing = 4;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
-constexpr float kRescaleGap = 8.f;      // P may reach 2^8 before the reference maximum is moved
+constexpr float kRescaleSum = 256.f;    // a tile's row sum of P above this moves the reference maximum (P <= 2^8 in bf16)
+constexpr int kRegsSoftmax = 184, kRegsBuilder = 96, kRegsAux = 48;   // 2 * 184 + 96 + 48 = 512 = 4 * 128
 
 struct AtSmem {   // byte offsets from a 1024-byte aligned base
   static constexpr uint32_t Q = 0;                          // 2 d-halves x [256 rows][128 B]
   static constexpr uint32_t K = Q + 4 * kAtHalf;            // 2 stages x (2 d-halves x 16 KB)
   static constexpr uint32_t V = K + 4 * kAtHalf;            // 2 stages x (2 d-halves x 16 KB)
-  static constexpr uint32_t CBK = V + 4 * kAtHalf;          // [G][C][16] fp32
-  static constexpr uint32_t CBV = CBK + 8192;
-  static constexpr uint32_t Bias = CBV + 8192;              // [ring][16] fp32, log2 domain
+  static constexpr uint32_t CBK = V + 4 * kAtHalf;          // [C][G][16] bf16: code z at z * 256 B, chunk ch at ch * 16 B
+  static constexpr uint32_t CBV = CBK + 4096;
+  static constexpr uint32_t StgC = CBV + 4096;              // staging of one pseudo tile: c [16][128] fp32
+  static constexpr uint32_t StgP = StgC + 8192;             //   p [16][128] fp32
+  static constexpr uint32_t StgZK = StgP + 8192;            //   codesK [16][8] u32
+  static constexpr uint32_t StgZV = StgZK + 512;            //   codesV
+  static constexpr uint32_t StgLn = StgZV + 512;            //   log n [16] fp32
+  static constexpr uint32_t StgKd = StgLn + 64;             //   kind [16] u8
+  static constexpr uint32_t Bias = StgKd + 64;              // [ring][16] fp32, log2 domain
   static constexpr uint32_t Bar = Bias + kAtBiasRing * kAtProto * 4;
   static constexpr uint32_t Total = Bar + 256;
 };
+constexpr uint32_t kStgBytes = 8192 + 8192 + 512 + 512 + 64 + 16;
 
 // Partition of the tile space shared by the kernel, the combine kernel and the host.
 struct AtPlan {
@@ -76,6 +88,32 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+__device__ __forceinline__ uint32_t add_bf16x2(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("add.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// packed fp32 pairs (sm_100 f32x2 arithmetic): one issue slot for two elements
+__device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack_f32x2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
 struct AtArgs {
   const void* Q;   // unused by the kernel (the tensor map addresses it); kept for the combine kernel's layout maths
@@ -133,42 +171,50 @@ __device__ __forceinline__ float at_row_max(uint32_t s_addr, float sc2, const fl
   return mx;
 }
 
-// One pass over the S tile of this row: P = exp2(x') packed to bf16 pairs, row sum and row max of x'.
+// One pass over the S tile of this row: P = exp2(x') packed to bf16 pairs and the row sum of P.  The 32-column chunks
+// are double-buffered: chunk c + 1 is in flight from TMEM while chunk c is exponentiated.
 template <bool RAGGED>
 __device__ __forceinline__ void at_row_pass(uint32_t s_addr, float sc2, const float (&bm)[16], int nvalid,
-                                            uint32_t (&pk)[64], float& lsum, float& mx) {
-  float l0 = 0.f, l1 = 0.f, m0 = -INFINITY, m1 = -INFINITY;
+                                            uint32_t (&pk)[64], float& lsum) {
+  const uint64_t sc22 = pack_f32x2(sc2, sc2);
+  uint64_t l2 = pack_f32x2(0.f, 0.f);
+  uint32_t a[2][32];
+  tmem_ld_32x32(s_addr, a[0]);
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
-    uint32_t a[32];
-    tmem_ld_32x32(s_addr + c * 32, a);
     tmem_ld_wait();
+    if (c < 3) tmem_ld_32x32(s_addr + (c + 1) * 32, a[(c + 1) & 1]);
 #pragma unroll
     for (int i = 0; i < 32; i += 2) {
-      float x0 = fmaf(__uint_as_float(a[i]), sc2, bm[(c * 32 + i) >> 3]);
-      float x1 = fmaf(__uint_as_float(a[i + 1]), sc2, bm[(c * 32 + i) >> 3]);
+      const float b = bm[(c * 32 + i) >> 3];
+      const uint64_t x2 = fma_f32x2(pack_f32x2(__uint_as_float(a[c & 1][i]), __uint_as_float(a[c & 1][i + 1])), sc22,
+                                    pack_f32x2(b, b));
+      float x0, x1;
+      unpack_f32x2(x2, x0, x1);
       if (RAGGED) {
         if (c * 32 + i >= nvalid) x0 = -INFINITY;
         if (c * 32 + i + 1 >= nvalid) x1 = -INFINITY;
       }
-      m0 = fmaxf(m0, x0); m1 = fmaxf(m1, x1);
       const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
-      l0 += p0; l1 += p1;
+      l2 = add_f32x2(l2, pack_f32x2(p0, p1));
       pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
     }
   }
+  float l0, l1;
+  unpack_f32x2(l2, l0, l1);
   lsum = l0 + l1;
-  mx = fmaxf(m0, m1);
 }
 
 struct AtBars {
-  uint64_t *q_full, *q_empty, *k_full, *k_empty, *v_full, *v_empty, *s_full, *p_full, *pv_done, *o_empty;
+  uint64_t *q_full, *q_empty, *k_full, *k_empty, *v_full, *v_empty, *s_full, *p_full, *pv_done, *o_empty, *stg_full,
+      *stg_empty;
   __device__ explicit AtBars(uint64_t* b)
       : q_full(b), q_empty(b + 1), k_full(b + 2), k_empty(b + 4), v_full(b + 6), v_empty(b + 8), s_full(b + 10),
-        p_full(b + 12), pv_done(b + 14), o_empty(b + 16) {}
+        p_full(b + 12), pv_done(b + 14), o_empty(b + 16), stg_full(b + 18), stg_empty(b + 19) {}
 };
+constexpr int kAtNumBars = 20;
 
-// ---- warp 0: MMA issuer -------------------------------------------------------------------------------------
+// ---- warp 12: MMA issuer ------------------------------------------------------------------------------------
 __device__ __forceinline__ void at_issue_s(uint32_t tmem_base, uint32_t q_addr, uint32_t k_addr, int w) {
   constexpr uint32_t idesc = idesc_bf16(128, 128, 0, 0);
 #pragma unroll
@@ -243,151 +289,171 @@ __device__ void at_mma_role(unsigned char* sm, const AtBars& B, uint32_t tmem_ba
   }
 }
 
-// ---- warps 1-4: producers -------------------------------------------------------------------------------------
-// Per-thread operands of a pseudo tile: thread (kk, ch) owns the 16-byte chunk ch (8 dims of subspace ch / 2) of
-// prototypes kk and kk + 8 of the tile, for all S pseudo-tokens of each.
+// ---- warp 13: loader (one lane) -------------------------------------------------------------------------------
+// Q boxes and near tiles by TMA straight into the operand stages; for pseudo tiles the raw operands of the tile
+// (centres, codes, kinds, log-masses of its 16 prototypes, all contiguous in the bank arrays) by bulk copies into the
+// single staging buffer, which the builders empty into registers before they build -- so the copies of tile j + 1
+// overlap the build of tile j.
+__device__ void at_loader_role(unsigned char* sm, const AtBars& B, const CUtensorMap* tmQ, const CUtensorMap* tmRK,
+                               const CUtensorMap* tmRV, const Dims& D, const Dev& V, const AtArgs& A, const AtPlan& P) {
+  const uint32_t qbytes = 256u * (uint32_t)D.group * (uint32_t)P.tb;   // two boxes {64 bf16, group, tb}
+  uint32_t tcnt = 0, pcnt = 0, ic = 0;
+  const long long g1 = at_span_begin(P, blockIdx.x + 1);
+  for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
+    const AtSeg sg = at_segment(P, D, A, g, g1);
+    g += sg.t1 - sg.t0;
+    mbar_wait(B.q_empty, (ic & 1) ^ 1);
+    mbar_arrive_expect_tx(B.q_full, qbytes);
+    const int tok = (sg.st * A.layer_count + sg.ll) * A.n_q + sg.rb * P.tb;
+    tma_load_3d(sm + AtSmem::Q, tmQ, 0, sg.hd * D.group, tok, B.q_full);
+    tma_load_3d(sm + AtSmem::Q + 2 * kAtHalf, tmQ, 64, sg.hd * D.group, tok, B.q_full);
+    ++ic;
+    for (int j = sg.t0; j < sg.t1; ++j, ++tcnt) {
+      const uint32_t stg = tcnt & 1, par = ((tcnt >> 1) & 1) ^ 1;
+      if (j < P.nt_near) {
+        unsigned char* ks = sm + AtSmem::K + stg * 2 * kAtHalf;
+        unsigned char* vs = sm + AtSmem::V + stg * 2 * kAtHalf;
+        const int row0 = sg.b * D.Wf * D.T + j * kAtCols;
+        mbar_wait(B.k_empty + stg, par);
+        mbar_arrive_expect_tx(B.k_full + stg, 2 * kAtHalf);
+        tma_load_2d(ks, tmRK, 0, row0, B.k_full + stg);
+        tma_load_2d(ks + kAtHalf, tmRK, 64, row0, B.k_full + stg);
+        mbar_wait(B.v_empty + stg, par);
+        mbar_arrive_expect_tx(B.v_full + stg, 2 * kAtHalf);
+        tma_load_2d(vs, tmRV, 0, row0, B.v_full + stg);
+        tma_load_2d(vs + kAtHalf, tmRV, 64, row0, B.v_full + stg);
+      } else {
+        const size_t pk0 = (size_t)sg.b * D.K + (size_t)(j - P.nt_near) * kAtProto;
+        mbar_wait(B.stg_empty, (pcnt & 1) ^ 1);
+        mbar_arrive_expect_tx(B.stg_full, kStgBytes);
+        bulk_load_1d(sm + AtSmem::StgC, V.c + pk0 * 128, 8192, B.stg_full);
+        bulk_load_1d(sm + AtSmem::StgP, V.p + pk0 * 128, 8192, B.stg_full);
+        bulk_load_1d(sm + AtSmem::StgZK, V.codesK + pk0 * 8, 512, B.stg_full);
+        bulk_load_1d(sm + AtSmem::StgZV, V.codesV + pk0 * 8, 512, B.stg_full);
+        bulk_load_1d(sm + AtSmem::StgLn, V.logn + pk0, 64, B.stg_full);
+        bulk_load_1d(sm + AtSmem::StgKd, V.kind + pk0, 16, B.stg_full);
+        ++pcnt;
+      }
+    }
+  }
+  if (ic > 0) mbar_wait(B.q_empty, (ic & 1) ^ 1);   // every MMA of this CTA has completed
+}
+
+// ---- warps 8-11: builders of the pseudo tiles ------------------------------------------------------------------
+// Thread (kk, ch) owns the 16-byte chunk ch (8 dims of subspace ch / 2) of prototypes kk and kk + 8 of the tile, for
+// all S pseudo-tokens of each.
 struct AtProtoRegs {
-  float x[2][8];        // centre chunk (c_k or p_k)
+  uint32_t x[2][4];     // centre chunk (c_k or p_k) as bf16 pairs
   uint32_t code[2][8];  // packed codes of the S modes (subspace g in bits [4g, 4g+4))
-  bool zero[2];         // zero residual (Alg. 4 l.3-4) or absent prototype
 };
 
-__device__ __forceinline__ void at_load_proto(AtProtoRegs& r, const float* centres, const uint32_t* codes,
-                                              const uint8_t* kind, size_t pk0, int k0, int n_act, int kk, int ch) {
+__device__ __forceinline__ void at_read_staged(AtProtoRegs& r, const unsigned char* centres, const unsigned char* codes,
+                                               int kk, int ch) {
 #pragma unroll
   for (int u = 0; u < 2; ++u) {
-    const int k = k0 + kk + 8 * u;
-    const size_t pk = pk0 + kk + 8 * u;
-    const int kd = k < n_act ? kind[pk] : 2;
-    r.zero[u] = kd != 0;
-    if (kd != 2) {
-      const float4 a = *reinterpret_cast<const float4*>(centres + pk * 128 + ch * 8);
-      const float4 b = *reinterpret_cast<const float4*>(centres + pk * 128 + ch * 8 + 4);
-      r.x[u][0] = a.x; r.x[u][1] = a.y; r.x[u][2] = a.z; r.x[u][3] = a.w;
-      r.x[u][4] = b.x; r.x[u][5] = b.y; r.x[u][6] = b.z; r.x[u][7] = b.w;
-    } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) r.x[u][i] = 0.f;
-    }
-    if (kd == 0) {
-      const uint4 a = *reinterpret_cast<const uint4*>(codes + pk * 8);
-      const uint4 b = *reinterpret_cast<const uint4*>(codes + pk * 8 + 4);
-      r.code[u][0] = a.x; r.code[u][1] = a.y; r.code[u][2] = a.z; r.code[u][3] = a.w;
-      r.code[u][4] = b.x; r.code[u][5] = b.y; r.code[u][6] = b.z; r.code[u][7] = b.w;
-    } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) r.code[u][i] = 0u;
-    }
+    const int kl = kk + 8 * u;
+    const float4 a = *reinterpret_cast<const float4*>(centres + kl * 512 + ch * 32);
+    const float4 b = *reinterpret_cast<const float4*>(centres + kl * 512 + ch * 32 + 16);
+    r.x[u][0] = pack_bf16(a.x, a.y); r.x[u][1] = pack_bf16(a.z, a.w);
+    r.x[u][2] = pack_bf16(b.x, b.y); r.x[u][3] = pack_bf16(b.z, b.w);
+    const uint4 c0 = *reinterpret_cast<const uint4*>(codes + kl * 32);
+    const uint4 c1 = *reinterpret_cast<const uint4*>(codes + kl * 32 + 16);
+    r.code[u][0] = c0.x; r.code[u][1] = c0.y; r.code[u][2] = c0.z; r.code[u][3] = c0.w;
+    r.code[u][4] = c1.x; r.code[u][5] = c1.y; r.code[u][6] = c1.z; r.code[u][7] = c1.w;
   }
 }
 
 // Writes rows (kl * 8 + s) of the tile (K-major, 128-byte swizzle, two d-halves) for this thread's two prototypes.
-__device__ __forceinline__ void at_build_tile(unsigned char* tile, const float* cb, const AtProtoRegs& r, int kk, int ch) {
-  const int g = ch >> 1;
-  const float* cbg = cb + g * 256 + (ch & 1) * 8;          // [C][16] block of subspace g, this chunk's 8 dims
+// kd: 0 decoded (centre + codeword), 1 zero residual (centre), 2 absent (zeros; its bias is -inf).
+__device__ __forceinline__ void at_build_tile(unsigned char* tile, const unsigned char* cb, const AtProtoRegs& r,
+                                              const int (&kd)[2], int kk, int ch) {
+  const int sh = (ch >> 1) * 4;
+  const unsigned char* cbt = cb + ch * 16;                 // + z * 256
   unsigned char* base = tile + (ch >> 3) * kAtHalf;
 #pragma unroll
   for (int u = 0; u < 2; ++u) {
+    uint4 x = make_uint4(r.x[u][0], r.x[u][1], r.x[u][2], r.x[u][3]);
+    if (kd[u] == 2) x = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
-      float o[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) o[i] = r.x[u][i];
-      if (!r.zero[u]) {
-        const uint32_t z = (r.code[u][s] >> (4 * g)) & 15u;
-        const float4 a = *reinterpret_cast<const float4*>(cbg + z * 16);
-        const float4 b = *reinterpret_cast<const float4*>(cbg + z * 16 + 4);
-        o[0] += a.x; o[1] += a.y; o[2] += a.z; o[3] += a.w;
-        o[4] += b.x; o[5] += b.y; o[6] += b.z; o[7] += b.w;
+      uint4 o = x;
+      if (kd[u] == 0) {
+        const uint32_t z = (r.code[u][s] >> sh) & 15u;
+        const uint4 e = *reinterpret_cast<const uint4*>(cbt + z * 256);
+        o.x = add_bf16x2(x.x, e.x); o.y = add_bf16x2(x.y, e.y); o.z = add_bf16x2(x.z, e.z); o.w = add_bf16x2(x.w, e.w);
       }
       const int row = (kk + 8 * u) * 8 + s;                // row & 7 == s
-      const uint4 w = make_uint4(pack_bf16(o[0], o[1]), pack_bf16(o[2], o[3]), pack_bf16(o[4], o[5]), pack_bf16(o[6], o[7]));
-      *reinterpret_cast<uint4*>(base + row * 128 + (((ch & 7) ^ s) << 4)) = w;
+      *reinterpret_cast<uint4*>(base + row * 128 + (((ch & 7) ^ s) << 4)) = o;
     }
   }
 }
 
-__device__ void at_producer_role(unsigned char* sm, const AtBars& B, const CUtensorMap* tmQ, const CUtensorMap* tmRK,
-                                 const CUtensorMap* tmRV, const Dims& D, const Dev& V, const AtArgs& A, const AtPlan& P,
-                                 int ptid) {
+__device__ void at_builder_role(unsigned char* sm, const AtBars& B, const Dims& D, const Dev& V, const AtArgs& A,
+                                const AtPlan& P, int ptid) {
   const int kk = ptid >> 4, ch = ptid & 15;
-  float* cbk_s = reinterpret_cast<float*>(sm + AtSmem::CBK);
-  float* cbv_s = reinterpret_cast<float*>(sm + AtSmem::CBV);
+  unsigned char* cbk_s = sm + AtSmem::CBK;
+  unsigned char* cbv_s = sm + AtSmem::CBV;
   float* bias_s = reinterpret_cast<float*>(sm + AtSmem::Bias);
-  const uint32_t qbytes = 256u * (uint32_t)D.group * (uint32_t)P.tb;   // two boxes {64 bf16, group, tb}
-  uint32_t tcnt = 0, ic = 0;
+  uint32_t tcnt = 0, pcnt = 0;
   int cur_bank = -1;
   const long long g1 = at_span_begin(P, blockIdx.x + 1);
   for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
     const AtSeg sg = at_segment(P, D, A, g, g1);
     g += sg.t1 - sg.t0;
-    if (ptid == 0) {
-      mbar_wait(B.q_empty, (ic & 1) ^ 1);
-      mbar_arrive_expect_tx(B.q_full, qbytes);
-      const int tok = (sg.st * A.layer_count + sg.ll) * A.n_q + sg.rb * P.tb;
-      tma_load_3d(sm + AtSmem::Q, tmQ, 0, sg.hd * D.group, tok, B.q_full);
-      tma_load_3d(sm + AtSmem::Q + 2 * kAtHalf, tmQ, 64, sg.hd * D.group, tok, B.q_full);
-    }
-    ++ic;
-    if (sg.b != cur_bank && sg.t1 > P.nt_near && V.cbk) {    // codebooks of this bank (only the builders read them)
+    if (sg.t1 <= P.nt_near) { tcnt += sg.t1 - sg.t0; continue; }
+    if (sg.b != cur_bank && V.cbk) {   // codebooks of this bank -> bf16, [z][g][16]
+      asm volatile("bar.sync 1, 128;" ::: "memory");      // nobody still builds with the previous bank's codebooks
       const float4* srck = reinterpret_cast<const float4*>(V.cbk + (size_t)sg.b * 2048);
       const float4* srcv = reinterpret_cast<const float4*>(V.cbv + (size_t)sg.b * 2048);
-      for (int e = ptid; e < 512; e += 128) {
-        reinterpret_cast<float4*>(cbk_s)[e] = srck[e];
-        reinterpret_cast<float4*>(cbv_s)[e] = srcv[e];
+      for (int e = ptid; e < 512; e += 128) {              // float4 e = (g, z, quarter)
+        const int gg = e >> 6, z = (e >> 2) & 15, qd = e & 3;
+        const float4 a = srck[e], b = srcv[e];
+        const uint32_t off = (uint32_t)(z * 256 + gg * 32 + qd * 8);
+        *reinterpret_cast<uint2*>(cbk_s + off) = make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w));
+        *reinterpret_cast<uint2*>(cbv_s + off) = make_uint2(pack_bf16(b.x, b.y), pack_bf16(b.z, b.w));
       }
       cur_bank = sg.b;
       asm volatile("bar.sync 1, 128;" ::: "memory");
     }
-    for (int j = sg.t0; j < sg.t1; ++j, ++tcnt) {
+    const int jb = sg.t0 > P.nt_near ? sg.t0 : P.nt_near;
+    tcnt += jb - sg.t0;
+    for (int j = jb; j < sg.t1; ++j, ++tcnt, ++pcnt) {
       const uint32_t stg = tcnt & 1, par = ((tcnt >> 1) & 1) ^ 1;
       unsigned char* ks = sm + AtSmem::K + stg * 2 * kAtHalf;
       unsigned char* vs = sm + AtSmem::V + stg * 2 * kAtHalf;
-      if (j < P.nt_near) {
-        // every producer thread observes every phase of the empty barriers (a parity wait is only meaningful for a
-        // waiter that is at most one phase behind); thread 0 alone issues the copies
-        const int row0 = sg.b * D.Wf * D.T + j * kAtCols;
-        mbar_wait(B.k_empty + stg, par);
-        if (ptid == 0) {
-          mbar_arrive_expect_tx(B.k_full + stg, 2 * kAtHalf);
-          tma_load_2d(ks, tmRK, 0, row0, B.k_full + stg);
-          tma_load_2d(ks + kAtHalf, tmRK, 64, row0, B.k_full + stg);
-        }
-        mbar_wait(B.v_empty + stg, par);
-        if (ptid == 0) {
-          mbar_arrive_expect_tx(B.v_full + stg, 2 * kAtHalf);
-          tma_load_2d(vs, tmRV, 0, row0, B.v_full + stg);
-          tma_load_2d(vs + kAtHalf, tmRV, 64, row0, B.v_full + stg);
-        }
-      } else {
-        const int k0 = (j - P.nt_near) * kAtProto;
-        const size_t pk0 = (size_t)sg.b * D.K + k0;
-        AtProtoRegs rk, rv;
-        at_load_proto(rk, V.c, V.codesK, V.kind, pk0, k0, A.n_act, kk, ch);
-        at_load_proto(rv, V.p, V.codesV, V.kind, pk0, k0, A.n_act, kk, ch);
-        if (ptid < kAtProto) {
-          const int k = k0 + ptid;
-          float bias = -INFINITY;
-          if (k < A.n_act && V.kind[pk0 + ptid] != 2) bias = A.use_bias ? V.logn[pk0 + ptid] * kLog2e : 0.f;
-          bias_s[(tcnt & (kAtBiasRing - 1)) * kAtProto + ptid] = bias;
-        }
-        mbar_wait(B.k_empty + stg, par);
-        at_build_tile(ks, cbk_s, rk, kk, ch);
-        fence_proxy_async_smem();
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        if (ptid == 0) mbar_arrive(B.k_full + stg);
-        mbar_wait(B.v_empty + stg, par);
-        at_build_tile(vs, cbv_s, rv, kk, ch);
-        fence_proxy_async_smem();
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        if (ptid == 0) mbar_arrive(B.v_full + stg);
+      const int k0 = (j - P.nt_near) * kAtProto;
+      mbar_wait(B.stg_full, pcnt & 1);
+      AtProtoRegs rk, rv;
+      at_read_staged(rk, sm + AtSmem::StgC, sm + AtSmem::StgZK, kk, ch);
+      at_read_staged(rv, sm + AtSmem::StgP, sm + AtSmem::StgZV, kk, ch);
+      int kd[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int kl = kk + 8 * u;
+        kd[u] = k0 + kl < A.n_act ? (int)sm[AtSmem::StgKd + kl] : 2;
       }
+      if (ptid < kAtProto) {
+        float bias = -INFINITY;
+        if (k0 + ptid < A.n_act && sm[AtSmem::StgKd + ptid] != 2)
+          bias = A.use_bias ? reinterpret_cast<const float*>(sm + AtSmem::StgLn)[ptid] * kLog2e : 0.f;
+        bias_s[(tcnt & (kAtBiasRing - 1)) * kAtProto + ptid] = bias;
+      }
+      mbar_arrive(B.stg_empty);                            // staged operands are in registers: next tile may land
+      mbar_wait(B.k_empty + stg, par);
+      at_build_tile(ks, cbk_s, rk, kd, kk, ch);
+      fence_proxy_async_smem();
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (ptid == 0) mbar_arrive(B.k_full + stg);
+      mbar_wait(B.v_empty + stg, par);
+      at_build_tile(vs, cbv_s, rv, kd, kk, ch);
+      fence_proxy_async_smem();
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (ptid == 0) mbar_arrive(B.v_full + stg);
     }
   }
-  if (ptid == 0 && ic > 0) mbar_wait(B.q_empty, (ic & 1) ^ 1);   // every MMA of this CTA has completed
 }
 
-// ---- warps 5-12: softmax (thread = query row of M tile w) -----------------------------------------------------
+// ---- warps 0-7: softmax (thread = query row of M tile w) ------------------------------------------------------
 constexpr int kPartStride = 132;   // floats per partial row: O[128], m (natural log units), l, 2 pad (16-byte rows)
 
 __device__ void at_softmax_role(unsigned char* sm, const AtBars& B, uint32_t tmem_base, const Dims& D, const AtArgs& A,
@@ -434,12 +500,15 @@ __device__ void at_softmax_role(unsigned char* sm, const AtBars& B, uint32_t tme
       }
       load_bm(m_ref);
       uint32_t pk[64];
-      float lsum, mx;
+      float lsum;
       for (;;) {
-        if (nvalid < kAtCols) at_row_pass<true>(s_addr, sc2, bm, nvalid, pk, lsum, mx);
-        else at_row_pass<false>(s_addr, sc2, bm, nvalid, pk, lsum, mx);
-        if (!__any_sync(0xffffffffu, mx > kRescaleGap)) break;
-        // some row of this warp ran past its reference maximum: move it and rescale l and O (rare)
+        if (nvalid < kAtCols) at_row_pass<true>(s_addr, sc2, bm, nvalid, pk, lsum);
+        else at_row_pass<false>(s_addr, sc2, bm, nvalid, pk, lsum);
+        if (!__any_sync(0xffffffffu, !(lsum <= kRescaleSum))) break;
+        // some row of this warp ran past its reference maximum (an element above 2^8 makes the sum exceed it): find
+        // the row maxima, move the references up and rescale l and O (rare)
+        const float mx = nvalid < kAtCols ? at_row_max<true>(s_addr, sc2, bm, nvalid)
+                                          : at_row_max<false>(s_addr, sc2, bm, nvalid);
         float alpha = 1.f;
         if (mx > 0.f) {
           alpha = ex2_approx(-mx);
@@ -498,7 +567,7 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* sm = (unsigned char*)(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(sm + AtSmem::Bar);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 18);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + kAtNumBars);
   const AtBars B(bars);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -511,28 +580,33 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
       mbar_init(B.s_full + i, 1); mbar_init(B.p_full + i, 128);
       mbar_init(B.pv_done + i, 1); mbar_init(B.o_empty + i, 128);
     }
+    mbar_init(B.stg_full, 1); mbar_init(B.stg_empty, 128);
     fence_barrier_init();
   }
   // rows of the Q staging area that no Q box ever writes must hold finite values
   for (uint32_t e = threadIdx.x; e < 4 * kAtHalf / 16; e += kAtThreads)
     reinterpret_cast<uint4*>(sm + AtSmem::Q)[e] = make_uint4(0u, 0u, 0u, 0u);
   fence_proxy_async_smem();
-  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  if (warp == 12) tmem_alloc(tmem_slot, 512);
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
 
-  if (warp == 0) {
-    if (lane == 0) at_mma_role(sm, B, tmem_base, D, A, P);
-  } else if (warp < 5) {
-    at_producer_role(sm, B, &tmQ, &tmRK, &tmRV, D, V, A, P, (int)threadIdx.x - 32);
+  if (warp < 8) {
+    reg_inc<kRegsSoftmax>();
+    at_softmax_role(sm, B, tmem_base, D, A, P, part, warp >> 2, warp & 3, lane);
+  } else if (warp < 12) {
+    reg_dec<kRegsBuilder>();
+    at_builder_role(sm, B, D, V, A, P, (int)threadIdx.x - 256);
   } else {
-    at_softmax_role(sm, B, tmem_base, D, A, P, part, (warp - 5) >> 2, warp & 3, lane);
+    reg_dec<kRegsAux>();
+    if (warp == 12 && lane == 0) at_mma_role(sm, B, tmem_base, D, A, P);
+    if (warp == 13 && lane == 0) at_loader_role(sm, B, &tmQ, &tmRK, &tmRV, D, V, A, P);
   }
   tc_fence_before_sync();
   __syncthreads();
-  if (warp == 0) {
+  if (warp == 12) {
     __syncwarp();
     tc_fence_after_sync();
     tmem_dealloc(tmem_base, 512);
@@ -588,7 +662,7 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
 // host side
 // ---------------------------------------------------------------------------------------------------------
 bool tc_attention_supported(const Dims& D) {
-  return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && D.group <= kAtRows;
+  return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && D.group <= kAtRows && D.K % kAtProto == 0;
 }
 
 static int at_rows_tb(const Dims& D, int n_q) {
