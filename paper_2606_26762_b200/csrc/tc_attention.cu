@@ -38,8 +38,14 @@ constexpr uint32_t kAtHalf = 128 * 128; // one [128 rows][64 bf16] swizzled box 
 constexpr int kAtBiasRing = 4;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
+// P is packed to bf16 by TRUNCATION (one PRMT per pair on the ALU pipe; cvt.rn.bf16x2 runs on the 4-lane XU pipe next
+// to MUFU.EX2, the pipe that bounds the softmax).  Truncation alone is biased by -2^-9 relative, so the exponent
+// carries +log2(1 + 2^-9): P^ = (1 + 2^-9) P truncated has zero mean error and the spread of round-to-nearest; the
+// row sum is accumulated from P^ and scaled back by 1 / (1 + 2^-9) once per tile.
+constexpr float kTruncBiasLog2 = 0.0028151f;
+constexpr float kTruncBiasInv = 0.99805068f;
 constexpr float kRescaleSum = 256.f;    // a tile's row sum of P above this moves the reference maximum (P <= 2^8 in bf16)
-constexpr int kRegsSoftmax = 184, kRegsBuilder = 96, kRegsAux = 48;   // 2 * 184 + 96 + 48 = 512 = 4 * 128
+constexpr int kRegsSoftmax = 200, kRegsBuilder = 72, kRegsAux = 40;   // 2 * 200 + 72 + 40 = 512 = 4 * 128
 
 struct AtSmem {   // byte offsets from a 1024-byte aligned base
   static constexpr uint32_t Q = 0;                          // 2 d-halves x [256 rows][128 B]
@@ -186,7 +192,7 @@ __device__ __forceinline__ void at_row_pass(uint32_t s_addr, float sc2, const fl
     if (c < 3) tmem_ld_32x32(s_addr + (c + 1) * 32, a[(c + 1) & 1]);
 #pragma unroll
     for (int i = 0; i < 32; i += 2) {
-      const float b = bm[(c * 32 + i) >> 3];
+      const float b = bm[(c * 32 + i) >> 3] + kTruncBiasLog2;
       const uint64_t x2 = fma_f32x2(pack_f32x2(__uint_as_float(a[c & 1][i]), __uint_as_float(a[c & 1][i + 1])), sc22,
                                     pack_f32x2(b, b));
       float x0, x1;
@@ -197,12 +203,12 @@ __device__ __forceinline__ void at_row_pass(uint32_t s_addr, float sc2, const fl
       }
       const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
       l2 = add_f32x2(l2, pack_f32x2(p0, p1));
-      pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+      pk[c * 16 + (i >> 1)] = __byte_perm(__float_as_uint(p0), __float_as_uint(p1), 0x7632);
     }
   }
   float l0, l1;
   unpack_f32x2(l2, l0, l1);
-  lsum = l0 + l1;
+  lsum = (l0 + l1) * kTruncBiasInv;
 }
 
 struct AtBars {
@@ -215,30 +221,34 @@ struct AtBars {
 constexpr int kAtNumBars = 20;
 
 // ---- warp 12: MMA issuer ------------------------------------------------------------------------------------
-__device__ __forceinline__ void at_issue_s(uint32_t tmem_base, uint32_t q_addr, uint32_t k_addr, int w) {
+// The whole warp runs the role converged (every lane observes every barrier phase); the tcgen05 instructions of a
+// block are issued by one elected lane, so the compiler emits no per-instruction election loop.  Descriptors are a
+// precomputed 64-bit base plus a small constant (the 14-bit address field never carries).
+__device__ __forceinline__ void at_issue_s(uint32_t d_tmem, uint64_t qd, uint64_t kd) {
   constexpr uint32_t idesc = idesc_bf16(128, 128, 0, 0);
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
 #pragma unroll
     for (int kk = 0; kk < 4; ++kk) {
-      const uint64_t ad = desc_kmajor_sw128(q_addr + half * 2 * kAtHalf + w * kAtHalf + kk * 32);
-      const uint64_t bd = desc_kmajor_sw128(k_addr + half * kAtHalf + kk * 32);
-      umma_bf16(tmem_base + w * 128, ad, bd, idesc, (half | kk) != 0);
+      const uint64_t ad = qd + (uint64_t)((half * 2 * kAtHalf + kk * 32) >> 4);
+      const uint64_t bd = kd + (uint64_t)((half * kAtHalf + kk * 32) >> 4);
+      umma_bf16(d_tmem, ad, bd, idesc, (half | kk) != 0);
     }
   }
 }
-__device__ __forceinline__ void at_issue_pv(uint32_t tmem_base, uint32_t v_addr, int w, bool acc) {
+__device__ __forceinline__ void at_issue_pv(uint32_t o_tmem, uint32_t p_tmem, uint64_t vd, bool acc) {
   constexpr uint32_t idesc = idesc_bf16(128, 128, 0, 1);   // B = V~ tile, MN-major (d contiguous)
 #pragma unroll
-  for (int kk = 0; kk < 8; ++kk) {                         // 16 context columns (= MMA K) per instruction
-    const uint64_t bd = desc_mnmajor_sw128(v_addr + kk * 2048, kAtHalf);
-    umma_bf16_ts(tmem_base + 256 + w * 128, tmem_base + w * 128 + kk * 8, bd, idesc, acc || kk != 0);
-  }
+  for (int kk = 0; kk < 8; ++kk)                           // 16 context columns (= MMA K) per instruction
+    umma_bf16_ts(o_tmem, p_tmem + kk * 8, vd + (uint64_t)((kk * 2048) >> 4), idesc, acc || kk != 0);
 }
 
 __device__ void at_mma_role(unsigned char* sm, const AtBars& B, uint32_t tmem_base, const Dims& D, const AtArgs& A,
                             const AtPlan& P) {
-  const uint32_t q_addr = smem_u32(sm + AtSmem::Q), k_addr = smem_u32(sm + AtSmem::K), v_addr = smem_u32(sm + AtSmem::V);
+  const uint64_t qd0 = desc_kmajor_sw128(smem_u32(sm + AtSmem::Q));
+  const uint64_t kd0 = desc_kmajor_sw128(smem_u32(sm + AtSmem::K));
+  const uint64_t vd0 = desc_mnmajor_sw128(smem_u32(sm + AtSmem::V), kAtHalf);
+  constexpr uint64_t kStage = (2 * kAtHalf) >> 4, kQTile = kAtHalf >> 4;
   uint32_t kc = 0, vc = 0, ic = 0, pc[2] = {0, 0}, oc[2] = {0, 0};
   const long long g1 = at_span_begin(P, blockIdx.x + 1);
   for (long long g = at_span_begin(P, blockIdx.x); g < g1;) {
@@ -248,11 +258,14 @@ __device__ void at_mma_role(unsigned char* sm, const AtBars& B, uint32_t tmem_ba
     mbar_wait(B.q_full, ic & 1);
     mbar_wait(B.k_full + (kc & 1), (kc >> 1) & 1);
     tc_fence_after_sync();
-    for (int w = 0; w < sg.ntm; ++w) {
-      at_issue_s(tmem_base, q_addr, k_addr + (kc & 1) * 2 * kAtHalf, w);
-      umma_commit(B.s_full + w);
+    if (elect_one_sync()) {
+      for (int w = 0; w < sg.ntm; ++w) {
+        at_issue_s(tmem_base + w * 128, qd0 + w * kQTile, kd0 + (kc & 1) * kStage);
+        umma_commit(B.s_full + w);
+      }
+      umma_commit(B.k_empty + (kc & 1));
     }
-    umma_commit(B.k_empty + (kc & 1));
+    __syncwarp();
     ++kc;
     for (int jj = 0; jj < n; ++jj) {
       const bool more = jj + 1 < n;
@@ -265,26 +278,27 @@ __device__ void at_mma_role(unsigned char* sm, const AtBars& B, uint32_t tmem_ba
           mbar_wait(B.o_empty + w, (oc[w] & 1) ^ 1);
           ++oc[w];
         }
+        if (more && w == 0) mbar_wait(B.k_full + (kc & 1), (kc >> 1) & 1);
         tc_fence_after_sync();
-        at_issue_pv(tmem_base, v_addr + sv * 2 * kAtHalf, w, jj > 0);
-        umma_commit(B.pv_done + w);
-        if (more) {
-          if (w == 0) {
-            mbar_wait(B.k_full + (kc & 1), (kc >> 1) & 1);
-            tc_fence_after_sync();
+        if (elect_one_sync()) {
+          at_issue_pv(tmem_base + 256 + w * 128, tmem_base + w * 128, vd0 + sv * kStage, jj > 0);
+          umma_commit(B.pv_done + w);
+          if (more) {              // S of the next tile goes after PV_w: P_w aliases S_w
+            at_issue_s(tmem_base + w * 128, qd0 + w * kQTile, kd0 + (kc & 1) * kStage);
+            umma_commit(B.s_full + w);
           }
-          at_issue_s(tmem_base, q_addr, k_addr + (kc & 1) * 2 * kAtHalf, w);   // after PV_w: P_w aliases S_w
-          umma_commit(B.s_full + w);
+          if (w + 1 == sg.ntm) {
+            umma_commit(B.v_empty + sv);
+            if (more) umma_commit(B.k_empty + (kc & 1));
+          }
         }
+        __syncwarp();
       }
-      umma_commit(B.v_empty + sv);
       ++vc;
-      if (more) {
-        umma_commit(B.k_empty + (kc & 1));
-        ++kc;
-      }
+      if (more) ++kc;
     }
-    umma_commit(B.q_empty);
+    if (elect_one_sync()) umma_commit(B.q_empty);
+    __syncwarp();
     ++ic;
   }
 }
@@ -423,9 +437,8 @@ __device__ void at_builder_role(unsigned char* sm, const AtBars& B, const Dims& 
       unsigned char* vs = sm + AtSmem::V + stg * 2 * kAtHalf;
       const int k0 = (j - P.nt_near) * kAtProto;
       mbar_wait(B.stg_full, pcnt & 1);
-      AtProtoRegs rk, rv;
-      at_read_staged(rk, sm + AtSmem::StgC, sm + AtSmem::StgZK, kk, ch);
-      at_read_staged(rv, sm + AtSmem::StgP, sm + AtSmem::StgZV, kk, ch);
+      AtProtoRegs r;
+      at_read_staged(r, sm + AtSmem::StgC, sm + AtSmem::StgZK, kk, ch);
       int kd[2];
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
@@ -438,14 +451,15 @@ __device__ void at_builder_role(unsigned char* sm, const AtBars& B, const Dims& 
           bias = A.use_bias ? reinterpret_cast<const float*>(sm + AtSmem::StgLn)[ptid] * kLog2e : 0.f;
         bias_s[(tcnt & (kAtBiasRing - 1)) * kAtProto + ptid] = bias;
       }
-      mbar_arrive(B.stg_empty);                            // staged operands are in registers: next tile may land
       mbar_wait(B.k_empty + stg, par);
-      at_build_tile(ks, cbk_s, rk, kd, kk, ch);
+      at_build_tile(ks, cbk_s, r, kd, kk, ch);
       fence_proxy_async_smem();
       asm volatile("bar.sync 1, 128;" ::: "memory");
       if (ptid == 0) mbar_arrive(B.k_full + stg);
+      at_read_staged(r, sm + AtSmem::StgP, sm + AtSmem::StgZV, kk, ch);
+      mbar_arrive(B.stg_empty);                            // staged operands are in registers: next tile may land
       mbar_wait(B.v_empty + stg, par);
-      at_build_tile(vs, cbv_s, rv, kd, kk, ch);
+      at_build_tile(vs, cbv_s, r, kd, kk, ch);
       fence_proxy_async_smem();
       asm volatile("bar.sync 1, 128;" ::: "memory");
       if (ptid == 0) mbar_arrive(B.v_full + stg);
@@ -601,7 +615,7 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
     at_builder_role(sm, B, D, V, A, P, (int)threadIdx.x - 256);
   } else {
     reg_dec<kRegsAux>();
-    if (warp == 12 && lane == 0) at_mma_role(sm, B, tmem_base, D, A, P);
+    if (warp == 12) at_mma_role(sm, B, tmem_base, D, A, P);
     if (warp == 13 && lane == 0) at_loader_role(sm, B, &tmQ, &tmRK, &tmRV, D, V, A, P);
   }
   tc_fence_before_sync();
