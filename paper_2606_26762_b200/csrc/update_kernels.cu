@@ -54,36 +54,49 @@ __device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const fl
 
 // ---------------------------------------------------------------------------------------------------------
 // U1 ring append (Alg. 1 l.1): frame f goes to slot f % Wf, transposed from the model-native
-// [stream][layer][T][Hkv][d] to the bank-major ring [bank][Wf][T][d].  16-byte vectors, one per thread.
-// grid.y = 0: K, 1: V.  The first threads of grid.y == 0 also copy grid_pos.
+// [stream][layer][T][Hkv][d] to the bank-major ring [bank][Wf][T][d].  A group of vpr lanes (16-byte vectors of one
+// row) copies kApRows rows of K and of V: all 2 * kApRows loads are in flight before the first store (the copy is
+// latency-bound otherwise), row indices are 32-bit.  The first threads also copy grid_pos and reset the keys.
 // ---------------------------------------------------------------------------------------------------------
+constexpr int kApRows = 4;
 template <bool BF16>
 __global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slot, const uint4* __restrict__ Kin,
                                                           const uint4* __restrict__ Vin,
                                                           const float* __restrict__ grid_pos, int vpr) {
-  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t total = (size_t)D.B * D.T * vpr;
-  if (blockIdx.y == 0) {
-    if (idx < (size_t)D.NS * D.T * 2) {
-      const int st = (int)(idx / (D.T * 2)), e = (int)(idx % (D.T * 2));
-      V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[idx];
-    }
-    if (idx < (size_t)D.B * D.T) V.akey[idx] = ~0ull;      // next frame's assignment keys (see tc_assign.cu)
+  const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (gtid < (uint32_t)(D.NS * D.T * 2)) {
+    const int st = (int)(gtid / (uint32_t)(D.T * 2)), e = (int)(gtid % (uint32_t)(D.T * 2));
+    V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[gtid];
   }
-  const bool valid = idx < total;                          // total is a multiple of vpr: whole rows are valid or not
-  const size_t id = valid ? idx : 0;
-  const int v = (int)(id % vpr);
-  const int j = (int)((id / vpr) % D.T);
-  const int b = (int)(id / ((size_t)vpr * D.T));
-  const int hd = b % D.Hkv, sl = b / D.Hkv;  // sl = stream * L + layer
-  const size_t src = (((size_t)sl * D.T + j) * D.Hkv + hd) * vpr + v;
-  const size_t row = ((size_t)b * D.Wf + slot) * D.T + j;
-  const uint4* in = blockIdx.y ? Vin : Kin;
-  uint4* out = (uint4*)(blockIdx.y ? V.ringV : V.ringK);
-  const uint4 w = in[src];
-  if (valid) out[row * vpr + v] = w;
-  if (blockIdx.y == 0) {                                   // |K_j|^2, reduced over the vpr lanes that hold the row
-    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+  for (uint32_t i = gtid; i < (uint32_t)(D.B * D.T); i += gridDim.x * blockDim.x)
+    V.akey[i] = ~0ull;                                     // next frame's assignment keys (see tc_assign.cu)
+  const uint32_t rows = (uint32_t)(D.B * D.T);
+  const uint32_t grp = gtid / (uint32_t)vpr, v = gtid % (uint32_t)vpr;
+  const uint32_t ngrp = gridDim.x * blockDim.x / (uint32_t)vpr;
+  uint4 wk[kApRows], wv[kApRows];
+  uint32_t orow[kApRows];
+#pragma unroll
+  for (int i = 0; i < kApRows; ++i) {
+    const uint32_t r = grp + (uint32_t)i * ngrp;           // r = b * T + j
+    const bool valid = r < rows;
+    const uint32_t rr = valid ? r : 0u;
+    const uint32_t b = rr / (uint32_t)D.T, j = rr - b * (uint32_t)D.T;
+    const uint32_t sl = b / (uint32_t)D.Hkv, hd = b - sl * (uint32_t)D.Hkv;   // sl = stream * L + layer
+    const size_t src = (((size_t)sl * D.T + j) * D.Hkv + hd) * vpr + v;
+    orow[i] = valid ? (b * (uint32_t)D.Wf + (uint32_t)slot) * (uint32_t)D.T + j : 0xffffffffu;
+    wk[i] = Kin[src];
+    wv[i] = Vin[src];
+  }
+  uint4* outK = (uint4*)V.ringK;
+  uint4* outV = (uint4*)V.ringV;
+#pragma unroll
+  for (int i = 0; i < kApRows; ++i) {
+    const bool valid = orow[i] != 0xffffffffu;
+    if (valid) {
+      outK[(size_t)orow[i] * vpr + v] = wk[i];
+      outV[(size_t)orow[i] * vpr + v] = wv[i];
+    }
+    const uint32_t ww[4] = {wk[i].x, wk[i].y, wk[i].z, wk[i].w};   // |K_j|^2, reduced over the lanes of the row
     float kk = 0.f;
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
@@ -96,15 +109,19 @@ __global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slo
       }
     }
     for (int o = vpr >> 1; o > 0; o >>= 1) kk += __shfl_xor_sync(0xffffffffu, kk, o);
-    if (valid && v == 0) V.ringN[row] = kk;
+    if (valid && v == 0) V.ringN[orow[i]] = kk;
   }
 }
 
 int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const void* Kin, const void* Vin,
                        const float* grid_pos, cudaStream_t s) {
-  const int vpr = D.d * (D.bf16 ? 2 : 4) / 16;
-  const size_t total = (size_t)D.B * D.T * vpr;
-  dim3 grid((unsigned)((total + 255) / 256), 2);
+  const int vpr = D.d * (D.bf16 ? 2 : 4) / 16;             // 8, 16 or 32 lanes per row: groups never straddle a warp
+  const size_t rows = (size_t)D.B * D.T;
+  const size_t groups = (rows + kApRows - 1) / kApRows;
+  size_t threads = groups * vpr;
+  const size_t need = (size_t)D.NS * D.T * 2;              // grid_pos copy
+  if (threads < need) threads = need;
+  const unsigned grid = (unsigned)((threads + 255) / 256);
   if (D.bf16) ring_append_kernel<true><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
   else ring_append_kernel<false><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
   return 1;
@@ -471,26 +488,46 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
 constexpr int kUfThreads = 256, kUfWarps = kUfThreads / 32;
 constexpr int kCbG = 68;   // float4 units per subspace block: 4 q x 16 z + 4 pad
 
-__device__ __forceinline__ void pq_pick(const float4* __restrict__ cb4, const float4* __restrict__ rsc, int g, int li,
-                                        int& code) {
-  float4 r[4];
+// packed fp32 pairs (sm_100 f32x2): one issue slot for two FMAs
+__device__ __forceinline__ uint64_t uf_pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ uint64_t uf_fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
+// Nearest codeword of subspace g to the residual (reading 10: squared L2, lowest index on ties) in the expanded form
+// argmin_z |C[z]|^2 - 2 r.C[z] (|r|^2 is common to all z): 8 packed FMAs per codeword instead of a subtract and an
+// FMA per dimension.  Lane (g, li) evaluates codewords li, li+4, li+8, li+12; a 2-step lexicographic (score, code)
+// min over the 4 lanes of the subspace picks the codeword.  cn = |C[z]|^2 per (g, z).
+__device__ __forceinline__ void pq_pick(const float4* __restrict__ cb4, const float* __restrict__ cn,
+                                        const float4* __restrict__ rsc, int g, int li, int& code) {
+  uint64_t r2[8];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) r[q] = rsc[g * 4 + q];
+  for (int q = 0; q < 4; ++q) {
+    const float4 r = rsc[g * 4 + q];
+    r2[2 * q] = uf_pack2(-2.f * r.x, -2.f * r.y);
+    r2[2 * q + 1] = uf_pack2(-2.f * r.z, -2.f * r.w);
+  }
   float bestd = INFINITY;
   int bz = 0;
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
     const int z = li + 4 * t;
-    float dist = 0.f;
+    uint64_t acc = uf_pack2(cn[g * 16 + z], 0.f);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const float4 cw = cb4[g * kCbG + q * 16 + z];
-      float e;
-      e = r[q].x - cw.x; dist = fmaf(e, e, dist);
-      e = r[q].y - cw.y; dist = fmaf(e, e, dist);
-      e = r[q].z - cw.z; dist = fmaf(e, e, dist);
-      e = r[q].w - cw.w; dist = fmaf(e, e, dist);
+      acc = uf_fma2(r2[2 * q], uf_pack2(cw.x, cw.y), acc);
+      acc = uf_fma2(r2[2 * q + 1], uf_pack2(cw.z, cw.w), acc);
     }
+    float a0, a1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(acc));
+    const float dist = a0 + a1;
     if (dist < bestd) { bestd = dist; bz = z; }           // increasing z within the lane: lowest z on ties
   }
 #pragma unroll
@@ -509,7 +546,9 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   float4* cbk4 = (float4*)smem_raw;                           // [8][68]
   float4* cbv4 = cbk4 + 8 * kCbG;
   float4* scratch = cbv4 + 8 * kCbG;                          // [warps][2][32]
-  uint32_t* keys = (uint32_t*)(scratch + kUfWarps * 64);      // [Tpad]
+  float* cnk = (float*)(scratch + kUfWarps * 64);             // [8][16] |C^K_g[z]|^2
+  float* cnv = cnk + 128;
+  uint32_t* keys = (uint32_t*)(cnv + 128);                    // [Tpad]
   uint32_t* sorted = keys + Tpad;                             // [Tpad]
   int* segstart = (int*)(sorted + Tpad);                      // [Tpad + 1]
   __shared__ int wtot[kUfWarps];
@@ -548,6 +587,17 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     }
   }
   __syncthreads();
+  if (has_cb) {                                               // codeword norms: thread = (side, g, z)
+    const int side = tid >> 7, gz = tid & 127, gg = gz >> 4, z = gz & 15;
+    const float4* cb = side ? cbv4 : cbk4;
+    float n2 = 0.f;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const float4 cw = cb[gg * kCbG + q * 16 + z];
+      n2 = fmaf(cw.x, cw.x, n2); n2 = fmaf(cw.y, cw.y, n2); n2 = fmaf(cw.z, cw.z, n2); n2 = fmaf(cw.w, cw.w, n2);
+    }
+    (side ? cnv : cnk)[gz] = n2;
+  }
   // ---- U4: rank counting sort, segment heads, segment table ----
   for (int i = tid; i < ntok; i += kUfThreads) {
     const uint32_t my = keys[i];
@@ -584,8 +634,8 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   const T* ringK = (const T*)V.ringK + rrow * DH;
   const T* ringV = (const T*)V.ringV + rrow * DH;
   const float* ringS = V.ringS + ((size_t)st * D.Wf + F.slot) * D.T * 2;
-  const double al = (double)H.alpha, be = (double)H.beta, et = (double)H.eta;
-  const double oma = 1.0 - al, omb = 1.0 - be, ome = 1.0 - et;
+  const double et = (double)H.eta, ome = 1.0 - et;
+  const float alf = H.alpha, bef = H.beta;
   const int g = lane >> 2, li = lane & 3;
   float4* rsc = scratch + warp * 64;
 
@@ -599,6 +649,8 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     const float2 mu2 = *(const float2*)(V.mu + pk * 2);
     float mu0 = mu2.x, mu1 = mu2.y;
     float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
+    const int n_old = V.n[pk];                                       // read now: the write-back must not wait for them
+    const uint32_t nres_old = has_cb ? V.nres[pk] : 0u;
     int jn = (int)(sorted[r0] & 0xfffu);
     float ken[4], ven[4];
     load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
@@ -619,8 +671,8 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       }
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
-        c[v] = ema_step(oma, al, c[v], ke[v]);                       // l.8
-        p[v] = ema_step(omb, be, p[v], ve[v]);                       // l.9
+        c[v] = fmaf(alf, ke[v] - c[v], c[v]);                        // l.8  (1 - a) c + a K  =  c + a (K - c)
+        p[v] = fmaf(bef, ve[v] - p[v], p[v]);                        // l.9
       }
       mu0 = ema_step(ome, et, mu0, s0);                              // l.11
       mu1 = ema_step(ome, et, mu1, s1);
@@ -635,8 +687,8 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
         rsc[32 + lane] = make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
         __syncwarp();
         int zk, zv;
-        pq_pick(cbk4, rsc, g, li, zk);
-        pq_pick(cbv4, rsc + 32, g, li, zv);
+        pq_pick(cbk4, cnk, rsc, g, li, zk);
+        pq_pick(cbv4, cnv, rsc + 32, g, li, zv);
         if (li == 0) {
           atomicAdd(V.hist + ((pk * 2 + 0) * 8 + g) * 16 + zk, 1u);
           atomicAdd(V.hist + ((pk * 2 + 1) * 8 + g) * 16 + zv, 1u);
@@ -655,13 +707,13 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     store_shadows<4>(V, pk * DH + lane * 4, c, inv_norm(cc));
     if (lane == 0) {
       const int m = r1 - r0;
-      const int n = V.n[pk] + m;                                     // l.10
+      const int n = n_old + m;                                       // l.10
       V.n[pk] = n;
       V.tau[pk] = F.t;
       V.pos[pk] = (long long)F.ev_frame * D.T + j;
       *(float2*)(V.mu + pk * 2) = make_float2(mu0, mu1);
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
-      if (has_cb) V.nres[pk] += (uint32_t)m;
+      if (has_cb) V.nres[pk] = nres_old + (uint32_t)m;
       V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
       V.logn[pk] = logf((float)n);
       mark_dirty(D, V, b, k, F.epoch);
@@ -676,7 +728,7 @@ int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& 
   if (ntok <= 0) return 0;
   if (D.d == 128 && D.G == 8 && D.C == 16) {
     const int Tpad = (ntok + 3) / 4 * 4;
-    const size_t sm = (size_t)(2 * 8 * kCbG + kUfWarps * 64) * 16 + (size_t)(3 * Tpad + 1) * 4;
+    const size_t sm = (size_t)(2 * 8 * kCbG + kUfWarps * 64) * 16 + 256 * 4 + (size_t)(3 * Tpad + 1) * 4;
     int nsplit = 4 * sm_count / D.B;
     const int max_split = (ntok + 2 * kUfWarps - 1) / (2 * kUfWarps);
     if (nsplit > max_split) nsplit = max_split;
