@@ -11,6 +11,7 @@
 namespace pkv {
 
 constexpr int kMaxS = 8, kMaxG = 8, kMaxC = 16;
+#define PKV_SYN_LOGTAB 4096
 constexpr int kCbPad = 16;  // floats of padding after each subspace's [C][sub] block in shared memory
 
 // Shapes, fixed at create.
@@ -65,6 +66,7 @@ struct Dev {
   ScoreRec* rec;   // [B][K]
   float* logn;     // [B][K]  log n_k (Eq. 4 bias)
   uint32_t* hist;  // [B][K][2][G][C]
+  const double* logtab;  // [PKV_SYN_LOGTAB] log(h + pq_eps), h = 0, 1, ...: built on the host at create (synthesis, Eq. 3)
   float* cbk;      // [B][G][C][sub]  (NULL when the state has no residual statistics)
   float* cbv;
   // synthesis result

@@ -3,6 +3,7 @@
 // update_kernels.cu / query_kernels.cu / tc_*.cu.
 #include <cstdarg>
 #include <cstdio>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -24,6 +25,7 @@ struct protokv_state {
   int last_ev_frame;  // index of the frame evicted by the last append, -1 if none
   int last_n_fill;
   bool codes_valid;   // codes/kind describe the current histograms
+  std::vector<double> logtab;   // host copy of Dev::logtab (source of an asynchronous copy: must outlive it)
   int epoch;          // synthesis epoch (see Dev::dirty_cnt)
   bool use_tc_assign;
   bool use_tc_attn;
@@ -158,6 +160,7 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   v.tau = (int*)take(BK * 4); v.pos = (long long*)take(BK * 8); v.nres = (uint32_t*)take(BK * 4);
   v.rec = (ScoreRec*)take(BK * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
   v.hist = (uint32_t*)take(BK * 2 * D.G * D.C * 4);
+  v.logtab = (const double*)take((size_t)PKV_SYN_LOGTAB * 8);
   if (has_cb) {
     v.cbk = (float*)take((size_t)D.B * D.G * D.C * D.sub * 4);
     v.cbv = (float*)take((size_t)D.B * D.G * D.C * D.sub * 4);
@@ -235,6 +238,11 @@ protokv_state* protokv_create(const protokv_config* cfg) {
     const size_t cb = (size_t)st->D.B * st->D.G * st->D.C * st->D.sub * 4;
     e = cudaMemcpyAsync(st->V.cbk, cfg->codebook_k, cb, cudaMemcpyDeviceToDevice, st->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st->V.cbv, cfg->codebook_v, cb, cudaMemcpyDeviceToDevice, st->stream);
+  }
+  if (e == cudaSuccess) {   // numerators of Eq. 3 in log form (the host's libm, like the definition reads)
+    st->logtab.resize(PKV_SYN_LOGTAB);
+    for (int h = 0; h < PKV_SYN_LOGTAB; ++h) st->logtab[h] = log((double)h + cfg->pq_eps);
+    e = cudaMemcpyAsync((void*)st->V.logtab, st->logtab.data(), (size_t)PKV_SYN_LOGTAB * 8, cudaMemcpyHostToDevice, st->stream);
   }
   if (e != cudaSuccess) {
     fail(PROTOKV_ECUDA, "state initialisation: %s", cudaGetErrorString(e));

@@ -21,6 +21,7 @@ namespace pkv {
 // and are reduced to the 8 best by bitonic merges.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSynThreads = 128;
+constexpr int kSynLogTab = PKV_SYN_LOGTAB;   // entries of Dev::logtab
 constexpr long long kSynInf = 1LL << 58;
 
 struct SynCand {
@@ -58,7 +59,71 @@ __device__ __forceinline__ SynCand syn_add(const SynCand& b, long long cost, uin
 // Work list: the prototypes stamped with the current epoch (Dev::dirty); the codes of the others are still valid.
 // Every block of a bank compacts the bank's stamps into the same list in shared memory (ballot + prefix), then the
 // blocks share the list entries by index.
-__device__ void synthesize_one(const Dims& D, const Hyper& H, const Dev& V, int n_act, size_t pk, int kv);
+//
+// One task = (prototype, K or V side) = one run of Alg. 3 over its G histogram rows, one thread per task.
+// log P = log(h + eps) - log(tot + C eps): the first term comes from a host-built table (Dev::logtab, libm), the
+// second is one fp64 log per subspace -- 8 device logs per task instead of up to 64.
+
+struct SynPrep {          // subspace g as prepared by lane g: the 8 most probable codes, best first
+  long long cost[8];      // -q(g, z) >= 0, kSynInf if there is no such code
+  uint32_t zc[8];
+};
+
+// Raw counts of subspace g (zero-padded to 16).
+__device__ __forceinline__ void syn_load_row(const Dims& D, const uint32_t* Hrow, int g, uint32_t (&h)[16]) {
+  if (D.C == 16) {
+    const uint4* h4 = reinterpret_cast<const uint4*>(Hrow + g * 16);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint4 v = h4[q];
+      h[4 * q] = v.x; h[4 * q + 1] = v.y; h[4 * q + 2] = v.z; h[4 * q + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int z = 0; z < 16; ++z) h[z] = z < D.C ? Hrow[g * D.C + z] : 0u;
+  }
+}
+
+__device__ __forceinline__ void syn_prepare(const Dims& D, const Hyper& H, const Dev& V, const uint32_t (&hrow)[16],
+                                            SynPrep& out) {
+  const int C = D.C;
+  // keys of the C codes: (count + 1) in the high bits, 15 - z in the low nibble; 0 = no such code
+  uint32_t key[16];
+  double tot = 0.0;
+#pragma unroll
+  for (int z = 0; z < 16; ++z) {
+    key[z] = 0u;
+    if (z < C) { tot += (double)hrow[z]; key[z] = ((hrow[z] + 1u) << 4) | (uint32_t)(15 - z); }
+  }
+  // descending bitonic sort of the 16 keys (the best 8 are needed, sorted)
+#pragma unroll
+  for (int kk = 2; kk <= 16; kk <<= 1) {
+#pragma unroll
+    for (int j = kk >> 1; j > 0; j >>= 1) {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const int l = i ^ j;
+        if (l > i) {
+          const uint32_t lo = min(key[i], key[l]), hi = max(key[i], key[l]);
+          const bool desc = (i & kk) == 0;
+          key[i] = desc ? hi : lo; key[l] = desc ? lo : hi;
+        }
+      }
+    }
+  }
+  const double logden = log(tot + (double)C * H.pq_eps);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    out.zc[i] = 15u - (key[i] & 15u);
+    if (key[i] == 0u) out.cost[i] = kSynInf;
+    else if (i > 0 && (key[i] >> 4) == (key[i - 1] >> 4)) out.cost[i] = out.cost[i - 1];
+    else {
+      const uint32_t h = (key[i] >> 4) - 1u;
+      const double lognum = h < (uint32_t)kSynLogTab ? V.logtab[h] : log((double)h + H.pq_eps);
+      out.cost[i] = -llround((lognum - logden) * 16777216.0);
+    }
+  }
+}
 
 __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act, int epoch) {
   extern __shared__ uint16_t syn_list[];      // [K]
@@ -66,112 +131,87 @@ __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H,
   const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t* flags = V.dirty + (size_t)b * D.K;
   int base = 0;
-  for (int k0 = 0; k0 < D.K; k0 += kSynThreads) {
-    const int k = k0 + tid;
-    const bool hit = k < D.K && flags[k] == (uint32_t)epoch;
-    const uint32_t bal = __ballot_sync(0xffffffffu, hit);
-    if (lane == 0) wcnt[warp] = __popc(bal);
-    __syncthreads();
-    int off = base, tot = 0;
+  for (int kb = 0; kb < D.K; kb += 8 * kSynThreads) {          // 8 independent loads in flight per thread
+    uint32_t fl[8];
 #pragma unroll
-    for (int w = 0; w < kSynThreads / 32; ++w) { const int c = wcnt[w]; if (w < warp) off += c; tot += c; }
-    if (hit) syn_list[off + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)k;
-    base += tot;
-    __syncthreads();
+    for (int u = 0; u < 8; ++u) {
+      const int k = kb + u * kSynThreads + tid;
+      fl[u] = k < D.K ? flags[k] : ~(uint32_t)epoch;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int k0 = kb + u * kSynThreads;
+      if (k0 >= D.K) break;                                    // block-uniform
+      const bool hit = fl[u] == (uint32_t)epoch;
+      const uint32_t bal = __ballot_sync(0xffffffffu, hit);
+      if (lane == 0) wcnt[warp] = __popc(bal);
+      __syncthreads();
+      int off = base, tot = 0;
+#pragma unroll
+      for (int w = 0; w < kSynThreads / 32; ++w) { const int c = wcnt[w]; if (w < warp) off += c; tot += c; }
+      if (hit) syn_list[off + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)(k0 + tid);
+      base += tot;
+      __syncthreads();
+    }
   }
-  const int cnt = base;
-  for (int idx = blockIdx.x * kSynThreads + tid; idx < 2 * cnt; idx += gridDim.x * kSynThreads)
-    synthesize_one(D, H, V, n_act, (size_t)b * D.K + syn_list[idx >> 1], idx & 1);
-}
-
-__device__ void synthesize_one(const Dims& D, const Hyper& H, const Dev& V, int n_act, size_t pk, int kv) {
-  const int k = (int)(pk % D.K);
+  const int ntask = 2 * base;
   const bool has_cb = V.cbk != nullptr;
-  const bool present = k < n_act && V.n[pk] >= 1;
-  const bool zero = !has_cb || V.nres[pk] == 0;
-  uint32_t* codes = (kv ? V.codesV : V.codesK) + pk * D.S;
-  if (kv == 0) V.kind[pk] = present ? (zero ? 1 : 0) : 2;
-  if (!present || zero) {
-    for (int s = 0; s < D.S; ++s) codes[s] = 0u;
-    return;
-  }
-  const uint32_t* Hrow = V.hist + (pk * 2 + kv) * D.G * D.C;
-  const int C = D.C, G = D.G;
-  SynCand beam[8];
-#pragma unroll
-  for (int i = 0; i < 8; ++i) { beam[i].c = kSynInf; beam[i].t = 0xffffffffu; }
-  beam[0].c = 0; beam[0].t = 0u;
-  for (int g = 0; g < G; ++g) {
-    // keys of the C codes: (count + 1) in the high bits, 15 - z in the low nibble; 0 = no such code
-    uint32_t key[16];
-    double tot = 0.0;
-#pragma unroll
-    for (int z = 0; z < 16; ++z) {
-      key[z] = 0u;
-      if (z < C) {
-        const uint32_t h = Hrow[g * C + z];
-        tot += (double)h;
-        key[z] = ((h + 1u) << 4) | (uint32_t)(15 - z);
-      }
+  for (int task = blockIdx.x * kSynThreads + tid; task < ntask; task += gridDim.x * kSynThreads) {
+    const int k = (int)syn_list[task >> 1];
+    const int kv = task & 1;
+    const size_t pk = (size_t)b * D.K + k;
+    const bool present = k < n_act && V.n[pk] >= 1;
+    const bool zero = !has_cb || !present || V.nres[pk] == 0;
+    uint32_t* codes = (kv ? V.codesV : V.codesK) + pk * D.S;
+    if (kv == 0) V.kind[pk] = present ? (zero ? 1 : 0) : 2;
+    if (zero) {
+      for (int s = 0; s < D.S; ++s) codes[s] = 0u;
+      continue;
     }
-    const double den = tot + (double)C * H.pq_eps;
-    // descending bitonic sort of the 16 keys (the best 8 are needed, sorted)
+    const uint32_t* Hrow = V.hist + (pk * 2 + kv) * D.G * D.C;
+    SynCand beam[8];
 #pragma unroll
-    for (int kk = 2; kk <= 16; kk <<= 1) {
+    for (int i = 0; i < 8; ++i) { beam[i].c = kSynInf; beam[i].t = 0xffffffffu; }
+    beam[0].c = 0; beam[0].t = 0u;
+    uint32_t hnext[16];
+    syn_load_row(D, Hrow, 0, hnext);
+    for (int g = 0; g < D.G; ++g) {
+      uint32_t hcur[16];
 #pragma unroll
-      for (int j = kk >> 1; j > 0; j >>= 1) {
+      for (int z = 0; z < 16; ++z) hcur[z] = hnext[z];
+      if (g + 1 < D.G) syn_load_row(D, Hrow, g + 1, hnext);    // next row in flight under this subspace's work
+      SynPrep pr;
+      syn_prepare(D, H, V, hcur, pr);
+      SynCand a[8], bb[8], c4[4];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          const int l = i ^ j;
-          if (l > i) {
-            const uint32_t lo = min(key[i], key[l]), hi = max(key[i], key[l]);
-            const bool desc = (i & kk) == 0;
-            key[i] = desc ? hi : lo; key[l] = desc ? lo : hi;
-          }
-        }
-      }
+      for (int j = 0; j < 8; ++j) a[j] = syn_add(beam[0], pr.cost[j], pr.zc[j]);           // R0, ascending
+#pragma unroll
+      for (int j = 0; j < 4; ++j) bb[j] = syn_add(beam[1], pr.cost[j], pr.zc[j]);          // R1
+#pragma unroll
+      for (int i = 0; i < 4; ++i) bb[7 - i] = syn_add(beam[4 + i], pr.cost[0], pr.zc[0]);  // R4 reversed: [R1, rev R4] is bitonic
+      syn_bitonic_merge<8>(bb);
+#pragma unroll
+      for (int j = 0; j < 2; ++j) c4[j] = syn_add(beam[2], pr.cost[j], pr.zc[j]);          // R2
+#pragma unroll
+      for (int j = 0; j < 2; ++j) c4[3 - j] = syn_add(beam[3], pr.cost[j], pr.zc[j]);      // R3 reversed
+      syn_bitonic_merge<4>(c4);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) a[i] = syn_min(a[i], bb[7 - i]);                         // 8 best of R0 u R1 u R4, bitonic
+      syn_bitonic_merge<8>(a);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) a[4 + i] = syn_min(a[4 + i], c4[3 - i]);                 // 8 best of all 20, bitonic
+      syn_bitonic_merge<8>(a);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) beam[i] = a[i];
     }
-    long long cost[8];
-    uint32_t zc[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      zc[i] = 15u - (key[i] & 15u);
-      if (key[i] == 0u) cost[i] = kSynInf;
-      else if (i > 0 && (key[i] >> 4) == (key[i - 1] >> 4)) cost[i] = cost[i - 1];
-      else {
-        const double P = ((double)((key[i] >> 4) - 1u) + H.pq_eps) / den;
-        cost[i] = -llround(log(P) * 16777216.0);
+    for (int s = 0; s < 8; ++s) {
+      if (s < D.S) {
+        uint32_t packed = 0u;
+        if (beam[s].c < kSynInf)
+          for (int g = 0; g < D.G; ++g) packed |= ((beam[s].t >> (4 * (D.G - 1 - g))) & 15u) << (4 * g);
+        codes[s] = packed;
       }
-    }
-    SynCand a[8], b[8], c4[4];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) a[j] = syn_add(beam[0], cost[j], zc[j]);                 // R0, ascending
-#pragma unroll
-    for (int j = 0; j < 4; ++j) b[j] = syn_add(beam[1], cost[j], zc[j]);                 // R1
-#pragma unroll
-    for (int i = 0; i < 4; ++i) b[7 - i] = syn_add(beam[4 + i], cost[0], zc[0]);         // R4 reversed: [R1, rev R4] is bitonic
-    syn_bitonic_merge<8>(b);
-#pragma unroll
-    for (int j = 0; j < 2; ++j) c4[j] = syn_add(beam[2], cost[j], zc[j]);                // R2
-#pragma unroll
-    for (int j = 0; j < 2; ++j) c4[3 - j] = syn_add(beam[3], cost[j], zc[j]);            // R3 reversed
-    syn_bitonic_merge<4>(c4);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) a[i] = syn_min(a[i], b[7 - i]);                          // 8 best of R0 u R1 u R4, bitonic
-    syn_bitonic_merge<8>(a);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) a[4 + i] = syn_min(a[4 + i], c4[3 - i]);                 // 8 best of all 20, bitonic
-    syn_bitonic_merge<8>(a);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) beam[i] = a[i];
-  }
-#pragma unroll
-  for (int s = 0; s < 8; ++s) {
-    if (s < D.S) {
-      uint32_t packed = 0u;
-      if (beam[s].c < kSynInf)
-        for (int g = 0; g < G; ++g) packed |= ((beam[s].t >> (4 * (G - 1 - g))) & 15u) << (4 * g);
-      codes[s] = packed;
     }
   }
 }
