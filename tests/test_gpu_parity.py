@@ -92,6 +92,25 @@ def test_c5_shape_multi_stream():
 
 
 # ---------------------------------------------------------------------------------------------------------
+# full sizes in the launch configuration bench.py times (C3: 112 banks, C5: 64 banks): the same grids, tile plans and
+# stream-K splits as the timed runs; the oracle follows a sample of banks (first, middle, last) frame by frame and
+# checks a sample of query rows -- every output it checks is computed one by one from the definition
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,banks,frames", [("c3", [0, 57, 111], 25), ("c5", [0, 31, 63], 13)])
+def test_full_size_bench_configuration_sampled(name, banks, frames):
+    spec = gen.spec_for(name, n_frames=frames)
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, banks)
+    stats = run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=frames - 1)
+    assert stats["scored"] > 0
+    compare_codes(gpu, oracles, spec.G)
+    rows = spec.n_query_tokens * (spec.n_q_heads // spec.n_kv_heads)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=True, rows_sample=range(0, rows, 11))
+    for b in banks:                                          # mass conservation on the sampled banks
+        assert int(gpu.export_state(b)["n"].sum()) == (spec.n_frames - spec.near_frames) * spec.T
+
+
+# ---------------------------------------------------------------------------------------------------------
 # config 4 cells (small ends of the sweep): K_max 256 with W_f 4, and a bank larger than the stream ever fills
 # ---------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("k_max,near", [(256, 4), (4096, 4)])
