@@ -7,8 +7,8 @@
 namespace pkv {
 
 // ---------------------------------------------------------------------------------------------------------
-// Q1 synthesis.  One thread per (bank, prototype, K|V); everything lives in registers (fully unrolled sorting
-// networks, no dynamically indexed arrays).
+// Q1 synthesis.  Task = (bank, prototype, K|V); sorting networks are fully unrolled and live in registers (no
+// dynamically indexed arrays).
 //
 // Scores are the fixed-point log-probabilities of Eq. 3, q(g,z) = llround(2^24 log((H[g,z]+eps)/(sum+C eps)))
 // (reading 13), tuples are ordered by (sum of q descending, tuple ascending lexicographically, z_1 most
@@ -20,27 +20,26 @@ namespace pkv {
 //   R4 = beam[4..7] + code[0]
 // and are reduced to the 8 best by bitonic merges.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kSynThreads = 128;
-constexpr int kSynLogTab = PKV_SYN_LOGTAB;   // entries of Dev::logtab
-constexpr long long kSynInf = 1LL << 58;
+constexpr int kSynThreads = 256;
+constexpr int kSynLanes = 4;                        // preparing lanes per task (each takes G / 4 subspaces)
+constexpr int kSynTasks = kSynThreads / kSynLanes;  // tasks per block and round
+constexpr int kSynLogTab = PKV_SYN_LOGTAB;          // entries of Dev::logtab
+constexpr int kSynWords = 9;                        // shared words per (task, subspace): 8 costs + 8 packed codes
 
-struct SynCand {
-  long long c;   // cost = -sum q  (>= 0), smaller is better
-  uint32_t t;    // tuple, z_1 in the most significant used nibble; smaller is better on equal cost
-};
+// A candidate is ONE 64-bit key: cost = -sum q (>= 0, smaller is better) in the high word, the tuple (z_1 in the most
+// significant used nibble; smaller is better on equal cost) in the low word -- the total order of reading 13 is the
+// order of the keys.  ~0 = no candidate.  A per-subspace cost is below 2^29 for every P >= 1e-13 (-log P * 2^24), the
+// sum over G = 8 subspaces is saturated at 2^32 - 2 (tuples that improbable never reach the top S).
+typedef unsigned long long SynKey;
+constexpr SynKey kSynNone = ~0ull;
+constexpr uint32_t kSynCostNone = 0xffffffffu;
 
-__device__ __forceinline__ void syn_ce(SynCand& a, SynCand& b) {   // afterwards a <= b
-  const bool sw = b.c < a.c || (b.c == a.c && b.t < a.t);
-  const long long c0 = sw ? b.c : a.c, c1 = sw ? a.c : b.c;
-  const uint32_t t0 = sw ? b.t : a.t, t1 = sw ? a.t : b.t;
-  a.c = c0; a.t = t0; b.c = c1; b.t = t1;
-}
-__device__ __forceinline__ SynCand syn_min(const SynCand& a, const SynCand& b) {
-  const bool sw = b.c < a.c || (b.c == a.c && b.t < a.t);
-  return sw ? b : a;
+__device__ __forceinline__ void syn_ce(SynKey& a, SynKey& b) {   // afterwards a <= b
+  const SynKey lo = a < b ? a : b, hi = a < b ? b : a;
+  a = lo; b = hi;
 }
 template <int N>
-__device__ __forceinline__ void syn_bitonic_merge(SynCand (&x)[N]) {   // bitonic input -> ascending
+__device__ __forceinline__ void syn_bitonic_merge(SynKey (&x)[N]) {   // bitonic input -> ascending
 #pragma unroll
   for (int j = N >> 1; j > 0; j >>= 1) {
 #pragma unroll
@@ -48,52 +47,42 @@ __device__ __forceinline__ void syn_bitonic_merge(SynCand (&x)[N]) {   // bitoni
       if ((i & j) == 0) syn_ce(x[i], x[i | j]);
   }
 }
-__device__ __forceinline__ SynCand syn_add(const SynCand& b, long long cost, uint32_t z) {
-  SynCand r;
-  r.c = b.c + cost;
-  r.c = r.c < kSynInf ? r.c : kSynInf;
-  r.t = (b.t << 4) | z;
-  return r;
+__device__ __forceinline__ SynKey syn_add(SynKey b, uint32_t cost, uint32_t z) {
+  if (b == kSynNone || cost == kSynCostNone) return kSynNone;
+  unsigned long long c = (b >> 32) + cost;
+  c = c < 0xfffffffeull ? c : 0xfffffffeull;
+  return (c << 32) | (uint32_t)(((uint32_t)b << 4) | z);
 }
 
-// Work list: the prototypes stamped with the current epoch (Dev::dirty); the codes of the others are still valid.
-// Every block of a bank compacts the bank's stamps into the same list in shared memory (ballot + prefix), then the
-// blocks share the list entries by index.
-//
-// One task = (prototype, K or V side) = one run of Alg. 3 over its G histogram rows, one thread per task.
+// Subspace g of one task: the 8 most probable codes, best first, as fixed-point costs -q(g, z) (kSynCostNone if there
+// is no such code) and the codes packed into nibbles (code i in bits [4i, 4i+4)).
 // log P = log(h + eps) - log(tot + C eps): the first term comes from a host-built table (Dev::logtab, libm), the
-// second is one fp64 log per subspace -- 8 device logs per task instead of up to 64.
-
-struct SynPrep {          // subspace g as prepared by lane g: the 8 most probable codes, best first
-  long long cost[8];      // -q(g, z) >= 0, kSynInf if there is no such code
-  uint32_t zc[8];
-};
-
-// Raw counts of subspace g (zero-padded to 16).
-__device__ __forceinline__ void syn_load_row(const Dims& D, const uint32_t* Hrow, int g, uint32_t (&h)[16]) {
-  if (D.C == 16) {
-    const uint4* h4 = reinterpret_cast<const uint4*>(Hrow + g * 16);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const uint4 v = h4[q];
-      h[4 * q] = v.x; h[4 * q + 1] = v.y; h[4 * q + 2] = v.z; h[4 * q + 3] = v.w;
-    }
-  } else {
-#pragma unroll
-    for (int z = 0; z < 16; ++z) h[z] = z < D.C ? Hrow[g * D.C + z] : 0u;
-  }
-}
-
-__device__ __forceinline__ void syn_prepare(const Dims& D, const Hyper& H, const Dev& V, const uint32_t (&hrow)[16],
-                                            SynPrep& out) {
+// second is one fp64 log.
+__device__ __forceinline__ void syn_prepare(const Dims& D, const Hyper& H, const Dev& V, const uint32_t* Hrow, int g,
+                                            uint32_t (&cost)[8], uint32_t& zpack) {
   const int C = D.C;
   // keys of the C codes: (count + 1) in the high bits, 15 - z in the low nibble; 0 = no such code
   uint32_t key[16];
   double tot = 0.0;
+  if (C == 16) {
+    const uint4* h4 = reinterpret_cast<const uint4*>(Hrow + g * 16);
 #pragma unroll
-  for (int z = 0; z < 16; ++z) {
-    key[z] = 0u;
-    if (z < C) { tot += (double)hrow[z]; key[z] = ((hrow[z] + 1u) << 4) | (uint32_t)(15 - z); }
+    for (int q = 0; q < 4; ++q) {
+      const uint4 v = h4[q];
+      key[4 * q] = v.x; key[4 * q + 1] = v.y; key[4 * q + 2] = v.z; key[4 * q + 3] = v.w;
+    }
+#pragma unroll
+    for (int z = 0; z < 16; ++z) { tot += (double)key[z]; key[z] = ((key[z] + 1u) << 4) | (uint32_t)(15 - z); }
+  } else {
+#pragma unroll
+    for (int z = 0; z < 16; ++z) {
+      key[z] = 0u;
+      if (z < C) {
+        const uint32_t h = Hrow[g * C + z];
+        tot += (double)h;
+        key[z] = ((h + 1u) << 4) | (uint32_t)(15 - z);
+      }
+    }
   }
   // descending bitonic sort of the 16 keys (the best 8 are needed, sorted)
 #pragma unroll
@@ -112,22 +101,35 @@ __device__ __forceinline__ void syn_prepare(const Dims& D, const Hyper& H, const
     }
   }
   const double logden = log(tot + (double)C * H.pq_eps);
+  zpack = 0u;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    out.zc[i] = 15u - (key[i] & 15u);
-    if (key[i] == 0u) out.cost[i] = kSynInf;
-    else if (i > 0 && (key[i] >> 4) == (key[i - 1] >> 4)) out.cost[i] = out.cost[i - 1];
+    zpack |= (15u - (key[i] & 15u)) << (4 * i);
+    if (key[i] == 0u) cost[i] = kSynCostNone;
+    else if (i > 0 && (key[i] >> 4) == (key[i - 1] >> 4)) cost[i] = cost[i - 1];
     else {
       const uint32_t h = (key[i] >> 4) - 1u;
       const double lognum = h < (uint32_t)kSynLogTab ? V.logtab[h] : log((double)h + H.pq_eps);
-      out.cost[i] = -llround((lognum - logden) * 16777216.0);
+      const long long q = -llround((lognum - logden) * 16777216.0);
+      cost[i] = (uint32_t)(q < 0 ? 0 : (q < 0xfffffffell ? q : 0xfffffffell));
     }
   }
 }
 
+// Work list: the prototypes stamped with the current epoch (Dev::dirty); the codes of the others are still valid.
+// Every block of a bank compacts the bank's stamps into the same list in shared memory (ballot + prefix), then the
+// blocks share the list entries by index.
+//
+// One task = (prototype, K or V side) = one run of Alg. 3 over its G histogram rows.  A block takes kSynTasks tasks per
+// round in two phases: (1) lane (task, g mod 4) prepares subspaces g, g + 4 -- loads the 16 counts, sorts the keys, turns the 8
+// best into fixed-point costs -- and parks them in shared memory ([g][word][task]: phase 2 reads are conflict-free);
+// (2) one thread per task walks the beam recurrence over g = 0..G-1.  Phase 1 is the 8-wide part of the work; phase 2
+// is the dependent chain that sets the kernel's duration, kept short by the single-key candidates.
 __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act, int epoch) {
   extern __shared__ uint16_t syn_list[];      // [K]
   __shared__ int wcnt[kSynThreads / 32];
+  __shared__ uint32_t prep[8 * kSynWords * kSynTasks];
+  __shared__ uint8_t tstate[kSynTasks];       // 0 decode, 1 zero residual / absent / no task
   const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t* flags = V.dirty + (size_t)b * D.K;
   int base = 0;
@@ -156,70 +158,97 @@ __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H,
   }
   const int ntask = 2 * base;
   const bool has_cb = V.cbk != nullptr;
-  for (int task = blockIdx.x * kSynThreads + tid; task < ntask; task += gridDim.x * kSynThreads) {
-    const int k = (int)syn_list[task >> 1];
-    const int kv = task & 1;
-    const size_t pk = (size_t)b * D.K + k;
-    const bool present = k < n_act && V.n[pk] >= 1;
-    const bool zero = !has_cb || !present || V.nres[pk] == 0;
-    uint32_t* codes = (kv ? V.codesV : V.codesK) + pk * D.S;
-    if (kv == 0) V.kind[pk] = present ? (zero ? 1 : 0) : 2;
-    if (zero) {
-      for (int s = 0; s < D.S; ++s) codes[s] = 0u;
-      continue;
-    }
-    const uint32_t* Hrow = V.hist + (pk * 2 + kv) * D.G * D.C;
-    SynCand beam[8];
+  for (int t0 = blockIdx.x * kSynTasks; t0 < ntask; t0 += gridDim.x * kSynTasks) {   // block-uniform
+    {   // ---- phase 1: thread = (task, subspace) ----
+      const int tl = tid / kSynLanes, g0 = tid % kSynLanes, task = t0 + tl;
+      bool decode = false;
+      size_t pk = 0;
+      int kv = 0;
+      if (task < ntask) {
+        const int k = (int)syn_list[task >> 1];
+        kv = task & 1;
+        pk = (size_t)b * D.K + k;
+        const bool present = k < n_act && V.n[pk] >= 1;
+        const bool zero = !has_cb || !present || V.nres[pk] == 0;
+        decode = !zero;
+        if (g0 == 0) {
+          tstate[tl] = zero ? 1 : 0;
+          if (kv == 0) V.kind[pk] = present ? (zero ? 1 : 0) : 2;
+        }
+      } else if (g0 == 0) {
+        tstate[tl] = 1;
+      }
+      if (decode) {
+        for (int g = g0; g < D.G; g += kSynLanes) {
+          uint32_t cost[8], zpack;
+          syn_prepare(D, H, V, V.hist + (pk * 2 + kv) * D.G * D.C, g, cost, zpack);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { beam[i].c = kSynInf; beam[i].t = 0xffffffffu; }
-    beam[0].c = 0; beam[0].t = 0u;
-    uint32_t hnext[16];
-    syn_load_row(D, Hrow, 0, hnext);
-    for (int g = 0; g < D.G; ++g) {
-      uint32_t hcur[16];
-#pragma unroll
-      for (int z = 0; z < 16; ++z) hcur[z] = hnext[z];
-      if (g + 1 < D.G) syn_load_row(D, Hrow, g + 1, hnext);    // next row in flight under this subspace's work
-      SynPrep pr;
-      syn_prepare(D, H, V, hcur, pr);
-      SynCand a[8], bb[8], c4[4];
-#pragma unroll
-      for (int j = 0; j < 8; ++j) a[j] = syn_add(beam[0], pr.cost[j], pr.zc[j]);           // R0, ascending
-#pragma unroll
-      for (int j = 0; j < 4; ++j) bb[j] = syn_add(beam[1], pr.cost[j], pr.zc[j]);          // R1
-#pragma unroll
-      for (int i = 0; i < 4; ++i) bb[7 - i] = syn_add(beam[4 + i], pr.cost[0], pr.zc[0]);  // R4 reversed: [R1, rev R4] is bitonic
-      syn_bitonic_merge<8>(bb);
-#pragma unroll
-      for (int j = 0; j < 2; ++j) c4[j] = syn_add(beam[2], pr.cost[j], pr.zc[j]);          // R2
-#pragma unroll
-      for (int j = 0; j < 2; ++j) c4[3 - j] = syn_add(beam[3], pr.cost[j], pr.zc[j]);      // R3 reversed
-      syn_bitonic_merge<4>(c4);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) a[i] = syn_min(a[i], bb[7 - i]);                         // 8 best of R0 u R1 u R4, bitonic
-      syn_bitonic_merge<8>(a);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) a[4 + i] = syn_min(a[4 + i], c4[3 - i]);                 // 8 best of all 20, bitonic
-      syn_bitonic_merge<8>(a);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) beam[i] = a[i];
-    }
-#pragma unroll
-    for (int s = 0; s < 8; ++s) {
-      if (s < D.S) {
-        uint32_t packed = 0u;
-        if (beam[s].c < kSynInf)
-          for (int g = 0; g < D.G; ++g) packed |= ((beam[s].t >> (4 * (D.G - 1 - g))) & 15u) << (4 * g);
-        codes[s] = packed;
+          for (int i = 0; i < 8; ++i) prep[(g * kSynWords + i) * kSynTasks + tl] = cost[i];
+          prep[(g * kSynWords + 8) * kSynTasks + tl] = zpack;
+        }
       }
     }
+    __syncthreads();
+    if (tid < kSynTasks && t0 + tid < ntask) {   // ---- phase 2: thread = task ----
+      const int task = t0 + tid;
+      const int k = (int)syn_list[task >> 1];
+      const size_t pk = (size_t)b * D.K + k;
+      uint32_t* codes = ((task & 1) ? V.codesV : V.codesK) + pk * D.S;
+      if (tstate[tid]) {
+        for (int s = 0; s < D.S; ++s) codes[s] = 0u;
+      } else {
+        SynKey beam[8];
+#pragma unroll
+        for (int i = 1; i < 8; ++i) beam[i] = kSynNone;
+        beam[0] = 0ull;
+        for (int g = 0; g < D.G; ++g) {
+          uint32_t cost[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) cost[i] = prep[(g * kSynWords + i) * kSynTasks + tid];
+          const uint32_t zp = prep[(g * kSynWords + 8) * kSynTasks + tid];
+          SynKey a[8], bb[8], c4[4];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) a[j] = syn_add(beam[0], cost[j], (zp >> (4 * j)) & 15u);          // R0, ascending
+#pragma unroll
+          for (int j = 0; j < 4; ++j) bb[j] = syn_add(beam[1], cost[j], (zp >> (4 * j)) & 15u);         // R1
+#pragma unroll
+          for (int i = 0; i < 4; ++i) bb[7 - i] = syn_add(beam[4 + i], cost[0], zp & 15u);              // R4 reversed: [R1, rev R4] is bitonic
+          syn_bitonic_merge<8>(bb);
+#pragma unroll
+          for (int j = 0; j < 2; ++j) c4[j] = syn_add(beam[2], cost[j], (zp >> (4 * j)) & 15u);         // R2
+#pragma unroll
+          for (int j = 0; j < 2; ++j) c4[3 - j] = syn_add(beam[3], cost[j], (zp >> (4 * j)) & 15u);     // R3 reversed
+          syn_bitonic_merge<4>(c4);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) a[i] = a[i] < bb[7 - i] ? a[i] : bb[7 - i];                       // 8 best of R0 u R1 u R4, bitonic
+          syn_bitonic_merge<8>(a);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) a[4 + i] = a[4 + i] < c4[3 - i] ? a[4 + i] : c4[3 - i];           // 8 best of all 20, bitonic
+          syn_bitonic_merge<8>(a);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) beam[i] = a[i];
+        }
+#pragma unroll
+        for (int s = 0; s < 8; ++s) {
+          if (s < D.S) {
+            uint32_t packed = 0u;
+            if (beam[s] != kSynNone) {
+              const uint32_t t = (uint32_t)beam[s];
+              for (int g = 0; g < D.G; ++g) packed |= ((t >> (4 * (D.G - 1 - g))) & 15u) << (4 * g);
+            }
+            codes[s] = packed;
+          }
+        }
+      }
+    }
+    __syncthreads();
   }
 }
 
 int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s) {
   // grid-stride over each bank's work list; its length is only known on the device
-  int per_bank = (2 * D.K + kSynThreads - 1) / kSynThreads;
-  const int cap = (6 * sm_count + D.B - 1) / D.B;
+  int per_bank = (2 * D.K + kSynTasks - 1) / kSynTasks;
+  const int cap = (8 * sm_count + D.B - 1) / D.B;
   if (per_bank > cap) per_bank = cap;
   if (per_bank < 1) per_bank = 1;
   synthesis_kernel<<<dim3(per_bank, D.B), kSynThreads, (size_t)D.K * 2, s>>>(D, H, V, n_act, epoch);
