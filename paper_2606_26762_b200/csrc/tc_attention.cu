@@ -646,22 +646,29 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
   }
   const float* base = part + ((size_t)item * P.nsplit * kAtRows + rin) * kPartStride;
   const size_t pstride = (size_t)kAtRows * kPartStride;
-  float M = -INFINITY;
-  for (int sp = 0; sp < np; ++sp) {
-    const float2 ml = *reinterpret_cast<const float2*>(base + sp * pstride + 128);
-    if (ml.y > 0.f) M = fmaxf(M, ml.x);
-  }
-  float l = 0.f;
+  // online merge, four pieces' loads in flight at a time
+  float M = -INFINITY, l = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  for (int sp = 0; sp < np; ++sp) {
-    const float* ps = base + sp * pstride;
-    const float2 ml = *reinterpret_cast<const float2*>(ps + 128);
-    if (!(ml.y > 0.f)) continue;
-    const float wgt = __expf(ml.x - M);
-    const float4 v = *reinterpret_cast<const float4*>(ps + lane * 4);
-    l = fmaf(ml.y, wgt, l);
-    acc.x = fmaf(v.x, wgt, acc.x); acc.y = fmaf(v.y, wgt, acc.y);
-    acc.z = fmaf(v.z, wgt, acc.z); acc.w = fmaf(v.w, wgt, acc.w);
+  for (int sp0 = 0; sp0 < np; sp0 += 4) {
+    float2 ml[4];
+    float4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int sp = sp0 + u < np ? sp0 + u : np - 1;        // clamp: a repeated piece is skipped below
+      const float* ps = base + sp * pstride;
+      ml[u] = *reinterpret_cast<const float2*>(ps + 128);
+      v[u] = *reinterpret_cast<const float4*>(ps + lane * 4);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (sp0 + u >= np || !(ml[u].y > 0.f)) continue;
+      const float Mn = fmaxf(M, ml[u].x);
+      const float so = __expf(M - Mn), sn = __expf(ml[u].x - Mn);   // M = -inf: so = 0
+      l = fmaf(l, so, ml[u].y * sn);
+      acc.x = fmaf(acc.x, so, v[u].x * sn); acc.y = fmaf(acc.y, so, v[u].y * sn);
+      acc.z = fmaf(acc.z, so, v[u].z * sn); acc.w = fmaf(acc.w, so, v[u].w * sn);
+      M = Mn;
+    }
   }
   const float inv = l > 0.f ? 1.f / l : 0.f;
   const size_t ooff = (((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh;
