@@ -124,6 +124,26 @@ def test_c4_cells(k_max, near):
 
 
 # ---------------------------------------------------------------------------------------------------------
+# Eq. 1's idle term and non-default hyper-parameters: with T_idle = 2 frames most prototypes are idle at any step
+# (the default 120 frames never triggers in a short stream), larger lambda_sp / lambda_idle move decisions, and the
+# EMA rates differ per statistic
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_idle_penalty_and_hyperparameters(force_simt):
+    spec = gen.spec_for("c2", n_frames=32)
+    hyper = dict(t_idle=2, lambda_idle=0.05, lambda_sp=0.3, alpha=0.1, beta=0.2, eta=0.02)
+    gpu = make_gpu(spec, flags=FORCE_SIMT if force_simt else 0, **hyper)
+    oracles = make_oracles(spec, [0, 3], **hyper)
+    stats = run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=8)
+    assert stats["scored"] > 0
+    st = oracles[0].state()
+    t_last = spec.n_frames - 1
+    idle = int(((t_last - st["tau"][st["active"].astype(bool)]) > hyper["t_idle"]).sum())
+    assert idle > 50, f"only {idle} idle prototypes: the idle term is not exercised"
+    _query_and_check(spec, gpu, oracles)
+
+
+# ---------------------------------------------------------------------------------------------------------
 # degenerate cases of the method
 # ---------------------------------------------------------------------------------------------------------
 def test_empty_and_near_only_states():
