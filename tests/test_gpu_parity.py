@@ -13,7 +13,7 @@ import torch
 
 import gen
 from gpu_helpers import (make_gpu, make_oracles, run_stream, compare_ring, compare_codes, compare_attention,
-                         compare_state, new_stats)
+                         compare_state, new_stats, step_teacher_forced)
 from oracle import FLAG_NEAR_ONLY, FLAG_FAR_ONLY, FLAG_NO_MASS_BIAS, FLAG_MAH_SQUARED
 from paper_2606_26762_b200 import ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT
 
@@ -141,6 +141,63 @@ def test_idle_penalty_and_hyperparameters(force_simt):
     idle = int(((t_last - st["tau"][st["active"].astype(bool)]) > hyper["t_idle"]).sum())
     assert idle > 50, f"only {idle} idle prototypes: the idle term is not exercised"
     _query_and_check(spec, gpu, oracles)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# long stream: the bank has been full for > 100 frames, segments hold several tokens per prototype, histograms are
+# deep, and with the default T_idle = 120 frames the idle term of Eq. 1 starts to fire near the end
+# ---------------------------------------------------------------------------------------------------------
+def test_c2_long_stream_steady_state():
+    spec = gen.spec_for("c2", n_frames=150)
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [1])
+    stats = run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=30)
+    assert stats["scored"] > 100 * spec.T
+    st = oracles[1].state()
+    assert int(st["n"].max()) >= 8                           # prototypes that absorbed many tokens
+    assert int(((spec.n_frames - 1 - st["tau"]) > 120).sum()) > 0, "no prototype went idle"
+    compare_ring(gpu, oracles)
+    _query_and_check(spec, gpu, oracles)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 2), run_synthesis=True, rows_sample=range(0, 224, 3))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the lazily moved reference maximum of the fused attention: keys of the later ring slots are 8x larger, so the
+# logits of later tiles exceed the first tile's row maximum by far more than the 2^8 head-room and O, l have to be
+# rescaled in flight (tcgen05 kernel) -- same inputs to the oracle, which has no such mechanism
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_attention_reference_maximum_moves(force_simt):
+    spec = gen.spec_for("c2", n_frames=24)
+    gpu = make_gpu(spec, flags=FORCE_SIMT if force_simt else 0)
+    oracles = make_oracles(spec, [0, 2])
+    stats = new_stats()
+    s = gen.grid_positions(spec)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        if f % spec.near_frames >= 6:                        # ring slot = f mod W_f; exact in bf16
+            K = K * 8
+        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats)
+    Q = gen.queries(spec, 0)
+    compare_codes(gpu, oracles, spec.G)
+    worst = compare_attention(spec, gpu, oracles, Q, run_synthesis=False)
+    # the construction does what it claims: the kernel walks the ring in slot order, slot 0 holds frame 16 (unscaled);
+    # for most rows the largest near-window logit lies far above the maximum over that first tile
+    from gpu_helpers import bank_frame
+    q = Q[0, 0, :, 0:7, :].float().numpy().reshape(-1, spec.head_dim)
+    first = None
+    top = np.full(q.shape[0], -np.inf)
+    for f in range(spec.n_frames - spec.near_frames, spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        if f % spec.near_frames >= 6:
+            K = K * 8
+        Kb = bank_frame(spec, K, V, s, 0)[0]
+        lg = q @ Kb.T / np.sqrt(spec.head_dim)
+        top = np.maximum(top, lg.max(axis=1))
+        if f % spec.near_frames == 0:
+            first = lg[:, :128].max(axis=1)
+    assert ((top - first) > 8 * np.log(2.0)).mean() > 0.5, "the reference maximum never has to move"
+    assert worst < 1e-1
 
 
 # ---------------------------------------------------------------------------------------------------------
