@@ -278,10 +278,13 @@ def roofline_objects(spec, res, peaks, steps):
     if src is None:   # a bandwidth-side kernel dominates: report the update path
         src = out["update_path"]
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # ncu dram bytes per launch (profiles/traffic.md)
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(spec.name, {}).get(dom)
+            for ln in open(tpath).read().splitlines()[1:]:
+                w, k, v = ln.split(",")
+                if w == spec.name and k == dom:
+                    traffic = float(v)
         except Exception:
             traffic = None
     roof = dict(bound=src["bound"], achieved=src["achieved"], peak=src["peak"], unit=src["unit"], frac=src["frac"],
