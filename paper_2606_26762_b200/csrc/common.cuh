@@ -44,6 +44,25 @@ struct __align__(16) ScoreRec {
   float v, tauf, invc;
   int tau;
 };
+// Storage of the records (Dev::rec): PAIRS of prototypes interleaved field by field, 16 floats per pair in the order
+// mux, muy, u, -w | v, tauf, invc, tau -- the tcgen05 epilogue scores two prototypes at a time with packed f32x2
+// arithmetic and wants each field of the pair as one aligned 64-bit operand (three 16-byte shared loads per pair).
+// w is stored negated so that y2 = dy v - dx w is one multiply and one fused multiply-add without a negation.
+__host__ __device__ inline size_t rec_slot(size_t pk, int field) { return (pk >> 1) * 16 + (size_t)field * 2 + (pk & 1); }
+__device__ __forceinline__ void store_rec(ScoreRec* base, size_t pk, const ScoreRec& r) {
+  float* f = reinterpret_cast<float*>(base);
+  f[rec_slot(pk, 0)] = r.mux; f[rec_slot(pk, 1)] = r.muy; f[rec_slot(pk, 2)] = r.u; f[rec_slot(pk, 3)] = -r.w;
+  f[rec_slot(pk, 4)] = r.v; f[rec_slot(pk, 5)] = r.tauf; f[rec_slot(pk, 6)] = r.invc;
+  f[rec_slot(pk, 7)] = __int_as_float(r.tau);
+}
+__device__ __forceinline__ ScoreRec load_rec(const ScoreRec* base, size_t pk) {
+  const float* f = reinterpret_cast<const float*>(base);
+  ScoreRec r;
+  r.mux = f[rec_slot(pk, 0)]; r.muy = f[rec_slot(pk, 1)]; r.u = f[rec_slot(pk, 2)]; r.w = -f[rec_slot(pk, 3)];
+  r.v = f[rec_slot(pk, 4)]; r.tauf = f[rec_slot(pk, 5)]; r.invc = f[rec_slot(pk, 6)];
+  r.tau = __float_as_int(f[rec_slot(pk, 7)]);
+  return r;
+}
 
 // Device pointers into the workspace.
 struct Dev {
@@ -63,7 +82,7 @@ struct Dev {
   int* tau;      // [B][K]
   long long* pos;  // [B][K]
   uint32_t* nres;  // [B][K]
-  ScoreRec* rec;   // [B][K]
+  ScoreRec* rec;   // [B * K / 2] pairs, see rec_slot()
   float* logn;     // [B][K]  log n_k (Eq. 4 bias)
   uint32_t* hist;  // [B][K][2][G][C]
   const double* logtab;  // [PKV_SYN_LOGTAB] log(h + pq_eps), h = 0, 1, ...: built on the host at create (synthesis, Eq. 3)

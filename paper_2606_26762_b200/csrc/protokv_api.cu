@@ -158,7 +158,7 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   }
   v.n = (int*)take(BK * 4); v.mu = (float*)take(BK * 8); v.sigma = (float*)take(BK * 12);
   v.tau = (int*)take(BK * 4); v.pos = (long long*)take(BK * 8); v.nres = (uint32_t*)take(BK * 4);
-  v.rec = (ScoreRec*)take(BK * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
+  v.rec = (ScoreRec*)take((BK + 1) * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
   v.hist = (uint32_t*)take(BK * 2 * D.G * D.C * 4);
   v.logtab = (const double*)take((size_t)PKV_SYN_LOGTAB * 8);
   if (has_cb) {

@@ -64,10 +64,35 @@ __device__ __forceinline__ uint32_t orderable(float f) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-// One row's scan over the (up to) 64 accumulator columns of a unit: rest of Eq. 1 + running argmin.
+// packed fp32 pairs (sm_100 f32x2 arithmetic): one issue slot for the two prototypes of a record pair
+__device__ __forceinline__ uint64_t as_pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void as_unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t as_fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t as_mul2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+// One row's scan over the (up to) 64 accumulator columns of a unit: rest of Eq. 1 + running argmin, two prototypes
+// per step.  The records arrive pair-interleaved (common.cuh rec_slot): {mux0, mux1, muy0, muy1}, {u0, u1, -w0, -w1},
+// {v0, v1, tauf0, tauf1}.  The scan maximises  acc - |K_j| (lambda_sp d_Mah + lambda_idle [idle])  = -|K_j| score.
 template <bool SQUARED, bool RAGGED>
 __device__ __forceinline__ void as_scan(uint32_t taddr, uint32_t rc, int ncol, float sx, float sy, float nk,
                                         float thr, float lam_idle, float& ub, int& ucol) {
+  const uint64_t sx2 = as_pack2(sx, sx), sy2 = as_pack2(sy, sy), m1 = as_pack2(-1.f, -1.f);
+  const uint64_t nnk2 = as_pack2(-nk, -nk), li2 = as_pack2(lam_idle, lam_idle);
+  float best = -ub;                                      // running maximum of -|K_j| score
 #pragma unroll
   for (int c0 = 0; c0 < kUN; c0 += 32) {
     if (!RAGGED || c0 < ncol) {
@@ -75,26 +100,39 @@ __device__ __forceinline__ void as_scan(uint32_t taddr, uint32_t rc, int ncol, f
       tmem_ld_32x32(taddr + c0, acc);
       tmem_ld_wait();
 #pragma unroll
-      for (int c = 0; c < 32; ++c) {
-        float4 r0;                                     // mux, muy, u, w
-        float2 r1;                                     // v, tauf
-        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w)
-                     : "r"(rc + (c0 + c) * 32) : "memory");
-        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r1.x), "=f"(r1.y) : "r"(rc + (c0 + c) * 32 + 16) : "memory");
-        const float dx = sx - r0.x, dy = sy - r0.y;
-        const float y1 = dx * r0.z;
-        const float y2 = fmaf(dy, r1.x, -(dx * r0.w));
-        const float qq = fmaf(y1, y1, y2 * y2);
-        float sp;
-        if (SQUARED) sp = qq;
-        else asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sp) : "f"(qq));
-        const float ee = fmaf(lam_idle, __saturatef(thr - r1.y), sp);
-        float sc = fmaf(nk, ee, -__uint_as_float(acc[c]));
-        if (RAGGED && c0 + c >= ncol) sc = INFINITY;
-        if (sc < ub) { ub = sc; ucol = c0 + c; }       // increasing k: lowest index on ties
+      for (int c = 0; c < 32; c += 2) {
+        uint64_t mu_x, mu_y, u2, wn2, v2, tf2;
+        const uint32_t ra = rc + ((c0 + c) >> 1) * 64;
+        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(mu_x), "=l"(mu_y) : "r"(ra) : "memory");
+        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(u2), "=l"(wn2) : "r"(ra + 16) : "memory");
+        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v2), "=l"(tf2) : "r"(ra + 32) : "memory");
+        const uint64_t dx = as_fma2(mu_x, m1, sx2), dy = as_fma2(mu_y, m1, sy2);     // s - mu
+        const uint64_t y1 = as_mul2(dx, u2);
+        const uint64_t y2 = as_fma2(dx, wn2, as_mul2(dy, v2));                       // dy v - dx w
+        const uint64_t qq = as_fma2(y1, y1, as_mul2(y2, y2));
+        float q0, q1, t0, t1;
+        as_unpack2(qq, q0, q1);
+        as_unpack2(tf2, t0, t1);
+        float s0, s1;
+        if (SQUARED) { s0 = q0; s1 = q1; }
+        else {
+          asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s0) : "f"(q0));
+          asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s1) : "f"(q1));
+        }
+        const uint64_t ee = as_fma2(li2, as_pack2(__saturatef(thr - t0), __saturatef(thr - t1)), as_pack2(s0, s1));
+        const uint64_t sc2 = as_fma2(nnk2, ee, as_pack2(__uint_as_float(acc[c]), __uint_as_float(acc[c + 1])));
+        float n0, n1;
+        as_unpack2(sc2, n0, n1);
+        if (RAGGED) {
+          if (c0 + c >= ncol) n0 = -INFINITY;
+          if (c0 + c + 1 >= ncol) n1 = -INFINITY;
+        }
+        if (n0 > best) { best = n0; ucol = c0 + c; }     // increasing k: lowest index on ties
+        if (n1 > best) { best = n1; ucol = c0 + c + 1; }
       }
     }
   }
+  ub = -best;
 }
 
 template <bool SQUARED>
@@ -162,7 +200,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
         tma_load_2d(dst + 3 * kBHalf, &tmClo, 64, prow, b_full + s);
         const int rs = i % kRecRing;
         mbar_wait(r_empty + rs, ((i / kRecRing) & 1) ^ 1);   // the epilogue of unit i - kRecRing has read this slot
-        const int nrec = min(kUN, D.K - x.nc * kUN);
+        const int nrec = (min(kUN, D.K - x.nc * kUN) + 1) & ~1;   // whole record pairs (prow is even: K % 64 == 0 here)
         mbar_arrive_expect_tx(r_full + rs, (uint32_t)nrec * sizeof(ScoreRec));
         bulk_load_1d(sm + AsSmem::Rec + rs * kRecBytes, V.rec + (size_t)prow, (uint32_t)nrec * sizeof(ScoreRec), r_full + rs);
       }
@@ -325,7 +363,7 @@ bool make_tmap_3d_bf16(CUtensorMap* out, const void* base, uint64_t n0, uint64_t
   return true;
 }
 
-bool tc_assign_supported(const Dims& D, const Hyper&) { return D.bf16 && D.d == 128; }
+bool tc_assign_supported(const Dims& D, const Hyper&) { return D.bf16 && D.d == 128 && D.K % 2 == 0; }   // record pairs
 
 bool tc_build_maps(const Dims& D, const Dev& V, TcMaps* maps) {
   const uint64_t ring_rows = (uint64_t)D.B * D.Wf * D.T, bank_rows = (uint64_t)D.B * D.K;

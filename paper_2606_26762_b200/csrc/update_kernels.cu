@@ -165,7 +165,7 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     V.tau[pk] = F.t;
     V.pos[pk] = (long long)F.ev_frame * D.T + j;
     V.nres[pk] = 0u;
-    V.rec[pk] = make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H);
+    store_rec(V.rec, pk, make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H));
     V.logn[pk] = 0.f;
     mark_dirty(D, V, b, k, F.epoch);
     V.assign[(size_t)b * D.T + j] = k;
@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(kScoreThreads) score_simt_kernel(Dims D, Hyper
     const int nk = min(kScoreKc, F.n_act - k0);
     const float4* src = (const float4*)(V.c + ((size_t)b * D.K + k0) * DH);
     for (int e = tid; e < nk * DH / 4; e += kScoreThreads) ((float4*)cs)[e] = src[e];
-    if (tid < nk) recs[tid] = V.rec[(size_t)b * D.K + k0 + tid];
+    if (tid < nk) recs[tid] = load_rec(V.rec, (size_t)b * D.K + k0 + tid);
     __syncthreads();
     float acc[8];
 #pragma unroll
@@ -465,7 +465,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       V.mu[pk * 2] = mu0; V.mu[pk * 2 + 1] = mu1;
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] += (uint32_t)m;
-      V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
+      store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
       V.logn[pk] = logf((float)n);
       mark_dirty(D, V, b, k, F.epoch);
     }
@@ -714,7 +714,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       *(float2*)(V.mu + pk * 2) = make_float2(mu0, mu1);
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] = nres_old + (uint32_t)m;
-      V.rec[pk] = make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H);
+      store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
       V.logn[pk] = logf((float)n);
       mark_dirty(D, V, b, k, F.epoch);
     }
@@ -781,8 +781,8 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b, int epoch)
     }
   }
   if (lane == 0) {
-    V.rec[pk] = make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
-                         V.sigma[pk * 3 + 2], V.tau[pk], H);
+    store_rec(V.rec, pk, make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
+                         V.sigma[pk * 3 + 2], V.tau[pk], H));
     const int n = V.n[pk];
     V.logn[pk] = n >= 1 ? logf((float)n) : 0.f;
     mark_dirty(D, V, b, k, epoch);
