@@ -206,6 +206,27 @@ def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=Tr
     tr = st.last_frame_trace()
     res["touched_per_bank"] = float(sum(len(set(a.tolist())) for a in tr["assign"]) / len(tr["assign"]))
 
+    # the same query as per-layer calls (layers are sequentially dependent in a real model): one
+    # synthesis of the dirty prototypes, then one protokv_query_attention_ex per layer, summed
+    if spec.n_layers > 1:
+        reps = max(3, min(10, steps // 10))
+        Ql = [Q[:, la:la + 1].contiguous() for la in range(spec.n_layers)]
+        Ol = [torch.empty_like(q) for q in Ql]
+        tot = 0.0
+        for i in range(reps):
+            K, V = pool[(warmup + i) % pool_n]
+            st.append_frame(K, V, s)                          # dirties prototypes like a timed step does
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            st.synthesize()
+            for la in range(spec.n_layers):
+                st.query_attention_ex(Ql[la], n_q=spec.n_query_tokens, layer_begin=la, layer_count=1, out=Ol[la],
+                                      run_synthesis=False)
+            e1.record()
+            torch.cuda.synchronize()
+            tot += e0.elapsed_time(e1)
+        res["per_layer_query_ms"] = tot / reps
+
     if do_profile:   # per-kernel durations: same steps again with the library's stage events switched on
         st.profile_enable(True)
         for i in range(steps):
@@ -417,6 +438,7 @@ def main():
                 roofline=roof, rooflines=stage_roofs,
                 stages_ms_per_step={k: v[0] / K for k, v in res.get("stages", {}).items()},
                 touched_prototypes_per_bank_frame=res["touched_per_bank"], state_bytes=res["state_bytes"],
+                query_attn_us_per_layer_calls=(res["per_layer_query_ms"] * 1e3 if "per_layer_query_ms" in res else None),
                 peaks=peaks)
     if world == 1 and args.extras:
         extras = {}
