@@ -227,6 +227,26 @@ def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=Tr
             tot += e0.elapsed_time(e1)
         res["per_layer_query_ms"] = tot / reps
 
+    # decode-style query: ONE query token (rows = GQA group per bank), memory-bound by construction -- the near window
+    # and the bank are streamed once for a handful of rows (north_star: HBM fraction of the decode-style attention)
+    if spec.dtype == "bf16":
+        Q1 = Q[:, :, :1].contiguous()
+        O1 = torch.empty_like(Q1)
+        st.synthesize()
+        st.query_attention_ex(Q1, n_q=1, out=O1, run_synthesis=False)
+        ts = []
+        for i in range(10):
+            if flush is not None:
+                flush.fill_(i & 255)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            st.query_attention_ex(Q1, n_q=1, out=O1, run_synthesis=False)
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ts.sort()
+        res["decode_ms"] = ts[len(ts) // 2]
+
     if do_profile:   # per-kernel durations: same steps again with the library's stage events switched on
         st.profile_enable(True)
         for i in range(steps):
@@ -259,6 +279,20 @@ def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=Tr
                           d2h=Q.numel() * Q.element_size())
     st.close()
     return res
+
+
+def decode_object(spec, res, peaks):
+    """One-token query (attention only, codes valid): us and fraction of the HBM roofline on its algorithmic bytes."""
+    if "decode_ms" not in res:
+        return None
+    elt = 2 if spec.dtype == "bf16" else 4
+    W = spec.near_frames * spec.T
+    rows = spec.n_q_heads // spec.n_kv_heads
+    per_bank = 2 * W * spec.head_dim * elt + spec.k_max * (2 * spec.head_dim * 4 + 8 * spec.G + 4) + 2 * rows * spec.head_dim * elt
+    b = per_bank * spec.n_banks
+    gbs = b / (res["decode_ms"] * 1e-3) / 1e9
+    return dict(n_query_tokens=1, attention_us=res["decode_ms"] * 1e3, algorithmic_bytes=b, bound="hbm", achieved=gbs,
+                unit="GB/s", peak=peaks["hbm"], frac=gbs / peaks["hbm"])
 
 
 def roofline_objects(spec, res, peaks, steps):
@@ -439,6 +473,7 @@ def main():
                 stages_ms_per_step={k: v[0] / K for k, v in res.get("stages", {}).items()},
                 touched_prototypes_per_bank_frame=res["touched_per_bank"], state_bytes=res["state_bytes"],
                 query_attn_us_per_layer_calls=(res["per_layer_query_ms"] * 1e3 if "per_layer_query_ms" in res else None),
+                decode_query=decode_object(spec, res, peaks),
                 peaks=peaks)
     if world == 1 and args.extras:
         extras = {}
