@@ -45,7 +45,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kTruncBiasLog2 = 0.0028151f;
 constexpr float kTruncBiasInv = 0.99805068f;
 constexpr float kRescaleSum = 256.f;    // a tile's row sum of P above this moves the reference maximum (P <= 2^8 in bf16)
-constexpr int kRegsSoftmax = 200, kRegsBuilder = 72, kRegsAux = 40;   // 2 * 200 + 72 + 40 = 512 = 4 * 128
+constexpr int kRegsSoftmax = 184, kRegsBuilder = 104, kRegsAux = 40;  // 2 * 184 + 104 + 40 = 512 = 4 * 128
 
 struct AtSmem {   // byte offsets from a 1024-byte aligned base
   static constexpr uint32_t Q = 0;                          // 2 d-halves x [256 rows][128 B]
