@@ -17,8 +17,10 @@
 // == sequential; forced replay; brute-force recomputation of the statistics from the assignment log (numpy);
 // constant-stream closed forms; exact attention over the full history when K_max >= evicted tokens; a mass-m
 // prototype == m duplicated tokens; torch SDPA on the materialised context; cosine nearest centroid; Euclidean
-// special case of d_Mah; beam == brute-force top-S.  What stays unpinned: the absolute values produced on the five
-// configs ("parity unpinned" beyond those pins).
+// special case of d_Mah; beam == brute-force top-S; closed forms after one absorption into a fresh slot (Sigma step
+// with delta against the NEW mean, Alg. 1 l.11-12; residual taken AFTER the token's own EMA step, l.8-9 before l.13).
+// What stays unpinned: the absolute values produced on the five configs ("parity unpinned" beyond those pins, see
+// DESIGN.md).
 #include <algorithm>
 #include <array>
 #include <cmath>

@@ -497,3 +497,55 @@ def test_zero_nres_gives_zero_residuals_and_no_codebooks_flag():
     o2 = make_oracle(spec, flags=FLAG_NO_RESIDUAL)
     run_stream(spec, o2, 30)
     assert int(o2.state()["nres"].sum()) == 0 and int(o2.state()["hist_k"].sum()) == 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# pins 13 + 14 (closed forms of Alg. 1 l.11-13 after ONE absorption into a fresh slot): they pin
+# the two statements the re-simulation of pin 5 only restates -- "Sigma uses delta = s_e - mu_NEW" (l.12 after l.11)
+# and "the residual is taken after the token's own EMA step" (l.13 after l.8-9, reading 7).
+#   slot opened by token 0: c = K0, p = V0, mu = s0, Sigma = I.  Token 1 absorbed:
+#     mu' = (1-eta) s0 + eta s1,  delta = s1 - mu' = (1-eta)(s1 - s0)
+#     Sigma' = (1-eta) I + eta (1-eta)^2 (s1-s0)(s1-s0)^T          [with the OLD mu it would be eta (s1-s0)(s1-s0)^T]
+#     r^K = K1 - c' = (1-alpha)(K1 - K0),  r^V = (1-beta)(V1 - V0)  [before the EMA step it would be K1 - K0]
+# ---------------------------------------------------------------------------------------------------------
+def _one_absorption(alpha, beta, eta, ck=None, cv=None, G=2, Cn=2, d=8, seed=7):
+    rng = np.random.default_rng(seed)
+    K = rng.normal(size=(3, 1, d)).astype(np.float32)
+    V = rng.normal(size=(3, 1, d)).astype(np.float32)
+    s = np.array([[[0.125, 0.75]], [[0.875, 0.25]], [[0.5, 0.5]]], np.float32)
+    o = OracleBank(1, 1, 1, d, ck, cv, G=G, C=Cn, S=1, beam=1, alpha=alpha, beta=beta, eta=eta)
+    traces = [o.append_frame(K[f], V[f], s[f]) for f in range(3)]   # f=1 evicts token 0 (fill), f=2 evicts token 1
+    assert traces[1]["n_fill"] == 1 and traces[2]["n_fill"] == 0 and traces[2]["assign"][0] == 0
+    return o.state(), K[:, 0], V[:, 0], s[:, 0], traces
+
+
+def test_sigma_after_one_absorption_closed_form():
+    eta = 0.25
+    st, K, V, s, _ = _one_absorption(0.5, 0.5, eta)
+    ds = s[1].astype(np.float64) - s[0].astype(np.float64)
+    want = (1 - eta) * np.eye(2) + eta * (1 - eta) ** 2 * np.outer(ds, ds)
+    got = st["sigma"][0].astype(np.float64)
+    assert np.allclose([got[0], got[1], got[2]], [want[0, 0], want[0, 1], want[1, 1]], rtol=0, atol=2e-7)
+    wrong = (1 - eta) * np.eye(2) + eta * np.outer(ds, ds)                    # delta against the old mean
+    assert abs(wrong[0, 0] - want[0, 0]) > 1e-2                               # the pin separates the two readings
+    assert np.allclose(st["mu"][0], (1 - eta) * s[0] + eta * s[1], rtol=0, atol=1e-7)
+
+
+def test_residual_is_taken_after_the_ema_step():
+    alpha, beta, d, G = 0.5, 0.25, 8, 2
+    sub = d // G
+    _, K, V, s, _ = _one_absorption(alpha, beta, 0.05, d=d)                   # same seeded tokens, no codebooks yet
+    # codeword 0 sits on the BEFORE-update residual K1-K0 (V1-V0), codeword 1 on the AFTER-update residual
+    # (1-alpha)(K1-K0): the literal order of Alg. 1 must hit codeword 1 in every subspace, the other order codeword 0
+    rk_before, rv_before = K[1] - K[0], V[1] - V[0]
+    ck = np.stack([rk_before.reshape(G, sub), ((1 - alpha) * rk_before).reshape(G, sub)], axis=1).astype(np.float32)
+    cv = np.stack([rv_before.reshape(G, sub), ((1 - beta) * rv_before).reshape(G, sub)], axis=1).astype(np.float32)
+    for g in range(G):                                                        # the two candidates are well separated
+        assert np.linalg.norm(ck[g, 0] - ck[g, 1]) > 0.05 and np.linalg.norm(cv[g, 0] - cv[g, 1]) > 0.05
+    st, K2, V2, _, tr = _one_absorption(alpha, beta, 0.05, ck=ck, cv=cv, d=d)
+    assert np.array_equal(K2, K) and np.array_equal(V2, V)
+    assert np.array_equal(st["hist_k"][0], np.tile([0, 1], (G, 1)))
+    assert np.array_equal(st["hist_v"][0], np.tile([0, 1], (G, 1)))
+    assert st["nres"][0] == 1 and st["n"][0] == 2
+    assert (tr[2]["codes_k"][0] == 1).all() and (tr[2]["codes_v"][0] == 1).all()
+    assert np.allclose(st["c"][0], (1 - alpha) * K[0] + alpha * K[1], atol=1e-7)
