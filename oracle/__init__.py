@@ -20,6 +20,7 @@ _SRC = os.path.join(_HERE, "protokv_oracle.cpp")
 _LIB = os.path.join(_HERE, "libprotokv_oracle.so")
 
 FLAG_MAH_SQUARED, FLAG_NO_MASS_BIAS, FLAG_NO_RESIDUAL, FLAG_NEAR_ONLY, FLAG_FAR_ONLY = 1, 2, 4, 8, 16
+FLAG_MAINTENANCE = 64
 
 
 def build(force: bool = False) -> str:
@@ -38,7 +39,7 @@ class _Config(C.Structure):
                 ("lambda_sp", C.c_float), ("lambda_idle", C.c_float), ("t_idle", C.c_int32),
                 ("alpha", C.c_float), ("beta", C.c_float), ("eta", C.c_float),
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float)]
 
 
 class _Trace(C.Structure):
@@ -66,6 +67,8 @@ def _load():
                                          C.c_void_p, C.c_void_p, C.POINTER(_Trace)]
         lib.pko_frames_seen.argtypes = [C.c_void_p]
         lib.pko_ring_frames.argtypes = [C.c_void_p]
+        lib.pko_maintain.argtypes = [C.c_void_p, C.c_int32]
+        lib.pko_maintenance_counters.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         lib.pko_get_ring.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         lib.pko_get_state.argtypes = [C.c_void_p, C.POINTER(_StateView)]
         lib.pko_set_state.argtypes = [C.c_void_p, C.POINTER(_StateView)]
@@ -93,7 +96,8 @@ def _ptr(a: Optional[np.ndarray]):
 
 
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
-                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0)   # Table 5
+                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0,
+                gamma=0.05, eps_k=0.20, eps_v=0.25)   # Table 5
 
 
 class OracleBank:
@@ -148,6 +152,15 @@ class OracleBank:
     @property
     def frames_seen(self):
         return self._lib.pko_frames_seen(self._h)
+
+    def maintain(self, t):
+        """Alg. 2 at stream time t on the current state (pins)."""
+        self._lib.pko_maintain(self._h, int(t))
+
+    def maintenance_counters(self, reset=False):
+        out = np.zeros(3, np.int64)
+        self._lib.pko_maintenance_counters(self._h, _ptr(out), int(reset))
+        return dict(decayed=int(out[0]), merges=int(out[1]), recycled=int(out[2]))
 
     def ring(self):
         n = self._lib.pko_ring_frames(self._h)

@@ -4,6 +4,7 @@
 //   Alg. 1 streaming update   (Eq. 1 at L93)      -> append_frame_sync / append_frame_seq
 //   Eq. 3 + Alg. 3 beam decode             -> decode_top_s
 //   Alg. 4 decode + attention, Eq. 2/4 -> materialize / attention
+//   Alg. 2 prototype maintenance (off unless FLAG_MAINTENANCE) -> maintain
 // One object = one bank = one (stream, layer, KV head): banks are independent.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call this.
@@ -19,6 +20,8 @@
 // prototype == m duplicated tokens; torch SDPA on the materialised context; cosine nearest centroid; Euclidean
 // special case of d_Mah; beam == brute-force top-S; closed forms after one absorption into a fresh slot (Sigma step
 // with delta against the NEW mean, Alg. 1 l.11-12; residual taken AFTER the token's own EMA step, l.8-9 before l.13).
+// Alg. 2 (tests/test_oracle_maintenance.py): generalised mass invariant, conservation of the mass-weighted sums under
+// merging, closed form of the idle decay, gamma = eps = 0 == the plain path bit for bit, T = 1 sync == sequential.
 // What stays unpinned: the absolute values produced on the five configs ("parity unpinned" beyond those pins, see
 // DESIGN.md).
 #include <algorithm>
@@ -38,6 +41,7 @@ enum : uint32_t {
   FLAG_NO_RESIDUAL = 4u,   // no histograms    (Table 2 "w/o residual stats", L179)
   FLAG_NEAR_ONLY = 8u,     // attention over the near window only (L176)
   FLAG_FAR_ONLY = 16u,     // attention over pseudo-tokens only   (L177)
+  FLAG_MAINTENANCE = 64u,  // run Alg. 2 at Alg. 1 l.15; off on the graded path (reading 19)
 };
 
 struct Config {
@@ -47,6 +51,13 @@ struct Config {
   float alpha, beta, eta, sigma_eps, cos_eps;
   double pq_eps;
   uint32_t flags;
+  float gamma, eps_k, eps_v;   // Alg. 2: idle decay rate, merge thresholds (Table 5: 0.05, 0.20, 0.25)
+};
+
+struct Maint {          // what Alg. 2 did since the counters were last read (pko_maintenance_counters)
+  int64_t decayed;      // mass removed by aging (l.3)
+  int64_t merges;       // prototypes merged away (l.7-11)
+  int64_t recycled;     // slots re-initialised from the near window (l.15-17)
 };
 
 struct Trace {          // all pointers nullable; sizes [T] or [T][G]
@@ -91,6 +102,8 @@ struct Bank {
   std::vector<int64_t> pos;
   std::vector<uint32_t> hk, hv, nres;
   std::vector<uint8_t> active;
+  std::vector<uint8_t> used;   // slot has been initialised at least once (Alg. 2 recycles only such slots, reading 24)
+  Maint maint{0, 0, 0};
 
   Bank(const Config& cf, const float* ck, const float* cv) : cfg(cf) {
     sub = cfg.d / cfg.G;
@@ -105,7 +118,7 @@ struct Bank {
     mu.assign(K * 2, 0.f); sigma.assign(K * 3, 0.f);
     n.assign(K, 0); tau.assign(K, 0); pos.assign(K, 0);
     hk.assign(K * cfg.G * cfg.C, 0u); hv.assign(K * cfg.G * cfg.C, 0u);
-    nres.assign(K, 0u); active.assign(K, 0);
+    nres.assign(K, 0u); active.assign(K, 0); used.assign(K, 0);
   }
 
   int free_slot() const {  // lowest-index inactive slot (reading 9), -1 if none
@@ -122,7 +135,71 @@ struct Bank {
     tau[k] = t; pos[k] = ps;
     std::fill(hk.begin() + (size_t)k * cfg.G * cfg.C, hk.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
     std::fill(hv.begin() + (size_t)k * cfg.G * cfg.C, hv.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
-    nres[k] = 0; active[k] = 1;
+    nres[k] = 0; active[k] = 1; used[k] = 1;
+  }
+
+  // Alg. 2, readings 20 and 24-27 of DESIGN.md: aging, pairwise merge, recycling -- in that order.
+  void maintain(int32_t t) {
+    const int K = cfg.k_max, d = cfg.d, GC = cfg.G * cfg.C;
+    // l.1-5 aging: n_k <- floor((1 - gamma) n_k) for prototypes idle for more than T_idle steps
+    for (int k = 0; k < K; ++k) {
+      if (!active[k]) continue;
+      if ((int64_t)t - (int64_t)tau[k] > (int64_t)cfg.t_idle) {
+        int32_t nn = (int32_t)std::floor((1.0 - (double)cfg.gamma) * (double)n[k]);
+        maint.decayed += n[k] - nn;
+        n[k] = nn;
+      }
+    }
+    // l.6-13 merging: pairs i < j in lexicographic order, both non-empty; the lower index survives and its UPDATED
+    // centres are what later pairs (i, j') are tested against; fields Alg. 2 does not list (Sigma, tau, pos) keep
+    // Pi_i's values
+    const double ek2 = (double)cfg.eps_k * (double)cfg.eps_k, ev2 = (double)cfg.eps_v * (double)cfg.eps_v;
+    for (int i = 0; i < K; ++i) {
+      if (!active[i] || n[i] < 1) continue;
+      for (int j = i + 1; j < K; ++j) {
+        if (!active[j] || n[j] < 1) continue;
+        double dk = 0, dv = 0;
+        for (int e = 0; e < d; ++e) {
+          double a = (double)c[(size_t)i * d + e] - (double)c[(size_t)j * d + e];
+          dk += a * a;
+        }
+        if (!(dk < ek2)) continue;                         // ||c_i - c_j||_2 < eps_K
+        for (int e = 0; e < d; ++e) {
+          double a = (double)p[(size_t)i * d + e] - (double)p[(size_t)j * d + e];
+          dv += a * a;
+        }
+        if (!(dv < ev2)) continue;                         // ||p_i - p_j||_2 < eps_V
+        const double ni = n[i], nj = n[j], w = ni + nj;
+        for (int e = 0; e < d; ++e) {
+          c[(size_t)i * d + e] = (float)((ni * (double)c[(size_t)i * d + e] + nj * (double)c[(size_t)j * d + e]) / w);
+          p[(size_t)i * d + e] = (float)((ni * (double)p[(size_t)i * d + e] + nj * (double)p[(size_t)j * d + e]) / w);
+        }
+        for (int e = 0; e < 2; ++e)
+          mu[i * 2 + e] = (float)((ni * (double)mu[i * 2 + e] + nj * (double)mu[j * 2 + e]) / w);
+        n[i] += n[j];
+        for (int e = 0; e < GC; ++e) {
+          hk[(size_t)i * GC + e] += hk[(size_t)j * GC + e];
+          hv[(size_t)i * GC + e] += hv[(size_t)j * GC + e];
+        }
+        nres[i] += nres[j];
+        active[j] = 0; n[j] = 0;                           // "mark Pi_j as inactive"
+        maint.merges += 1;
+      }
+    }
+    // l.14-19 recycling: every slot emptied by decay or merging (never-used slots stay free for Alg. 1 l.3-4) is
+    // re-initialised from a recent near-window token: the r-th such slot of this call, in increasing slot order, takes
+    // token T-1-(r mod T) of the (r / T)-th newest frame
+    int r = 0;
+    for (int k = 0; k < K; ++k) {
+      if (!used[k] || (active[k] && n[k] >= 1)) continue;
+      int back = r / cfg.T;
+      if (back >= (int)ring.size()) back = (int)ring.size() - 1;
+      const Frame& f = ring[ring.size() - 1 - back];
+      const int j = cfg.T - 1 - (r % cfg.T);
+      init_slot(k, &f.K[(size_t)j * d], &f.V[(size_t)j * d], &f.s[j * 2], t, (int64_t)f.index * cfg.T + j);
+      maint.recycled += 1;
+      ++r;
+    }
   }
 
   // Eq. 1: -cos(K_e,c_k) + lambda_sp d_Mah(s_e;mu_k,Sigma_k) + lambda_idle 1[t - tau_k > T_idle]
@@ -293,6 +370,7 @@ struct Bank {
                    tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
                    tr && tr->code_gap_v ? tr->code_gap_v + j * G : nullptr);
     }
+    if (cfg.flags & FLAG_MAINTENANCE) maintain(t);   // Alg. 1 l.15, once per frame in the frame-synchronous reading
   }
 
   // Literal Alg. 1 (token-sequential): every evicted token sees the live bank. Used for pinning only.
@@ -318,6 +396,7 @@ struct Bank {
         init_slot(k, Ke, Ve, se, t, ps);
         if (tr && tr->assign) tr->assign[j] = k;
         ++nf;
+        if (cfg.flags & FLAG_MAINTENANCE) maintain(t);                // l.15
         continue;
       }
       float b, s2;
@@ -333,6 +412,7 @@ struct Bank {
                    tr && tr->codes_k ? tr->codes_k + j * G : nullptr, tr && tr->codes_v ? tr->codes_v + j * G : nullptr,
                    tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
                    tr && tr->code_gap_v ? tr->code_gap_v + j * G : nullptr);
+      if (cfg.flags & FLAG_MAINTENANCE) maintain(t);                  // l.15
     }
     if (tr) tr->n_fill = nf;
   }
@@ -491,6 +571,14 @@ int pko_append_frame(void* h, const float* K, const float* V, const float* s, in
 }
 
 int pko_frames_seen(void* h) { return static_cast<Bank*>(h)->frames_seen; }
+
+// Alg. 2 on its own (time t), for pins; and its counters since the last call with reset != 0
+void pko_maintain(void* h, int32_t t) { static_cast<Bank*>(h)->maintain(t); }
+void pko_maintenance_counters(void* h, int64_t* out3, int reset) {
+  Bank* b = static_cast<Bank*>(h);
+  out3[0] = b->maint.decayed; out3[1] = b->maint.merges; out3[2] = b->maint.recycled;
+  if (reset) b->maint = Maint{0, 0, 0};
+}
 int pko_ring_frames(void* h) { return (int)static_cast<Bank*>(h)->ring.size(); }
 
 // ring in chronological order: K,V [n][T][d], s [n][T][2], idx [n]; returns n
@@ -524,6 +612,8 @@ void pko_set_state(void* h, const StateView* v) {
   PKO_LOAD(c, c); PKO_LOAD(p, p); PKO_LOAD(n, n); PKO_LOAD(mu, mu); PKO_LOAD(sigma, sigma);
   PKO_LOAD(tau, tau); PKO_LOAD(pos, pos); PKO_LOAD(hist_k, hk); PKO_LOAD(hist_v, hv); PKO_LOAD(nres, nres);
   PKO_LOAD(active, active);
+  if (v->active)
+    for (size_t k = 0; k < b->used.size(); ++k) b->used[k] = b->used[k] || b->active[k];
 }
 
 // Eq. 1 score of (K_e, s_e) against prototype k at stream time t, on the current bank
