@@ -295,12 +295,24 @@ def decode_object(spec, res, peaks):
                 unit="GB/s", peak=peaks["hbm"], frac=gbs / peaks["hbm"])
 
 
-def roofline_objects(spec, res, peaks, steps):
-    """roofline of the dominant kernel + one object per stage group."""
+def tensor_peak(peaks, clocks):
+    """Which measured bf16 peak applies to this run (MEASURED_PEAKS.json holds a burst and a sustained figure): a timed
+    region of milliseconds that the sampler saw at the maximum SM clock without a power cap ran under burst conditions;
+    a power-capped or down-clocked region is compared with the sustained figure."""
+    burst = True
+    if clocks and clocks.get("sm_mhz") and clocks.get("sm_max_mhz"):
+        burst = clocks["sm_mhz"] >= 0.95 * clocks["sm_max_mhz"] and "sw_power_cap" not in (clocks.get("reasons") or [])
+    return (peaks["bf16_burst"], "burst") if burst else (peaks["bf16_sustained"], "sustained")
+
+
+def roofline_objects(spec, res, peaks, steps, clocks=None):
+    """roofline of the dominant kernel + one object per stage group, all on SURVEY.md 8(d)'s ALGORITHMIC counts
+    (DESIGN.md "Measurement"): frac = (time the roofline allows for the algorithmic bytes / flops) / (measured time)."""
     out = {}
     stages = res.get("stages")
     if not stages:
         return None, out
+    tpeak, tkind = tensor_peak(peaks, clocks if clocks is not None else res.get("clocks"))
     ub = update_bytes_per_frame(spec, res["touched_per_bank"])
     qb = query_bytes(spec)
     fact, dense = query_flops(spec)
@@ -310,23 +322,29 @@ def roofline_objects(spec, res, peaks, steps):
     out["update_path"]["frac"] = out["update_path"]["achieved"] / peaks["hbm"]
     sc_ms = stages["score"][0] / max(1, stages["score"][1])
     af = assign_flops_per_frame(spec)
-    out["score"] = dict(bound="tensor", achieved=af / (sc_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
-                        algorithmic_flops=af, ms=sc_ms, note="T x K_max x d contraction, 1x flops (hi+lo split doubles the MMA work)")
-    out["score"]["frac"] = out["score"]["achieved"] / peaks["bf16_sustained"]
+    out["score"] = dict(bound="tensor", achieved=af / (sc_ms * 1e-3) / 1e12, peak=tpeak, unit="TFLOP/s",
+                        algorithmic_flops=af, ms=sc_ms, peak_kind=tkind,
+                        note="T x K_max x d contraction, 1x flops (the hi+lo split issues 2x that on the tensor pipe)")
+    out["score"]["frac"] = out["score"]["achieved"] / tpeak
     at_ms = stages["attention"][0] / max(1, stages["attention"][1])
-    # The kernel issues the dense contraction 4 rows L_context d on the tensor pipe (the "factorised"
-    # count of SURVEY 8(d) is not reachable -- its per-(row, pseudo-token) code gathers are themselves G*C = d wide), so
-    # `achieved` is dense-equivalent TFLOP/s = tensor-pipe utilisation; the stricter factorised figures ride along.
-    t_dense = max(qb / (peaks["hbm"] * 1e9), dense / (peaks["bf16_sustained"] * 1e12))
-    t_fact = max(qb / (peaks["hbm"] * 1e9), fact / (peaks["bf16_sustained"] * 1e12))
-    out["attention"] = dict(bound="tensor", achieved=dense / (at_ms * 1e-3) / 1e12, peak=peaks["bf16_sustained"], unit="TFLOP/s",
-                            frac=dense / (at_ms * 1e-3) / 1e12 / peaks["bf16_sustained"], algorithmic_flops=dense,
-                            factorised_flops=fact, factorised_tflops=fact / (at_ms * 1e-3) / 1e12,
-                            algorithmic_bytes=qb, hbm_gbs=qb / (at_ms * 1e-3) / 1e9, hbm_frac=qb / (at_ms * 1e-3) / 1e9 / peaks["hbm"],
-                            roofline_us=t_dense * 1e6, frac_of_roofline_time=t_dense * 1e3 / at_ms,
-                            factorised_roofline_us=t_fact * 1e6, frac_of_factorised_roofline_time=t_fact * 1e3 / at_ms, ms=at_ms)
+    # the attention's roofline is max(algorithmic bytes / HBM, FACTORISED flops / tensor peak).  The kernel
+    # issues the dense contraction 4 rows L_context d (DESIGN.md 6.1 says why the factorised form does not shrink the
+    # MMA volume); its utilisation of the tensor pipe rides along as tensor_pipe_util, it is not `frac`.
+    t_hbm, t_tc = qb / (peaks["hbm"] * 1e9), fact / (tpeak * 1e12)
+    t_roof = max(t_hbm, t_tc)
+    if t_hbm >= t_tc:
+        att = dict(bound="hbm", achieved=qb / (at_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s")
+    else:
+        att = dict(bound="tensor", achieved=fact / (at_ms * 1e-3) / 1e12, peak=tpeak, unit="TFLOP/s")
+    att.update(frac=att["achieved"] / att["peak"], algorithmic_bytes=qb, algorithmic_flops=fact,
+               roofline_us=t_roof * 1e6, ms=at_ms, peak_kind=tkind,
+               dense_flops=dense, dense_tflops=dense / (at_ms * 1e-3) / 1e12,
+               tensor_pipe_util=dense / (at_ms * 1e-3) / 1e12 / tpeak,
+               dense_roofline_us=max(t_hbm, dense / (tpeak * 1e12)) * 1e6)
+    out["attention"] = att
     sy_ms = stages["synthesis"][0] / max(1, stages["synthesis"][1])
-    out["synthesis"] = dict(ms=sy_ms)
+    syb = spec.k_max * (2 * spec.G * spec.C * 4 + 8 * spec.G) * spec.n_banks      # if run for every prototype (8(d))
+    out["synthesis"] = dict(ms=sy_ms, bound="hbm", algorithmic_bytes_all_prototypes=syb)
     # dominant kernel of the step = the stage with the largest summed device time
     dom = max(("score", "update", "attention", "synthesis", "append", "fill"), key=lambda k: stages[k][0])
     src = {"score": out["score"], "attention": out["attention"]}.get(dom)
@@ -343,54 +361,102 @@ def roofline_objects(spec, res, peaks, steps):
         except Exception:
             traffic = None
     roof = dict(bound=src["bound"], achieved=src["achieved"], peak=src["peak"], unit=src["unit"], frac=src["frac"],
-                traffic=traffic, kernel=dom, peak_source=peaks["source"] + (" sustained bf16 (kernel timed inside a long step)"
-                                                                         if src["unit"] == "TFLOP/s" else " copy bandwidth"))
+                traffic=traffic, kernel=dom,
+                peak_source=peaks["source"] + (f" {tkind} bf16" if src["unit"] == "TFLOP/s" else " copy bandwidth"))
+    if dom == "attention":
+        roof["tensor_pipe_util"] = src["tensor_pipe_util"]
     return roof, out
 
 
 # ---------------------------------------------------------------------------------------------------------------
 # the oracle arm (cpu_baseline and --impl reference)
 # ---------------------------------------------------------------------------------------------------------------
-def oracle_sample(spec, budget_s=15.0, query_rows=16):
-    """Times the CPU oracle, as it stands, on one bank of the workload in steady state: seconds per bank-frame and
-    seconds per query row; returns whole-workload figures by multiplying with the bank / row counts."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from helpers import frame_for_bank, codebooks_for_bank, query_rows_for_bank
-    from oracle import OracleBank
+def _oracle_subspec(spec, nb):
+    """The smallest spec whose first nb banks are the first nb banks of `spec` (the generator is counter-based, so the
+    sub-spec yields exactly the values those banks have in the full workload)."""
     import dataclasses
-    # bank 0 = (stream 0, layer 0, head 0): the generator is counter-based, so the one-layer / one-stream spec yields
-    # exactly the values bank 0 has in the full workload without generating the other banks.
-    one = dataclasses.replace(spec, n_layers=1, n_streams=1)
-    ck, cv = codebooks_for_bank(one, 0)
-    o = OracleBank(one.T, one.near_frames, one.k_max, one.head_dim, ck, cv, G=one.G, C=one.C)
-    prime = steady_state_frames(one)
-    for f in range(prime):
-        K, V, s = frame_for_bank(one, f, 0)
-        o.append_frame(K, V, s, trace=False)
-    n, t_upd = 0, 0.0
-    while t_upd < budget_s * 0.6 and n < 200:
-        K, V, s = frame_for_bank(one, prime + n, 0)
+    per_stream = spec.n_layers * spec.n_kv_heads
+    if nb <= per_stream:
+        return dataclasses.replace(spec, n_streams=1, n_layers=min(spec.n_layers, math.ceil(nb / spec.n_kv_heads)))
+    return dataclasses.replace(spec, n_streams=min(spec.n_streams, math.ceil(nb / per_stream)))
+
+
+def oracle_arm(spec, steps, warmup, query_rows=2, max_cores=None):
+    """The CPU oracle, as it stands, on the box's host cores.  One oracle object per bank (banks are independent,
+    PAPER.md:L312); nb = min(banks, cores) banks run in parallel threads (the ctypes call drops the GIL), each
+    single-threaded.  One STEP = one steady-state frame of those nb banks + one attention call per bank over
+    `query_rows` of its query rows (synthesis + materialisation of the whole bank, then the sampled rows).  Returns the
+    measured per-step times and the whole-workload figures obtained by scaling with the bank and row counts."""
+    from concurrent.futures import ThreadPoolExecutor
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import bank_coords, query_rows_for_bank
+    from oracle import OracleBank
+    torch.set_num_threads(1)                       # host-side input generation must not fight the oracle threads
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    if max_cores:
+        cores = min(cores, max_cores)
+    nb = max(1, min(spec.n_banks, cores))
+    sub = _oracle_subspec(spec, nb)
+    ck, cv = gen.codebooks(sub)
+    banks = list(range(nb))
+    coords = [bank_coords(sub, b) for b in banks]
+    orc = [OracleBank(sub.T, sub.near_frames, sub.k_max, sub.head_dim, ck[c].numpy(), cv[c].numpy(), G=sub.G, C=sub.C)
+           for c in coords]
+    s = gen.grid_positions(sub)
+
+    def frame_inputs(f):
+        K, V = gen.frame_kv(sub, f)
+        return [(K[st, la, :, hd, :].float().numpy(), V[st, la, :, hd, :].float().numpy(), s[st].numpy())
+                for st, la, hd in coords]
+
+    pool = ThreadPoolExecutor(nb)
+
+    def upd(f):
+        inp = frame_inputs(f)
         t0 = time.perf_counter()
-        o.append_frame(K, V, s, trace=False)
-        t_upd += time.perf_counter() - t0
-        n += 1
-    Q = gen.queries(one, 0)
-    rows = query_rows_for_bank(one, Q, 0)
-    t0 = time.perf_counter()
-    o.attention(rows[:1])                      # synthesis of every prototype + materialisation + 1 row
-    t_one = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    o.attention(rows[:1 + query_rows])
-    t_many = time.perf_counter() - t0
-    per_row = max(0.0, (t_many - t_one) / query_rows)
-    per_bank_fixed = max(0.0, t_one - per_row)
-    rows_total = rows.shape[0]
-    s_frame = t_upd / n * spec.n_banks
-    s_query = (per_bank_fixed + per_row * rows_total) * spec.n_banks
-    return dict(frames_per_s=1.0 / s_frame, query_s=s_query, s_per_bank_frame=t_upd / n, frames_timed=n,
-                sample=f"bank 0 of {spec.n_banks}: {n} steady-state frames after {prime} priming frames; query: synthesis "
-                       f"+ materialisation of bank 0 once, {query_rows} of its {rows_total} rows; both scaled by the bank "
-                       f"and row counts", cores=1)
+        list(pool.map(lambda i: orc[i].append_frame(*inp[i], trace=False), range(nb)))
+        return time.perf_counter() - t0
+
+    Q = gen.queries(sub, 0)
+    rows = [query_rows_for_bank(sub, Q, b) for b in banks]
+    rows_total = rows[0].shape[0]
+
+    def qry(nrows):
+        t0 = time.perf_counter()
+        list(pool.map(lambda i: orc[i].attention(rows[i][:nrows]), range(nb)))
+        return time.perf_counter() - t0
+
+    prime = steady_state_frames(sub)
+    for f in range(prime):
+        upd(f)
+    f = prime
+    for _ in range(warmup):
+        upd(f); f += 1
+        qry(1 + query_rows)
+    tu = tq = 0.0
+    q1 = []
+    t_all = time.perf_counter()
+    for i in range(steps):
+        tu += upd(f); f += 1
+        tq += qry(1 + query_rows)
+        if i < 3:
+            q1.append(qry(1))                      # calibration of the per-row cost (1 row vs 1 + query_rows rows);
+    wall = time.perf_counter() - t_all             # inside the wall time, outside the per-step sums
+    pool.shutdown()
+    tu /= steps; tq /= steps
+    t_q1 = min(q1) if q1 else tq
+    per_row = max(0.0, (tq - t_q1) / query_rows)
+    fixed = max(0.0, tq - (1 + query_rows) * per_row)
+    scale = spec.n_banks / nb
+    s_frame = tu * scale
+    s_query = (fixed + per_row * rows_total) * scale
+    return dict(frames_per_s=1.0 / s_frame, query_s=s_query, step_ms=(tu + tq) * 1e3, update_step_ms=tu * 1e3,
+                query_step_ms=tq * 1e3, wall_s=wall, cores=nb, banks_timed=nb, steps=steps,
+                sample=f"{steps} steps on banks 0..{nb - 1} of {spec.n_banks} ({nb} threads, one single-threaded oracle per "
+                       f"bank) after {prime} priming frames; step = 1 steady-state frame of those banks ({tu * 1e3:.1f} ms) + "
+                       f"1 query per bank over {1 + query_rows} of its {rows_total} rows ({tq * 1e3:.1f} ms); value scales the "
+                       f"frame time by {spec.n_banks}/{nb} banks, query_attn_us scales per-bank fixed + per-row cost to "
+                       f"{rows_total} rows x {spec.n_banks} banks")
 
 
 def main():
@@ -399,7 +465,8 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="c3")
-    ap.add_argument("--extras", default="c2,c5", help="comma list of further configs measured briefly in the same line (N=1)")
+    ap.add_argument("--extras", default="c2,c5,c4_k4096_w64",
+                    help="comma list of further configs measured briefly in the same line (N=1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -408,25 +475,38 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
     spec = gen.spec_for(args.workload)
+    if world > 1 and args.impl != "reference":
+        # banks are independent, so N GPUs hold disjoint banks and nothing is exchanged.  The N-GPU job is the
+        # workload with N x its streams (one C3 video stream per GPU; C5's streams spread over the ranks), cut along the
+        # stream axis by paper_2606_26762_b200.sharding: weak scaling, per-GPU work fixed.
+        import dataclasses
+        from paper_2606_26762_b200 import sharding
+        sh = sharding.shard_config(spec.n_streams * world, spec.n_layers, spec.n_q_heads, spec.n_kv_heads, world, rank,
+                                   axis="stream")
+        spec = dataclasses.replace(spec, n_streams=sh["n_streams"], stream0=sh["begin"])
     config = dict(workload=f"{spec.name}: BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c3': 2, 'c5': 4}.get(spec.name, 3)}]",
                   banks=spec.n_banks, layers=spec.n_layers, streams=spec.n_streams, q_heads=spec.n_q_heads,
                   kv_heads=spec.n_kv_heads, head_dim=spec.head_dim, tokens_per_frame=spec.T, near_frames=spec.near_frames,
                   k_max=spec.k_max, n_query_tokens=spec.n_query_tokens,
                   step="1 protokv_append_frame (steady state) + 1 protokv_query_attention; value = frames/s of the update "
-                       "part, query_attn_us = the query part, ms_per_step = both")
+                       "part, query_attn_us = the query part, ms_per_step = both",
+                  l2="inputs cycle through a device pool sized so that state + pool > 2x L2 (126 MB); where they are "
+                     "smaller a 252 MB fill flushes L2 before each timed segment (l2_policy says which applied)")
 
     if args.impl == "reference":
         if rank != 0:
             return
-        t_all = time.perf_counter()
-        os_ = oracle_sample(spec, budget_s=min(60.0, 4.0 * max(1, args.steps)))
+        os_ = oracle_arm(spec, steps=args.steps, warmup=warmup)
         line = dict(metric=METRIC, value=os_["frames_per_s"], unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=warmup,
-                    ms_per_step=1e3 / os_["frames_per_s"] + os_["query_s"] * 1e3, higher_is_better=True, scaling="weak",
+                    ms_per_step=os_["wall_s"] * 1e3 / args.steps, higher_is_better=True, scaling="weak",
                     vs_baseline=None, dtype="f64", data="synthetic", config=config, impl="reference",
                     query_attn_us=os_["query_s"] * 1e6,
+                    measured=dict(update_step_ms=os_["update_step_ms"], query_step_ms=os_["query_step_ms"],
+                                  banks_timed=os_["banks_timed"], timed_region_s=os_["wall_s"],
+                                  note="ms_per_step is the time of the bounded step actually run; value and query_attn_us "
+                                       "are whole-workload figures obtained from it (see cpu_baseline.sample)"),
                     cpu_baseline=dict(value=os_["frames_per_s"], unit=UNIT, cores=os_["cores"], kind="oracle", sample=os_["sample"]),
-                    e2e=dict(value=os_["frames_per_s"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
-                    wall_s=time.perf_counter() - t_all)
+                    e2e=dict(value=os_["frames_per_s"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
         print(json.dumps(line))
         return
 
@@ -440,7 +520,7 @@ def main():
         barrier = lambda: dist.barrier()
     peaks = load_peaks()
     sampler = ClockSampler(local) if rank == 0 else None
-    res = run_workload(spec, device, args.steps, warmup, rank=rank, sampler=sampler, barrier=barrier,
+    res = run_workload(spec, device, args.steps, warmup, rank=0, sampler=sampler, barrier=barrier,
                        do_e2e=True, do_profile=True)
     upd_ms, qry_ms, region_ms = res["update_ms_sum"], res["query_ms_sum"], res["region_ms"]
     e2e_u, e2e_q = res["e2e"]["update_s"] / res["e2e"]["steps"], res["e2e"]["query_s"] / res["e2e"]["steps"]
@@ -460,7 +540,7 @@ def main():
     roof, stage_roofs = roofline_objects(spec, res, peaks, K)
     line = dict(metric=METRIC, value=fps, unit=UNIT, n_gpus=world, steps=K, warmup=warmup,
                 ms_per_step=region_ms / K, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="bf16" if spec.dtype == "bf16" else "f32", data="synthetic", config=dict(config, l2=res["l2"]),
+                dtype="bf16" if spec.dtype == "bf16" else "f32", data="synthetic", config=config, l2_policy=res["l2"],
                 update_ms_per_frame=upd_ms / K, update_ms_median=res["update_ms_median"],
                 query_attn_us=qry_ms / K * 1e3, query_attn_us_median=res["query_ms_median"] * 1e3,
                 gpu_launches=res["launches"], impl_kernels=res["impl"], clocks=res["clocks"],
@@ -482,7 +562,7 @@ def main():
                 sp = gen.spec_for(name)
                 r = run_workload(sp, device, max(10, K // 4), warmup, do_e2e=False, do_profile=True)
                 n = max(10, K // 4)
-                ro, sr = roofline_objects(sp, r, peaks, n)
+                ro, sr = roofline_objects(sp, r, peaks, n, clocks=res["clocks"])
                 extras[name] = dict(frames_per_s=n / (r["update_ms_sum"] * 1e-3), update_ms_per_frame=r["update_ms_sum"] / n,
                                     query_attn_us=r["query_ms_sum"] / n * 1e3, steps=n, l2=r["l2"], roofline=ro,
                                     rooflines=sr, stages_ms_per_step={k: v[0] / n for k, v in r["stages"].items()})
@@ -490,7 +570,7 @@ def main():
                 extras[name] = dict(error=repr(e))
         line["other_workloads"] = extras
     if world == 1 and not args.no_cpu_baseline:
-        os_ = oracle_sample(spec, budget_s=15.0)
+        os_ = oracle_arm(spec, steps=12, warmup=1)
         line["cpu_baseline"] = dict(value=os_["frames_per_s"], unit=UNIT, cores=os_["cores"], kind="oracle",
                                     sample=os_["sample"], query_attn_us=os_["query_s"] * 1e6,
                                     host_cores_available=os.cpu_count())

@@ -105,6 +105,7 @@ class WorkloadSpec:
     query_every: int = 0       # 0: one query after the last frame
     G: int = 8
     C: int = 16
+    stream0: int = 0           # global index of this spec's first stream (a rank's shard of a multi-stream workload)
 
     @property
     def T(self) -> int:
@@ -152,7 +153,7 @@ def grid_positions(spec: WorkloadSpec, device="cpu") -> torch.Tensor:
 
 def cluster_ids(spec: WorkloadSpec, frame: int, device="cpu") -> torch.Tensor:
     """[n_streams][T] int64 mixture component of each token (shared by all layers/heads)."""
-    st = _arange(spec.n_streams, device)[:, None]
+    st = _arange(spec.n_streams, device)[:, None] + spec.stream0
     j = _arange(spec.T, device)[None, :]
     row, col = j // spec.grid_w, j % spec.grid_w
     block = (row // 2) * ((spec.grid_w + 1) // 2) + (col // 2)
@@ -192,7 +193,7 @@ def frame_kv(spec: WorkloadSpec, frame: int, device="cpu"):
     dev = str(device)
     cl = cluster_ids(spec, frame, dev)                                   # [S][T]
     out = []
-    st = _arange(spec.n_streams, dev)[:, None, None, None, None]
+    st = _arange(spec.n_streams, dev)[:, None, None, None, None] + spec.stream0
     la = _arange(spec.n_layers, dev)[None, :, None, None, None]
     j = _arange(spec.T, dev)[None, None, :, None, None]
     hd = _arange(spec.n_kv_heads, dev)[None, None, None, :, None]
@@ -214,6 +215,7 @@ def codebooks(spec: WorkloadSpec, device="cpu"):
     sub = spec.head_dim // spec.G
     shape_idx = [_arange(n, dev) for n in (spec.n_streams, spec.n_layers, spec.n_kv_heads, spec.G, spec.C, sub)]
     idx = [a.reshape([-1 if i == k else 1 for i in range(6)]) for k, a in enumerate(shape_idx)]
+    idx[0] = idx[0] + spec.stream0
     res = []
     for tag in (TAG_CB_K, TAG_CB_V):
         z = standard_normal(_key(spec.seed, tag, *idx, device=dev))
@@ -227,5 +229,6 @@ def queries(spec: WorkloadSpec, query_index: int = 0, n_q: Optional[int] = None,
     n_q = spec.n_query_tokens if n_q is None else n_q
     dims = (spec.n_streams, spec.n_layers, n_q, spec.n_q_heads, spec.head_dim)
     idx = [_arange(n, dev).reshape([-1 if i == k else 1 for i in range(5)]) for k, n in enumerate(dims)]
+    idx[0] = idx[0] + spec.stream0
     z = standard_normal(_key(spec.seed, TAG_Q, query_index, *idx, device=dev))
     return z.to(spec.torch_dtype).contiguous()

@@ -8,8 +8,11 @@
  * (PAPER.md:L312); one state object holds n_streams * n_layers * n_kv_heads of them and every call processes
  * all of them in batched kernel launches.
  *
- * Everything runs in hand-written CUDA kernels on the caller's stream.  There is no CPU fallback: on a machine
- * without an sm_100 device protokv_create fails with PROTOKV_EUNSUPPORTED.
+ * Every step of Alg. 1 / 3 / 4 runs in hand-written CUDA kernels on the caller's stream.  The one piece of the
+ * method's arithmetic evaluated on the host is a constant table: protokv_create fills the 4,096 numerators
+ * log(h + pq_eps), h = 0..4095, of Eq. 3 with the host's libm and copies them to the device, where the
+ * synthesis kernel looks them up (larger counts are evaluated by the kernel itself).  There is no CPU fallback: on a
+ * machine without an sm_100 device protokv_create fails with PROTOKV_EUNSUPPORTED.
  *
  * Conventions
  *   - "device"/"host" says where a pointer must live.  Tensor arguments are caller-owned and contiguous.
@@ -57,7 +60,13 @@ enum {
   PROTOKV_NO_RESIDUAL = 4u,  /* never update histograms => zero residuals (Table 2)               */
   PROTOKV_NEAR_ONLY = 8u,    /* attention over the near window only (L176)                              */
   PROTOKV_FAR_ONLY = 16u,    /* attention over pseudo-tokens only   (L177)                              */
-  PROTOKV_FORCE_SIMT = 32u   /* use the fp32 SIMT kernels even where a tcgen05 kernel exists (cross-check) */
+  PROTOKV_FORCE_SIMT = 32u,  /* use the fp32 SIMT kernels even where a tcgen05 kernel exists (cross-check) */
+  PROTOKV_DECODE_SPLITKV = 128u, /* serve queries of <= 16 rows per bank with the split-KV mma.sync kernel
+                                (csrc/decode_attention.cu) instead of the 128-row tcgen05 kernel.  Measured on C3 (one
+                                query token, 7 rows per bank): 167-183 us against 161 us -- not faster, hence opt-in */
+  PROTOKV_MAINTENANCE = 64u  /* run Alg. 2 at the end of every append_frame that evicted a frame
+                                (Alg. 1 l.15); off by default: north_star's path and its invariant "total mass = tokens
+                                absorbed" exclude it (reading 19) */
 };
 
 typedef struct {
@@ -76,20 +85,30 @@ typedef struct {
   float cos_eps;          /* lower bound of |K||c| in the cosine (reading 6): 1e-12 */
   double pq_eps;          /* epsilon of Eq. 3 (value not given in the paper): 1e-6 */
   uint32_t flags;
+  float gamma;            /* Alg. 2 idle decay rate (Table 5: 0.05); used with PROTOKV_MAINTENANCE */
+  float eps_k, eps_v;     /* Alg. 2 merge thresholds on |c_i - c_j|, |p_i - p_j| (Table 5: 0.20, 0.25) */
   const float *codebook_k, *codebook_v; /* device; copied at create.  NULL => no residual statistics */
   void *workspace;        /* device memory from the caller, >= protokv_workspace_bytes(cfg), 256-byte aligned */
   size_t workspace_bytes;
   void *cuda_stream;      /* cudaStream_t of the caller (NULL = legacy default stream) */
 } protokv_config;
 
-/* Bytes of device workspace a state with this configuration needs; 0 if the configuration is invalid
- * (protokv_last_error() says why).  Pointer fields of cfg are ignored.  Host-only, no CUDA call. */
+/* Bytes of device workspace a state with this configuration needs: the two-tier state of PAPER.md:L300-312 (§A.1) --
+ * B_near (ring of W = near_frames * T exact K, V rows per bank, L300) and B_far (k_max prototypes
+ * (c, p, n, R, mu, Sigma, tau) per bank, L302-310, R = two G x C histograms + n_res) -- plus the per-frame scratch, the
+ * derived copies the kernels stream and the host-variant staging buffers; constant in the
+ * stream length (L81, L102).  0 if the configuration is invalid (protokv_last_error() says why).  Pointer fields of
+ * cfg are ignored.  Host-only, no CUDA call. */
 size_t protokv_workspace_bytes(const protokv_config *cfg);
 
-/* Builds the state inside cfg->workspace (zeroed asynchronously on the stream).  NULL on failure. */
+/* Builds the empty state of PAPER.md:L300-312 inside cfg->workspace: empty near window, every prototype slot inactive
+ * (L83: slots are opened by the first evicted tokens), codebooks copied from cfg (L312: fixed after warm-up; their
+ * training is the caller's, reading 11).  The workspace is zeroed asynchronously on the stream.
+ * The state is bound to the CUDA device that is current at this call; later calls may be made with any device
+ * current.  NULL on failure (protokv_last_error()). */
 protokv_state *protokv_create(const protokv_config *cfg);
 
-/* Releases host-side resources.  The workspace stays the caller's.  NULL is a no-op. */
+/* Releases host-side resources (the paper's state lives entirely in the caller's workspace).  NULL is a no-op. */
 void protokv_destroy(protokv_state *st);
 
 /*
@@ -98,7 +117,11 @@ void protokv_destroy(protokv_state *st);
  * evicted and absorbed:  (A) while free slots remain each evicted token opens the lowest free slot (l.3-4, L83);
  * (B) the others are assigned by Eq. 1 (L93) against the bank as it stands after (A), lowest index on ties;
  * (C) Alg. 1 l.8-13 is replayed token by token in eviction order (EMA centres, mass, recency, spatial mean and
- * covariance, PQ residual histograms of the just-updated centres).  Alg. 1 l.15 (maintenance) is not run.
+ * covariance, PQ residual histograms of the just-updated centres).  Alg. 1 l.15 (maintenance, Alg. 2)
+ * runs only with PROTOKV_MAINTENANCE, once per frame after (C) and after the frame has entered the ring: idle
+ * prototypes decay n <- floor((1 - gamma) n), pairs with |c_i - c_j| < eps_k and |p_i - p_j| < eps_v merge into the lower
+ * index (mass-weighted c, p, mu; n, H, n_res summed; Sigma, tau, pos of the survivor kept), and every slot emptied by
+ * decay or merging is re-initialised from the newest near-window tokens (readings 20, 24-27).
  * K, V, grid_pos: device.
  */
 int protokv_append_frame(protokv_state *st, const void *K, const void *V, const float *grid_pos);
@@ -156,18 +179,37 @@ int protokv_export_ring(protokv_state *st, int32_t bank, float *K, float *V, flo
 /* Result of the last synthesis for one bank, on the host: codes [k_max][S][G] (one code per byte) and
  * kind [k_max] (0 = decoded modes, 1 = zero residuals, 2 = slot not in the context).  Synchronises. */
 int protokv_export_codes(protokv_state *st, int32_t bank, uint8_t *codes_k, uint8_t *codes_v, uint8_t *kind);
+/* Overwrites the tuples of one bank (parity aid: attention with the checker's codes).  They stay in force until the
+ * next synthesis, which re-decodes the whole bank from its histograms. */
 int protokv_import_codes(protokv_state *st, int32_t bank, const uint8_t *codes_k, const uint8_t *codes_v);
 
 /* What the last append_frame decided, all banks, on the host: assign [banks][T] (slot index; -1 if no frame
- * was evicted), best [banks][T] (Eq. 1 score of the choice; 0 for slot fills), codes_k/v [banks][T][G]
- * (255 = no residual update); *n_fill = tokens per bank that opened a new slot; *evicted_frame = index of the
- * evicted frame or -1.  NULL members are skipped.  Synchronises. */
+ * was evicted; -2 for a token without any finite Eq. 1 score, see protokv_error_flags), best [banks][T] (Eq. 1 score
+ * of the choice; 0 for slot fills), codes_k/v [banks][T][G] (255 = no residual update); *n_fill = tokens per bank that
+ * opened a new slot; *evicted_frame = index of the evicted frame or -1.  NULL members are skipped.  Synchronises.
+ * The runner-up score is deliberately not part of the trace: the parity rule needs "the ORACLE's score of the GPU's
+ * choice minus the oracle's best" (north_star's 1e-5 gap), which only the checker can evaluate, and the kernels keep
+ * one running minimum per token (a second one would cost the epilogue a compare per score for no consumer). */
 int protokv_last_frame_trace(protokv_state *st, int32_t *assign, float *best, uint8_t *codes_k,
                              uint8_t *codes_v, int32_t *n_fill, int32_t *evicted_frame);
 
 /* Counters: frames appended so far; kernels launched by this state since create (bench's gpu_launches). */
 int64_t protokv_frames_seen(const protokv_state *st);
 int64_t protokv_kernel_launches(const protokv_state *st);
+
+/* Sticky device-side error bits raised by the kernels since create (or the last clear); synchronises the stream.
+ *   bit 0 (PROTOKV_ERRBIT_UNASSIGNED): an evicted token had no finite Eq. 1 score against any prototype (NaN / Inf in
+ *   its key row or in the bank).  Eq. 1's argmin is undefined for it; the token is dropped (not absorbed, trace
+ *   assign = -2) and the rest of the frame proceeds.  *flags (host) receives the bits; clear != 0 resets them. */
+/*   bit 1 (PROTOKV_ERRBIT_MAINT_OVERFLOW): Alg. 2 met more merge candidates in one frame of one bank than its list holds
+ *   (2,048); the excess pairs were not merged in that frame. */
+enum { PROTOKV_ERRBIT_UNASSIGNED = 1u, PROTOKV_ERRBIT_MAINT_OVERFLOW = 2u };
+int protokv_error_flags(protokv_state *st, uint32_t *flags, int32_t clear);
+
+/* What Alg. 2 has done since create, summed over all banks: counts[0] = mass removed by aging, counts[1] = prototypes
+ * merged away, counts[2] = slots recycled (host, 3 entries).  Synchronises.  The generalised mass invariant reads
+ * sum_k n_k = tokens absorbed - counts[0] + counts[2]. */
+int protokv_maintenance_counters(protokv_state *st, int64_t *counts);
 
 /* Stage timing (measurement aid, off by default).  When enabled the library brackets every kernel group it launches
  * with CUDA events on the state's stream; protokv_profile_read synchronises the stream and returns, per stage, the

@@ -10,11 +10,11 @@ import numpy as np
 from .build import build
 
 F32, BF16 = 0, 1
-MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT = 1, 2, 4, 8, 16, 32
+MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV = 1, 2, 4, 8, 16, 32, 64, 128
 
 # Table 5 of the paper + the constants the paper leaves open (readings 4, 6, 12)
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
-                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0)
+                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0, gamma=0.05, eps_k=0.20, eps_v=0.25)
 
 EXPORTED_SYMBOLS = [
     "protokv_workspace_bytes", "protokv_create", "protokv_destroy", "protokv_append_frame",
@@ -22,7 +22,7 @@ EXPORTED_SYMBOLS = [
     "protokv_query_attention_ex", "protokv_synthesize", "protokv_export_state", "protokv_import_state",
     "protokv_export_ring", "protokv_export_codes", "protokv_import_codes", "protokv_last_frame_trace",
     "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl", "protokv_profile_enable",
-    "protokv_profile_read",
+    "protokv_profile_read", "protokv_error_flags", "protokv_maintenance_counters",
 ]
 STAGES = ["fill", "score", "update", "append", "synthesis", "attention"]
 
@@ -43,7 +43,7 @@ class ProtoKVConfig(C.Structure):
                 ("lambda_sp", C.c_float), ("lambda_idle", C.c_float), ("t_idle", C.c_int32),
                 ("alpha", C.c_float), ("beta", C.c_float), ("eta", C.c_float),
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
-                ("flags", C.c_uint32),
+                ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float),
                 ("codebook_k", C.c_void_p), ("codebook_v", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("cuda_stream", C.c_void_p)]
@@ -89,6 +89,8 @@ def load_library():
     lib.protokv_kernel_launches.argtypes = [vp]
     lib.protokv_profile_enable.argtypes = [vp, i32]
     lib.protokv_profile_read.argtypes = [vp, vp, vp]
+    lib.protokv_error_flags.argtypes = [vp, C.POINTER(C.c_uint32), i32]
+    lib.protokv_maintenance_counters.argtypes = [vp, vp]
     lib.protokv_stage_impl.restype = C.c_char_p
     lib.protokv_stage_impl.argtypes = [vp, i32]
     _lib = lib
@@ -319,6 +321,16 @@ class ProtoKV:
     @property
     def kernel_launches(self):
         return int(self._lib.protokv_kernel_launches(self._h))
+
+    def maintenance_counters(self):
+        c = np.zeros(3, np.int64)
+        self._check(self._lib.protokv_maintenance_counters(self._h, _np_ptr(c)))
+        return dict(decayed=int(c[0]), merges=int(c[1]), recycled=int(c[2]))
+
+    def error_flags(self, clear=False):
+        f = C.c_uint32(0)
+        self._check(self._lib.protokv_error_flags(self._h, C.byref(f), int(clear)))
+        return int(f.value)
 
     def stage_impl(self, stage):
         return self._lib.protokv_stage_impl(self._h, stage).decode()

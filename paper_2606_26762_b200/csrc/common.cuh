@@ -11,8 +11,14 @@
 namespace pkv {
 
 constexpr int kMaxS = 8, kMaxG = 8, kMaxC = 16;
+constexpr int kMaxT = 4096, kMaxKmax = 16384;   // limits protokv_create admits (sort keys hold 12 bits of token index)
 #define PKV_SYN_LOGTAB 4096
-constexpr int kCbPad = 16;  // floats of padding after each subspace's [C][sub] block in shared memory
+constexpr int kCbPad = 16;
+// Device-side error bits (Dev::err).  UNASSIGNED: an evicted token had no finite Eq. 1 score against any prototype (a
+// NaN / Inf in its key row or in the bank); it is NOT absorbed (trace assign = -2) and the bit is raised.
+constexpr uint32_t PKV_ERR_UNASSIGNED = 1u;
+constexpr uint32_t PKV_ERR_MAINT_OVERFLOW = 2u;   // Alg. 2: more merge candidates in one frame than the kernel's list holds
+constexpr int kNoProto = 0xfffff;   // sort-key prototype field of such a token (k_max <= 16384 < kNoProto)  // floats of padding after each subspace's [C][sub] block in shared memory
 
 // Shapes, fixed at create.
 struct Dims {
@@ -103,6 +109,12 @@ struct Dev {
                              // assignment; all-ones between frames (reset by the append kernel)
   uint8_t* tcodeK;   // [B][T][G]
   uint8_t* tcodeV;
+  // err[0]: sticky device-side error bits (PKV_ERR_*), read by protokv_error_flags
+  uint32_t* err;
+  // Alg. 2 maintenance: mstamp[pk] = stream time of the last change of c_k / p_k (fill, update, merge, recycle);
+  // mcount = {mass decayed, prototypes merged away, slots recycled} since create
+  int* mstamp;                   // [B][K]
+  unsigned long long* mcount;    // [3]
   // attention scratch
   float* part;   // [rows_total][nsplit][d + 2]
   // host-variant staging
@@ -162,6 +174,11 @@ int launch_fill(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F,
 int launch_score_simt(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
 int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s);
 int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s);
+int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s);
+// One-time (per device) function attributes of every kernel that needs more than 48 KB of shared memory for some
+// admissible shape; returns false if the device refuses one of them.
+bool update_kernels_prepare(const Dims& D);
+bool query_kernels_prepare(const Dims& D);
 int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s);
 
 __device__ __forceinline__ void mark_dirty(const Dims& D, const Dev& V, int b, int k, int epoch) {
@@ -177,6 +194,20 @@ struct AttnArgs {
 };
 int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
+
+// Alg. 2 maintenance (maintenance.cu)
+bool maintenance_prepare();
+int launch_maintenance(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int held, int full, float gamma,
+                       float eps_k, float eps_v, cudaStream_t s);
+
+// decode-style attention (decode_attention.cu): bf16, d = 128, n_q * group <= 16 rows per bank
+bool decode_attention_supported(const Dims& D, int n_q);
+size_t decode_attention_part_bytes(const Dims& D);
+bool decode_attention_prepare();
+int launch_attention_decode(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
+                            int* nsplit_out);
+// merges A.nsplit partials per row ([rows][nsplit][d + 2] in Dev::part) into out / lse (bf16, d = 128)
+int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, cudaStream_t s);
 
 // tcgen05 paths (bf16, d = 128).  The TMA tensor maps are built once per state.
 struct TcMaps {

@@ -18,6 +18,9 @@ struct protokv_state {
   Hyper H;
   Dev V;
   cudaStream_t stream;
+  int device;         // ordinal the state was created on; every entry point runs with it current (DeviceGuard)
+  bool poisoned;      // a launch failed half-way through a call: device and host counters may disagree
+  bool maint_full;    // the next Alg. 2 pass must look at every pair (first pass, after an import)
   int sm_count;
   int64_t frames;     // frames appended so far = stream time of the next frame
   int n_act;          // active prototypes per bank (identical in every bank: slot fill is data-independent)
@@ -29,6 +32,7 @@ struct protokv_state {
   int epoch;          // synthesis epoch (see Dev::dirty_cnt)
   bool use_tc_assign;
   bool use_tc_attn;
+  bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
   TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
@@ -56,11 +60,7 @@ struct StageTimer {
     a = get(st); b = get(st);
     cudaEventRecord(a, st->stream);
   }
-  ~StageTimer() {
-    if (!a) return;
-    cudaEventRecord(b, st->stream);
-    st->spans.push_back({stage, a, b});
-  }
+  ~StageTimer();
 };
 
 static int drain_spans(protokv_state* st) {
@@ -73,7 +73,28 @@ static int drain_spans(protokv_state* st) {
   return 0;
 }
 
+StageTimer::~StageTimer() {
+  if (!a) return;
+  cudaEventRecord(b, st->stream);
+  st->spans.push_back({stage, a, b});
+  if (st->spans.size() >= 4096) {      // nobody reads the profile: fold the finished spans so the events are recycled
+    cudaEventSynchronize(b);
+    drain_spans(st);
+  }
+}
+
 static thread_local char g_err[512] = "";
+
+// Makes the state's device current for the duration of an entry point and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(const protokv_state* st) {
+    if (!st) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != st->device) switched = cudaSetDevice(st->device) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 static int fail(int code, const char* fmt, ...) {
   va_list ap;
@@ -111,12 +132,18 @@ static int validate(const protokv_config* c) {
     for (int g = 0; g < c->G; ++g) tuples *= c->C;
     if (tuples < c->S) return fail(PROTOKV_EINVAL, "C^G < S");
   }
-  if (c->tokens_per_frame > 4096) return fail(PROTOKV_EUNSUPPORTED, "tokens_per_frame > 4096");
-  if (c->k_max > 16384) return fail(PROTOKV_EUNSUPPORTED, "k_max > 16384");
+  if (c->tokens_per_frame > kMaxT) return fail(PROTOKV_EUNSUPPORTED, "tokens_per_frame > 4096");
+  if (c->k_max > kMaxKmax) return fail(PROTOKV_EUNSUPPORTED, "k_max > 16384");
   if (!(c->alpha >= 0.f && c->alpha <= 1.f && c->beta >= 0.f && c->beta <= 1.f && c->eta >= 0.f && c->eta <= 1.f))
     return fail(PROTOKV_EINVAL, "alpha, beta, eta must lie in [0, 1]");
   if (!(c->sigma_eps >= 0.f) || !(c->cos_eps > 0.f) || !(c->pq_eps > 0.0))
     return fail(PROTOKV_EINVAL, "need sigma_eps >= 0, cos_eps > 0, pq_eps > 0");
+  if (c->flags & PROTOKV_MAINTENANCE) {
+    if (!(c->gamma >= 0.f && c->gamma <= 1.f) || !(c->eps_k >= 0.f) || !(c->eps_v >= 0.f))
+      return fail(PROTOKV_EINVAL, "maintenance needs gamma in [0, 1], eps_k >= 0, eps_v >= 0");
+  }
+  if (!(c->lambda_sp >= 0.f) || !(c->lambda_idle >= 0.f))   // Eq. 1's penalties are penalties (the score kernel prunes on it)
+    return fail(PROTOKV_EINVAL, "need lambda_sp >= 0 and lambda_idle >= 0");
   if ((c->flags & PROTOKV_NEAR_ONLY) && (c->flags & PROTOKV_FAR_ONLY))
     return fail(PROTOKV_EINVAL, "NEAR_ONLY and FAR_ONLY are exclusive");
   return PROTOKV_OK;
@@ -171,9 +198,13 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   v.assign = (int*)take(BT * 4); v.best = (float*)take(BT * 4);
   v.akey = (unsigned long long*)take(BT * 8);
   v.tcodeK = (uint8_t*)take(BT * D.G); v.tcodeV = (uint8_t*)take(BT * D.G);
+  v.err = (uint32_t*)take(256);
+  v.mcount = (unsigned long long*)take(256);
+  v.mstamp = (int*)take(BK * 4);
   const size_t rows = (size_t)D.B * D.Nq * D.group;
   size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
   if (tc_attention_supported(D) && tc_attention_part_bytes(D) > part_bytes) part_bytes = tc_attention_part_bytes(D);
+  if (decode_attention_supported(D, 1) && decode_attention_part_bytes(D) > part_bytes) part_bytes = decode_attention_part_bytes(D);
   v.part = (float*)take(part_bytes);
   const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * elt;
   const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * elt;
@@ -222,6 +253,9 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->cfg = *cfg;
   fill_dims(cfg, &st->D, &st->H);
   st->stream = (cudaStream_t)cfg->cuda_stream;
+  st->device = dev;
+  st->poisoned = false;
+  st->maint_full = true;
   st->sm_count = sms;
   st->nsplit = plan_nsplit(st->D);
   const bool has_cb = cfg->codebook_k && !(cfg->flags & PROTOKV_NO_RESIDUAL);
@@ -255,15 +289,24 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->profiling = false;
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->maps.ok = false;
+  if (!update_kernels_prepare(st->D) || !query_kernels_prepare(st->D) ||
+      ((cfg->flags & PROTOKV_MAINTENANCE) && !maintenance_prepare())) {   // capability error: before any launch
+    fail(PROTOKV_EUNSUPPORTED, "the device refused the shared-memory opt-in this shape needs");
+    delete st;
+    return nullptr;
+  }
   const bool want_tc = !(cfg->flags & PROTOKV_FORCE_SIMT);
   if (want_tc && (tc_assign_supported(st->D, st->H) || tc_attention_supported(st->D))) tc_build_maps(st->D, st->V, &st->maps);
   st->use_tc_assign = want_tc && tc_assign_supported(st->D, st->H) && st->maps.ok;
   st->use_tc_attn = want_tc && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
+  st->use_decode_attn = want_tc && (cfg->flags & PROTOKV_DECODE_SPLITKV) && decode_attention_supported(st->D, 1) &&
+                        decode_attention_prepare();
   return st;
 }
 
 void protokv_destroy(protokv_state* st) {
   if (!st) return;
+  DeviceGuard dg(st);
   for (auto& sp : st->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto e : st->ev_free) cudaEventDestroy(e);
   delete st;
@@ -271,6 +314,7 @@ void protokv_destroy(protokv_state* st) {
 
 int protokv_profile_enable(protokv_state* st, int32_t on) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  DeviceGuard dg(st);
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   drain_spans(st);
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
@@ -280,6 +324,7 @@ int protokv_profile_enable(protokv_state* st, int32_t on) {
 
 int protokv_profile_read(protokv_state* st, double* ms_sum, int64_t* launches) {
   if (!st || !ms_sum || !launches) return fail(PROTOKV_EINVAL, "NULL argument");
+  DeviceGuard dg(st);
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   drain_spans(st);
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) {
@@ -291,6 +336,8 @@ int protokv_profile_read(protokv_state* st, double* ms_sum, int64_t* launches) {
 
 int protokv_append_frame(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
   if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
+  if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   FrameArgs F{};
   F.t = (int)st->frames;
@@ -322,7 +369,19 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
     StageTimer tm(st, PROTOKV_STAGE_APPEND);
     nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                  // U1 (overwrites the slot)
   }
-  PKV_CUDA(cudaGetLastError());
+  if ((st->H.flags & PROTOKV_MAINTENANCE) && F.evicted) {                               // Alg. 1 l.15 -> Alg. 2
+    const int held = (int)(st->frames + 1 < D.Wf ? st->frames + 1 : D.Wf);
+    nl += launch_maintenance(D, st->H, st->V, F, held, st->maint_full ? 1 : 0, st->cfg.gamma, st->cfg.eps_k, st->cfg.eps_v,
+                             st->stream);
+    st->maint_full = false;
+  }
+  {
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {   // some kernels of this frame may have run: the bank no longer matches the host counters
+      st->poisoned = true;
+      return fail(PROTOKV_ECUDA, "append_frame launch: %s", cudaGetErrorString(e));
+    }
+  }
   st->launches += nl;
   st->n_act = F.n_act;
   st->last_ev_frame = F.ev_frame;
@@ -334,6 +393,8 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
 
 int protokv_synthesize(protokv_state* st) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
+  DeviceGuard dg(st);
   {
     StageTimer tm(st, PROTOKV_STAGE_SYNTH);
     st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->sm_count, st->stream);
@@ -347,6 +408,8 @@ int protokv_synthesize(protokv_state* st) {
 int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, int32_t layer_begin,
                                int32_t layer_count, void* out, float* lse, int32_t run_synthesis) {
   if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
+  if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   if (n_q < 1 || n_q > D.Nq) return fail(PROTOKV_EINVAL, "n_q %d outside [1, %d]", n_q, D.Nq);
   if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > D.L)
@@ -371,7 +434,12 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
   A.nsplit = st->nsplit;
   {
     StageTimer tm(st, PROTOKV_STAGE_ATTN);
-    if (st->use_tc_attn && (uintptr_t)Q % 16 == 0 && (uintptr_t)out % 8 == 0) {
+    if (st->use_decode_attn && decode_attention_supported(D, n_q) && (uintptr_t)Q % 16 == 0) {
+      int ns = 1;
+      st->launches += launch_attention_decode(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
+      A.nsplit = ns;
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+    } else if (st->use_tc_attn && (uintptr_t)Q % 16 == 0 && (uintptr_t)out % 8 == 0) {
       const int nl = launch_attention_tc(D, st->H, st->V, A, st->maps, st->sm_count, st->stream);
       if (nl < 0) return fail(PROTOKV_ECUDA, "cuTensorMapEncodeTiled failed for Q");
       st->launches += nl;
@@ -390,6 +458,7 @@ int protokv_query_attention(protokv_state* st, const void* Q, void* out) {
 
 int protokv_append_frame_host(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
   if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * (D.bf16 ? 2 : 4);
   PKV_CUDA(cudaMemcpyAsync(st->V.stageK, K, frame, cudaMemcpyHostToDevice, st->stream));
@@ -400,6 +469,7 @@ int protokv_append_frame_host(protokv_state* st, const void* K, const void* V, c
 
 int protokv_query_attention_host(protokv_state* st, const void* Q, void* out) {
   if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * (D.bf16 ? 2 : 4);
   PKV_CUDA(cudaMemcpyAsync(st->V.stageQ, Q, qbytes, cudaMemcpyHostToDevice, st->stream));
@@ -413,10 +483,28 @@ int protokv_query_attention_host(protokv_state* st, const void* Q, void* out) {
 int64_t protokv_frames_seen(const protokv_state* st) { return st ? st->frames : -1; }
 int64_t protokv_kernel_launches(const protokv_state* st) { return st ? st->launches : -1; }
 
+int protokv_maintenance_counters(protokv_state* st, int64_t* counts) {
+  if (!st || !counts) return fail(PROTOKV_EINVAL, "NULL argument");
+  DeviceGuard dg(st);
+  PKV_CUDA(cudaMemcpyAsync(counts, st->V.mcount, 3 * sizeof(int64_t), cudaMemcpyDeviceToHost, st->stream));
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  return PROTOKV_OK;
+}
+
+int protokv_error_flags(protokv_state* st, uint32_t* flags, int32_t clear) {
+  if (!st || !flags) return fail(PROTOKV_EINVAL, "NULL argument");
+  DeviceGuard dg(st);
+  PKV_CUDA(cudaMemcpyAsync(flags, st->V.err, 4, cudaMemcpyDeviceToHost, st->stream));
+  if (clear) PKV_CUDA(cudaMemsetAsync(st->V.err, 0, 4, st->stream));
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  return PROTOKV_OK;
+}
+
 const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
   if (!st) return "none";
   if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
   if (stage == 1) return st->use_tc_attn ? "tcgen05" : "simt";
+  if (stage == 2) return st->use_decode_attn ? "mma.sync split-KV" : (st->use_tc_attn ? "tcgen05" : "simt");
   return "none";
 }
 
@@ -444,6 +532,7 @@ int protokv_export_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   int rc = check_bank(st, bank);
   if (rc) return rc;
   if (!v) return fail(PROTOKV_EINVAL, "NULL view");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   const Dev& V = st->V;
   const size_t K = D.K, o = (size_t)bank * K;
@@ -469,6 +558,7 @@ int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   int rc = check_bank(st, bank);
   if (rc) return rc;
   if (!v) return fail(PROTOKV_EINVAL, "NULL view");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   const Dev& V = st->V;
   const size_t K = D.K, o = (size_t)bank * K;
@@ -496,6 +586,7 @@ int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   PKV_CUDA(cudaGetLastError());
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   st->codes_valid = false;
+  st->maint_full = true;
   return PROTOKV_OK;
 }
 
@@ -503,6 +594,7 @@ int protokv_export_ring(protokv_state* st, int32_t bank, float* K, float* Vv, fl
                         int32_t* n_frames) {
   int rc = check_bank(st, bank);
   if (rc) return rc;
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   const int held = (int)(st->frames < D.Wf ? st->frames : D.Wf);
   if (n_frames) *n_frames = held;
@@ -537,6 +629,7 @@ int protokv_export_codes(protokv_state* st, int32_t bank, uint8_t* codes_k, uint
   int rc = check_bank(st, bank);
   if (rc) return rc;
   if (!st->codes_valid) return fail(PROTOKV_ESTATE, "no synthesis result for the current state");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   std::vector<uint32_t> tmp((size_t)D.K * D.S);
@@ -556,6 +649,7 @@ int protokv_import_codes(protokv_state* st, int32_t bank, const uint8_t* codes_k
   int rc = check_bank(st, bank);
   if (rc) return rc;
   if (!st->codes_valid) return fail(PROTOKV_ESTATE, "run protokv_synthesize first (kind[] comes from it)");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   std::vector<uint32_t> tmp((size_t)D.K * D.S);
@@ -573,6 +667,11 @@ int protokv_import_codes(protokv_state* st, int32_t bank, const uint8_t* codes_k
     PKV_CUDA(cudaMemcpy((kv ? st->V.codesV : st->V.codesK) + (size_t)bank * D.K * D.S, tmp.data(), tmp.size() * 4,
                         cudaMemcpyHostToDevice));
   }
+  // Forced codes last until the next synthesis: the whole bank is stamped with the epoch the next synthesis decodes,
+  // so that it re-derives every tuple from the histograms instead of keeping forced ones on untouched prototypes.
+  st->launches += launch_fill_u32(st->V.dirty + (size_t)bank * D.K, (uint32_t)st->epoch, (size_t)D.K, st->stream);
+  PKV_CUDA(cudaGetLastError());
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
   return PROTOKV_OK;
 }
 
@@ -580,6 +679,7 @@ int protokv_last_frame_trace(protokv_state* st, int32_t* assign, float* best, ui
                              int32_t* n_fill, int32_t* evicted_frame) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
   if (st->frames == 0) return fail(PROTOKV_ESTATE, "no frame appended yet");
+  DeviceGuard dg(st);
   const Dims& D = st->D;
   if (n_fill) *n_fill = st->last_n_fill;
   if (evicted_frame) *evicted_frame = st->last_ev_frame;

@@ -245,6 +245,13 @@ __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H,
   }
 }
 
+bool query_kernels_prepare(const Dims&) {
+  // function attributes are per device, not per state: size for the largest k_max protokv_create admits
+  if (cudaFuncSetAttribute(synthesis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxKmax * 2) == cudaSuccess) return true;
+  cudaGetLastError();
+  return false;
+}
+
 int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s) {
   // grid-stride over each bank's work list; its length is only known on the device
   int per_bank = (2 * D.K + kSynTasks - 1) / kSynTasks;
@@ -416,7 +423,12 @@ __global__ void __launch_bounds__(128) attention_combine_kernel(Dims D, Dev V, A
   const int qi = row / D.group, h = hd * D.group + row % D.group;
   const float* part = V.part + (size_t)gr * A.nsplit * (DH + 2);
   float M = -INFINITY;
-  for (int sp = 0; sp < A.nsplit; ++sp) M = fmaxf(M, part[sp * (DH + 2) + DH]);
+  bool poisoned = false;   // a partial with a NaN maximum or row sum (non-finite logits): the row is NaN
+  for (int sp = 0; sp < A.nsplit; ++sp) {
+    const float m = part[sp * (DH + 2) + DH], ls = part[sp * (DH + 2) + DH + 1];
+    poisoned = poisoned || m != m || ls != ls;
+    M = fmaxf(M, m);
+  }
   float l = 0.f, acc[VEC];
 #pragma unroll
   for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
@@ -429,12 +441,17 @@ __global__ void __launch_bounds__(128) attention_combine_kernel(Dims D, Dev V, A
       for (int v = 0; v < VEC; ++v) acc[v] = fmaf(ps[lane * VEC + v], w, acc[v]);
     }
   }
-  const float inv = l > 0.f ? 1.f / l : 0.f;
+  float inv = l > 0.f ? 1.f / l : 0.f;
+  if (poisoned) {
+    inv = __int_as_float(0x7fc00000);
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) acc[v] = 1.f;
+  }
   const size_t ooff = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + h);
   T* out = (T*)A.out + ooff * DH + lane * VEC;
 #pragma unroll
   for (int v = 0; v < VEC; ++v) out[v] = from_f32<T>(acc[v] * inv);
-  if (A.lse && lane == 0) A.lse[ooff] = l > 0.f ? M + logf(l) : -INFINITY;
+  if (A.lse && lane == 0) A.lse[ooff] = poisoned ? inv : (l > 0.f ? M + logf(l) : -INFINITY);
 }
 
 int attention_simt_splits(const Dims& D, int sm_count) {
@@ -457,6 +474,12 @@ static int attention_simt_launch(const Dims& D, const Hyper& H, const Dev& V, co
   const int rows_total = nb * R;
   attention_combine_kernel<T, DH><<<(rows_total + 3) / 4, 128, 0, s>>>(D, V, A, rows_total);
   return 2;
+}
+
+int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, cudaStream_t s) {
+  const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
+  attention_combine_kernel<__nv_bfloat16, 128><<<(rows_total + 3) / 4, 128, 0, s>>>(D, V, A, rows_total);
+  return 1;
 }
 
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s) {

@@ -515,10 +515,13 @@ __device__ void at_softmax_role(unsigned char* sm, const AtBars& B, uint32_t tme
       load_bm(m_ref);
       uint32_t pk[64];
       float lsum;
-      for (;;) {
+      // At most one retry: after re-referencing to the true row maximum a tile's row sum is <= 128, so a second
+      // failure can only come from non-finite logits (NaN / Inf in Q, K or a centre) -- those rows then produce NaN
+      // like the SIMT path does, instead of spinning a persistent CTA forever.
+      for (int attempt = 0;; ++attempt) {
         if (nvalid < kAtCols) at_row_pass<true>(s_addr, sc2, bm, nvalid, pk, lsum);
         else at_row_pass<false>(s_addr, sc2, bm, nvalid, pk, lsum);
-        if (!__any_sync(0xffffffffu, !(lsum <= kRescaleSum))) break;
+        if (attempt == 1 || !__any_sync(0xffffffffu, !(lsum <= kRescaleSum))) break;
         // some row of this warp ran past its reference maximum (an element above 2^8 makes the sum exceed it): find
         // the row maxima, move the references up and rescale l and O (rare)
         const float mx = nvalid < kAtCols ? at_row_max<true>(s_addr, sc2, bm, nvalid)
@@ -649,6 +652,7 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
   // online merge, four pieces' loads in flight at a time
   float M = -INFINITY, l = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  bool poisoned = false;   // a piece with a NaN row sum (non-finite logits): the row is NaN, like the SIMT path returns it
   for (int sp0 = 0; sp0 < np; sp0 += 4) {
     float2 ml[4];
     float4 v[4];
@@ -661,6 +665,7 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
+      if (sp0 + u < np && ml[u].y != ml[u].y) poisoned = true;
       if (sp0 + u >= np || !(ml[u].y > 0.f)) continue;
       const float Mn = fmaxf(M, ml[u].x);
       const float so = __expf(M - Mn), sn = __expf(ml[u].x - Mn);   // M = -inf: so = 0
@@ -670,13 +675,14 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
       M = Mn;
     }
   }
-  const float inv = l > 0.f ? 1.f / l : 0.f;
+  float inv = l > 0.f ? 1.f / l : 0.f;
+  if (poisoned) { inv = __int_as_float(0x7fc00000); acc = make_float4(1.f, 1.f, 1.f, 1.f); l = inv; }
   const size_t ooff = (((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh;
   uint2 o;
   o.x = pack_bf16(acc.x * inv, acc.y * inv);
   o.y = pack_bf16(acc.z * inv, acc.w * inv);
   *reinterpret_cast<uint2*>(out + ooff * 128 + lane * 4) = o;
-  if (lse && lane == 0) lse[ooff] = l > 0.f ? M + logf(l) : -INFINITY;
+  if (lse && lane == 0) lse[ooff] = poisoned ? inv : (l > 0.f ? M + logf(l) : -INFINITY);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -2,55 +2,9 @@
 // SIMT variant), segmenting and the segmented prototype update with PQ residual histograms.
 // See DESIGN.md "Kernels".  All launchers are asynchronous on the caller's stream.
 #include "common.cuh"
+#include "derived.cuh"
 
 namespace pkv {
-
-// Token-independent part of Eq. 1 for one prototype.  Sigma + eps I = R R^T (Cholesky),
-// d_Mah^2 = |R^-1 delta|^2 = (dx/r11)^2 + ((dy - r21 dx/r11)/r22)^2.  Evaluated in fp64 from the fp32 state.
-__device__ __forceinline__ float inv_norm(float cc);
-__device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, float sxx, float sxy, float syy, int tau,
-                                             const Hyper& H) {
-  ScoreRec r;
-  r.invc = inv_norm(cc);
-  r.mux = mux; r.muy = muy;
-  const double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
-  const double i11 = rsqrt(a);                 // 1 / r11
-  const double r21 = b * i11;
-  const double t = e - r21 * r21;              // r22^2
-  const double i22 = t > 0.0 ? rsqrt(t) : (double)INFINITY;
-  // lambda_sp * d_Mah = sqrt(q) with factors scaled by lambda_sp; for MAH_SQUARED scale by sqrt(lambda_sp).
-  const double lam = (H.flags & PROTOKV_MAH_SQUARED) ? sqrt((double)H.lambda_sp) : (double)H.lambda_sp;
-  r.u = (float)(lam * i11);
-  r.v = (float)(lam * i22);
-  r.w = (float)(lam * r21 * i11 * i22);
-  r.tau = tau;
-  r.tauf = (float)tau;
-  return r;
-}
-
-__device__ __forceinline__ void split_bf16(float x, __nv_bfloat16& hi, __nv_bfloat16& lo) {
-  hi = __float2bfloat16_rn(x);
-  lo = __float2bfloat16_rn(x - __bfloat162float(hi));
-}
-
-__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)rsqrt((double)cc) : 0.f; }
-
-// bf16 shadows of the NORMALISED key centre c / |c| = hi + lo (+ O(2^-17)): the tcgen05 assignment contracts the
-// evicted keys with these, so its accumulator is |K_j| cos(K_j, c_k) and Eq. 1 needs no per-column scale.
-template <int VEC>
-__device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const float (&c)[VEC], float invc) {
-  if (!V.c_hi) return;
-  __nv_bfloat16 hi[VEC], lo[VEC];
-#pragma unroll
-  for (int v = 0; v < VEC; ++v) split_bf16(c[v] * invc, hi[v], lo[v]);
-  if (VEC == 4) {
-    *reinterpret_cast<uint2*>(V.c_hi + off) = *reinterpret_cast<const uint2*>(hi);
-    *reinterpret_cast<uint2*>(V.c_lo + off) = *reinterpret_cast<const uint2*>(lo);
-  } else {
-#pragma unroll
-    for (int v = 0; v < VEC; ++v) { V.c_hi[off + v] = hi[v]; V.c_lo[off + v] = lo[v]; }
-  }
-}
 
 // ---------------------------------------------------------------------------------------------------------
 // U1 ring append (Alg. 1 l.1): frame f goes to slot f % Wf, transposed from the model-native
@@ -140,11 +94,13 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
   const T* Ve = (const T*)V.ringV + (((size_t)b * D.Wf + F.slot) * D.T + j) * D.d;
   const size_t pk = (size_t)b * D.K + k;
   float cc = 0.f;
-  for (int i = lane; i < D.d; i += 32) {
+  const int vec = D.d / 32;   // same per-lane order as update_kernel / refresh_derived_kernel: derived values agree bit for bit
+  for (int v = 0; v < vec; ++v) {
+    const int i = lane * vec + v;
     float kf = to_f32(Ke[i]), vf = to_f32(Ve[i]);
     V.c[pk * D.d + i] = kf;
     V.p[pk * D.d + i] = vf;
-    cc += kf * kf;
+    cc = fmaf(kf, kf, cc);
   }
   cc = warp_sum(cc);
   if (V.c_hi) {
@@ -167,6 +123,7 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     V.nres[pk] = 0u;
     store_rec(V.rec, pk, make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H));
     V.logn[pk] = 0.f;
+    V.mstamp[pk] = F.t;
     mark_dirty(D, V, b, k, F.epoch);
     V.assign[(size_t)b * D.T + j] = k;
     V.best[(size_t)b * D.T + j] = 0.f;
@@ -284,11 +241,6 @@ template <typename T, int DH>
 static void score_simt_launch(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, dim3 grid,
                               cudaStream_t s) {
   const size_t sm = score_simt_smem(DH);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(score_simt_kernel<T, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    attr_done = true;
-  }
   score_simt_kernel<T, DH><<<grid, kScoreThreads, sm, s>>>(D, H, V, F);
 }
 
@@ -355,6 +307,10 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       } else {
         a = V.assign[(size_t)b * D.T + j];
       }
+      if ((uint32_t)a >= (uint32_t)F.n_act) {   // no finite score (non-finite key or bank): not absorbed, flagged
+        a = kNoProto;
+        if (blockIdx.x == 0) { V.assign[(size_t)b * D.T + j] = -2; atomicOr(V.err, PKV_ERR_UNASSIGNED); }
+      }
       key = ((uint32_t)a << 12) | (uint32_t)j;
     }
     keys[i] = key;
@@ -392,6 +348,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
   for (int i = blockIdx.x * kUpdWarps + warp; i < ntok; i += gridDim.x * kUpdWarps) {
     const uint32_t key = keys[i];
     const int k = (int)(key >> 12);
+    if (k == kNoProto) break;                               // unassigned tokens sort last
     if (i > 0 && (int)(keys[i - 1] >> 12) == k) continue;   // not a segment head
     const size_t pk = (size_t)b * D.K + k;
     float c[VEC], p[VEC];
@@ -467,6 +424,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       if (has_cb) V.nres[pk] += (uint32_t)m;
       store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
       V.logn[pk] = logf((float)n);
+      V.mstamp[pk] = F.t;
       mark_dirty(D, V, b, k, F.epoch);
     }
   }
@@ -575,6 +533,10 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     } else {
       a = V.assign[bt + j];
     }
+    if ((uint32_t)a >= (uint32_t)F.n_act) {   // no finite score (non-finite key or bank): not absorbed, flagged
+      a = kNoProto;
+      if (blockIdx.x == 0) { V.assign[bt + j] = -2; atomicOr(V.err, PKV_ERR_UNASSIGNED); }
+    }
     keys[i] = ((uint32_t)a << 12) | (uint32_t)j;
   }
   if (has_cb) {
@@ -642,6 +604,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   for (int seg = blockIdx.x * kUfWarps + warp; seg < nseg; seg += gridDim.x * kUfWarps) {
     const int r0 = segstart[seg], r1 = segstart[seg + 1];
     const int k = (int)(sorted[r0] >> 12);
+    if (k == kNoProto) continue;                                     // the segment of unassigned tokens
     const size_t pk = (size_t)b * D.K + k;
     float c[4], p[4];
     load_vec<float, 4>(V.c + pk * DH + lane * 4, c);
@@ -716,6 +679,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       if (has_cb) V.nres[pk] = nres_old + (uint32_t)m;
       store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
       V.logn[pk] = logf((float)n);
+      V.mstamp[pk] = F.t;
       mark_dirty(D, V, b, k, F.epoch);
     }
   }
@@ -723,12 +687,45 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
 
 static int next_pow2(int x) { int p = 2; while (p < x) p <<= 1; return p; }
 
+static size_t update_fast_smem(int ntok) {
+  const int Tpad = (ntok + 3) / 4 * 4;
+  return (size_t)(2 * 8 * kCbG + kUfWarps * 64) * 16 + 256 * 4 + (size_t)(3 * Tpad + 1) * 4;
+}
+static size_t update_generic_smem(const Dims& D, int ntok) {
+  return (size_t)next_pow2(ntok) * 4 + 2 * (size_t)D.G * (D.C * D.sub + kCbPad) * 4;
+}
+
+template <typename K> static bool set_smem(K kernel, size_t bytes) {
+  if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess) return true;
+  cudaGetLastError();
+  return false;
+}
+
+bool update_kernels_prepare(const Dims& D0) {
+  // function attributes are per device, not per state: size for the largest frame / PQ shape protokv_create admits
+  Dims D = D0;
+  D.T = kMaxT; D.G = kMaxG; D.C = kMaxC; D.sub = 128 / kMaxG;   // G (C sub + pad) is largest at G = 8
+  bool ok = true;
+  ok &= set_smem(score_simt_kernel<__nv_bfloat16, 128>, score_simt_smem(128));
+  ok &= set_smem(score_simt_kernel<__nv_bfloat16, 64>, score_simt_smem(64));
+  ok &= set_smem(score_simt_kernel<float, 128>, score_simt_smem(128));
+  ok &= set_smem(score_simt_kernel<float, 64>, score_simt_smem(64));
+  const size_t uf = update_fast_smem(D.T), ug = update_generic_smem(D, D.T);
+  ok &= set_smem(update_fast_kernel<__nv_bfloat16>, uf);
+  ok &= set_smem(update_fast_kernel<float>, uf);
+  ok &= set_smem(update_kernel<__nv_bfloat16, 128>, ug);
+  ok &= set_smem(update_kernel<__nv_bfloat16, 64>, ug);
+  ok &= set_smem(update_kernel<float, 128>, ug);
+  ok &= set_smem(update_kernel<float, 64>, ug);
+  return ok;
+}
+
 int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s) {
   const int ntok = D.T - F.n_fill;
   if (ntok <= 0) return 0;
   if (D.d == 128 && D.G == 8 && D.C == 16) {
     const int Tpad = (ntok + 3) / 4 * 4;
-    const size_t sm = (size_t)(2 * 8 * kCbG + kUfWarps * 64) * 16 + 256 * 4 + (size_t)(3 * Tpad + 1) * 4;
+    const size_t sm = update_fast_smem(ntok);
     int nsplit = 4 * sm_count / D.B;
     const int max_split = (ntok + 2 * kUfWarps - 1) / (2 * kUfWarps);
     if (nsplit > max_split) nsplit = max_split;
@@ -744,7 +741,7 @@ int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& 
   const int max_chunk = (ntok + kUpdWarps - 1) / kUpdWarps;
   if (nchunk > max_chunk) nchunk = max_chunk;
   if (nchunk > 32) nchunk = 32;
-  const size_t sm = (size_t)P * 4 + 2 * (size_t)D.G * (D.C * D.sub + kCbPad) * 4;
+  const size_t sm = update_generic_smem(D, ntok);
   dim3 grid(nchunk, D.B);
   if (D.bf16) {
     if (D.d == 128) update_kernel<__nv_bfloat16, 128><<<grid, kUpdThreads, sm, s>>>(D, H, V, F, P);
@@ -787,6 +784,16 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b, int epoch)
     V.logn[pk] = n >= 1 ? logf((float)n) : 0.f;
     mark_dirty(D, V, b, k, epoch);
   }
+}
+
+__global__ void fill_u32_kernel(uint32_t* dst, uint32_t value, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) dst[i] = value;
+}
+int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s) {
+  if (n == 0) return 0;
+  const unsigned grid = (unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
+  fill_u32_kernel<<<grid, 256, 0, s>>>(dst, value, n);
+  return 1;
 }
 
 int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s) {

@@ -9,6 +9,11 @@ if ROOT not in sys.path:
 
 
 def pytest_configure(config):
+    try:   # the generator's integer hashing on CPU is memory-bound elementwise work: intra-op threads only contend with
+        import torch   # the oracle's worker threads (and with each other inside a CPU-limited container)
+        torch.set_num_threads(1)
+    except Exception:
+        pass
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 

@@ -54,67 +54,101 @@ def compare_state(gs, os_, where=""):
         assert (err <= tol).all(), f"{where}: {f} max err {err.max():.3e}"
 
 
-def step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats, with_codebooks=True):
+def _follow_bank(spec, f, b, o, Kb, Vb, sb, tr, with_codebooks):
+    """Oracle side of one bank-frame: checks the GPU's decisions against the oracle's own and advances the oracle in
+    follow mode.  Returns the counters of this bank-frame.  Runs on a worker thread (ctypes drops the GIL)."""
+    st = new_stats()
+    _check_bank_frame(spec, f, b, o, Kb, Vb, sb, tr, st, with_codebooks)
+    return st
+
+
+def step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats, with_codebooks=True, pool=None):
     """Append frame f on the GPU, check its decisions against the oracle's own, then advance every oracle bank with
-    the GPU's decisions (follow mode)."""
+    the GPU's decisions (follow mode).  K, V, s may live on the device (only the followed banks are pulled to the
+    host); with a thread pool the oracle banks advance in parallel."""
     dev = gpu.device
     gpu.append_frame(K.to(dev), V.to(dev), s.to(dev))
     tr = gpu.last_frame_trace()
+    if K.is_cuda:
+        s_host = s.cpu()
+        frames = {}
+        for b in oracles:
+            st_, la, hd = bank_coords(spec, b)
+            frames[b] = (K[st_, la, :, hd, :].float().cpu().numpy(), V[st_, la, :, hd, :].float().cpu().numpy(),
+                         s_host[st_].numpy())
+    else:
+        frames = {b: bank_frame(spec, K, V, s, b) for b in oracles}
+    if pool is not None:
+        futs = [pool.submit(_follow_bank, spec, f, b, o, *frames[b], tr, with_codebooks) for b, o in oracles.items()]
+        for fu in futs:
+            for k, v in fu.result().items():
+                stats[k] = max(stats[k], v) if k == "max_score_err" else stats[k] + v
+        return
     for b, o in oracles.items():
-        Kb, Vb, sb = bank_frame(spec, K, V, s, b)
-        ga = tr["assign"][b]
-        evicted = tr["evicted_frame"] >= 0
-        forced = ga.copy()
-        fk = tr["codes_k"][b] if with_codebooks else None
-        fv = tr["codes_v"][b] if with_codebooks else None
-        if evicted and with_codebooks:
-            # fills carry 255 in the GPU trace; the oracle ignores forced codes for fills
-            fk = np.where(fk == 255, 0, fk).astype(np.uint8)
-            fv = np.where(fv == 255, 0, fv).astype(np.uint8)
-        ot = o.append_frame(Kb, Vb, sb, mode=0, forced_assign=forced if evicted else None,
-                            forced_codes_k=fk if evicted else None, forced_codes_v=fv if evicted else None)
-        assert bool(ot["evicted"]) == evicted, f"frame {f} bank {b}: eviction mismatch"
-        if not evicted:
-            assert (ga == -1).all()
-            continue
-        assert ot["n_fill"] == tr["n_fill"]
-        nf = ot["n_fill"]
-        assert np.array_equal(ga[:nf], ot["assign"][:nf]), f"frame {f} bank {b}: slot fill differs"
-        diff = ga[nf:] != ot["assign"][nf:]
-        excess = ot["forced_excess"][nf:]
-        bad = diff & ~(excess <= ASSIGN_GAP)
-        assert not bad.any(), (f"frame {f} bank {b}: {bad.sum()} assignments differ beyond the 1e-5 gap rule; "
-                               f"worst excess {excess[bad].max():.3e}")
-        stats["scored"] += int(diff.size)
-        stats["assign_flips"] += int(diff.sum())
-        # the GPU's score of its choice vs the oracle's score of that choice
-        sc_err = np.abs(tr["best"][b][nf:] - (ot["best"][nf:] + excess))
-        stats["max_score_err"] = max(stats["max_score_err"], float(sc_err.max()) if sc_err.size else 0.0)
-        assert (sc_err <= ASSIGN_GAP).all(), f"frame {f} bank {b}: score error {sc_err.max():.3e}"
-        if with_codebooks:
-            for name, gc, oc, gap in (("K", tr["codes_k"][b], ot["codes_k"], ot["code_gap_k"]),
-                                      ("V", tr["codes_v"][b], ot["codes_v"], ot["code_gap_v"])):
-                assert (gc[:nf] == 255).all()
-                d = gc[nf:] != oc[nf:]
-                badc = d & ~(gap[nf:] <= CODE_GAP)
-                assert not badc.any(), f"frame {f} bank {b}: {badc.sum()} PQ codes ({name}) differ beyond the gap rule"
-                stats["codes"] += int(d.size)
-                stats["code_flips"] += int(d.sum())
+        _check_bank_frame(spec, f, b, o, *frames[b], tr, stats, with_codebooks)
+
+
+def _check_bank_frame(spec, f, b, o, Kb, Vb, sb, tr, stats, with_codebooks):
+    ga = tr["assign"][b]
+    evicted = tr["evicted_frame"] >= 0
+    forced = ga.copy()
+    fk = tr["codes_k"][b] if with_codebooks else None
+    fv = tr["codes_v"][b] if with_codebooks else None
+    if evicted and with_codebooks:
+        # fills carry 255 in the GPU trace; the oracle ignores forced codes for fills
+        fk = np.where(fk == 255, 0, fk).astype(np.uint8)
+        fv = np.where(fv == 255, 0, fv).astype(np.uint8)
+    ot = o.append_frame(Kb, Vb, sb, mode=0, forced_assign=forced if evicted else None,
+                        forced_codes_k=fk if evicted else None, forced_codes_v=fv if evicted else None)
+    assert bool(ot["evicted"]) == evicted, f"frame {f} bank {b}: eviction mismatch"
+    if not evicted:
+        assert (ga == -1).all()
+        return
+    assert ot["n_fill"] == tr["n_fill"]
+    nf = ot["n_fill"]
+    assert np.array_equal(ga[:nf], ot["assign"][:nf]), f"frame {f} bank {b}: slot fill differs"
+    diff = ga[nf:] != ot["assign"][nf:]
+    excess = ot["forced_excess"][nf:]
+    bad = diff & ~(excess <= ASSIGN_GAP)
+    assert not bad.any(), (f"frame {f} bank {b}: {bad.sum()} assignments differ beyond the 1e-5 gap rule; "
+                           f"worst excess {excess[bad].max():.3e}")
+    stats["scored"] += int(diff.size)
+    stats["assign_flips"] += int(diff.sum())
+    # the GPU's score of its choice vs the oracle's score of that choice
+    sc_err = np.abs(tr["best"][b][nf:] - (ot["best"][nf:] + excess))
+    stats["max_score_err"] = max(stats["max_score_err"], float(sc_err.max()) if sc_err.size else 0.0)
+    assert (sc_err <= ASSIGN_GAP).all(), f"frame {f} bank {b}: score error {sc_err.max():.3e}"
+    if with_codebooks:
+        for name, gc, oc, gap in (("K", tr["codes_k"][b], ot["codes_k"], ot["code_gap_k"]),
+                                  ("V", tr["codes_v"][b], ot["codes_v"], ot["code_gap_v"])):
+            assert (gc[:nf] == 255).all()
+            d = gc[nf:] != oc[nf:]
+            badc = d & ~(gap[nf:] <= CODE_GAP)
+            assert not badc.any(), f"frame {f} bank {b}: {badc.sum()} PQ codes ({name}) differ beyond the gap rule"
+            stats["codes"] += int(d.size)
+            stats["code_flips"] += int(d.sum())
 
 
 def new_stats():
     return dict(scored=0, assign_flips=0, max_score_err=0.0, codes=0, code_flips=0)
 
 
-def run_stream(spec, gpu, oracles, n_frames, check_state_every=8, with_codebooks=True, stats=None, first_frame=0):
+def run_stream(spec, gpu, oracles, n_frames, check_state_every=8, with_codebooks=True, stats=None, first_frame=0,
+               on_device=False, pool=None, after_frame=None):
+    """Teacher-forced stream of frames [first_frame, first_frame + n_frames).  on_device: frames are generated on the
+    GPU (bit-identical generator) and only the followed banks are pulled to the host -- what makes the full-length
+    streams of BASELINE.json's configs affordable.  after_frame(f) is called after frame f has been checked."""
     stats = stats if stats is not None else new_stats()
-    s = gen.grid_positions(spec)
+    dev = str(gpu.device) if on_device else "cpu"
+    s = gen.grid_positions(spec, device=dev)
     for f in range(first_frame, first_frame + n_frames):
-        K, V = gen.frame_kv(spec, f)
-        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats, with_codebooks)
+        K, V = gen.frame_kv(spec, f, device=dev)
+        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats, with_codebooks, pool=pool)
         if check_state_every and ((f + 1) % check_state_every == 0 or f == first_frame + n_frames - 1):
             for b, o in oracles.items():
                 compare_state(gpu.export_state(b), o.state(), f"frame {f} bank {b}")
+        if after_frame is not None:
+            after_frame(f)
     return stats
 
 

@@ -69,6 +69,14 @@ def _worker(rank, world, port, axis, q):
             K, V = gen.frame_kv(spec, f)                       # the full job's frame ...
             Kl, Vl = sharding.slice_kv(K, sh), sharding.slice_kv(V, sh)   # ... and what this rank's state would be fed
             sl = sharding.slice_grid_pos(s_all, sh)
+            if axis == "stream":   # what bench.py --gpus N feeds a rank: the shard generated directly (stream0 = begin)
+                shard = dataclasses.replace(local, stream0=sh["begin"])
+                Kd, Vd = gen.frame_kv(shard, f)
+                assert torch.equal(Kd, Kl) and torch.equal(Vd, Vl)
+                if f == 0:
+                    group = spec.n_q_heads // spec.n_kv_heads
+                    assert torch.equal(gen.queries(shard, 3), sharding.slice_q(gen.queries(spec, 3), sh, group))
+                    assert torch.equal(gen.codebooks(shard)[0], gen.codebooks(spec)[0][sh["begin"]:sh["end"]])
             for i, b in enumerate(banks):                      # rank-local bank i  <->  global bank b
                 st, la, hd = bank_coords(local, i)
                 k_loc, v_loc = Kl[st, la, :, hd].float().numpy(), Vl[st, la, :, hd].float().numpy()

@@ -15,7 +15,8 @@ import gen
 from gpu_helpers import (make_gpu, make_oracles, run_stream, compare_ring, compare_codes, compare_attention,
                          compare_state, new_stats, step_teacher_forced)
 from oracle import FLAG_NEAR_ONLY, FLAG_FAR_ONLY, FLAG_NO_MASS_BIAS, FLAG_MAH_SQUARED
-from paper_2606_26762_b200 import ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT
+from paper_2606_26762_b200 import (ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT,
+                                   DECODE_SPLITKV)
 
 pytestmark = pytest.mark.gpu
 
@@ -300,7 +301,9 @@ def test_import_state_round_trip():
     a.append_frame(K.cuda(), V.cuda(), s)
     b.append_frame(K.cuda(), V.cuda(), s)
     ta, tb = a.last_frame_trace(), b.last_frame_trace()
-    assert np.array_equal(ta["assign"], tb["assign"]) and np.allclose(ta["best"], tb["best"], rtol=0, atol=1e-6)
+    # bit for bit: the slot fill, the update kernels and refresh_derived_kernel all reduce |c|^2 in the same per-lane
+    # order, so the derived 1/|c| (and with it every score) is reproduced exactly after an import
+    assert np.array_equal(ta["assign"], tb["assign"]) and np.array_equal(ta["best"], tb["best"])
     for f in ("c", "p", "n", "hist_k", "mu", "sigma"):
         assert np.array_equal(a.export_state(0)[f], b.export_state(0)[f])
 
@@ -342,3 +345,160 @@ def test_errors_leave_state_unchanged():
         make_gpu(dataclasses.replace(spec, head_dim=96))
     with pytest.raises(ProtoKVError):
         gpu.export_codes(0)                                                        # nothing synthesised yet
+
+
+# ---------------------------------------------------------------------------------------------------------
+# non-finite inputs are contained: a NaN / Inf key row has no finite Eq. 1 score -- the token is dropped
+# and flagged instead of indexing a prototype with garbage; a NaN query row yields NaN for that row only and the
+# persistent attention kernel terminates
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,force_simt", [("c2", False), ("c2", True), ("c1", False)])
+def test_nonfinite_key_row_is_dropped_and_flagged(name, force_simt):
+    spec = gen.spec_for(name, n_frames=spec_frames(name))
+    gpu = make_gpu(spec, flags=FORCE_SIMT if force_simt else 0)
+    s = gen.grid_positions(spec).cuda()
+    bad_frame, bad_tok = spec.n_frames - spec.near_frames - 2, 5
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        if f == bad_frame:
+            K[0, 0, bad_tok, 0, 3] = float("nan")
+            K[0, 0, bad_tok + 1, 0, 7] = float("inf")
+        gpu.append_frame(K.cuda(), V.cuda(), s)
+        tr = gpu.last_frame_trace()
+        if tr["evicted_frame"] == bad_frame:
+            a = tr["assign"][0]
+            assert a[bad_tok] == -2 and a[bad_tok + 1] == -2
+            assert (np.delete(a, [bad_tok, bad_tok + 1]) >= 0).all()
+            assert (tr["assign"][1:] >= 0).all()                 # the other banks are untouched by it
+    assert gpu.error_flags() & 1
+    st = gpu.export_state(0)
+    evicted = (spec.n_frames - spec.near_frames) * spec.T
+    assert int(st["n"].sum()) == evicted - 2                     # exactly the two tokens are missing from the mass
+    assert np.isfinite(st["c"]).all() and np.isfinite(st["p"]).all()
+    assert gpu.error_flags(clear=True) & 1 and gpu.error_flags() == 0
+
+
+def spec_frames(name):
+    return 14 if name == "c1" else 26
+
+
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_nan_query_row_stays_in_its_row(force_simt):
+    spec = gen.spec_for("c2", n_frames=24)
+    gpu = make_gpu(spec, flags=FORCE_SIMT if force_simt else 0)
+    s = gen.grid_positions(spec).cuda()
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        gpu.append_frame(K.cuda(), V.cuda(), s)
+    Q = gen.queries(spec, 0)
+    ref = gpu.query_attention(Q.cuda()).float().cpu()
+    Qn = Q.clone()
+    Qn[0, 0, 3, 9, 17] = float("nan")            # query token 3, query head 9 (KV head 1)
+    Qn[0, 0, 5, 20, 1] = float("inf")
+    out = gpu.query_attention(Qn.cuda()).float().cpu()   # must return (a hang would trip the suite's timeout)
+    assert torch.isnan(out[0, 0, 3, 9]).all() and not torch.isfinite(out[0, 0, 5, 20]).any()
+    mask = torch.ones(out.shape[:4], dtype=torch.bool)
+    mask[0, 0, 3, 9] = False
+    mask[0, 0, 5, 20] = False
+    # (a NaN row makes its warp re-reference its rows' maxima once: other rows may differ in rounding, not in value)
+    assert torch.allclose(out[mask], ref[mask], atol=1e-2, rtol=2e-2)
+
+
+def test_imported_codes_last_until_the_next_synthesis():
+    spec = gen.spec_for("c1", n_frames=20)
+    gpu = make_gpu(spec)
+    s = gen.grid_positions(spec).cuda()
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        gpu.append_frame(K.cuda(), V.cuda(), s)
+    gpu.synthesize()
+    ck, cv, kind = gpu.export_codes(0)
+    forced_k, forced_v = (ck + 1) % spec.C, (cv + 3) % spec.C
+    gpu.import_codes(0, forced_k, forced_v)
+    assert np.array_equal(gpu.export_codes(0)[0], forced_k)      # in force for queries with run_synthesis = 0
+    K, V = gen.frame_kv(spec, spec.n_frames)
+    gpu.append_frame(K.cuda(), V.cuda(), s)                       # touches only a few prototypes
+    gpu.synthesize()
+    ck2, cv2, kind2 = gpu.export_codes(0)
+    fresh = make_gpu(spec)
+    for f in range(spec.n_frames + 1):
+        K, V = gen.frame_kv(spec, f)
+        fresh.append_frame(K.cuda(), V.cuda(), s)
+    fresh.synthesize()
+    ek, ev, ekind = fresh.export_codes(0)
+    assert np.array_equal(ck2, ek) and np.array_equal(cv2, ev) and np.array_equal(kind2, ekind)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# synthesis with deep histograms: counts beyond the 4,096-entry numerator table of Eq. 3 take the kernel's own
+# log() branch; masses in the thousands enter the log n_k bias
+# ---------------------------------------------------------------------------------------------------------
+def test_synthesis_and_bias_with_counts_beyond_the_log_table():
+    spec = gen.spec_for("c1", n_frames=16)
+    gpu = make_gpu(spec)
+    oracles = make_oracles(spec, [0])
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=0)
+    st = oracles[0].state()
+    rng = np.random.default_rng(11)
+    act = st["active"].astype(bool)
+    big = rng.integers(0, 3, size=st["hist_k"].shape) * rng.integers(3000, 200000, size=st["hist_k"].shape)
+    hk = (st["hist_k"].astype(np.int64) + big).astype(np.uint32)
+    hv = np.roll(hk, 1, axis=2)
+    # rows of a prototype must all sum to n_res: top the first bin of every row up to a common total
+    tot = max(int(hk.sum(axis=2).max()), int(hv.sum(axis=2).max())) + 5
+    for H in (hk, hv):
+        H[:, :, 0] += (tot - H.sum(axis=2)).astype(np.uint32)
+    hk[~act] = 0
+    hv[~act] = 0
+    st["hist_k"], st["hist_v"] = hk, hv
+    st["nres"] = np.where(act, tot, 0).astype(np.uint32)
+    st["n"] = np.where(act, tot + 1, 0).astype(np.int32)
+    assert hk.max() > 4095
+    oracles[0].set_state(**st)
+    gpu.import_state(0, **st)
+    compare_codes(gpu, oracles, spec.G)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# decode-style queries (<= 16 rows per bank) through the opt-in split-KV mma.sync kernel (csrc/decode_attention.cu): one- and
+# two-token queries against the oracle at every stage of a stream -- partial window (ragged near tail), bank still
+# filling (ragged prototype tail, zero-residual prototypes), steady state -- and under the ablation flags
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flags,oflags", [(0, 0), (NEAR_ONLY, FLAG_NEAR_ONLY), (FAR_ONLY, FLAG_FAR_ONLY),
+                                          (NO_MASS_BIAS, FLAG_NO_MASS_BIAS)])
+def test_decode_query_kernel(flags, oflags):
+    spec = gen.spec_for("c2", n_frames=40)
+    gpu = make_gpu(spec, flags=flags | DECODE_SPLITKV)
+    assert gpu.stage_impl(2).startswith("mma.sync")
+    oracles = make_oracles(spec, [0, 3], flags=oflags)
+    Q = gen.queries(spec, 5)
+    checkpoints = {2: 1, 9: 2, 17: 1, 19: 2, 23: 1, 39: 2}      # frame -> query tokens (7 or 14 rows per bank)
+    stats = new_stats()
+    s = gen.grid_positions(spec)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats)
+        if f in checkpoints:
+            nq = checkpoints[f]
+            if not (flags & NEAR_ONLY):
+                compare_codes(gpu, oracles, spec.G)
+            Qs = Q[:, :, 3:3 + nq].contiguous()
+            compare_attention(spec, gpu, oracles, Qs, run_synthesis=True)
+            # and against the 128-row tcgen05 kernel on the same state (a 3-token query has 21 rows)
+            Q3 = Q[:, :, 3:6].contiguous()
+            o3 = gpu.query_attention_ex(Q3.cuda(), n_q=3, run_synthesis=False).float().cpu()
+            o1 = gpu.query_attention_ex(Qs.cuda(), n_q=nq, run_synthesis=False).float().cpu()
+            assert torch.allclose(o1, o3[:, :, :nq], atol=1e-2, rtol=2e-2)
+
+
+def test_decode_query_full_size_c3_sampled():
+    spec = gen.spec_for("c3", n_frames=24)
+    for flags in (0, DECODE_SPLITKV):                # the default route (tcgen05 kernel) and the opt-in one
+        gpu = make_gpu(spec, flags=flags)
+        banks = [0, 57, 111]
+        oracles = make_oracles(spec, banks)
+        run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=0, on_device=True)
+        Q = gen.queries(spec, 1)[:, :, :1].contiguous()
+        compare_attention(spec, gpu, oracles, Q, run_synthesis=True)
+        gpu.close()
