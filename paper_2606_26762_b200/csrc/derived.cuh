@@ -6,7 +6,18 @@
 
 namespace pkv {
 
-__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)rsqrt((double)cc) : 0.f; }
+// 1 / sqrt(x) in fp64 from the fp32 hardware estimate and two Newton steps (2^-22 -> 2^-44 -> below fp64 rounding): the
+// library rsqrt(double) costs ~40 instructions and three of them per touched prototype were 8 % of the update kernel
+// (profiles/r02_experiments.md).  Every writer of derived data goes through these helpers, so they agree bit for bit.
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y = (double)rsqrtf((float)x);
+  y = y * fma(-0.5 * x * y, y, 1.5);
+  y = y * fma(-0.5 * x * y, y, 1.5);
+  return y;
+}
+__device__ __forceinline__ float inv_norm(float cc) { return cc > 0.f ? (float)rsqrt_nr((double)cc) : 0.f; }
+// log n_k of Eq. 4 (bias of the pseudo-tokens; consumed in bf16 attention: 1e-6 relative is ample)
+__device__ __forceinline__ float log_mass(int n) { return n >= 1 ? __logf((float)n) : 0.f; }
 
 // Token-independent part of Eq. 1 for one prototype.  Sigma + eps I = R R^T (Cholesky),
 // d_Mah^2 = |R^-1 delta|^2 = (dx/r11)^2 + ((dy - r21 dx/r11)/r22)^2.  Evaluated in fp64 from the fp32 state.
@@ -16,10 +27,10 @@ __device__ __forceinline__ ScoreRec make_rec(float cc, float mux, float muy, flo
   r.invc = inv_norm(cc);
   r.mux = mux; r.muy = muy;
   const double a = (double)sxx + (double)H.sigma_eps, b = (double)sxy, e = (double)syy + (double)H.sigma_eps;
-  const double i11 = rsqrt(a);                 // 1 / r11
+  const double i11 = rsqrt_nr(a);              // 1 / r11
   const double r21 = b * i11;
   const double t = e - r21 * r21;              // r22^2
-  const double i22 = t > 0.0 ? rsqrt(t) : (double)INFINITY;
+  const double i22 = t > 0.0 ? rsqrt_nr(t) : (double)INFINITY;
   // lambda_sp * d_Mah = sqrt(q) with factors scaled by lambda_sp; for MAH_SQUARED scale by sqrt(lambda_sp).
   const double lam = (H.flags & PROTOKV_MAH_SQUARED) ? sqrt((double)H.lambda_sp) : (double)H.lambda_sp;
   r.u = (float)(lam * i11);

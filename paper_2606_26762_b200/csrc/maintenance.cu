@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
         if (nn != n) {
           atomicAdd(V.mcount + 0, (unsigned long long)(n - nn));
           V.n[pk] = nn;
-          V.logn[pk] = nn >= 1 ? logf((float)nn) : 0.f;
+          V.logn[pk] = log_mass(nn);
           n = nn;
         }
       }
@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
     if (lane == 0) {
       store_rec(V.rec, pk, make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
                                     V.sigma[pk * 3 + 2], V.tau[pk], H));
-      V.logn[pk] = logf((float)V.n[pk]);
+      V.logn[pk] = log_mass(V.n[pk]);
       V.mstamp[pk] = A.t + 1;   // its pairs with lower-index rows are only looked at again by the next pass
       mark_dirty(D, V, b, k, A.epoch);
     }

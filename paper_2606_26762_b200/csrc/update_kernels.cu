@@ -423,7 +423,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] += (uint32_t)m;
       store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
-      V.logn[pk] = logf((float)n);
+      V.logn[pk] = log_mass(n);
       V.mstamp[pk] = F.t;
       mark_dirty(D, V, b, k, F.epoch);
     }
@@ -510,14 +510,18 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   uint32_t* sorted = keys + Tpad;                             // [Tpad]
   int* segstart = (int*)(sorted + Tpad);                      // [Tpad + 1]
   __shared__ int wtot[kUfWarps];
-  __shared__ int nseg_s;
+  __shared__ int nseg_s, nmine_s;
 
   const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int ntok = D.T - F.n_fill;
+  const int ntok_all = D.T - F.n_fill;
   const bool has_cb = V.cbk != nullptr;
   const size_t bt = (size_t)b * D.T;
   const size_t rrow = ((size_t)b * D.Wf + F.slot) * D.T;      // ring row of evicted token 0
-  for (int i = tid; i < ntok; i += kUfThreads) {
+  if (tid == 0) nmine_s = 0;
+  __syncthreads();
+  // CTA x of the bank's gridDim.x CTAs owns the prototypes k with k mod gridDim.x == x: it keeps only the tokens
+  // assigned to those, so that the sort below is over ~T / gridDim.x keys instead of T in every CTA
+  for (int i = tid; i < ntok_all; i += kUfThreads) {
     const int j = F.n_fill + i;
     int a;
     if (F.keys) {   // tcgen05 assignment: (orderable(|K_j| * score) << 32 | k), see tc_assign.cu
@@ -534,10 +538,10 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       a = V.assign[bt + j];
     }
     if ((uint32_t)a >= (uint32_t)F.n_act) {   // no finite score (non-finite key or bank): not absorbed, flagged
-      a = kNoProto;
       if (blockIdx.x == 0) { V.assign[bt + j] = -2; atomicOr(V.err, PKV_ERR_UNASSIGNED); }
+    } else if ((uint32_t)a % gridDim.x == blockIdx.x) {
+      keys[atomicAdd(&nmine_s, 1)] = ((uint32_t)a << 12) | (uint32_t)j;   // any order: the keys are distinct
     }
-    keys[i] = ((uint32_t)a << 12) | (uint32_t)j;
   }
   if (has_cb) {
     const float4* sk = (const float4*)(V.cbk + (size_t)b * 2048);
@@ -560,7 +564,8 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     }
     (side ? cnv : cnk)[gz] = n2;
   }
-  // ---- U4: rank counting sort, segment heads, segment table ----
+  // ---- U4: rank counting sort of this CTA's keys, segment heads, segment table ----
+  const int ntok = nmine_s;
   for (int i = tid; i < ntok; i += kUfThreads) {
     const uint32_t my = keys[i];
     int r = 0;
@@ -601,10 +606,9 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   const int g = lane >> 2, li = lane & 3;
   float4* rsc = scratch + warp * 64;
 
-  for (int seg = blockIdx.x * kUfWarps + warp; seg < nseg; seg += gridDim.x * kUfWarps) {
+  for (int seg = warp; seg < nseg; seg += kUfWarps) {
     const int r0 = segstart[seg], r1 = segstart[seg + 1];
     const int k = (int)(sorted[r0] >> 12);
-    if (k == kNoProto) continue;                                     // the segment of unassigned tokens
     const size_t pk = (size_t)b * D.K + k;
     float c[4], p[4];
     load_vec<float, 4>(V.c + pk * DH + lane * 4, c);
@@ -678,7 +682,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] = nres_old + (uint32_t)m;
       store_rec(V.rec, pk, make_rec(cc, mu0, mu1, sxx, sxy, syy, F.t, H));
-      V.logn[pk] = logf((float)n);
+      V.logn[pk] = log_mass(n);
       V.mstamp[pk] = F.t;
       mark_dirty(D, V, b, k, F.epoch);
     }
@@ -781,7 +785,7 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b, int epoch)
     store_rec(V.rec, pk, make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
                          V.sigma[pk * 3 + 2], V.tau[pk], H));
     const int n = V.n[pk];
-    V.logn[pk] = n >= 1 ? logf((float)n) : 0.f;
+    V.logn[pk] = log_mass(n);
     mark_dirty(D, V, b, k, epoch);
   }
 }
