@@ -21,6 +21,7 @@ _LIB = os.path.join(_HERE, "libprotokv_oracle.so")
 
 FLAG_MAH_SQUARED, FLAG_NO_MASS_BIAS, FLAG_NO_RESIDUAL, FLAG_NEAR_ONLY, FLAG_FAR_ONLY = 1, 2, 4, 8, 16
 FLAG_MAINTENANCE = 64
+FLAG_ROPE = 256
 
 
 def build(force: bool = False) -> str:
@@ -39,7 +40,8 @@ class _Config(C.Structure):
                 ("lambda_sp", C.c_float), ("lambda_idle", C.c_float), ("t_idle", C.c_int32),
                 ("alpha", C.c_float), ("beta", C.c_float), ("eta", C.c_float),
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
-                ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float)]
+                ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float),
+                ("rope_theta", C.c_double), ("rope_anchor", C.c_int32), ("pos0", C.c_int64)]
 
 
 class _Trace(C.Structure):
@@ -50,7 +52,7 @@ class _Trace(C.Structure):
 
 class _StateView(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("c", "p", "n", "mu", "sigma", "tau", "pos", "hist_k", "hist_v",
-                                          "nres", "active")]
+                                          "nres", "active", "pos_first", "pos_sum", "pos_cnt")]
 
 
 _lib = None
@@ -80,9 +82,9 @@ def _load():
         lib.pko_tuple_score.restype = C.c_int64
         lib.pko_tuple_score.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         lib.pko_context_len.argtypes = [C.c_void_p]
-        lib.pko_materialize.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        lib.pko_materialize.argtypes = [C.c_void_p] + [C.c_void_p] * 6 + [C.c_int]
         lib.pko_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
-                                      C.c_void_p]
+                                      C.c_void_p, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -97,7 +99,8 @@ def _ptr(a: Optional[np.ndarray]):
 
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
                 eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0,
-                gamma=0.05, eps_k=0.20, eps_v=0.25)   # Table 5
+                gamma=0.05, eps_k=0.20, eps_v=0.25,   # Table 5
+                rope_theta=1.0e6, rope_anchor=0, pos0=0)   # readings 28-30 (the paper fixes no rotary base)
 
 
 class OracleBank:
@@ -177,7 +180,8 @@ class OracleBank:
                     mu=np.zeros((k, 2), np.float32), sigma=np.zeros((k, 3), np.float32), tau=np.zeros(k, np.int32),
                     pos=np.zeros(k, np.int64), hist_k=np.zeros((k, G, Cc), np.uint32),
                     hist_v=np.zeros((k, G, Cc), np.uint32), nres=np.zeros(k, np.uint32),
-                    active=np.zeros(k, np.uint8))
+                    active=np.zeros(k, np.uint8), pos_first=np.zeros(k, np.int64), pos_sum=np.zeros(k, np.int64),
+                    pos_cnt=np.zeros(k, np.int32))
 
     def state(self):
         st = self._state_arrays()
@@ -226,18 +230,21 @@ class OracleBank:
         return int(self._lib.pko_tuple_score(self._h, int(k), int(which), _ptr(z)))
 
     # ---- attention ----------------------------------------------------------------------------------------
-    def materialize(self, forced_codes_k=None, forced_codes_v=None):
+    def materialize(self, forced_codes_k=None, forced_codes_v=None, positions=False, rotate=True):
+        """[near || pseudo] keys, values, bias (fp64).  positions=True also returns the stream position of every
+        element; rotate=False returns the keys before the rotary embedding (FLAG_ROPE only)."""
         fk = None if forced_codes_k is None else np.ascontiguousarray(forced_codes_k, dtype=np.uint8)
         fv = None if forced_codes_v is None else np.ascontiguousarray(forced_codes_v, dtype=np.uint8)
         L = self._lib.pko_context_len(self._h)
         Kt = np.empty((L, self.d), np.float64)
         Vt = np.empty((L, self.d), np.float64)
         b = np.empty(L, np.float64)
-        self._lib.pko_materialize(self._h, _ptr(fk), _ptr(fv), _ptr(Kt), _ptr(Vt), _ptr(b))
-        return Kt, Vt, b
+        ps = np.empty(L, np.float64)
+        self._lib.pko_materialize(self._h, _ptr(fk), _ptr(fv), _ptr(Kt), _ptr(Vt), _ptr(b), _ptr(ps), int(rotate))
+        return (Kt, Vt, b, ps) if positions else (Kt, Vt, b)
 
-    def attention(self, Q, forced_codes_k=None, forced_codes_v=None, return_lse=False):
-        """Q [rows][d] -> O [rows][d] fp32 (Alg. 4)."""
+    def attention(self, Q, forced_codes_k=None, forced_codes_v=None, return_lse=False, qpos=None):
+        """Q [rows][d] -> O [rows][d] fp32 (Alg. 4).  qpos [rows] int64: stream positions of the query rows (FLAG_ROPE)."""
         Q = _f32(Q)
         rows = Q.shape[0]
         assert Q.shape == (rows, self.d)
@@ -245,6 +252,8 @@ class OracleBank:
         fv = None if forced_codes_v is None else np.ascontiguousarray(forced_codes_v, dtype=np.uint8)
         out = np.empty((rows, self.d), np.float32)
         lse = np.empty(rows, np.float64)
-        rc = self._lib.pko_attention(self._h, _ptr(Q), rows, _ptr(fk), _ptr(fv), _ptr(out), _ptr(lse))
+        qp = None if qpos is None else np.ascontiguousarray(qpos, dtype=np.int64)
+        assert qp is None or qp.shape == (rows,)
+        rc = self._lib.pko_attention(self._h, _ptr(Q), rows, _ptr(fk), _ptr(fv), _ptr(out), _ptr(lse), _ptr(qp))
         assert rc == 0
         return (out, lse) if return_lse else out

@@ -22,6 +22,9 @@
 // with delta against the NEW mean, Alg. 1 l.11-12; residual taken AFTER the token's own EMA step, l.8-9 before l.13).
 // Alg. 2 (tests/test_oracle_maintenance.py): generalised mass invariant, conservation of the mass-weighted sums under
 // merging, closed form of the idle decay, gamma = eps = 0 == the plain path bit for bit, T = 1 sync == sequential.
+// Rotary anchoring (FLAG_ROPE, tests/test_oracle_rope.py): rotated keys and attention against the rotate-half routine of
+// the `transformers` package + torch SDPA, relative-position property (a common shift of all positions changes nothing),
+// norm preservation, anchor fields (first / average / most recent) recomputed from the assignment log.
 // What stays unpinned: the absolute values produced on the five configs ("parity unpinned" beyond those pins, see
 // DESIGN.md).
 #include <algorithm>
@@ -41,6 +44,7 @@ enum : uint32_t {
   FLAG_NO_RESIDUAL = 4u,   // no histograms    (Table 2 "w/o residual stats", L179)
   FLAG_NEAR_ONLY = 8u,     // attention over the near window only (L176)
   FLAG_FAR_ONLY = 16u,     // attention over pseudo-tokens only   (L177)
+  FLAG_ROPE = 256u,        // rotary position anchoring of L126 / D.1 (readings 28-31): K and Q are given un-rotated
   FLAG_MAINTENANCE = 64u,  // run Alg. 2 at Alg. 1 l.15; off on the graded path (reading 19)
 };
 
@@ -52,6 +56,9 @@ struct Config {
   double pq_eps;
   uint32_t flags;
   float gamma, eps_k, eps_v;   // Alg. 2: idle decay rate, merge thresholds (Table 5: 0.05, 0.20, 0.25)
+  double rope_theta;           // rotary base (reading 28); angle of pair i at position p = p * theta^(-2 i / d)
+  int32_t rope_anchor;         // D.1 (L578-596): 0 most recent absorbed position (default), 1 first, 2 average
+  int64_t pos0;                // stream position of token 0 of frame 0 (positions are pos0 + f T + j)
 };
 
 struct Maint {          // what Alg. 2 did since the counters were last read (pko_maintenance_counters)
@@ -81,6 +88,9 @@ struct StateView {      // host pointers, any may be NULL
   uint32_t* hist_k; uint32_t* hist_v;  // [k_max][G][C]
   uint32_t* nres;               // [k_max]
   uint8_t* active;              // [k_max]
+  int64_t* pos_first;           // [k_max] stream position of the initialising token (D.1 "first")
+  int64_t* pos_sum;             // [k_max] sum of the positions of all absorbed tokens (D.1 "average" = pos_sum / pos_cnt)
+  int32_t* pos_cnt;             // [k_max]
 };
 
 struct Frame {
@@ -99,7 +109,8 @@ struct Bank {
   int32_t frames_seen = 0;
   std::vector<float> c, p, mu, sigma;
   std::vector<int32_t> n, tau;
-  std::vector<int64_t> pos;
+  std::vector<int64_t> pos, pos_first, pos_sum;
+  std::vector<int32_t> pos_cnt;
   std::vector<uint32_t> hk, hv, nres;
   std::vector<uint8_t> active;
   std::vector<uint8_t> used;   // slot has been initialised at least once (Alg. 2 recycles only such slots, reading 24)
@@ -117,6 +128,7 @@ struct Bank {
     c.assign(K * d, 0.f); p.assign(K * d, 0.f);
     mu.assign(K * 2, 0.f); sigma.assign(K * 3, 0.f);
     n.assign(K, 0); tau.assign(K, 0); pos.assign(K, 0);
+    pos_first.assign(K, 0); pos_sum.assign(K, 0); pos_cnt.assign(K, 0);
     hk.assign(K * cfg.G * cfg.C, 0u); hv.assign(K * cfg.G * cfg.C, 0u);
     nres.assign(K, 0u); active.assign(K, 0); used.assign(K, 0);
   }
@@ -133,6 +145,7 @@ struct Bank {
     n[k] = 1; mu[k * 2] = se[0]; mu[k * 2 + 1] = se[1];
     sigma[k * 3] = 1.f; sigma[k * 3 + 1] = 0.f; sigma[k * 3 + 2] = 1.f;
     tau[k] = t; pos[k] = ps;
+    pos_first[k] = ps; pos_sum[k] = ps; pos_cnt[k] = 1;
     std::fill(hk.begin() + (size_t)k * cfg.G * cfg.C, hk.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
     std::fill(hv.begin() + (size_t)k * cfg.G * cfg.C, hv.begin() + (size_t)(k + 1) * cfg.G * cfg.C, 0u);
     nres[k] = 0; active[k] = 1; used[k] = 1;
@@ -182,6 +195,8 @@ struct Bank {
           hv[(size_t)i * GC + e] += hv[(size_t)j * GC + e];
         }
         nres[i] += nres[j];
+        pos_first[i] = std::min(pos_first[i], pos_first[j]);   // anchors of the union of the absorbed tokens (reading 30)
+        pos_sum[i] += pos_sum[j]; pos_cnt[i] += pos_cnt[j];
         active[j] = 0; n[j] = 0;                           // "mark Pi_j as inactive"
         maint.merges += 1;
       }
@@ -196,7 +211,7 @@ struct Bank {
       if (back >= (int)ring.size()) back = (int)ring.size() - 1;
       const Frame& f = ring[ring.size() - 1 - back];
       const int j = cfg.T - 1 - (r % cfg.T);
-      init_slot(k, &f.K[(size_t)j * d], &f.V[(size_t)j * d], &f.s[j * 2], t, (int64_t)f.index * cfg.T + j);
+      init_slot(k, &f.K[(size_t)j * d], &f.V[(size_t)j * d], &f.s[j * 2], t, cfg.pos0 + (int64_t)f.index * cfg.T + j);
       maint.recycled += 1;
       ++r;
     }
@@ -265,6 +280,7 @@ struct Bank {
       pk[i] = (float)((1.0 - be) * (double)pk[i] + be * (double)Ve[i]);   // l.9
     }
     n[k] += 1; tau[k] = t; pos[k] = ps;                                   // l.10
+    pos_sum[k] += ps; pos_cnt[k] += 1;                                    // D.1 anchors (pos_first stays)
     mu[k * 2] = (float)((1.0 - et) * (double)mu[k * 2] + et * (double)se[0]);          // l.11
     mu[k * 2 + 1] = (float)((1.0 - et) * (double)mu[k * 2 + 1] + et * (double)se[1]);
     double dx = (double)se[0] - (double)mu[k * 2], dy = (double)se[1] - (double)mu[k * 2 + 1];  // new mu
@@ -345,7 +361,7 @@ struct Bank {
     for (; j < T; ++j) {                        // (A)
       int k = free_slot();
       if (k < 0) break;
-      init_slot(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, (int64_t)E.index * T + j);
+      init_slot(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, cfg.pos0 + (int64_t)E.index * T + j);
       if (tr && tr->assign) tr->assign[j] = k;
     }
     const int nf = j;
@@ -364,7 +380,7 @@ struct Bank {
     }
     for (j = nf; j < T; ++j) {                  // (C)
       int k = forced ? forced[j] : own[j];
-      update_proto(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, (int64_t)E.index * T + j,
+      update_proto(k, &E.K[(size_t)j * d], &E.V[(size_t)j * d], &E.s[j * 2], t, cfg.pos0 + (int64_t)E.index * T + j,
                    fck ? fck + j * G : nullptr, fcv ? fcv + j * G : nullptr,
                    tr && tr->codes_k ? tr->codes_k + j * G : nullptr, tr && tr->codes_v ? tr->codes_v + j * G : nullptr,
                    tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
@@ -390,7 +406,7 @@ struct Bank {
       const float* Ke = &E.K[(size_t)j * d];
       const float* Ve = &E.V[(size_t)j * d];
       const float* se = &E.s[j * 2];
-      int64_t ps = (int64_t)E.index * T + j;
+      int64_t ps = cfg.pos0 + (int64_t)E.index * T + j;
       int k = free_slot();
       if (k >= 0) {                                                   // l.3-4
         init_slot(k, Ke, Ve, se, t, ps);
@@ -473,15 +489,40 @@ struct Bank {
   }
 
   // Alg. 4 l.1-13: [near || pseudo] keys/values and bias b
+  // Rotary embedding of one vector at (possibly fractional) position p, rotate-half convention (reading 28):
+  // pair (i, i + d/2), angle p * theta^(-2 i / d); everything in fp64.
+  void rope(double* x, double p) const {
+    const int h = cfg.d / 2;
+    for (int i = 0; i < h; ++i) {
+      const double ang = p * std::pow(cfg.rope_theta, -2.0 * (double)i / (double)cfg.d);
+      const double cs = std::cos(ang), sn = std::sin(ang);
+      const double a = x[i], b2 = x[i + h];
+      x[i] = a * cs - b2 * sn;
+      x[i + h] = b2 * cs + a * sn;
+    }
+  }
+  // Rotary anchor of prototype k (D.1 L578-596): most recent / first / average absorbed position
+  double anchor(int k) const {
+    if (cfg.rope_anchor == 1) return (double)pos_first[k];
+    if (cfg.rope_anchor == 2) return (double)pos_sum[k] / (double)pos_cnt[k];
+    return (double)pos[k];
+  }
+
+  // positions (optional out): stream position of every context element (near: original, pseudo: the anchor)
   void materialize(const uint8_t* fck, const uint8_t* fcv, std::vector<double>& Kt, std::vector<double>& Vt,
-                   std::vector<double>& b) const {
+                   std::vector<double>& b, std::vector<double>* positions = nullptr, bool rotate = true) const {
     const int d = cfg.d, S = cfg.S, G = cfg.G;
+    const bool do_rope = (cfg.flags & FLAG_ROPE) && rotate;
     Kt.clear(); Vt.clear(); b.clear();
+    if (positions) positions->clear();
     if (!(cfg.flags & FLAG_FAR_ONLY))
       for (const Frame& f : ring)
         for (int j = 0; j < cfg.T; ++j) {
           for (int i = 0; i < d; ++i) { Kt.push_back(f.K[(size_t)j * d + i]); Vt.push_back(f.V[(size_t)j * d + i]); }
           b.push_back(0.0);                                                   // near tokens carry zero bias (L407)
+          const double ps = (double)(cfg.pos0 + (int64_t)f.index * cfg.T + j);   // near tokens keep their positions (L126)
+          if (positions) positions->push_back(ps);
+          if (do_rope) rope(&Kt[Kt.size() - d], ps);
         }
     if (cfg.flags & FLAG_NEAR_ONLY) return;
     std::vector<Tuple> zk, zv;
@@ -514,24 +555,29 @@ struct Bank {
           Vt.push_back((double)p[(size_t)k * d + i] + rv);
         }
         b.push_back(bias);
+        if (positions) positions->push_back(anchor(k));                       // all S pseudo-tokens share tau_k (L126)
+        if (do_rope) rope(&Kt[Kt.size() - d], anchor(k));
       }
     }
   }
 
   // Alg. 4 l.14-15: A = Q K~^T / sqrt(d) + b ; O = softmax(A) V~   (no mask, reading 17)
-  void attention(const float* Q, int rows, const uint8_t* fck, const uint8_t* fcv, float* out, double* lse) const {
+  // qpos: stream position of every query row (used with FLAG_ROPE only; NULL = every row at the next stream position)
+  void attention(const float* Q, int rows, const uint8_t* fck, const uint8_t* fcv, float* out, double* lse,
+                 const int64_t* qpos = nullptr) const {
     const int d = cfg.d;
     std::vector<double> Kt, Vt, b;
     materialize(fck, fcv, Kt, Vt, b);
     const size_t L = b.size();
     const double scale = 1.0 / std::sqrt((double)d);
-    std::vector<double> logit(L), acc(d);
+    std::vector<double> logit(L), acc(d), q(d);
     for (int r = 0; r < rows; ++r) {
-      const float* q = Q + (size_t)r * d;
+      for (int i = 0; i < d; ++i) q[i] = (double)Q[(size_t)r * d + i];
+      if (cfg.flags & FLAG_ROPE) rope(q.data(), (double)(qpos ? qpos[r] : cfg.pos0 + (int64_t)frames_seen * cfg.T));
       double m = -std::numeric_limits<double>::infinity();
       for (size_t j = 0; j < L; ++j) {
         double dot = 0;
-        for (int i = 0; i < d; ++i) dot += (double)q[i] * Kt[j * d + i];
+        for (int i = 0; i < d; ++i) dot += q[i] * Kt[j * d + i];
         logit[j] = dot * scale + b[j];
         m = std::max(m, logit[j]);
       }
@@ -605,13 +651,13 @@ void pko_get_state(void* h, StateView* v) {
   Bank* b = static_cast<Bank*>(h);
   PKO_COPY(c, c); PKO_COPY(p, p); PKO_COPY(n, n); PKO_COPY(mu, mu); PKO_COPY(sigma, sigma);
   PKO_COPY(tau, tau); PKO_COPY(pos, pos); PKO_COPY(hist_k, hk); PKO_COPY(hist_v, hv); PKO_COPY(nres, nres);
-  PKO_COPY(active, active);
+  PKO_COPY(active, active); PKO_COPY(pos_first, pos_first); PKO_COPY(pos_sum, pos_sum); PKO_COPY(pos_cnt, pos_cnt);
 }
 void pko_set_state(void* h, const StateView* v) {
   Bank* b = static_cast<Bank*>(h);
   PKO_LOAD(c, c); PKO_LOAD(p, p); PKO_LOAD(n, n); PKO_LOAD(mu, mu); PKO_LOAD(sigma, sigma);
   PKO_LOAD(tau, tau); PKO_LOAD(pos, pos); PKO_LOAD(hist_k, hk); PKO_LOAD(hist_v, hv); PKO_LOAD(nres, nres);
-  PKO_LOAD(active, active);
+  PKO_LOAD(active, active); PKO_LOAD(pos_first, pos_first); PKO_LOAD(pos_sum, pos_sum); PKO_LOAD(pos_cnt, pos_cnt);
   if (v->active)
     for (size_t k = 0; k < b->used.size(); ++k) b->used[k] = b->used[k] || b->active[k];
 }
@@ -676,11 +722,13 @@ int pko_context_len(void* h) {
   return (int)bb.size();
 }
 // [near || pseudo] as doubles: Kt, Vt [L][d], bias [L]; returns L (call pko_context_len first)
+// positions (optional): stream position of every context element; rotate = 0 returns the keys un-rotated under FLAG_ROPE
 int pko_materialize(void* h, const uint8_t* forced_codes_k, const uint8_t* forced_codes_v, double* Kt, double* Vt,
-                    double* bias) {
+                    double* bias, double* positions, int rotate) {
   Bank* b = static_cast<Bank*>(h);
-  std::vector<double> k, v, bb;
-  b->materialize(forced_codes_k, forced_codes_v, k, v, bb);
+  std::vector<double> k, v, bb, ps;
+  b->materialize(forced_codes_k, forced_codes_v, k, v, bb, &ps, rotate != 0);
+  if (positions) std::memcpy(positions, ps.data(), ps.size() * sizeof(double));
   if (Kt) std::memcpy(Kt, k.data(), k.size() * sizeof(double));
   if (Vt) std::memcpy(Vt, v.data(), v.size() * sizeof(double));
   if (bias) std::memcpy(bias, bb.data(), bb.size() * sizeof(double));
@@ -689,10 +737,10 @@ int pko_materialize(void* h, const uint8_t* forced_codes_k, const uint8_t* force
 
 // Q [rows][d] fp32 (bf16 inputs widened exactly by the caller); out [rows][d] fp32; lse [rows] or NULL
 int pko_attention(void* h, const float* Q, int rows, const uint8_t* forced_codes_k, const uint8_t* forced_codes_v,
-                  float* out, double* lse) {
+                  float* out, double* lse, const int64_t* qpos) {
   Bank* b = static_cast<Bank*>(h);
   if (!b || !Q || !out || rows < 0) return 1;
-  b->attention(Q, rows, forced_codes_k, forced_codes_v, out, lse);
+  b->attention(Q, rows, forced_codes_k, forced_codes_v, out, lse, qpos);
   return 0;
 }
 
