@@ -64,6 +64,10 @@ enum {
   PROTOKV_DECODE_SPLITKV = 128u, /* serve queries of <= 16 rows per bank with the split-KV mma.sync kernel
                                 (csrc/decode_attention.cu) instead of the 128-row tcgen05 kernel.  Measured on C3 (one
                                 query token, 7 rows per bank): 167-183 us against 161 us -- not faster, hence opt-in */
+  PROTOKV_ROPE = 256u,       /* rotary position anchoring (D.1 L578-596; readings 28-31): K and Q
+                                are given UN-ROTATED; the attention rotates near tokens at their stream positions, the S
+                                pseudo-tokens of prototype k at its anchor and the query tokens at q_pos0 + i.  Served by
+                                the fp32 SIMT attention kernel (the tcgen05 kernel has no rotation stage) */
   PROTOKV_MAINTENANCE = 64u  /* run Alg. 2 at the end of every append_frame that evicted a frame
                                 (Alg. 1 l.15); off by default: north_star's path and its invariant "total mass = tokens
                                 absorbed" exclude it (reading 19) */
@@ -87,6 +91,10 @@ typedef struct {
   uint32_t flags;
   float gamma;            /* Alg. 2 idle decay rate (Table 5: 0.05); used with PROTOKV_MAINTENANCE */
   float eps_k, eps_v;     /* Alg. 2 merge thresholds on |c_i - c_j|, |p_i - p_j| (Table 5: 0.20, 0.25) */
+  double rope_theta;      /* rotary base (rotate-half convention, angle of pair (i, i + d/2) at position p = p theta^(-2i/d));
+                             the paper fixes none: 1e6 (Qwen2-family backbones).  Used with PROTOKV_ROPE */
+  int32_t rope_anchor;    /* D.1: 0 = most recent absorbed position (default), 1 = first, 2 = average */
+  int64_t pos0;           /* stream position of token 0 of frame 0; token j of frame f sits at pos0 + f T + j */
   const float *codebook_k, *codebook_v; /* device; copied at create.  NULL => no residual statistics */
   void *workspace;        /* device memory from the caller, >= protokv_workspace_bytes(cfg), 256-byte aligned */
   size_t workspace_bytes;
@@ -154,6 +162,11 @@ const char *protokv_last_error(void);
 int protokv_query_attention_ex(protokv_state *st, const void *Q, int32_t n_q, int32_t layer_begin,
                                int32_t layer_count, void *out, float *lse, int32_t run_synthesis);
 
+/* The same with the stream position of the first query token given explicitly (PROTOKV_ROPE; query token i is rotated
+ * at q_pos0 + i).  protokv_query_attention(_ex) use q_pos0 = pos0 + frames_seen * T, the next stream position. */
+int protokv_query_attention_at(protokv_state *st, const void *Q, int32_t n_q, int32_t layer_begin, int32_t layer_count,
+                               void *out, float *lse, int32_t run_synthesis, int64_t q_pos0);
+
 /* Alg. 3 for every bank without the attention (timing / parity of the synthesis kernel alone). */
 int protokv_synthesize(protokv_state *st);
 
@@ -167,6 +180,8 @@ typedef struct {
   uint32_t *hist_k, *hist_v;    /* [k_max][G][C]                                                          */
   uint32_t *nres;               /* [k_max]                                                                */
   uint8_t *active;              /* [k_max]                                                                */
+  int64_t *pos_first, *pos_sum; /* [k_max] D.1 anchors: position of the initialising token; sum of all absorbed positions */
+  int32_t *pos_cnt;             /* [k_max] number of absorbed positions (average anchor = pos_sum / pos_cnt)           */
 } protokv_bank_view;
 int protokv_export_state(protokv_state *st, int32_t bank, const protokv_bank_view *host_dst);
 int protokv_import_state(protokv_state *st, int32_t bank, const protokv_bank_view *host_src);

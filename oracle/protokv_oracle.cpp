@@ -562,7 +562,8 @@ struct Bank {
   }
 
   // Alg. 4 l.14-15: A = Q K~^T / sqrt(d) + b ; O = softmax(A) V~   (no mask, reading 17)
-  // qpos: stream position of every query row (used with FLAG_ROPE only; NULL = every row at the next stream position)
+  // qpos: stream position of every query row (used with FLAG_ROPE only; a query token i sits at q_pos0 + i and all heads
+  // of a token share its position -- the caller expands that to rows; NULL = every row at the next stream position)
   void attention(const float* Q, int rows, const uint8_t* fck, const uint8_t* fcv, float* out, double* lse,
                  const int64_t* qpos = nullptr) const {
     const int d = cfg.d;

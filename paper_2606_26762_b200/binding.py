@@ -10,11 +10,12 @@ import numpy as np
 from .build import build
 
 F32, BF16 = 0, 1
-MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV = 1, 2, 4, 8, 16, 32, 64, 128
+MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV, ROPE = 1, 2, 4, 8, 16, 32, 64, 128, 256
 
 # Table 5 of the paper + the constants the paper leaves open (readings 4, 6, 12)
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
-                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0, gamma=0.05, eps_k=0.20, eps_v=0.25)
+                eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0, gamma=0.05, eps_k=0.20, eps_v=0.25,
+                rope_theta=1.0e6, rope_anchor=0, pos0=0)
 
 EXPORTED_SYMBOLS = [
     "protokv_workspace_bytes", "protokv_create", "protokv_destroy", "protokv_append_frame",
@@ -22,7 +23,7 @@ EXPORTED_SYMBOLS = [
     "protokv_query_attention_ex", "protokv_synthesize", "protokv_export_state", "protokv_import_state",
     "protokv_export_ring", "protokv_export_codes", "protokv_import_codes", "protokv_last_frame_trace",
     "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl", "protokv_profile_enable",
-    "protokv_profile_read", "protokv_error_flags", "protokv_maintenance_counters",
+    "protokv_profile_read", "protokv_error_flags", "protokv_maintenance_counters", "protokv_query_attention_at",
 ]
 STAGES = ["fill", "score", "update", "append", "synthesis", "attention"]
 
@@ -44,6 +45,7 @@ class ProtoKVConfig(C.Structure):
                 ("alpha", C.c_float), ("beta", C.c_float), ("eta", C.c_float),
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
                 ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float),
+                ("rope_theta", C.c_double), ("rope_anchor", C.c_int32), ("pos0", C.c_int64),
                 ("codebook_k", C.c_void_p), ("codebook_v", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("cuda_stream", C.c_void_p)]
@@ -51,7 +53,7 @@ class ProtoKVConfig(C.Structure):
 
 class _BankView(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("c", "p", "n", "mu", "sigma", "tau", "pos", "hist_k", "hist_v", "nres",
-                                          "active")]
+                                          "active", "pos_first", "pos_sum", "pos_cnt")]
 
 
 _lib = None
@@ -76,6 +78,7 @@ def load_library():
     lib.protokv_query_attention_host.argtypes = [vp, vp, vp]
     lib.protokv_last_error.restype = C.c_char_p
     lib.protokv_query_attention_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32]
+    lib.protokv_query_attention_at.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, C.c_int64]
     lib.protokv_synthesize.argtypes = [vp]
     lib.protokv_export_state.argtypes = [vp, i32, C.POINTER(_BankView)]
     lib.protokv_import_state.argtypes = [vp, i32, C.POINTER(_BankView)]
@@ -228,7 +231,7 @@ class ProtoKV:
 
     # ---- parity / debug surface -----------------------------------------------------------------------------
     def query_attention_ex(self, Q, n_q=None, layer_begin=0, layer_count=None, out=None, return_lse=False,
-                           run_synthesis=True):
+                           run_synthesis=True, q_pos0=None):
         c = self.cfg
         n_q = c.n_query_tokens if n_q is None else n_q
         layer_count = c.n_layers if layer_count is None else layer_count
@@ -239,9 +242,12 @@ class ProtoKV:
         if return_lse:
             lse = self._torch.empty((c.n_streams, layer_count, n_q, c.n_q_heads), dtype=self._torch.float32,
                                     device=self.device)
-        self._check(self._lib.protokv_query_attention_ex(
-            self._h, self._dev(Q, self.torch_dtype, n), n_q, layer_begin, layer_count,
-            self._dev(out, self.torch_dtype, n), lse.data_ptr() if lse is not None else None, int(run_synthesis)))
+        args = (self._h, self._dev(Q, self.torch_dtype, n), n_q, layer_begin, layer_count,
+                self._dev(out, self.torch_dtype, n), lse.data_ptr() if lse is not None else None, int(run_synthesis))
+        if q_pos0 is None:
+            self._check(self._lib.protokv_query_attention_ex(*args))
+        else:
+            self._check(self._lib.protokv_query_attention_at(*args, int(q_pos0)))
         return (out, lse) if return_lse else out
 
     def synthesize(self):
@@ -254,7 +260,8 @@ class ProtoKV:
                     mu=np.zeros((k, 2), np.float32), sigma=np.zeros((k, 3), np.float32), tau=np.zeros(k, np.int32),
                     pos=np.zeros(k, np.int64), hist_k=np.zeros((k, G, Cc), np.uint32),
                     hist_v=np.zeros((k, G, Cc), np.uint32), nres=np.zeros(k, np.uint32),
-                    active=np.zeros(k, np.uint8))
+                    active=np.zeros(k, np.uint8), pos_first=np.zeros(k, np.int64), pos_sum=np.zeros(k, np.int64),
+                    pos_cnt=np.zeros(k, np.int32))
 
     def export_state(self, bank):
         st = self._state_arrays()

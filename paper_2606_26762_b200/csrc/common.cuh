@@ -38,6 +38,9 @@ struct Hyper {
   float alpha, beta, eta, sigma_eps, cos_eps;
   double pq_eps;
   uint32_t flags;
+  double rope_theta;     // PROTOKV_ROPE
+  int rope_anchor;
+  long long pos0;        // stream position of token 0 of frame 0
 };
 
 // Per-prototype scoring record (Eq. 1 terms that do not depend on the token), 32 bytes.
@@ -86,7 +89,15 @@ struct Dev {
   float* mu;     // [B][K][2]
   float* sigma;  // [B][K][3]
   int* tau;      // [B][K]
-  long long* pos;  // [B][K]
+  long long* pos;  // [B][K]  stream position of the most recently absorbed token (D.1 default anchor)
+  long long* pos_first;  // [B][K] ... of the initialising token
+  long long* pos_sum;    // [B][K] sum over all absorbed tokens
+  int* pos_cnt;          // [B][K]
+  // rotary tables (PROTOKV_ROPE only), rebuilt by every query: cis(angle) as float2 from fp64 sincos
+  float2* ropeJ;         // [T][d/2]        token offset j inside a frame
+  float2* ropeF;         // [Wf][d/2]       first position of the frame held in each ring slot
+  float2* ropeP;         // [B][K][d/2]     anchor of every prototype
+  float2* ropeQ;         // [Nq][d/2]       query tokens
   uint32_t* nres;  // [B][K]
   ScoreRec* rec;   // [B * K / 2] pairs, see rec_slot()
   float* logn;     // [B][K]  log n_k (Eq. 4 bias)
@@ -186,6 +197,8 @@ __device__ __forceinline__ void mark_dirty(const Dims& D, const Dev& V, int b, i
 }
 
 struct AttnArgs {
+  long long q_pos0;    // stream position of query token 0 (PROTOKV_ROPE)
+  long long frames;    // frames appended so far (ring slot s holds frame ... see launch_rope_tables)
   const void* Q; void* out; float* lse;
   int n_q, layer_begin, layer_count;
   int n_near;          // near-window tokens currently held (frames held * T): ring rows [0, n_near) of each bank
@@ -194,6 +207,7 @@ struct AttnArgs {
 };
 int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
+int launch_rope_tables(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
 
 // Alg. 2 maintenance (maintenance.cu)
 bool maintenance_prepare();

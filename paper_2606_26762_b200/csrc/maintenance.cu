@@ -207,6 +207,9 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
       if (tid == 0) {
         V.n[pi] = (int)(ni + nj);
         V.nres[pi] += V.nres[pj];
+        V.pos_first[pi] = V.pos_first[pi] < V.pos_first[pj] ? V.pos_first[pi] : V.pos_first[pj];   // reading 30
+        V.pos_sum[pi] += V.pos_sum[pj];
+        V.pos_cnt[pi] += V.pos_cnt[pj];
         V.n[pj] = 0;
         alive[j >> 5] &= ~(1u << (j & 31));
         atomicAdd(V.mcount + 1, 1ull);
@@ -327,7 +330,8 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
       V.mu[pk * 2] = se[0]; V.mu[pk * 2 + 1] = se[1];
       V.sigma[pk * 3] = 1.f; V.sigma[pk * 3 + 1] = 0.f; V.sigma[pk * 3 + 2] = 1.f;
       V.tau[pk] = A.t;
-      V.pos[pk] = (long long)(A.t - back) * D.T + j;
+      const long long ps = H.pos0 + (long long)(A.t - back) * D.T + j;
+      V.pos[pk] = ps; V.pos_first[pk] = ps; V.pos_sum[pk] = ps; V.pos_cnt[pk] = 1;
       V.nres[pk] = 0u;
       store_rec(V.rec, pk, make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, A.t, H));
       V.logn[pk] = 0.f;

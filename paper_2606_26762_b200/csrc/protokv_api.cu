@@ -142,6 +142,10 @@ static int validate(const protokv_config* c) {
     if (!(c->gamma >= 0.f && c->gamma <= 1.f) || !(c->eps_k >= 0.f) || !(c->eps_v >= 0.f))
       return fail(PROTOKV_EINVAL, "maintenance needs gamma in [0, 1], eps_k >= 0, eps_v >= 0");
   }
+  if (c->flags & PROTOKV_ROPE) {
+    if (!(c->rope_theta > 1.0) || c->rope_anchor < 0 || c->rope_anchor > 2)
+      return fail(PROTOKV_EINVAL, "rope needs rope_theta > 1 and rope_anchor in {0, 1, 2}");
+  }
   if (!(c->lambda_sp >= 0.f) || !(c->lambda_idle >= 0.f))   // Eq. 1's penalties are penalties (the score kernel prunes on it)
     return fail(PROTOKV_EINVAL, "need lambda_sp >= 0 and lambda_idle >= 0");
   if ((c->flags & PROTOKV_NEAR_ONLY) && (c->flags & PROTOKV_FAR_ONLY))
@@ -160,10 +164,11 @@ static void fill_dims(const protokv_config* c, Dims* D, Hyper* H) {
   H->lambda_sp = c->lambda_sp; H->lambda_idle = c->lambda_idle; H->t_idle = c->t_idle;
   H->alpha = c->alpha; H->beta = c->beta; H->eta = c->eta;
   H->sigma_eps = c->sigma_eps; H->cos_eps = c->cos_eps; H->pq_eps = c->pq_eps; H->flags = c->flags;
+  H->rope_theta = c->rope_theta; H->rope_anchor = c->rope_anchor; H->pos0 = (long long)c->pos0;
 }
 
 // Lays the state out in the workspace (base may be NULL to only measure).  Every array is 256-byte aligned.
-static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) {
+static size_t carve(const Dims& D, bool has_cb, bool rope, int nsplit, char* base, Dev* V) {
   size_t off = 0;
   auto take = [&](size_t bytes) -> void* {
     off = align_up(off, 256);
@@ -185,6 +190,12 @@ static size_t carve(const Dims& D, bool has_cb, int nsplit, char* base, Dev* V) 
   }
   v.n = (int*)take(BK * 4); v.mu = (float*)take(BK * 8); v.sigma = (float*)take(BK * 12);
   v.tau = (int*)take(BK * 4); v.pos = (long long*)take(BK * 8); v.nres = (uint32_t*)take(BK * 4);
+  v.pos_first = (long long*)take(BK * 8); v.pos_sum = (long long*)take(BK * 8); v.pos_cnt = (int*)take(BK * 4);
+  if (rope) {
+    const size_t h = (size_t)D.d / 2;
+    v.ropeJ = (float2*)take((size_t)D.T * h * 8); v.ropeF = (float2*)take((size_t)D.Wf * h * 8);
+    v.ropeP = (float2*)take(BK * h * 8); v.ropeQ = (float2*)take((size_t)D.Nq * h * 8);
+  }
   v.rec = (ScoreRec*)take((BK + 1) * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
   v.hist = (uint32_t*)take(BK * 2 * D.G * D.C * 4);
   v.logtab = (const double*)take((size_t)PKV_SYN_LOGTAB * 8);
@@ -227,7 +238,7 @@ size_t protokv_workspace_bytes(const protokv_config* cfg) {
   Dims D; Hyper H;
   fill_dims(cfg, &D, &H);
   const bool has_cb = !(cfg->flags & PROTOKV_NO_RESIDUAL);   // sized as if codebooks were given
-  return carve(D, has_cb, plan_nsplit(D), nullptr, nullptr);
+  return carve(D, has_cb, (cfg->flags & PROTOKV_ROPE) != 0, plan_nsplit(D), nullptr, nullptr);
 }
 
 protokv_state* protokv_create(const protokv_config* cfg) {
@@ -259,7 +270,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->sm_count = sms;
   st->nsplit = plan_nsplit(st->D);
   const bool has_cb = cfg->codebook_k && !(cfg->flags & PROTOKV_NO_RESIDUAL);
-  const size_t need = carve(st->D, has_cb, st->nsplit, (char*)cfg->workspace, &st->V);
+  const size_t need = carve(st->D, has_cb, (cfg->flags & PROTOKV_ROPE) != 0, st->nsplit, (char*)cfg->workspace, &st->V);
   if (need > cfg->workspace_bytes) {
     fail(PROTOKV_ENOMEM, "workspace too small: need %zu bytes, got %zu", need, cfg->workspace_bytes);
     delete st;
@@ -298,8 +309,9 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   const bool want_tc = !(cfg->flags & PROTOKV_FORCE_SIMT);
   if (want_tc && (tc_assign_supported(st->D, st->H) || tc_attention_supported(st->D))) tc_build_maps(st->D, st->V, &st->maps);
   st->use_tc_assign = want_tc && tc_assign_supported(st->D, st->H) && st->maps.ok;
-  st->use_tc_attn = want_tc && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
-  st->use_decode_attn = want_tc && (cfg->flags & PROTOKV_DECODE_SPLITKV) && decode_attention_supported(st->D, 1) &&
+  const bool rope = (cfg->flags & PROTOKV_ROPE) != 0;   // the rotation stage exists in the SIMT attention kernel only
+  st->use_tc_attn = want_tc && !rope && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
+  st->use_decode_attn = want_tc && !rope && (cfg->flags & PROTOKV_DECODE_SPLITKV) && decode_attention_supported(st->D, 1) &&
                         decode_attention_prepare();
   return st;
 }
@@ -407,6 +419,13 @@ int protokv_synthesize(protokv_state* st) {
 
 int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, int32_t layer_begin,
                                int32_t layer_count, void* out, float* lse, int32_t run_synthesis) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL argument");
+  return protokv_query_attention_at(st, Q, n_q, layer_begin, layer_count, out, lse, run_synthesis,
+                                    (int64_t)st->H.pos0 + st->frames * st->D.T);
+}
+
+int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, int32_t layer_begin, int32_t layer_count,
+                               void* out, float* lse, int32_t run_synthesis, int64_t q_pos0) {
   if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
   if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
   DeviceGuard dg(st);
@@ -427,6 +446,7 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
   }
   AttnArgs A{};
   A.Q = Q; A.out = out; A.lse = lse;
+  A.q_pos0 = (long long)q_pos0; A.frames = st->frames;
   A.n_q = n_q; A.layer_begin = layer_begin; A.layer_count = layer_count;
   const int64_t held = st->frames < D.Wf ? st->frames : D.Wf;
   A.n_near = (int)(held * D.T);
@@ -444,6 +464,7 @@ int protokv_query_attention_ex(protokv_state* st, const void* Q, int32_t n_q, in
       if (nl < 0) return fail(PROTOKV_ECUDA, "cuTensorMapEncodeTiled failed for Q");
       st->launches += nl;
     } else {
+      if (st->H.flags & PROTOKV_ROPE) st->launches += launch_rope_tables(D, st->H, st->V, A, st->stream);
       st->launches += launch_attention_simt(D, st->H, st->V, A, st->stream);
     }
   }
@@ -545,6 +566,9 @@ int protokv_export_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   if (v->tau) PKV_CUDA(cudaMemcpy(v->tau, V.tau + o, K * 4, cudaMemcpyDeviceToHost));
   if (v->pos) PKV_CUDA(cudaMemcpy(v->pos, V.pos + o, K * 8, cudaMemcpyDeviceToHost));
   if (v->nres) PKV_CUDA(cudaMemcpy(v->nres, V.nres + o, K * 4, cudaMemcpyDeviceToHost));
+  if (v->pos_first) PKV_CUDA(cudaMemcpy(v->pos_first, V.pos_first + o, K * 8, cudaMemcpyDeviceToHost));
+  if (v->pos_sum) PKV_CUDA(cudaMemcpy(v->pos_sum, V.pos_sum + o, K * 8, cudaMemcpyDeviceToHost));
+  if (v->pos_cnt) PKV_CUDA(cudaMemcpy(v->pos_cnt, V.pos_cnt + o, K * 4, cudaMemcpyDeviceToHost));
   const size_t gc = (size_t)D.G * D.C * 4;
   if (v->hist_k) PKV_CUDA(cudaMemcpy2D(v->hist_k, gc, V.hist + o * 2 * D.G * D.C, 2 * gc, gc, K, cudaMemcpyDeviceToHost));
   if (v->hist_v)
@@ -578,6 +602,9 @@ int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   if (v->tau) PKV_CUDA(cudaMemcpy(V.tau + o, v->tau, K * 4, cudaMemcpyHostToDevice));
   if (v->pos) PKV_CUDA(cudaMemcpy(V.pos + o, v->pos, K * 8, cudaMemcpyHostToDevice));
   if (v->nres) PKV_CUDA(cudaMemcpy(V.nres + o, v->nres, K * 4, cudaMemcpyHostToDevice));
+  if (v->pos_first) PKV_CUDA(cudaMemcpy(V.pos_first + o, v->pos_first, K * 8, cudaMemcpyHostToDevice));
+  if (v->pos_sum) PKV_CUDA(cudaMemcpy(V.pos_sum + o, v->pos_sum, K * 8, cudaMemcpyHostToDevice));
+  if (v->pos_cnt) PKV_CUDA(cudaMemcpy(V.pos_cnt + o, v->pos_cnt, K * 4, cudaMemcpyHostToDevice));
   const size_t gc = (size_t)D.G * D.C * 4;
   if (v->hist_k) PKV_CUDA(cudaMemcpy2D(V.hist + o * 2 * D.G * D.C, 2 * gc, v->hist_k, gc, gc, K, cudaMemcpyHostToDevice));
   if (v->hist_v)

@@ -290,7 +290,75 @@ __device__ __forceinline__ void online_update(Softmax1& st, float (&acc)[VEC], f
   }
 }
 
-template <typename T, int DH>
+// ---- rotary position anchoring (PROTOKV_ROPE, D.1; readings 28-31) --------------------
+// Rotate-half convention: pair (i, i + d/2) of a vector at position p turns by p * theta^(-2i/d).  A lane of the
+// attention warp holds VEC consecutive dims, so its partner dims live in lane ^ 16 at the same v.  The angles are
+// evaluated in fp64 by rope_tables_kernel (positions reach ~1e6, fp32 angles would be off by 0.05 rad) and kept as
+// float2 (cos, sin): J[j] for the token offset inside a frame, F[slot] for the first position of the frame held in a
+// ring slot (a near token's rotation is the product of the two), P[k] for the anchor of every prototype (all S
+// pseudo-tokens of a prototype share it), Qc[i] for the query tokens.
+template <int VEC>
+__device__ __forceinline__ void rope_apply(float (&x)[VEC], const float2 (&cs)[VEC], int lane) {
+  const float sgn = lane < 16 ? -1.f : 1.f;
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) {
+    const float partner = __shfl_xor_sync(0xffffffffu, x[v], 16);
+    x[v] = fmaf(sgn * partner, cs[v].y, x[v] * cs[v].x);
+  }
+}
+__device__ __forceinline__ float2 cis_mul(float2 a, float2 b) {
+  return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.y, b.x, a.x * b.y));
+}
+
+__global__ void rope_tables_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
+  extern __shared__ double inv_freq[];                 // [d/2]
+  const int h = D.d / 2;
+  for (int i = threadIdx.x; i < h; i += blockDim.x) inv_freq[i] = pow(H.rope_theta, -2.0 * (double)i / (double)D.d);
+  __syncthreads();
+  const long long nJ = (long long)D.T * h, nF = (long long)D.Wf * h, nQ = (long long)A.n_q * h;
+  const long long nP = (long long)D.B * D.K * h, total = nJ + nF + nQ + nP;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    double p;
+    float2* dst;
+    int i;
+    if (e < nJ) { i = (int)(e % h); p = (double)(e / h); dst = V.ropeJ + e; }
+    else if (e < nJ + nF) {
+      const long long x = e - nJ;
+      i = (int)(x % h);
+      const long long slot = x / h, last = A.frames - 1;
+      const long long f = last >= slot ? last - ((last - slot) % D.Wf) : 0;   // the frame the slot holds (0 if none yet)
+      p = (double)(H.pos0 + f * D.T);
+      dst = V.ropeF + x;
+    } else if (e < nJ + nF + nQ) {
+      const long long x = e - nJ - nF;
+      i = (int)(x % h);
+      p = (double)(A.q_pos0 + x / h);
+      dst = V.ropeQ + x;
+    } else {
+      const long long x = e - nJ - nF - nQ;
+      i = (int)(x % h);
+      const long long pk = x / h;
+      if ((int)(pk % D.K) >= A.n_act) continue;
+      if (H.rope_anchor == 1) p = (double)V.pos_first[pk];
+      else if (H.rope_anchor == 2) p = (double)V.pos_sum[pk] / (double)max(V.pos_cnt[pk], 1);
+      else p = (double)V.pos[pk];
+      dst = V.ropeP + x;
+    }
+    double sn, cs;
+    sincos(p * inv_freq[i], &sn, &cs);
+    *dst = make_float2((float)cs, (float)sn);
+  }
+}
+
+int launch_rope_tables(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s) {
+  const int h = D.d / 2;
+  const long long total = (long long)(D.T + D.Wf + A.n_q) * h + (long long)D.B * D.K * h;
+  const unsigned grid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+  rope_tables_kernel<<<grid, 256, (size_t)h * 8, s>>>(D, H, V, A);
+  return 1;
+}
+
+template <typename T, int DH, bool ROPE>
 __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
   constexpr int VEC = DH / 32;
   extern __shared__ __align__(16) float cb_s[];
@@ -320,6 +388,14 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
   const size_t qoff = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + h) * DH;
   float q[VEC];
   load_vec<T, VEC>((const T*)A.Q + qoff + lane * VEC, q);
+  constexpr int HH = DH / 2;
+  const int ri = (lane & 15) * VEC;                    // pair index of this lane's first dim (ROPE)
+  if (ROPE) {
+    float2 cs[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) cs[v] = V.ropeQ[(size_t)qi * HH + ri + v];
+    rope_apply<VEC>(q, cs, lane);
+  }
   const float scale = 1.0f / sqrtf((float)DH);
 #pragma unroll
   for (int v = 0; v < VEC; ++v) q[v] *= scale;
@@ -346,6 +422,16 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
       load_vec<T, VEC>(rK + (size_t)(e + u) * DH + lane * VEC, kk[u]);
       load_vec<T, VEC>(rV + (size_t)(e + u) * DH + lane * VEC, vv[u]);
     }
+    if (ROPE) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int slot = (e + u) / D.T, j = (e + u) - slot * D.T;
+        float2 cs[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) cs[v] = cis_mul(V.ropeF[slot * HH + ri + v], V.ropeJ[(size_t)j * HH + ri + v]);
+        rope_apply<VEC>(kk[u], cs, lane);
+      }
+    }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       dot[u] = 0.f;
@@ -364,6 +450,13 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
     float kk[VEC], vv[VEC];
     load_vec<T, VEC>(rK + (size_t)e * DH + lane * VEC, kk);
     load_vec<T, VEC>(rV + (size_t)e * DH + lane * VEC, vv);
+    if (ROPE) {
+      const int slot = e / D.T, j = e - slot * D.T;
+      float2 cs[VEC];
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) cs[v] = cis_mul(V.ropeF[slot * HH + ri + v], V.ropeJ[(size_t)j * HH + ri + v]);
+      rope_apply<VEC>(kk, cs, lane);
+    }
     float dot = 0.f;
 #pragma unroll
     for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], kk[v], dot);
@@ -384,10 +477,19 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
       load_vec<float, VEC>(V.c + pk * DH + lane * VEC, c);
       load_vec<float, VEC>(V.p + pk * DH + lane * VEC, p);
       const float bias = use_bias ? V.logn[pk] : 0.f;
+      float2 pcs[VEC];
+      if (ROPE) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) pcs[v] = V.ropeP[pk * HH + ri + v];
+      }
       if (kind == 1) {             // zero residuals: S identical pseudo-tokens (Alg. 4 l.3-4)
+        float kc[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) kc[v] = c[v];
+        if (ROPE) rope_apply<VEC>(kc, pcs, lane);
         float dot = 0.f;
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], c[v], dot);
+        for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], kc[v], dot);
         dot = warp_sum(dot) + bias;
         for (int s = s_lo; s < s_hi; ++s) online_update<VEC>(sm, acc, dot, p);
         continue;
@@ -400,7 +502,10 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
         load_vec<float, VEC>(cbv_s + g * gstride + zv * D.sub + li * VEC, rv);
         float dot = 0.f;
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) { dot = fmaf(q[v], c[v] + rk[v], dot); rv[v] += p[v]; }
+        for (int v = 0; v < VEC; ++v) { rk[v] += c[v]; rv[v] += p[v]; }
+        if (ROPE) rope_apply<VEC>(rk, pcs, lane);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) dot = fmaf(q[v], rk[v], dot);
         dot = warp_sum(dot) + bias;
         online_update<VEC>(sm, acc, dot, rv);
       }
@@ -470,7 +575,8 @@ static int attention_simt_launch(const Dims& D, const Hyper& H, const Dev& V, co
   const int rgroups = (R + kAttWarps - 1) / kAttWarps;
   const size_t sm = V.cbk ? 2 * (size_t)D.G * (D.C * D.sub + kCbPad) * 4 : 0;
   dim3 grid(nb * rgroups, A.nsplit);
-  attention_simt_kernel<T, DH><<<grid, kAttWarps * 32, sm, s>>>(D, H, V, A);
+  if (H.flags & PROTOKV_ROPE) attention_simt_kernel<T, DH, true><<<grid, kAttWarps * 32, sm, s>>>(D, H, V, A);
+  else attention_simt_kernel<T, DH, false><<<grid, kAttWarps * 32, sm, s>>>(D, H, V, A);
   const int rows_total = nb * R;
   attention_combine_kernel<T, DH><<<(rows_total + 3) / 4, 128, 0, s>>>(D, V, A, rows_total);
   return 2;

@@ -119,7 +119,8 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     V.mu[pk * 2] = se[0]; V.mu[pk * 2 + 1] = se[1];
     V.sigma[pk * 3] = 1.f; V.sigma[pk * 3 + 1] = 0.f; V.sigma[pk * 3 + 2] = 1.f;
     V.tau[pk] = F.t;
-    V.pos[pk] = (long long)F.ev_frame * D.T + j;
+    const long long ps = H.pos0 + (long long)F.ev_frame * D.T + j;
+    V.pos[pk] = ps; V.pos_first[pk] = ps; V.pos_sum[pk] = ps; V.pos_cnt[pk] = 1;   // D.1 anchors
     V.nres[pk] = 0u;
     store_rec(V.rec, pk, make_rec(cc, se[0], se[1], 1.f, 0.f, 1.f, F.t, H));
     V.logn[pk] = 0.f;
@@ -357,7 +358,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
     float mu0 = V.mu[pk * 2], mu1 = V.mu[pk * 2 + 1];
     float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
     int n = V.n[pk];
-    int m = 0, jlast = 0;
+    int m = 0, jlast = 0, jsum = 0;
     for (int ii = i; ii < ntok && (int)(keys[ii] >> 12) == k; ++ii) {
       const int j = (int)(keys[ii] & 0xfffu);
       float ke[VEC], ve[VEC];
@@ -369,7 +370,7 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
         c[v] = ema_step(oma, al, c[v], ke[v]);                       // l.8
         p[v] = ema_step(omb, be, p[v], ve[v]);                       // l.9
       }
-      n += 1; ++m; jlast = j;                                        // l.10
+      n += 1; ++m; jlast = j; jsum += j;                             // l.10
       mu0 = ema_step(ome, et, mu0, s0);                              // l.11
       mu1 = ema_step(ome, et, mu1, s1);
       const double dx = (double)s0 - (double)mu0, dy = (double)s1 - (double)mu1;   // new mu
@@ -418,7 +419,9 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
     if (lane == 0) {
       V.n[pk] = n;
       V.tau[pk] = F.t;
-      V.pos[pk] = (long long)F.ev_frame * D.T + jlast;
+      const long long ps0 = H.pos0 + (long long)F.ev_frame * D.T;
+      V.pos[pk] = ps0 + jlast;
+      V.pos_sum[pk] += ps0 * m + jsum; V.pos_cnt[pk] += m;
       V.mu[pk * 2] = mu0; V.mu[pk * 2 + 1] = mu1;
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] += (uint32_t)m;
@@ -618,6 +621,9 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
     const int n_old = V.n[pk];                                       // read now: the write-back must not wait for them
     const uint32_t nres_old = has_cb ? V.nres[pk] : 0u;
+    const long long psum_old = V.pos_sum[pk];
+    const int pcnt_old = V.pos_cnt[pk];
+    int jsum = 0;
     int jn = (int)(sorted[r0] & 0xfffu);
     float ken[4], ven[4];
     load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
@@ -626,6 +632,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     int j = jn;
     for (int r = r0; r < r1; ++r) {
       j = jn;
+      jsum += j;
       float ke[4], ve[4];
 #pragma unroll
       for (int v = 0; v < 4; ++v) { ke[v] = ken[v]; ve[v] = ven[v]; }
@@ -677,7 +684,9 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       const int n = n_old + m;                                       // l.10
       V.n[pk] = n;
       V.tau[pk] = F.t;
-      V.pos[pk] = (long long)F.ev_frame * D.T + j;
+      const long long ps0 = H.pos0 + (long long)F.ev_frame * D.T;
+      V.pos[pk] = ps0 + j;
+      V.pos_sum[pk] = psum_old + ps0 * m + jsum; V.pos_cnt[pk] = pcnt_old + m;       // D.1 anchors
       *(float2*)(V.mu + pk * 2) = make_float2(mu0, mu1);
       V.sigma[pk * 3] = sxx; V.sigma[pk * 3 + 1] = sxy; V.sigma[pk * 3 + 2] = syy;
       if (has_cb) V.nres[pk] = nres_old + (uint32_t)m;

@@ -44,7 +44,7 @@ def bank_frame(spec, K, V, s, bank):
 
 def compare_state(gs, os_, where=""):
     """GPU state dict vs oracle state dict of one bank."""
-    for f in ("n", "tau", "pos", "nres", "active", "hist_k", "hist_v"):
+    for f in ("n", "tau", "pos", "nres", "active", "hist_k", "hist_v", "pos_first", "pos_sum", "pos_cnt"):
         assert np.array_equal(gs[f], os_[f]), f"{where}: {f} differs"
     act = os_["active"].astype(bool)
     for f in ("c", "p", "mu", "sigma"):
@@ -190,13 +190,13 @@ def attention_tolerance(spec):
 
 
 def compare_attention(spec, gpu, oracles, Q, n_q=None, layer_begin=0, layer_count=None, run_synthesis=True,
-                      use_gpu_codes=False, rows_sample=None):
+                      use_gpu_codes=False, rows_sample=None, q_pos0=None):
     """GPU attention of all banks vs the oracle on the given banks.  Q: CPU tensor in the ABI layout
     [n_streams][layer_count][n_q][Hq][d]."""
     n_q = Q.shape[2]
     layer_count = Q.shape[1]
     out, lse = gpu.query_attention_ex(Q.to(gpu.device), n_q=n_q, layer_begin=layer_begin, layer_count=layer_count,
-                                      return_lse=True, run_synthesis=run_synthesis)
+                                      return_lse=True, run_synthesis=run_synthesis, q_pos0=q_pos0)
     out = out.float().cpu()
     lse = lse.cpu().numpy()
     atol, rtol = attention_tolerance(spec)
@@ -214,7 +214,11 @@ def compare_attention(spec, gpu, oracles, Q, n_q=None, layer_begin=0, layer_coun
         fk = fv = None
         if use_gpu_codes:
             fk, fv, _ = gpu.export_codes(b)
-        ref, rl = o.attention(q[rows], forced_codes_k=fk, forced_codes_v=fv, return_lse=True)
+        # query token i sits at q_pos0 + i (default: the next stream position); row = token * group + head.  Ignored by
+        # the oracle unless FLAG_ROPE is set.
+        qp0 = q_pos0 if q_pos0 is not None else int(gpu.cfg.pos0) + gpu.frames_seen * spec.T
+        qpos = (qp0 + rows // group).astype(np.int64)
+        ref, rl = o.attention(q[rows], forced_codes_k=fk, forced_codes_v=fv, return_lse=True, qpos=qpos)
         ref_r = torch.from_numpy(ref).to(spec.torch_dtype).float().numpy()   # output rounded to the I/O dtype
         err = np.abs(g[rows] - ref_r)
         tol = atol + rtol * np.abs(ref_r)
