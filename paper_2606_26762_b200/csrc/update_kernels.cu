@@ -609,13 +609,47 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   const int g = lane >> 2, li = lane & 3;
   float4* rsc = scratch + warp * 64;
 
-  for (int seg = warp; seg < nseg; seg += kUfWarps) {
+  // A task = (segment, side): the key side replays c, mu, Sigma and the K histogram, the value side p and the V
+  // histogram -- two independent dependency chains, so a segment's latency is that of the longer one
+  for (int task = warp; task < 2 * nseg; task += kUfWarps) {
+    const int seg = task >> 1, side = task & 1;
     const int r0 = segstart[seg], r1 = segstart[seg + 1];
     const int k = (int)(sorted[r0] >> 12);
     const size_t pk = (size_t)b * D.K + k;
-    float c[4], p[4];
+    int jn = (int)(sorted[r0] & 0xfffu);
+    if (side) {                                                        // ---- value side: l.9 and the V half of l.13
+      float p[4], ven[4];
+      load_vec<float, 4>(V.p + pk * DH + lane * 4, p);
+      load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
+      for (int r = r0; r < r1; ++r) {
+        const int j = jn;
+        float ve[4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v) ve[v] = ven[v];
+        if (r + 1 < r1) {
+          jn = (int)(sorted[r + 1] & 0xfffu);
+          load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
+        }
+#pragma unroll
+        for (int v = 0; v < 4; ++v) p[v] = fmaf(bef, ve[v] - p[v], p[v]);              // l.9
+        if (has_cb) {
+          __syncwarp();
+          rsc[lane] = make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
+          __syncwarp();
+          int zv;
+          pq_pick(cbv4, cnv, rsc, g, li, zv);
+          if (li == 0) {
+            atomicAdd(V.hist + ((pk * 2 + 1) * 8 + g) * 16 + zv, 1u);
+            V.tcodeV[(bt + j) * 8 + g] = (uint8_t)zv;
+          }
+        }
+      }
+      *(float4*)(V.p + pk * DH + lane * 4) = make_float4(p[0], p[1], p[2], p[3]);
+      continue;
+    }
+    // ---- key side: l.8, l.10-12, the K half of l.13 and everything derived from the prototype
+    float c[4];
     load_vec<float, 4>(V.c + pk * DH + lane * 4, c);
-    load_vec<float, 4>(V.p + pk * DH + lane * 4, p);
     const float2 mu2 = *(const float2*)(V.mu + pk * 2);
     float mu0 = mu2.x, mu1 = mu2.y;
     float sxx = V.sigma[pk * 3], sxy = V.sigma[pk * 3 + 1], syy = V.sigma[pk * 3 + 2];
@@ -624,30 +658,24 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     const long long psum_old = V.pos_sum[pk];
     const int pcnt_old = V.pos_cnt[pk];
     int jsum = 0;
-    int jn = (int)(sorted[r0] & 0xfffu);
-    float ken[4], ven[4];
+    float ken[4];
     load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
-    load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
     float2 sn = *(const float2*)(ringS + jn * 2);
     int j = jn;
     for (int r = r0; r < r1; ++r) {
       j = jn;
       jsum += j;
-      float ke[4], ve[4];
+      float ke[4];
 #pragma unroll
-      for (int v = 0; v < 4; ++v) { ke[v] = ken[v]; ve[v] = ven[v]; }
+      for (int v = 0; v < 4; ++v) ke[v] = ken[v];
       const float s0 = sn.x, s1 = sn.y;
       if (r + 1 < r1) {                                              // prefetch the next token of the segment
         jn = (int)(sorted[r + 1] & 0xfffu);
         load_vec<T, 4>(ringK + (size_t)jn * DH + lane * 4, ken);
-        load_vec<T, 4>(ringV + (size_t)jn * DH + lane * 4, ven);
         sn = *(const float2*)(ringS + jn * 2);
       }
 #pragma unroll
-      for (int v = 0; v < 4; ++v) {
-        c[v] = fmaf(alf, ke[v] - c[v], c[v]);                        // l.8  (1 - a) c + a K  =  c + a (K - c)
-        p[v] = fmaf(bef, ve[v] - p[v], p[v]);                        // l.9
-      }
+      for (int v = 0; v < 4; ++v) c[v] = fmaf(alf, ke[v] - c[v], c[v]);                // l.8  (1 - a) c + a K  =  c + a (K - c)
       mu0 = ema_step(ome, et, mu0, s0);                              // l.11
       mu1 = ema_step(ome, et, mu1, s1);
       const double dx = (double)s0 - (double)mu0, dy = (double)s1 - (double)mu1;   // new mu
@@ -655,25 +683,20 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       sxx = (float)__dadd_rn(__dmul_rn(ome, (double)sxx), __dmul_rn(edx, dx));     // l.12
       sxy = (float)__dadd_rn(__dmul_rn(ome, (double)sxy), __dmul_rn(edx, dy));
       syy = (float)__dadd_rn(__dmul_rn(ome, (double)syy), __dmul_rn(edy, dy));
-      if (has_cb) {                                                  // l.13, residual of the updated centres
+      if (has_cb) {                                                  // l.13, residual of the updated centre
         __syncwarp();
         rsc[lane] = make_float4(ke[0] - c[0], ke[1] - c[1], ke[2] - c[2], ke[3] - c[3]);
-        rsc[32 + lane] = make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
         __syncwarp();
-        int zk, zv;
+        int zk;
         pq_pick(cbk4, cnk, rsc, g, li, zk);
-        pq_pick(cbv4, cnv, rsc + 32, g, li, zv);
         if (li == 0) {
           atomicAdd(V.hist + ((pk * 2 + 0) * 8 + g) * 16 + zk, 1u);
-          atomicAdd(V.hist + ((pk * 2 + 1) * 8 + g) * 16 + zv, 1u);
           V.tcodeK[(bt + j) * 8 + g] = (uint8_t)zk;
-          V.tcodeV[(bt + j) * 8 + g] = (uint8_t)zv;
         }
       }
     }
     // write back the prototype and everything derived from it
     *(float4*)(V.c + pk * DH + lane * 4) = make_float4(c[0], c[1], c[2], c[3]);
-    *(float4*)(V.p + pk * DH + lane * 4) = make_float4(p[0], p[1], p[2], p[3]);
     float cc = 0.f;
 #pragma unroll
     for (int v = 0; v < 4; ++v) cc = fmaf(c[v], c[v], cc);
