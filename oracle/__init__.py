@@ -22,6 +22,7 @@ _LIB = os.path.join(_HERE, "libprotokv_oracle.so")
 FLAG_MAH_SQUARED, FLAG_NO_MASS_BIAS, FLAG_NO_RESIDUAL, FLAG_NEAR_ONLY, FLAG_FAR_ONLY = 1, 2, 4, 8, 16
 FLAG_MAINTENANCE = 64
 FLAG_ROPE = 256
+FLAG_WARMUP, FLAG_WARMUP_MANUAL, FLAG_VAR_ALLOC = 512, 1024, 2048
 
 
 def build(force: bool = False) -> str:
@@ -41,7 +42,9 @@ class _Config(C.Structure):
                 ("alpha", C.c_float), ("beta", C.c_float), ("eta", C.c_float),
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
                 ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float),
-                ("rope_theta", C.c_double), ("rope_anchor", C.c_int32), ("pos0", C.c_int64)]
+                ("rope_theta", C.c_double), ("rope_anchor", C.c_int32), ("pos0", C.c_int64),
+                ("t_warm", C.c_int32), ("warm_reservoir", C.c_int32), ("km_iters", C.c_int32),
+                ("km_batch", C.c_int32), ("km_seed", C.c_uint64), ("s_cap", C.c_int32)]
 
 
 class _Trace(C.Structure):
@@ -76,7 +79,16 @@ def _load():
         lib.pko_set_state.argtypes = [C.c_void_p, C.POINTER(_StateView)]
         lib.pko_score.restype = C.c_float
         lib.pko_score.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int32]
-        lib.pko_synthesize.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        lib.pko_synthesize.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        lib.pko_reservoir.restype = C.c_int64
+        lib.pko_reservoir.argtypes = [C.c_void_p] * 4
+        lib.pko_set_reservoir.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64]
+        lib.pko_train_codebooks.argtypes = [C.c_void_p]
+        lib.pko_codebooks.argtypes = [C.c_void_p] * 3
+        lib.pko_draw.restype = C.c_uint64
+        lib.pko_draw.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
+        lib.pko_reservoir_slot.argtypes = [C.c_void_p, C.c_int64]
+        lib.pko_allocation.argtypes = [C.c_void_p] * 3
         lib.pko_decode_hist.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pko_log_table.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pko_tuple_score.restype = C.c_int64
@@ -100,7 +112,9 @@ def _ptr(a: Optional[np.ndarray]):
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
                 eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0,
                 gamma=0.05, eps_k=0.20, eps_v=0.25,   # Table 5
-                rope_theta=1.0e6, rope_anchor=0, pos0=0)   # readings 28-30 (the paper fixes no rotary base)
+                rope_theta=1.0e6, rope_anchor=0, pos0=0,   # readings 28-30 (the paper fixes no rotary base)
+                t_warm=0, warm_reservoir=2048, km_iters=32, km_batch=256, km_seed=0,   # readings 32-36 (L312, L478)
+                s_cap=32)                                  # reading 39 (D.3)
 
 
 class OracleBank:
@@ -112,6 +126,7 @@ class OracleBank:
         self.cfg = _Config(T=T, near_frames=near_frames, k_max=k_max, d=d, **p)
         self.T, self.near_frames, self.k_max, self.d = T, near_frames, k_max, d
         self.S, self.G, self.C = p["S"], p["G"], p["C"]
+        self.smax = p["s_cap"] if p["flags"] & FLAG_VAR_ALLOC else self.S   # rows per slot of code arrays
         self._lib = _load()
         ck = _f32(codebook_k) if codebook_k is not None else None
         cv = _f32(codebook_v) if codebook_v is not None else None
@@ -203,13 +218,49 @@ class OracleBank:
 
     # ---- synthesis ----------------------------------------------------------------------------------------
     def synthesize(self):
-        k, S, G = self.k_max, self.S, self.G
+        k, S, G = self.k_max, self.smax, self.G
         out = dict(codes_k=np.zeros((k, S, G), np.uint8), codes_v=np.zeros((k, S, G), np.uint8),
                    scores_k=np.zeros((k, S), np.int64), scores_v=np.zeros((k, S), np.int64),
-                   zero=np.zeros(k, np.uint8))
+                   zero=np.zeros(k, np.uint8), s_count=np.zeros(k, np.int32))
         self._lib.pko_synthesize(self._h, *[_ptr(out[f]) for f in ("codes_k", "codes_v", "scores_k", "scores_v",
-                                                                    "zero")])
+                                                                    "zero", "s_count")])
         return out
+
+    # ---- PQ codebook warm-up and D.3 allocation ---------------------------------------------
+    def reservoir(self):
+        """(r^K [n][d], r^V [n][d], residuals offered so far)."""
+        R = self.cfg.warm_reservoir
+        rk = np.zeros((R, self.d), np.float32)
+        rv = np.zeros((R, self.d), np.float32)
+        seen = np.zeros(1, np.int64)
+        n = self._lib.pko_reservoir(self._h, _ptr(rk), _ptr(rv), _ptr(seen))
+        return rk[:n], rv[:n], int(seen[0])
+
+    def set_reservoir(self, rk, rv):
+        rk, rv = _f32(rk), _f32(rv)
+        assert rk.shape == rv.shape and rk.shape[1] == self.d and rk.shape[0] <= self.cfg.warm_reservoir
+        self._lib.pko_set_reservoir(self._h, _ptr(rk), _ptr(rv), rk.shape[0])
+
+    def train_codebooks(self):
+        return int(self._lib.pko_train_codebooks(self._h))
+
+    def codebooks(self):
+        sub = self.d // self.G
+        ck = np.zeros((self.G, self.C, sub), np.float32)
+        cv = np.zeros_like(ck)
+        return (ck, cv) if self._lib.pko_codebooks(self._h, _ptr(ck), _ptr(cv)) else None
+
+    def draw(self, stream, counter):
+        return int(self._lib.pko_draw(self._h, int(stream), int(counter)))
+
+    def reservoir_slot(self, i):
+        return int(self._lib.pko_reservoir_slot(self._h, int(i)))
+
+    def allocation(self):
+        v = np.zeros(self.k_max, np.int64)
+        sk = np.zeros(self.k_max, np.int32)
+        self._lib.pko_allocation(self._h, _ptr(v), _ptr(sk))
+        return v, sk
 
     def decode_hist(self, H):
         H = np.ascontiguousarray(H, dtype=np.uint32)

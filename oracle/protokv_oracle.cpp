@@ -5,6 +5,8 @@
 //   Eq. 3 + Alg. 3 beam decode             -> decode_top_s
 //   Alg. 4 decode + attention, Eq. 2/4 -> materialize / attention
 //   Alg. 2 prototype maintenance (off unless FLAG_MAINTENANCE) -> maintain
+//   PQ codebook warm-up (FLAG_WARMUP) -> reservoir_offer / kmeans_subspace / train_codebooks
+//   D.3 variance-aware pseudo-token allocation (FLAG_VAR_ALLOC) -> variance_fx / allocate
 // One object = one bank = one (stream, layer, KV head): banks are independent.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call this.
@@ -25,6 +27,10 @@
 // Rotary anchoring (FLAG_ROPE, tests/test_oracle_rope.py): rotated keys and attention against the rotate-half routine of
 // the `transformers` package + torch SDPA, relative-position property (a common shift of all positions changes nothing),
 // norm preservation, anchor fields (first / average / most recent) recomputed from the assignment log.
+// PQ codebook warm-up (FLAG_WARMUP, tests/test_oracle_warmup.py): generator against the published
+// SplitMix64 vector, reservoir against uniform sampling and numpy residuals, mini-batch k-means against the running-mean
+// closed form, separated blobs and scikit-learn KMeans.  D.3 allocation (FLAG_VAR_ALLOC, tests/test_oracle_alloc.py;
+// PAPER.md:L608-625): Var(H_k) against numpy's population variance, shares against hand-worked examples and invariants.
 // What stays unpinned: the absolute values produced on the five configs ("parity unpinned" beyond those pins, see
 // DESIGN.md).
 #include <algorithm>
@@ -46,6 +52,10 @@ enum : uint32_t {
   FLAG_FAR_ONLY = 16u,     // attention over pseudo-tokens only   (L177)
   FLAG_ROPE = 256u,        // rotary position anchoring of L126 / D.1 (readings 28-31): K and Q are given un-rotated
   FLAG_MAINTENANCE = 64u,  // run Alg. 2 at Alg. 1 l.15; off on the graded path (reading 19)
+  FLAG_WARMUP = 512u,      // PQ codebook warm-up (readings 32-36): residual reservoir over the first t_warm
+                           // steps, then mini-batch k-means per subspace and side; codebooks given at create are ignored
+  FLAG_WARMUP_MANUAL = 1024u,  // with FLAG_WARMUP: training is not started by the frame t_warm - 1 but by pko_train_codebooks
+  FLAG_VAR_ALLOC = 2048u,  // variance-aware pseudo-token allocation S_k (D.3; readings 37-40)
 };
 
 struct Config {
@@ -59,6 +69,11 @@ struct Config {
   double rope_theta;           // rotary base (reading 28); angle of pair i at position p = p * theta^(-2 i / d)
   int32_t rope_anchor;         // D.1 (L578-596): 0 most recent absorbed position (default), 1 first, 2 average
   int64_t pos0;                // stream position of token 0 of frame 0 (positions are pos0 + f T + j)
+  int32_t t_warm;              // warm-up length in streaming steps (frames, reading 2): residuals of steps t < t_warm are collected
+  int32_t warm_reservoir;      // reservoir capacity R (residual pairs per bank)
+  int32_t km_iters, km_batch;  // mini-batch k-means: iterations, samples per iteration
+  uint64_t km_seed;            // seed of this bank's counter-based generator (reservoir replacement, batch sampling)
+  int32_t s_cap;               // D.3: upper bound of S_k (<= beam); S_tot = k_max * S
 };
 
 struct Maint {          // what Alg. 2 did since the counters were last read (pko_maintenance_counters)
@@ -115,10 +130,18 @@ struct Bank {
   std::vector<uint8_t> active;
   std::vector<uint8_t> used;   // slot has been initialised at least once (Alg. 2 recycles only such slots, reading 24)
   Maint maint{0, 0, 0};
+  // PQ codebook warm-up: reservoir of residual pairs (r^K, r^V) of absorbed tokens, [R][d] each
+  std::vector<float> resK, resV;
+  int64_t res_seen = 0;        // residuals offered to the reservoir so far
+  bool trained = false;        // codebooks have been trained (warm-up is over)
 
   Bank(const Config& cf, const float* ck, const float* cv) : cfg(cf) {
     sub = cfg.d / cfg.G;
-    has_cb = ck && cv && !(cfg.flags & FLAG_NO_RESIDUAL);
+    has_cb = ck && cv && !(cfg.flags & (FLAG_NO_RESIDUAL | FLAG_WARMUP));
+    if ((cfg.flags & FLAG_WARMUP) && !(cfg.flags & FLAG_NO_RESIDUAL)) {
+      resK.assign((size_t)cfg.warm_reservoir * cfg.d, 0.f);
+      resV.assign((size_t)cfg.warm_reservoir * cfg.d, 0.f);
+    }
     if (has_cb) {
       size_t nn = (size_t)cfg.G * cfg.C * sub;
       cbk.assign(ck, ck + nn);
@@ -217,6 +240,103 @@ struct Bank {
     }
   }
 
+  // ---- PQ codebook warm-up ("mini-batch k-means on a warm-up reservoir of residuals collected during the
+  // first T_warm streaming steps, run separately for each subspace and for key/value"; readings 32-36) ----
+  // Counter-based generator: the SplitMix64 output function (Steele, Lea & Flood 2014) of a counter.
+  static uint64_t mix64(uint64_t x) {
+    uint64_t z = x + 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+  }
+  uint64_t draw(uint64_t stream, uint64_t counter) const { return mix64(cfg.km_seed ^ mix64(2 * counter + stream)); }
+  bool warming(int32_t t) const {
+    return (cfg.flags & FLAG_WARMUP) && !(cfg.flags & FLAG_NO_RESIDUAL) && !trained && t < cfg.t_warm;
+  }
+  // Reservoir sampling (Vitter's Algorithm R): the i-th residual pair offered (i = 0, 1, ...) fills slot i while
+  // i < R, afterwards it replaces slot u = draw mod (i + 1) if u < R.  Returns the slot or -1.
+  int reservoir_slot(int64_t i) const {
+    const int64_t R = cfg.warm_reservoir;
+    if (i < R) return (int)i;
+    const uint64_t u = draw(0, (uint64_t)i) % (uint64_t)(i + 1);
+    return u < (uint64_t)R ? (int)u : -1;
+  }
+  void reservoir_offer(const float* Ke, const float* Ve, const float* ck, const float* pk) {
+    const int64_t i = res_seen++;
+    const int slot = reservoir_slot(i);
+    if (slot < 0) return;
+    for (int e = 0; e < cfg.d; ++e) {      // r = x - centre (the just-updated one, reading 7), one rounding to fp32
+      resK[(size_t)slot * cfg.d + e] = (float)((double)Ke[e] - (double)ck[e]);
+      resV[(size_t)slot * cfg.d + e] = (float)((double)Ve[e] - (double)pk[e]);
+    }
+  }
+  int64_t reservoir_fill() const { return std::min<int64_t>(res_seen, cfg.warm_reservoir); }
+
+  // Mini-batch k-means (Sculley 2010, Alg. 1) of the rows X[0, n) restricted to subspace g: C centres of `sub` dims.
+  // Reading 34: centre z starts at row floor(z n / C); per iteration `km_batch` rows are drawn with replacement by the
+  // counter-based generator (the same rows for every subspace and side), assigned to their nearest centre with the
+  // centres frozen, then applied in batch order with the per-centre rate 1 / v_z, v_z = samples ever assigned to z.
+  // Reading 35: these decisions are taken in fp32, operation by operation (no fused multiply-add), so that another
+  // implementation can reproduce them bit for bit: dist = sum_m (x_m - c_m)^2 accumulated left to right from 0.
+  void kmeans_subspace(const std::vector<float>& X, int64_t n, int g, float* out /*[C][sub]*/) const {
+    const int Cn = cfg.C, d = cfg.d;
+    std::vector<float> cen((size_t)Cn * sub);
+    std::vector<int64_t> v(Cn, 0);
+    for (int z = 0; z < Cn; ++z) {
+      const int64_t row = (int64_t)z * n / Cn;
+      for (int m = 0; m < sub; ++m) cen[(size_t)z * sub + m] = X[(size_t)row * d + g * sub + m];
+    }
+    std::vector<int64_t> rows(cfg.km_batch);
+    std::vector<int> asg(cfg.km_batch);
+    for (int it = 0; it < cfg.km_iters; ++it) {
+      for (int q = 0; q < cfg.km_batch; ++q) {
+        rows[q] = (int64_t)(draw(1, (uint64_t)it * (uint64_t)cfg.km_batch + (uint64_t)q) % (uint64_t)n);
+        const float* x = &X[(size_t)rows[q] * d + g * sub];
+        int zb = 0;
+        float db = std::numeric_limits<float>::infinity();
+        for (int z = 0; z < Cn; ++z) {
+          float acc = 0.f;
+          for (int m = 0; m < sub; ++m) {
+            const float t = x[m] - cen[(size_t)z * sub + m];
+            const float t2 = t * t;
+            acc = acc + t2;
+          }
+          if (acc < db) { db = acc; zb = z; }             // lowest index on ties
+        }
+        asg[q] = zb;
+      }
+      for (int q = 0; q < cfg.km_batch; ++q) {
+        const int z = asg[q];
+        v[z] += 1;
+        const float eta = 1.0f / (float)v[z];
+        const float keep = 1.0f - eta;
+        const float* x = &X[(size_t)rows[q] * d + g * sub];
+        for (int m = 0; m < sub; ++m) {
+          const float a = keep * cen[(size_t)z * sub + m];
+          const float b2 = eta * x[m];
+          cen[(size_t)z * sub + m] = a + b2;
+        }
+      }
+    }
+    std::memcpy(out, cen.data(), cen.size() * sizeof(float));
+  }
+  // Ends the warm-up: trains C^K_g, C^V_g for every subspace from the reservoir.  Fewer than C residuals: no codebooks
+  // (the state keeps running without residual statistics).  Returns 1 if codebooks now exist.
+  int train_codebooks() {
+    if (!(cfg.flags & FLAG_WARMUP) || (cfg.flags & FLAG_NO_RESIDUAL) || trained) return has_cb ? 1 : 0;
+    trained = true;
+    const int64_t n = reservoir_fill();
+    if (n < cfg.C) return 0;
+    cbk.assign((size_t)cfg.G * cfg.C * sub, 0.f);
+    cbv.assign((size_t)cfg.G * cfg.C * sub, 0.f);
+    for (int g = 0; g < cfg.G; ++g) {
+      kmeans_subspace(resK, n, g, &cbk[(size_t)g * cfg.C * sub]);
+      kmeans_subspace(resV, n, g, &cbv[(size_t)g * cfg.C * sub]);
+    }
+    has_cb = true;
+    return 1;
+  }
+
   // Eq. 1: -cos(K_e,c_k) + lambda_sp d_Mah(s_e;mu_k,Sigma_k) + lambda_idle 1[t - tau_k > T_idle]
   float score(const float* Ke, const float* se, int k, int32_t t) const {
     int d = cfg.d;
@@ -287,6 +407,7 @@ struct Bank {
     sigma[k * 3] = (float)((1.0 - et) * (double)sigma[k * 3] + et * dx * dx);          // l.12
     sigma[k * 3 + 1] = (float)((1.0 - et) * (double)sigma[k * 3 + 1] + et * dx * dy);
     sigma[k * 3 + 2] = (float)((1.0 - et) * (double)sigma[k * 3 + 2] + et * dy * dy);
+    if (warming(t)) reservoir_offer(Ke, Ve, ck, pk);                     // L312: residuals of the warm-up steps
     if (!has_cb) return;
     std::vector<double> r(sub);
     std::vector<float> dist(cfg.C);
@@ -355,7 +476,7 @@ struct Bank {
     push(K, V, s);
     const int32_t t = frames_seen;             // stream time = frame index (reading 2)
     frames_seen += 1;
-    if (!ev) return;
+    if (!ev) { end_of_step(t); return; }
     if (tr) tr->evicted = 1;
     int j = 0;
     for (; j < T; ++j) {                        // (A)
@@ -386,6 +507,7 @@ struct Bank {
                    tr && tr->code_gap_k ? tr->code_gap_k + j * G : nullptr,
                    tr && tr->code_gap_v ? tr->code_gap_v + j * G : nullptr);
     }
+    end_of_step(t);
     if (cfg.flags & FLAG_MAINTENANCE) maintain(t);   // Alg. 1 l.15, once per frame in the frame-synchronous reading
   }
 
@@ -399,7 +521,7 @@ struct Bank {
     push(K, V, s);
     const int32_t t = frames_seen;
     frames_seen += 1;
-    if (!ev) return;
+    if (!ev) { end_of_step(t); return; }
     if (tr) tr->evicted = 1;
     int nf = 0;
     for (int j = 0; j < T; ++j) {
@@ -431,6 +553,11 @@ struct Bank {
       if (cfg.flags & FLAG_MAINTENANCE) maintain(t);                  // l.15
     }
     if (tr) tr->n_fill = nf;
+    end_of_step(t);
+  }
+  // the last warm-up step trains the codebooks (reading 33) unless the caller does it (FLAG_WARMUP_MANUAL)
+  void end_of_step(int32_t t) {
+    if ((cfg.flags & FLAG_WARMUP) && !(cfg.flags & FLAG_WARMUP_MANUAL) && !trained && t == cfg.t_warm - 1) train_codebooks();
   }
 
   // Eq. 3 in fixed point (reading 13): q(g,c) = llround(2^24 * log P(g,c))
@@ -449,7 +576,8 @@ struct Bank {
 
   // Alg. 3: beam search over subquantisers, beam width B, output the top S tuples.
   // Order: score descending, then tuple ascending lexicographically (z_1 most significant).
-  void decode_top_s(const uint32_t* H, std::vector<Tuple>& out, std::vector<int64_t>* out_scores) const {
+  void decode_top_s(const uint32_t* H, std::vector<Tuple>& out, std::vector<int64_t>* out_scores, int S_out = -1) const {
+    if (S_out < 0) S_out = cfg.S;
     std::vector<int64_t> q;
     log_table(H, q);
     struct Item { int64_t a; Tuple z; };
@@ -473,9 +601,82 @@ struct Bank {
     }
     out.clear();
     if (out_scores) out_scores->clear();
-    for (int s = 0; s < cfg.S && s < (int)beam.size(); ++s) {    // TopS, l.12
+    for (int s = 0; s < S_out && s < (int)beam.size(); ++s) {    // TopS, l.12
       out.push_back(beam[s].z);
       if (out_scores) out_scores->push_back(beam[s].a);
+    }
+  }
+
+  // ---- D.3 dynamic pseudo-token allocation: S_k = S_tot Var(H_k) / sum_j Var(H_j), S_tot = K_max S.
+  // Reading 37: Var(H_k) = total variance of the residual distribution the histograms describe -- for each side and
+  // subspace the codewords C_g[z] weighted by the empirical frequencies H[g,z] / sum_z H[g,z]:
+  //   var_g = sum_z H_z |C_g[z] - mean_g|^2 / tot,  mean_g = sum_z H_z C_g[z] / tot;  Var = sum over (K then V, g ascending).
+  // fp64, every product and sum rounded separately in the order written (reading 38: the value is then fixed to
+  // v_k = floor(Var 2^20 + 1/2), so that the allocation is integer arithmetic another implementation reproduces exactly).
+  int64_t variance_fx(int k) const {
+    if (!has_cb || nres[k] == 0) return 0;
+    double total = 0.0;
+    std::vector<double> mean(sub);
+    for (int kv = 0; kv < 2; ++kv) {
+      const std::vector<uint32_t>& H = kv ? hv : hk;
+      const std::vector<float>& cb = kv ? cbv : cbk;
+      for (int g = 0; g < cfg.G; ++g) {
+        const uint32_t* h = &H[((size_t)k * cfg.G + g) * cfg.C];
+        double tot = 0.0;
+        for (int z = 0; z < cfg.C; ++z) tot = tot + (double)h[z];
+        if (tot == 0.0) continue;
+        for (int m = 0; m < sub; ++m) {
+          double a = 0.0;
+          for (int z = 0; z < cfg.C; ++z) a = a + (double)h[z] * (double)cb[((size_t)g * cfg.C + z) * sub + m];
+          mean[m] = a / tot;
+        }
+        double var = 0.0;
+        for (int z = 0; z < cfg.C; ++z) {
+          double dz = 0.0;
+          for (int m = 0; m < sub; ++m) {
+            const double t = (double)cb[((size_t)g * cfg.C + z) * sub + m] - mean[m];
+            dz = dz + t * t;
+          }
+          var = var + (double)h[z] * dz;
+        }
+        total = total + var / tot;
+      }
+    }
+    return (int64_t)std::floor(total * 1048576.0 + 0.5);
+  }
+  // Reading 39: integer shares.  Every prototype in the context (active, n >= 1) gets one pseudo-token, the remaining
+  // budget S_tot - |A| is split in proportion to v_k (floor), capped at s_cap; what flooring and capping leave over goes
+  // one unit at a time to the prototypes below the cap in the order (remainder of the proportional split descending,
+  // index ascending), round after round.  sum_j v_j = 0: the fixed default min(S, s_cap) each.
+  void allocate(std::vector<int32_t>& Sk) const {
+    const int K = cfg.k_max;
+    Sk.assign(K, 0);
+    std::vector<int> A;
+    for (int k = 0; k < K; ++k) if (active[k] && n[k] >= 1) A.push_back(k);
+    if (A.empty()) return;
+    if (!(cfg.flags & FLAG_VAR_ALLOC)) { for (int k : A) Sk[k] = cfg.S; return; }
+    std::vector<int64_t> v(K, 0), rem(K, 0);
+    int64_t vsum = 0;
+    for (int k : A) { v[k] = variance_fx(k); vsum += v[k]; }
+    if (vsum == 0) { for (int k : A) Sk[k] = std::min(cfg.S, cfg.s_cap); return; }
+    const int64_t stot = (int64_t)K * cfg.S, bud = stot - (int64_t)A.size();
+    int64_t used = 0;
+    for (int k : A) {
+      const int64_t prod = bud * v[k];
+      Sk[k] = (int32_t)std::min<int64_t>(cfg.s_cap, 1 + prod / vsum);
+      rem[k] = prod % vsum;
+      used += Sk[k];
+    }
+    int64_t left = stot - used;
+    std::vector<int> order(A);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b2) { return rem[a] > rem[b2]; });
+    while (left > 0) {
+      bool any = false;
+      for (int k : order) {
+        if (left == 0) break;
+        if (Sk[k] < cfg.s_cap) { Sk[k] += 1; left -= 1; any = true; }
+      }
+      if (!any) break;
     }
   }
 
@@ -501,6 +702,7 @@ struct Bank {
       x[i + h] = b2 * cs + a * sn;
     }
   }
+  int stride_s() const { return (cfg.flags & FLAG_VAR_ALLOC) ? cfg.s_cap : cfg.S; }
   // Rotary anchor of prototype k (D.1 L578-596): most recent / first / average absorbed position
   double anchor(int k) const {
     if (cfg.rope_anchor == 1) return (double)pos_first[k];
@@ -511,7 +713,7 @@ struct Bank {
   // positions (optional out): stream position of every context element (near: original, pseudo: the anchor)
   void materialize(const uint8_t* fck, const uint8_t* fcv, std::vector<double>& Kt, std::vector<double>& Vt,
                    std::vector<double>& b, std::vector<double>* positions = nullptr, bool rotate = true) const {
-    const int d = cfg.d, S = cfg.S, G = cfg.G;
+    const int d = cfg.d, G = cfg.G;
     const bool do_rope = (cfg.flags & FLAG_ROPE) && rotate;
     Kt.clear(); Vt.clear(); b.clear();
     if (positions) positions->clear();
@@ -526,20 +728,24 @@ struct Bank {
         }
     if (cfg.flags & FLAG_NEAR_ONLY) return;
     std::vector<Tuple> zk, zv;
+    std::vector<int32_t> Sk;
+    allocate(Sk);                                                             // S_k = S, or the D.3 shares (FLAG_VAR_ALLOC)
+    const int smax = stride_s();                                              // row stride of forced code arrays
     for (int k = 0; k < cfg.k_max; ++k) {
       if (!active[k] || n[k] < 1) continue;                                   // l.2 "each active prototype"
       bool zero = (!has_cb) || nres[k] == 0;                                  // l.3-4
+      const int S = Sk[k];
       if (!zero) {
         if (fck && fcv) {
           zk.assign(S, Tuple{}); zv.assign(S, Tuple{});
           for (int s = 0; s < S; ++s)
             for (int g = 0; g < G; ++g) {
-              zk[s][g] = fck[((size_t)k * S + s) * G + g];
-              zv[s][g] = fcv[((size_t)k * S + s) * G + g];
+              zk[s][g] = fck[((size_t)k * smax + s) * G + g];
+              zv[s][g] = fcv[((size_t)k * smax + s) * G + g];
             }
         } else {
-          decode_top_s(&hk[(size_t)k * G * cfg.C], zk, nullptr);              // l.5
-          decode_top_s(&hv[(size_t)k * G * cfg.C], zv, nullptr);              // l.6
+          decode_top_s(&hk[(size_t)k * G * cfg.C], zk, nullptr, S);           // l.5
+          decode_top_s(&hv[(size_t)k * G * cfg.C], zv, nullptr, S);           // l.6
         }
       }
       double bias = (cfg.flags & FLAG_NO_MASS_BIAS) ? 0.0 : std::log((double)n[k]);   // Eq. 4, natural log
@@ -603,6 +809,9 @@ void* pko_create(const Config* cfg, const float* codebook_k, const float* codebo
   if (!cfg || cfg->d <= 0 || cfg->G <= 0 || cfg->d % cfg->G || cfg->C <= 0 || cfg->C > 255 || cfg->G > 16 ||
       cfg->S <= 0 || cfg->beam < cfg->S || cfg->T <= 0 || cfg->near_frames <= 0 || cfg->k_max <= 0)
     return nullptr;
+  if ((cfg->flags & FLAG_WARMUP) && (cfg->t_warm < 1 || cfg->warm_reservoir < 1 || cfg->km_iters < 0 || cfg->km_batch < 1))
+    return nullptr;
+  if ((cfg->flags & FLAG_VAR_ALLOC) && (cfg->s_cap < 1 || cfg->s_cap > cfg->beam)) return nullptr;
   return new Bank(*cfg, codebook_k, codebook_v);
 }
 void pko_destroy(void* h) { delete static_cast<Bank*>(h); }
@@ -670,23 +879,28 @@ float pko_score(void* h, const float* Ke, const float* se, int k, int32_t t) {
 
 // Alg. 3 for every slot: codes [k_max][S][G] (K and V), scores [k_max][S] (fixed-point), zero[k_max] = 1 when
 // the slot contributes zero residuals (n_res = 0 or no codebooks), 2 when the slot is not in the context at all.
-void pko_synthesize(void* h, uint8_t* codes_k, uint8_t* codes_v, int64_t* scores_k, int64_t* scores_v, uint8_t* zero) {
+void pko_synthesize(void* h, uint8_t* codes_k, uint8_t* codes_v, int64_t* scores_k, int64_t* scores_v, uint8_t* zero,
+                    int32_t* s_count) {
   Bank* b = static_cast<Bank*>(h);
   const Config& cf = b->cfg;
   std::vector<Tuple> z;
   std::vector<int64_t> sc;
+  std::vector<int32_t> Sk;
+  b->allocate(Sk);
+  const int smax = b->stride_s();      // rows per slot in the outputs: S, or s_cap with FLAG_VAR_ALLOC
   for (int k = 0; k < cf.k_max; ++k) {
     bool present = b->active[k] && b->n[k] >= 1;
     bool zr = !b->has_cb || b->nres[k] == 0;
     if (zero) zero[k] = present ? (zr ? 1 : 0) : 2;
+    if (s_count) s_count[k] = Sk[k];
     for (int kv = 0; kv < 2; ++kv) {
       uint8_t* oc = kv ? codes_v : codes_k;
       int64_t* os = kv ? scores_v : scores_k;
-      if (present && !zr) b->decode_top_s(&(kv ? b->hv : b->hk)[(size_t)k * cf.G * cf.C], z, &sc);
-      for (int s = 0; s < cf.S; ++s) {
+      if (present && !zr) b->decode_top_s(&(kv ? b->hv : b->hk)[(size_t)k * cf.G * cf.C], z, &sc, Sk[k]);
+      for (int s = 0; s < smax; ++s) {
         bool have = present && !zr && s < (int)z.size();
-        if (oc) for (int g = 0; g < cf.G; ++g) oc[((size_t)k * cf.S + s) * cf.G + g] = have ? z[s][g] : 0;
-        if (os) os[(size_t)k * cf.S + s] = have ? sc[s] : 0;
+        if (oc) for (int g = 0; g < cf.G; ++g) oc[((size_t)k * smax + s) * cf.G + g] = have ? z[s][g] : 0;
+        if (os) os[(size_t)k * smax + s] = have ? sc[s] : 0;
       }
     }
   }
@@ -713,6 +927,44 @@ void pko_log_table(void* h, const uint32_t* H, int64_t* q) {
 }
 int64_t pko_tuple_score(void* h, int k, int which, const uint8_t* z) {
   return static_cast<Bank*>(h)->tuple_score(k, which, z);
+}
+
+// PQ codebook warm-up: reservoir contents [fill][d] x 2 and the number of residuals offered so far
+int64_t pko_reservoir(void* h, float* rK, float* rV, int64_t* seen) {
+  Bank* b = static_cast<Bank*>(h);
+  const int64_t n = b->reservoir_fill();
+  if (rK) std::memcpy(rK, b->resK.data(), (size_t)n * b->cfg.d * sizeof(float));
+  if (rV) std::memcpy(rV, b->resV.data(), (size_t)n * b->cfg.d * sizeof(float));
+  if (seen) *seen = b->res_seen;
+  return n;
+}
+// overwrite the reservoir (pins): n rows, counted as n residuals offered
+void pko_set_reservoir(void* h, const float* rK, const float* rV, int64_t n) {
+  Bank* b = static_cast<Bank*>(h);
+  std::memcpy(b->resK.data(), rK, (size_t)n * b->cfg.d * sizeof(float));
+  std::memcpy(b->resV.data(), rV, (size_t)n * b->cfg.d * sizeof(float));
+  b->res_seen = n;
+}
+int pko_train_codebooks(void* h) { return static_cast<Bank*>(h)->train_codebooks(); }
+// current codebooks [G][C][sub] x 2; returns 0 if the bank has none
+int pko_codebooks(void* h, float* ck, float* cv) {
+  Bank* b = static_cast<Bank*>(h);
+  if (!b->has_cb) return 0;
+  if (ck) std::memcpy(ck, b->cbk.data(), b->cbk.size() * sizeof(float));
+  if (cv) std::memcpy(cv, b->cbv.data(), b->cbv.size() * sizeof(float));
+  return 1;
+}
+uint64_t pko_draw(void* h, uint64_t stream, uint64_t counter) { return static_cast<Bank*>(h)->draw(stream, counter); }
+int pko_reservoir_slot(void* h, int64_t i) { return static_cast<Bank*>(h)->reservoir_slot(i); }
+// D.3: fixed-point variances v_k [k_max] and the shares S_k [k_max] of the current state
+void pko_allocation(void* h, int64_t* v, int32_t* Sk) {
+  Bank* b = static_cast<Bank*>(h);
+  std::vector<int32_t> s;
+  b->allocate(s);
+  for (int k = 0; k < b->cfg.k_max; ++k) {
+    if (v) v[k] = (b->active[k] && b->n[k] >= 1) ? b->variance_fx(k) : 0;
+    if (Sk) Sk[k] = s[k];
+  }
 }
 
 // context length of the current state
