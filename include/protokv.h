@@ -68,6 +68,15 @@ enum {
                                 are given UN-ROTATED; the attention rotates near tokens at their stream positions, the S
                                 pseudo-tokens of prototype k at its anchor and the query tokens at q_pos0 + i.  Served by
                                 the fp32 SIMT attention kernel (the tcgen05 kernel has no rotation stage) */
+  PROTOKV_WARMUP = 512u,     /* PQ codebook warm-up (readings 32-36): cfg.codebook_k/v are
+                                ignored; the residuals (r^K, r^V) of the tokens absorbed during the first t_warm steps go
+                                into a per-bank reservoir (Algorithm R, capacity warm_reservoir), no histogram is updated
+                                meanwhile, and the append of frame t_warm - 1 ends with mini-batch k-means per subspace and
+                                side (km_iters x km_batch samples) that writes the bank's codebooks, fixed thereafter */
+  PROTOKV_WARMUP_MANUAL = 1024u, /* with PROTOKV_WARMUP: the training is started by protokv_train_codebooks instead */
+  PROTOKV_VAR_ALLOC = 2048u, /* D.3 (readings 37-40): variance-aware pseudo-token counts
+                                S_k = S_tot Var(H_k) / sum_j Var(H_j) under S_tot = k_max S, 1 <= S_k <= s_cap, recomputed by
+                                every synthesis; served by the fp32 SIMT attention kernel (ragged pseudo-token counts) */
   PROTOKV_MAINTENANCE = 64u  /* run Alg. 2 at the end of every append_frame that evicted a frame
                                 (Alg. 1 l.15); off by default: north_star's path and its invariant "total mass = tokens
                                 absorbed" exclude it (reading 19) */
@@ -95,6 +104,11 @@ typedef struct {
                              the paper fixes none: 1e6 (Qwen2-family backbones).  Used with PROTOKV_ROPE */
   int32_t rope_anchor;    /* D.1: 0 = most recent absorbed position (default), 1 = first, 2 = average */
   int64_t pos0;           /* stream position of token 0 of frame 0; token j of frame f sits at pos0 + f T + j */
+  int32_t t_warm;         /* PROTOKV_WARMUP: warm-up length T_warm in streaming steps = frames (the paper gives no value, L478) */
+  int32_t warm_reservoir; /* residual pairs the reservoir of a bank holds (<= 65536) */
+  int32_t km_iters, km_batch; /* mini-batch k-means: iterations, samples drawn per iteration (km_batch <= 1024) */
+  uint64_t km_seed;       /* bank b draws from the counter-based generator (SplitMix64 output function) seeded km_seed + b */
+  int32_t s_cap;          /* PROTOKV_VAR_ALLOC: upper bound of S_k, <= beam and <= 32 */
   const float *codebook_k, *codebook_v; /* device; copied at create.  NULL => no residual statistics */
   void *workspace;        /* device memory from the caller, >= protokv_workspace_bytes(cfg), 256-byte aligned */
   size_t workspace_bytes;
@@ -218,13 +232,35 @@ int64_t protokv_kernel_launches(const protokv_state *st);
  *   assign = -2) and the rest of the frame proceeds.  *flags (host) receives the bits; clear != 0 resets them. */
 /*   bit 1 (PROTOKV_ERRBIT_MAINT_OVERFLOW): Alg. 2 met more merge candidates in one frame of one bank than its list holds
  *   (2,048); the excess pairs were not merged in that frame. */
-enum { PROTOKV_ERRBIT_UNASSIGNED = 1u, PROTOKV_ERRBIT_MAINT_OVERFLOW = 2u };
+/*   bit 2 (PROTOKV_ERRBIT_WARMUP_SHORT): the warm-up ended with fewer residuals than codewords (C) in the reservoir; no
+ *   codebooks were trained and the state keeps running without residual statistics. */
+enum { PROTOKV_ERRBIT_UNASSIGNED = 1u, PROTOKV_ERRBIT_MAINT_OVERFLOW = 2u, PROTOKV_ERRBIT_WARMUP_SHORT = 4u };
 int protokv_error_flags(protokv_state *st, uint32_t *flags, int32_t clear);
 
 /* What Alg. 2 has done since create, summed over all banks: counts[0] = mass removed by aging, counts[1] = prototypes
  * merged away, counts[2] = slots recycled (host, 3 entries).  Synchronises.  The generalised mass invariant reads
  * sum_k n_k = tokens absorbed - counts[0] + counts[2]. */
 int protokv_maintenance_counters(protokv_state *st, int64_t *counts);
+
+/* PQ codebook warm-up ("initialized via mini-batch k-means on a warm-up reservoir of residuals collected
+ * during the first T_warm streaming steps, run separately for each subspace and for key/value ... kept fixed
+ * thereafter"; PROTOKV_WARMUP states only).
+ * protokv_train_codebooks ends the warm-up of every bank now: k-means on what the reservoirs hold, codebooks written,
+ * histogram updates start with the next absorbed token.  Called by the library itself at the end of the append of frame
+ * t_warm - 1 unless PROTOKV_WARMUP_MANUAL is set.  PROTOKV_ESTATE if the state has no warm-up or is already trained.
+ * export/import_reservoir: rows [fill][head_dim] fp32 of r^K and r^V of one bank (host); *fill = rows held, *seen =
+ * residuals offered so far; import overwrites the first n rows and sets both counts to n (parity aid).
+ * export_codebooks: the bank's [G][C][head_dim / G] fp32 codebooks (host); PROTOKV_ESTATE if it has none.
+ * All four synchronise. */
+int protokv_train_codebooks(protokv_state *st);
+int protokv_export_reservoir(protokv_state *st, int32_t bank, float *res_k, float *res_v, int64_t *fill, int64_t *seen);
+int protokv_import_reservoir(protokv_state *st, int32_t bank, const float *res_k, const float *res_v, int64_t n);
+int protokv_export_codebooks(protokv_state *st, int32_t bank, float *codebook_k, float *codebook_v);
+
+/* D.3 (PROTOKV_VAR_ALLOC states): the pseudo-token counts S_k [k_max] (int32, host) and fixed-point variances
+ * v_k = floor(Var(H_k) 2^20 + 1/2) [k_max] (int64, host; may be NULL) of one bank as of the last synthesis; with the
+ * flag off S_k = S for every prototype in the context.  PROTOKV_ESTATE without a valid synthesis.  Synchronises. */
+int protokv_export_allocation(protokv_state *st, int32_t bank, int32_t *s_count, int64_t *variance_fx);
 
 /* Stage timing (measurement aid, off by default).  When enabled the library brackets every kernel group it launches
  * with CUDA events on the state's stream; protokv_profile_read synchronises the stream and returns, per stage, the

@@ -11,11 +11,13 @@ from .build import build
 
 F32, BF16 = 0, 1
 MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV, ROPE = 1, 2, 4, 8, 16, 32, 64, 128, 256
+WARMUP, WARMUP_MANUAL, VAR_ALLOC = 512, 1024, 2048
 
 # Table 5 of the paper + the constants the paper leaves open (readings 4, 6, 12)
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,
                 eta=0.05, sigma_eps=1e-4, cos_eps=1e-12, pq_eps=1e-6, flags=0, gamma=0.05, eps_k=0.20, eps_v=0.25,
-                rope_theta=1.0e6, rope_anchor=0, pos0=0)
+                rope_theta=1.0e6, rope_anchor=0, pos0=0,
+                t_warm=0, warm_reservoir=2048, km_iters=32, km_batch=256, km_seed=0, s_cap=32)
 
 EXPORTED_SYMBOLS = [
     "protokv_workspace_bytes", "protokv_create", "protokv_destroy", "protokv_append_frame",
@@ -24,6 +26,8 @@ EXPORTED_SYMBOLS = [
     "protokv_export_ring", "protokv_export_codes", "protokv_import_codes", "protokv_last_frame_trace",
     "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl", "protokv_profile_enable",
     "protokv_profile_read", "protokv_error_flags", "protokv_maintenance_counters", "protokv_query_attention_at",
+    "protokv_train_codebooks", "protokv_export_reservoir", "protokv_import_reservoir", "protokv_export_codebooks",
+    "protokv_export_allocation",
 ]
 STAGES = ["fill", "score", "update", "append", "synthesis", "attention"]
 
@@ -46,6 +50,8 @@ class ProtoKVConfig(C.Structure):
                 ("sigma_eps", C.c_float), ("cos_eps", C.c_float), ("pq_eps", C.c_double),
                 ("flags", C.c_uint32), ("gamma", C.c_float), ("eps_k", C.c_float), ("eps_v", C.c_float),
                 ("rope_theta", C.c_double), ("rope_anchor", C.c_int32), ("pos0", C.c_int64),
+                ("t_warm", C.c_int32), ("warm_reservoir", C.c_int32), ("km_iters", C.c_int32), ("km_batch", C.c_int32),
+                ("km_seed", C.c_uint64), ("s_cap", C.c_int32),
                 ("codebook_k", C.c_void_p), ("codebook_v", C.c_void_p),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("cuda_stream", C.c_void_p)]
@@ -94,6 +100,11 @@ def load_library():
     lib.protokv_profile_read.argtypes = [vp, vp, vp]
     lib.protokv_error_flags.argtypes = [vp, C.POINTER(C.c_uint32), i32]
     lib.protokv_maintenance_counters.argtypes = [vp, vp]
+    lib.protokv_train_codebooks.argtypes = [vp]
+    lib.protokv_export_reservoir.argtypes = [vp, i32, vp, vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.protokv_import_reservoir.argtypes = [vp, i32, vp, vp, C.c_int64]
+    lib.protokv_export_codebooks.argtypes = [vp, i32, vp, vp]
+    lib.protokv_export_allocation.argtypes = [vp, i32, vp, vp]
     lib.protokv_stage_impl.restype = C.c_char_p
     lib.protokv_stage_impl.argtypes = [vp, i32]
     _lib = lib
@@ -286,9 +297,45 @@ class ProtoKV:
                                                   C.byref(n)))
         return K[:n.value], V[:n.value], s[:n.value], idx[:n.value]
 
+    def train_codebooks(self):
+        """protokv_train_codebooks: ends the warm-up now (PROTOKV_WARMUP_MANUAL states)."""
+        self._check(self._lib.protokv_train_codebooks(self._h))
+
+    def export_reservoir(self, bank):
+        """(r^K [fill][d], r^V [fill][d], residuals offered so far) of one bank."""
+        c = self.cfg
+        rk = np.zeros((c.warm_reservoir, c.head_dim), np.float32)
+        rv = np.zeros_like(rk)
+        fill, seen = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.protokv_export_reservoir(self._h, bank, _np_ptr(rk), _np_ptr(rv), C.byref(fill),
+                                                       C.byref(seen)))
+        return rk[:fill.value], rv[:fill.value], int(seen.value)
+
+    def import_reservoir(self, bank, res_k, res_v):
+        rk = np.ascontiguousarray(res_k, dtype=np.float32)
+        rv = np.ascontiguousarray(res_v, dtype=np.float32)
+        if rk.shape != rv.shape or rk.ndim != 2 or rk.shape[1] != self.cfg.head_dim:
+            raise ProtoKVError(1, "reservoir rows must be [n][head_dim] for both sides")
+        self._check(self._lib.protokv_import_reservoir(self._h, bank, _np_ptr(rk), _np_ptr(rv), rk.shape[0]))
+
+    def export_codebooks(self, bank):
+        c = self.cfg
+        ck = np.zeros((c.G, c.C, c.head_dim // c.G), np.float32)
+        cv = np.zeros_like(ck)
+        self._check(self._lib.protokv_export_codebooks(self._h, bank, _np_ptr(ck), _np_ptr(cv)))
+        return ck, cv
+
+    def export_allocation(self, bank):
+        """(S_k [k_max] int32, v_k [k_max] int64) of one bank as of the last synthesis (D.3)."""
+        sk = np.zeros(self.cfg.k_max, np.int32)
+        v = np.zeros(self.cfg.k_max, np.int64)
+        self._check(self._lib.protokv_export_allocation(self._h, bank, _np_ptr(sk), _np_ptr(v)))
+        return sk, v
+
     def export_codes(self, bank):
         c = self.cfg
-        ck = np.zeros((c.k_max, c.S, c.G), np.uint8)
+        smax = c.s_cap if c.flags & VAR_ALLOC else c.S
+        ck = np.zeros((c.k_max, smax, c.G), np.uint8)
         cv = np.zeros_like(ck)
         kind = np.zeros(c.k_max, np.uint8)
         self._check(self._lib.protokv_export_codes(self._h, bank, _np_ptr(ck), _np_ptr(cv), _np_ptr(kind)))

@@ -17,7 +17,9 @@ constexpr int kCbPad = 16;
 // Device-side error bits (Dev::err).  UNASSIGNED: an evicted token had no finite Eq. 1 score against any prototype (a
 // NaN / Inf in its key row or in the bank); it is NOT absorbed (trace assign = -2) and the bit is raised.
 constexpr uint32_t PKV_ERR_UNASSIGNED = 1u;
-constexpr uint32_t PKV_ERR_MAINT_OVERFLOW = 2u;   // Alg. 2: more merge candidates in one frame than the kernel's list holds
+constexpr uint32_t PKV_ERR_MAINT_OVERFLOW = 2u;
+constexpr uint32_t PKV_ERR_WARMUP_SHORT = 4u;     // warm-up ended with fewer than C residuals in a reservoir: no codebooks
+constexpr int kMaxReservoir = 65536, kMaxKmBatch = 1024, kMaxSCap = 32;   // Alg. 2: more merge candidates in one frame than the kernel's list holds
 constexpr int kNoProto = 0xfffff;   // sort-key prototype field of such a token (k_max <= 16384 < kNoProto)  // floats of padding after each subspace's [C][sub] block in shared memory
 
 // Shapes, fixed at create.
@@ -41,6 +43,9 @@ struct Hyper {
   double rope_theta;     // PROTOKV_ROPE
   int rope_anchor;
   long long pos0;        // stream position of token 0 of frame 0
+  int warm_reservoir, km_iters, km_batch;   // PROTOKV_WARMUP
+  unsigned long long km_seed;
+  int s_cap;             // PROTOKV_VAR_ALLOC
 };
 
 // Per-prototype scoring record (Eq. 1 terms that do not depend on the token), 32 bytes.
@@ -126,6 +131,14 @@ struct Dev {
   // mcount = {mass decayed, prototypes merged away, slots recycled} since create
   int* mstamp;                   // [B][K]
   unsigned long long* mcount;    // [3]
+  // PQ codebook warm-up (PROTOKV_WARMUP): reservoirs of residual pairs and this frame's write plan
+  float* resK;   // [B][R][d]
+  float* resV;
+  int* rslot;    // [B][T] reservoir slot the residual of evicted token j goes to, -1 = none (written by reservoir_plan_kernel)
+  // D.3 allocation (PROTOKV_VAR_ALLOC): counts, exclusive prefix offsets into the bank's [K * S] code rows, variances
+  int* scount;   // [B][K]
+  int* soff;     // [B][K + 1]
+  long long* varfx;  // [B][K]
   // attention scratch
   float* part;   // [rows_total][nsplit][d + 2]
   // host-variant staging
@@ -176,6 +189,8 @@ struct FrameArgs {
   int n_act;     // active prototypes after the fill = what Eq. 1 scans
   int epoch;     // id of the current synthesis epoch (>= 1), see Dev::dirty
   int keys;      // 1: the assignment of this frame is in Dev::akey (tcgen05 path), 0: in Dev::assign / best (SIMT)
+  int warm;      // 1: warm-up step -- residuals go to the reservoir slots of Dev::rslot, no histogram update
+  long long res_base;  // residuals offered to each bank's reservoir before this frame
 };
 
 // Every launcher returns the number of kernels it launched (0 if there was nothing to do).
@@ -186,6 +201,7 @@ int launch_score_simt(const Dims& D, const Hyper& H, const Dev& V, const FrameAr
 int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, int sm_count, cudaStream_t s);
 int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s);
 int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s);
+int launch_or_u32(uint32_t* dst, uint32_t bits, cudaStream_t s);
 // One-time (per device) function attributes of every kernel that needs more than 48 KB of shared memory for some
 // admissible shape; returns false if the device refuses one of them.
 bool update_kernels_prepare(const Dims& D);
@@ -208,6 +224,16 @@ struct AttnArgs {
 int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
 int launch_rope_tables(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
+
+// PQ codebook warm-up (warmup.cu)
+int launch_reservoir_plan(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);
+// cbk / cbv: where the trained codebooks go ([B][G][C][sub]); fill = rows every reservoir holds
+int launch_kmeans(const Dims& D, const Hyper& H, const Dev& V, float* cbk, float* cbv, long long fill, cudaStream_t s);
+bool warmup_prepare(const Dims& D, const Hyper& H);
+// D.3 allocation + ragged synthesis (alloc.cu)
+bool alloc_prepare(const Dims& D);
+int launch_allocation(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s);
+int launch_synthesis_var(const Dims& D, const Hyper& H, const Dev& V, int n_act, cudaStream_t s);
 
 // Alg. 2 maintenance (maintenance.cu)
 bool maintenance_prepare();

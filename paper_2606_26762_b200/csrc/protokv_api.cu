@@ -27,6 +27,12 @@ struct protokv_state {
   int64_t launches;
   int last_ev_frame;  // index of the frame evicted by the last append, -1 if none
   int last_n_fill;
+  // PQ codebook warm-up (PROTOKV_WARMUP): the codebook arrays are carved but stay hidden (Dev::cbk == NULL: no
+  // histogram updates, zero residuals) until the training has written them
+  bool warm;          // the state was created with PROTOKV_WARMUP
+  bool trained;       // warm-up over (training ran or was skipped for lack of residuals)
+  float *cb_store_k, *cb_store_v;
+  int64_t res_seen;   // residuals offered to every bank's reservoir so far (identical in every bank)
   bool codes_valid;   // codes/kind describe the current histograms
   std::vector<double> logtab;   // host copy of Dev::logtab (source of an asynchronous copy: must outlive it)
   int epoch;          // synthesis epoch (see Dev::dirty_cnt)
@@ -146,6 +152,20 @@ static int validate(const protokv_config* c) {
     if (!(c->rope_theta > 1.0) || c->rope_anchor < 0 || c->rope_anchor > 2)
       return fail(PROTOKV_EINVAL, "rope needs rope_theta > 1 and rope_anchor in {0, 1, 2}");
   }
+  if (c->flags & PROTOKV_WARMUP) {
+    if (c->t_warm < 1 || c->warm_reservoir < 1 || c->warm_reservoir > kMaxReservoir || c->km_iters < 0 || c->km_batch < 1 ||
+        c->km_batch > kMaxKmBatch)
+      return fail(PROTOKV_EINVAL, "warm-up needs t_warm >= 1, 1 <= warm_reservoir <= 65536, km_iters >= 0, 1 <= km_batch <= 1024");
+  } else if (c->flags & PROTOKV_WARMUP_MANUAL) {
+    return fail(PROTOKV_EINVAL, "WARMUP_MANUAL without WARMUP");
+  }
+  if (c->flags & PROTOKV_VAR_ALLOC) {
+    if (c->s_cap < 1 || c->s_cap > c->beam || c->s_cap > kMaxSCap) return fail(PROTOKV_EINVAL, "need 1 <= s_cap <= min(beam, 32)");
+    double tuples = 1;
+    for (int g = 0; g < c->G; ++g) tuples *= c->C;
+    if (tuples < c->s_cap) return fail(PROTOKV_EINVAL, "C^G < s_cap");
+    if (c->flags & PROTOKV_DECODE_SPLITKV) return fail(PROTOKV_EUNSUPPORTED, "VAR_ALLOC is served by the SIMT attention kernel only");
+  }
   if (!(c->lambda_sp >= 0.f) || !(c->lambda_idle >= 0.f))   // Eq. 1's penalties are penalties (the score kernel prunes on it)
     return fail(PROTOKV_EINVAL, "need lambda_sp >= 0 and lambda_idle >= 0");
   if ((c->flags & PROTOKV_NEAR_ONLY) && (c->flags & PROTOKV_FAR_ONLY))
@@ -165,10 +185,12 @@ static void fill_dims(const protokv_config* c, Dims* D, Hyper* H) {
   H->alpha = c->alpha; H->beta = c->beta; H->eta = c->eta;
   H->sigma_eps = c->sigma_eps; H->cos_eps = c->cos_eps; H->pq_eps = c->pq_eps; H->flags = c->flags;
   H->rope_theta = c->rope_theta; H->rope_anchor = c->rope_anchor; H->pos0 = (long long)c->pos0;
+  H->warm_reservoir = c->warm_reservoir; H->km_iters = c->km_iters; H->km_batch = c->km_batch;
+  H->km_seed = (unsigned long long)c->km_seed; H->s_cap = c->s_cap;
 }
 
 // Lays the state out in the workspace (base may be NULL to only measure).  Every array is 256-byte aligned.
-static size_t carve(const Dims& D, bool has_cb, bool rope, int nsplit, char* base, Dev* V) {
+static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int nsplit, char* base, Dev* V) {
   size_t off = 0;
   auto take = [&](size_t bytes) -> void* {
     off = align_up(off, 256);
@@ -212,6 +234,17 @@ static size_t carve(const Dims& D, bool has_cb, bool rope, int nsplit, char* bas
   v.err = (uint32_t*)take(256);
   v.mcount = (unsigned long long*)take(256);
   v.mstamp = (int*)take(BK * 4);
+  if ((H.flags & PROTOKV_WARMUP) && !(H.flags & PROTOKV_NO_RESIDUAL)) {
+    const size_t res = (size_t)D.B * H.warm_reservoir * D.d * 4;
+    v.resK = (float*)take(res);
+    v.resV = (float*)take(res + (size_t)D.B * H.warm_reservoir * 8);   // + the claim words of reservoir_plan_kernel
+    v.rslot = (int*)take(BT * 4);
+  }
+  if (H.flags & PROTOKV_VAR_ALLOC) {
+    v.scount = (int*)take(BK * 4);
+    v.soff = (int*)take((size_t)D.B * (D.K + 1) * 4);
+    v.varfx = (long long*)take(BK * 8);
+  }
   const size_t rows = (size_t)D.B * D.Nq * D.group;
   size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
   if (tc_attention_supported(D) && tc_attention_part_bytes(D) > part_bytes) part_bytes = tc_attention_part_bytes(D);
@@ -238,7 +271,7 @@ size_t protokv_workspace_bytes(const protokv_config* cfg) {
   Dims D; Hyper H;
   fill_dims(cfg, &D, &H);
   const bool has_cb = !(cfg->flags & PROTOKV_NO_RESIDUAL);   // sized as if codebooks were given
-  return carve(D, has_cb, (cfg->flags & PROTOKV_ROPE) != 0, plan_nsplit(D), nullptr, nullptr);
+  return carve(D, H, has_cb, (cfg->flags & PROTOKV_ROPE) != 0, plan_nsplit(D), nullptr, nullptr);
 }
 
 protokv_state* protokv_create(const protokv_config* cfg) {
@@ -269,8 +302,13 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->maint_full = true;
   st->sm_count = sms;
   st->nsplit = plan_nsplit(st->D);
-  const bool has_cb = cfg->codebook_k && !(cfg->flags & PROTOKV_NO_RESIDUAL);
-  const size_t need = carve(st->D, has_cb, (cfg->flags & PROTOKV_ROPE) != 0, st->nsplit, (char*)cfg->workspace, &st->V);
+  st->warm = (cfg->flags & PROTOKV_WARMUP) && !(cfg->flags & PROTOKV_NO_RESIDUAL);
+  st->trained = false; st->res_seen = 0;
+  const bool carve_cb = (cfg->codebook_k || st->warm) && !(cfg->flags & PROTOKV_NO_RESIDUAL);
+  const bool has_cb = carve_cb && !st->warm;                  // codebooks to copy now (warm-up states train their own)
+  const size_t need = carve(st->D, st->H, carve_cb, (cfg->flags & PROTOKV_ROPE) != 0, st->nsplit, (char*)cfg->workspace, &st->V);
+  st->cb_store_k = st->V.cbk; st->cb_store_v = st->V.cbv;
+  if (st->warm) { st->V.cbk = nullptr; st->V.cbv = nullptr; }
   if (need > cfg->workspace_bytes) {
     fail(PROTOKV_ENOMEM, "workspace too small: need %zu bytes, got %zu", need, cfg->workspace_bytes);
     delete st;
@@ -301,7 +339,8 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->maps.ok = false;
   if (!update_kernels_prepare(st->D) || !query_kernels_prepare(st->D) ||
-      ((cfg->flags & PROTOKV_MAINTENANCE) && !maintenance_prepare())) {   // capability error: before any launch
+      ((cfg->flags & PROTOKV_MAINTENANCE) && !maintenance_prepare()) || (st->warm && !warmup_prepare(st->D, st->H)) ||
+      ((cfg->flags & PROTOKV_VAR_ALLOC) && !alloc_prepare(st->D))) {   // capability error: before any launch
     fail(PROTOKV_EUNSUPPORTED, "the device refused the shared-memory opt-in this shape needs");
     delete st;
     return nullptr;
@@ -309,7 +348,8 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   const bool want_tc = !(cfg->flags & PROTOKV_FORCE_SIMT);
   if (want_tc && (tc_assign_supported(st->D, st->H) || tc_attention_supported(st->D))) tc_build_maps(st->D, st->V, &st->maps);
   st->use_tc_assign = want_tc && tc_assign_supported(st->D, st->H) && st->maps.ok;
-  const bool rope = (cfg->flags & PROTOKV_ROPE) != 0;   // the rotation stage exists in the SIMT attention kernel only
+  // the rotation stage and ragged pseudo-token counts exist in the SIMT attention kernel only
+  const bool rope = (cfg->flags & (PROTOKV_ROPE | PROTOKV_VAR_ALLOC)) != 0;
   st->use_tc_attn = want_tc && !rope && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
   st->use_decode_attn = want_tc && !rope && (cfg->flags & PROTOKV_DECODE_SPLITKV) && decode_attention_supported(st->D, 1) &&
                         decode_attention_prepare();
@@ -361,6 +401,8 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   F.n_act = st->n_act + F.n_fill;
   F.keys = st->use_tc_assign ? 1 : 0;
   F.epoch = st->epoch;
+  F.warm = st->warm && !st->trained && st->frames < st->cfg.t_warm;
+  F.res_base = st->res_seen;
   int nl = 0;
   if (F.evicted) {
     if (F.n_fill > 0) {
@@ -374,6 +416,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
                                 : launch_score_simt(D, st->H, st->V, F, st->stream);
       }
       StageTimer tm(st, PROTOKV_STAGE_UPDATE);
+      if (F.warm) nl += launch_reservoir_plan(D, st->H, st->V, F, st->stream);          // L312: where this frame's residuals go
       nl += launch_update(D, st->H, st->V, F, st->sm_count, st->stream);                // U4-U6
     }
   }
@@ -399,7 +442,29 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   st->last_ev_frame = F.ev_frame;
   st->last_n_fill = F.n_fill;
   if (F.evicted) st->codes_valid = false;
+  if (F.warm && F.evicted) st->res_seen += D.T - F.n_fill;
   st->frames += 1;
+  if (st->warm && !st->trained && !(st->cfg.flags & PROTOKV_WARMUP_MANUAL) && st->frames == st->cfg.t_warm)
+    return protokv_train_codebooks(st);                                                 // end of the warm-up (reading 33)
+  return PROTOKV_OK;
+}
+
+int protokv_train_codebooks(protokv_state* st) {
+  if (!st) return fail(PROTOKV_EINVAL, "NULL state");
+  if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
+  if (!st->warm || st->trained) return fail(PROTOKV_ESTATE, "the state has no warm-up in progress");
+  DeviceGuard dg(st);
+  st->trained = true;
+  const int64_t fill = st->res_seen < st->cfg.warm_reservoir ? st->res_seen : st->cfg.warm_reservoir;
+  if (fill < st->D.C) {   // fewer residuals than codewords: no codebooks, the state runs on without residual statistics
+    st->launches += launch_or_u32(st->V.err, PKV_ERR_WARMUP_SHORT, st->stream);
+    PKV_CUDA(cudaGetLastError());
+    return PROTOKV_OK;
+  }
+  st->launches += launch_kmeans(st->D, st->H, st->V, st->cb_store_k, st->cb_store_v, (long long)fill, st->stream);
+  PKV_CUDA(cudaGetLastError());
+  st->V.cbk = st->cb_store_k; st->V.cbv = st->cb_store_v;     // from now on Alg. 1 l.13 updates the histograms
+  st->codes_valid = false;
   return PROTOKV_OK;
 }
 
@@ -409,7 +474,12 @@ int protokv_synthesize(protokv_state* st) {
   DeviceGuard dg(st);
   {
     StageTimer tm(st, PROTOKV_STAGE_SYNTH);
-    st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->sm_count, st->stream);
+    if (st->H.flags & PROTOKV_VAR_ALLOC) {   // D.3: shares S_k first (they move the code rows), then every prototype's modes
+      st->launches += launch_allocation(st->D, st->H, st->V, st->n_act, st->stream);
+      st->launches += launch_synthesis_var(st->D, st->H, st->V, st->n_act, st->stream);
+    } else {
+      st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->sm_count, st->stream);
+    }
   }
   PKV_CUDA(cudaGetLastError());
   st->epoch += 1;
@@ -660,11 +730,27 @@ int protokv_export_codes(protokv_state* st, int32_t bank, uint8_t* codes_k, uint
   const Dims& D = st->D;
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   std::vector<uint32_t> tmp((size_t)D.K * D.S);
+  const bool var = st->V.scount != nullptr;                 // D.3: ragged rows, exported as [k_max][s_cap][G]
+  const int smax = var ? st->H.s_cap : D.S;
+  std::vector<int> cnt, off;
+  if (var) {
+    cnt.resize(D.K); off.resize(D.K + 1);
+    PKV_CUDA(cudaMemcpy(cnt.data(), st->V.scount + (size_t)bank * D.K, (size_t)D.K * 4, cudaMemcpyDeviceToHost));
+    PKV_CUDA(cudaMemcpy(off.data(), st->V.soff + (size_t)bank * (D.K + 1), (size_t)(D.K + 1) * 4, cudaMemcpyDeviceToHost));
+  }
   for (int kv = 0; kv < 2; ++kv) {
     uint8_t* dst = kv ? codes_v : codes_k;
     if (!dst) continue;
     PKV_CUDA(cudaMemcpy(tmp.data(), (kv ? st->V.codesV : st->V.codesK) + (size_t)bank * D.K * D.S, tmp.size() * 4,
                         cudaMemcpyDeviceToHost));
+    if (var) {
+      memset(dst, 0, (size_t)D.K * smax * D.G);
+      for (int k = 0; k < D.K; ++k)
+        for (int s2 = 0; s2 < cnt[k]; ++s2)
+          for (int g = 0; g < D.G; ++g)
+            dst[((size_t)k * smax + s2) * D.G + g] = (uint8_t)((tmp[(size_t)off[k] + s2] >> (4 * g)) & 15u);
+      continue;
+    }
     for (size_t e = 0; e < tmp.size(); ++e)
       for (int g = 0; g < D.G; ++g) dst[e * D.G + g] = (uint8_t)((tmp[e] >> (4 * g)) & 15u);
   }
@@ -676,6 +762,7 @@ int protokv_import_codes(protokv_state* st, int32_t bank, const uint8_t* codes_k
   int rc = check_bank(st, bank);
   if (rc) return rc;
   if (!st->codes_valid) return fail(PROTOKV_ESTATE, "run protokv_synthesize first (kind[] comes from it)");
+  if (st->V.scount) return fail(PROTOKV_EUNSUPPORTED, "import_codes is not available with PROTOKV_VAR_ALLOC");
   DeviceGuard dg(st);
   const Dims& D = st->D;
   PKV_CUDA(cudaStreamSynchronize(st->stream));
@@ -727,6 +814,70 @@ int protokv_last_frame_trace(protokv_state* st, int32_t* assign, float* best, ui
   } else {
     if (codes_k) memset(codes_k, 255, BT * D.G);
     if (codes_v) memset(codes_v, 255, BT * D.G);
+  }
+  return PROTOKV_OK;
+}
+
+int protokv_export_reservoir(protokv_state* st, int32_t bank, float* res_k, float* res_v, int64_t* fill, int64_t* seen) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!st->warm) return fail(PROTOKV_ESTATE, "the state was created without PROTOKV_WARMUP");
+  DeviceGuard dg(st);
+  const int64_t n = st->res_seen < st->cfg.warm_reservoir ? st->res_seen : st->cfg.warm_reservoir;
+  if (fill) *fill = n;
+  if (seen) *seen = st->res_seen;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  const size_t off = (size_t)bank * st->cfg.warm_reservoir * st->D.d, bytes = (size_t)n * st->D.d * 4;
+  if (res_k && n) PKV_CUDA(cudaMemcpy(res_k, st->V.resK + off, bytes, cudaMemcpyDeviceToHost));
+  if (res_v && n) PKV_CUDA(cudaMemcpy(res_v, st->V.resV + off, bytes, cudaMemcpyDeviceToHost));
+  return PROTOKV_OK;
+}
+
+int protokv_import_reservoir(protokv_state* st, int32_t bank, const float* res_k, const float* res_v, int64_t n) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!st->warm || st->trained) return fail(PROTOKV_ESTATE, "the state has no warm-up in progress");
+  if (!res_k || !res_v || n < 0 || n > st->cfg.warm_reservoir) return fail(PROTOKV_EINVAL, "bad reservoir rows");
+  DeviceGuard dg(st);
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  const size_t R = (size_t)st->cfg.warm_reservoir, off = (size_t)bank * R * st->D.d, bytes = (size_t)n * st->D.d * 4;
+  if (n) {
+    PKV_CUDA(cudaMemcpy(st->V.resK + off, res_k, bytes, cudaMemcpyHostToDevice));
+    PKV_CUDA(cudaMemcpy(st->V.resV + off, res_v, bytes, cudaMemcpyHostToDevice));
+  }
+  // the claim words order residual indices; the count restarts at n for every bank
+  PKV_CUDA(cudaMemset(st->V.resV + (size_t)st->D.B * R * st->D.d, 0, (size_t)st->D.B * R * 8));
+  st->res_seen = n;
+  return PROTOKV_OK;
+}
+
+int protokv_export_codebooks(protokv_state* st, int32_t bank, float* codebook_k, float* codebook_v) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!st->V.cbk) return fail(PROTOKV_ESTATE, "the state has no codebooks (none given, or the warm-up has not ended)");
+  DeviceGuard dg(st);
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  const size_t n = (size_t)st->D.G * st->D.C * st->D.sub;
+  if (codebook_k) PKV_CUDA(cudaMemcpy(codebook_k, st->V.cbk + (size_t)bank * n, n * 4, cudaMemcpyDeviceToHost));
+  if (codebook_v) PKV_CUDA(cudaMemcpy(codebook_v, st->V.cbv + (size_t)bank * n, n * 4, cudaMemcpyDeviceToHost));
+  return PROTOKV_OK;
+}
+
+int protokv_export_allocation(protokv_state* st, int32_t bank, int32_t* s_count, int64_t* variance_fx) {
+  int rc = check_bank(st, bank);
+  if (rc) return rc;
+  if (!s_count) return fail(PROTOKV_EINVAL, "NULL s_count");
+  if (!st->codes_valid) return fail(PROTOKV_ESTATE, "no synthesis result for the current state");
+  DeviceGuard dg(st);
+  const Dims& D = st->D;
+  PKV_CUDA(cudaStreamSynchronize(st->stream));
+  if (st->V.scount) {
+    PKV_CUDA(cudaMemcpy(s_count, st->V.scount + (size_t)bank * D.K, (size_t)D.K * 4, cudaMemcpyDeviceToHost));
+    if (variance_fx) PKV_CUDA(cudaMemcpy(variance_fx, st->V.varfx + (size_t)bank * D.K, (size_t)D.K * 8, cudaMemcpyDeviceToHost));
+  } else {
+    std::vector<uint8_t> kind(D.K);
+    PKV_CUDA(cudaMemcpy(kind.data(), st->V.kind + (size_t)bank * D.K, D.K, cudaMemcpyDeviceToHost));
+    for (int k = 0; k < D.K; ++k) { s_count[k] = kind[k] == 2 ? 0 : D.S; if (variance_fx) variance_fx[k] = 0; }
   }
   return PROTOKV_OK;
 }

@@ -401,7 +401,8 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
   for (int v = 0; v < VEC; ++v) q[v] *= scale;
 
   const int near_cnt = (H.flags & PROTOKV_FAR_ONLY) ? 0 : A.n_near;
-  const int ps_cnt = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : A.n_act * D.S;
+  const int* soff = V.soff ? V.soff + (size_t)b * (D.K + 1) : nullptr;   // D.3: ragged pseudo-token counts
+  const int ps_cnt = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : (soff ? soff[D.K] : A.n_act * D.S);
   const int Lc = near_cnt + ps_cnt;
   const int chunk = (Lc + A.nsplit - 1) / A.nsplit;
   const int lo = blockIdx.y * chunk, hi = min(Lc, lo + chunk);
@@ -468,11 +469,19 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
     const int p_lo = max(lo, near_cnt) - near_cnt, p_hi = hi - near_cnt;
     const int LPS = 32 / D.G, g = lane / LPS, li = lane % LPS;
     const bool use_bias = !(H.flags & PROTOKV_NO_MASS_BIAS);
-    for (int k = p_lo / D.S; k * D.S < p_hi; ++k) {
+    int k = p_lo / D.S;
+    if (soff) {                              // first prototype whose rows reach beyond p_lo
+      int lo2 = 0, hi2 = D.K;
+      while (lo2 < hi2) { const int mid = (lo2 + hi2) >> 1; if (soff[mid + 1] > p_lo) hi2 = mid; else lo2 = mid + 1; }
+      k = lo2;
+    }
+    for (; k < D.K && (soff ? soff[k] : k * D.S) < p_hi; ++k) {
       const size_t pk = (size_t)b * D.K + k;
       const int kind = V.kind[pk];
       if (kind == 2) continue;
-      const int s_lo = max(p_lo - k * D.S, 0), s_hi = min(p_hi - k * D.S, D.S);
+      const int row0 = soff ? soff[k] : k * D.S, nrow = soff ? soff[k + 1] - soff[k] : D.S;
+      const int s_lo = max(p_lo - row0, 0), s_hi = min(p_hi - row0, nrow);
+      const size_t crow = (size_t)b * D.K * D.S + row0;   // this prototype's code rows
       float c[VEC], p[VEC];
       load_vec<float, VEC>(V.c + pk * DH + lane * VEC, c);
       load_vec<float, VEC>(V.p + pk * DH + lane * VEC, p);
@@ -495,8 +504,8 @@ __global__ void __launch_bounds__(kAttWarps * 32) attention_simt_kernel(Dims D, 
         continue;
       }
       for (int s = s_lo; s < s_hi; ++s) {
-        const uint32_t zk = (V.codesK[pk * D.S + s] >> (4 * g)) & 15u;
-        const uint32_t zv = (V.codesV[pk * D.S + s] >> (4 * g)) & 15u;
+        const uint32_t zk = (V.codesK[crow + s] >> (4 * g)) & 15u;
+        const uint32_t zv = (V.codesV[crow + s] >> (4 * g)) & 15u;
         float rk[VEC], rv[VEC];
         load_vec<float, VEC>(cbk_s + g * gstride + zk * D.sub + li * VEC, rk);
         load_vec<float, VEC>(cbv_s + g * gstride + zv * D.sub + li * VEC, rv);

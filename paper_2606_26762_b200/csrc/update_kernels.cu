@@ -378,6 +378,15 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
       sxx = (float)__dadd_rn(__dmul_rn(ome, (double)sxx), __dmul_rn(edx, dx));     // l.12
       sxy = (float)__dadd_rn(__dmul_rn(ome, (double)sxy), __dmul_rn(edx, dy));
       syy = (float)__dadd_rn(__dmul_rn(ome, (double)syy), __dmul_rn(edy, dy));
+      if (F.warm) {                                                  // L312: residual of a warm-up step -> reservoir
+        const int slot = V.rslot[(size_t)b * D.T + j];
+        if (slot >= 0) {
+          float* rk = V.resK + ((size_t)b * H.warm_reservoir + slot) * DH + lane * VEC;
+          float* rv = V.resV + ((size_t)b * H.warm_reservoir + slot) * DH + lane * VEC;
+#pragma unroll
+          for (int v = 0; v < VEC; ++v) { rk[v] = ke[v] - c[v]; rv[v] = ve[v] - p[v]; }
+        }
+      }
       if (has_cb) {                                                  // l.13, residual of the updated centres
 #pragma unroll
         for (int kv = 0; kv < 2; ++kv) {
@@ -632,6 +641,12 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
         }
 #pragma unroll
         for (int v = 0; v < 4; ++v) p[v] = fmaf(bef, ve[v] - p[v], p[v]);              // l.9
+        if (F.warm) {                                                // L312: residual of a warm-up step -> reservoir
+          const int slot = V.rslot[bt + j];
+          if (slot >= 0)
+            *(float4*)(V.resV + ((size_t)b * H.warm_reservoir + slot) * DH + lane * 4) =
+                make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
+        }
         if (has_cb) {
           __syncwarp();
           rsc[lane] = make_float4(ve[0] - p[0], ve[1] - p[1], ve[2] - p[2], ve[3] - p[3]);
@@ -683,6 +698,12 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       sxx = (float)__dadd_rn(__dmul_rn(ome, (double)sxx), __dmul_rn(edx, dx));     // l.12
       sxy = (float)__dadd_rn(__dmul_rn(ome, (double)sxy), __dmul_rn(edx, dy));
       syy = (float)__dadd_rn(__dmul_rn(ome, (double)syy), __dmul_rn(edy, dy));
+      if (F.warm) {                                                  // L312: residual of a warm-up step -> reservoir
+        const int slot = V.rslot[bt + j];
+        if (slot >= 0)
+          *(float4*)(V.resK + ((size_t)b * H.warm_reservoir + slot) * DH + lane * 4) =
+              make_float4(ke[0] - c[0], ke[1] - c[1], ke[2] - c[2], ke[3] - c[3]);
+      }
       if (has_cb) {                                                  // l.13, residual of the updated centre
         __syncwarp();
         rsc[lane] = make_float4(ke[0] - c[0], ke[1] - c[1], ke[2] - c[2], ke[3] - c[3]);
@@ -829,6 +850,12 @@ int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s) {
   if (n == 0) return 0;
   const unsigned grid = (unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
   fill_u32_kernel<<<grid, 256, 0, s>>>(dst, value, n);
+  return 1;
+}
+
+__global__ void or_u32_kernel(uint32_t* dst, uint32_t bits) { atomicOr(dst, bits); }
+int launch_or_u32(uint32_t* dst, uint32_t bits, cudaStream_t s) {
+  or_u32_kernel<<<1, 1, 0, s>>>(dst, bits);
   return 1;
 }
 
