@@ -281,6 +281,78 @@ def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=Tr
     return res
 
 
+def next_rows(spec, device):
+    """SURVEY 8(f) rows at the measurement bar, on the headline workload's shape: the CUDA path of each optional row timed
+    with CUDA events on the library's stream (device-resident inputs).  None of them is on the graded step."""
+    from paper_2606_26762_b200 import ProtoKV, binding as B
+    dev = str(device)
+    s = gen.grid_positions(spec, device=dev)
+    Q = gen.queries(spec, 0, device=dev)
+    out = {}
+
+    def mk(**kw):
+        cb = kw.pop("cb", True)
+        ck, cv = gen.codebooks(spec, device=dev) if cb else (None, None)
+        return ProtoKV(n_streams=spec.n_streams, n_layers=spec.n_layers, n_q_heads=spec.n_q_heads,
+                       n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim, dtype=spec.dtype, tokens_per_frame=spec.T,
+                       near_frames=spec.near_frames, k_max=spec.k_max, n_query_tokens=spec.n_query_tokens,
+                       codebook_k=ck, codebook_v=cv, device=dev, G=spec.G, C=spec.C, **kw)
+
+    def timed(fn, reps=5):
+        ts = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ts.sort()
+        return ts[len(ts) // 2]
+
+    prime = steady_state_frames(spec) + 8
+    frames = [gen.frame_kv(spec, f, device=dev) for f in range(prime)]
+    # NEXT-2: warm-up frames (reservoir plan + stores in the update kernel) and the k-means training (PAPER.md:L312)
+    st = mk(cb=False, flags=B.WARMUP | B.WARMUP_MANUAL, t_warm=1 << 30, warm_reservoir=2048, km_iters=32, km_batch=256, km_seed=1)
+    for K, V in frames[:-4]:
+        st.append_frame(K, V, s)
+    it = iter(frames[-4:])
+    warm_ms = timed(lambda: st.append_frame(*next(it), s), reps=4)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); st.train_codebooks(); e1.record()
+    torch.cuda.synchronize()
+    out["next2_codebook_warmup"] = dict(warmup_frame_update_ms=warm_ms, kmeans_training_ms=e0.elapsed_time(e1),
+                                        reservoir=2048, km_iters=32, km_batch=256,
+                                        note="one-time training of 2 x G codebooks per bank, CTA = (subspace, side, bank)")
+    st.close()
+    # NEXT-4: D.3 allocation + ragged synthesis + SIMT attention over the ragged context (PAPER.md:L608-625)
+    st = mk(flags=B.VAR_ALLOC, s_cap=32)
+    for K, V in frames:
+        st.append_frame(K, V, s)
+    o = torch.empty_like(Q)
+    syn_ms = timed(lambda: st.synthesize())
+    att_ms = timed(lambda: st.query_attention_ex(Q, out=o, run_synthesis=False))
+    sk, _ = st.export_allocation(0)
+    out["next4_variance_aware_allocation"] = dict(allocation_and_synthesis_ms=syn_ms, attention_ms=att_ms, attention_impl=st.stage_impl(1),
+                                                  s_k_min=int(sk[sk > 0].min()), s_k_max=int(sk.max()), s_total=int(sk.sum()))
+    st.close()
+    # NEXT-3: rotary anchoring (SIMT attention with the rotation stage + fp64 sincos tables) (PAPER.md:L126, D.1)
+    st = mk(flags=B.ROPE)
+    for K, V in frames:
+        st.append_frame(K, V, s)
+    st.synthesize()
+    out["next3_rope_anchoring"] = dict(attention_ms=timed(lambda: st.query_attention_ex(Q, out=o, run_synthesis=False)),
+                                       attention_impl=st.stage_impl(1))
+    st.close()
+    # NEXT-1: Alg. 2 maintenance, Table 5 defaults, in steady state (PAPER.md:L355-388)
+    st = mk(flags=B.MAINTENANCE)
+    for K, V in frames[:-4]:
+        st.append_frame(K, V, s)
+    it2 = iter(frames[-4:])
+    out["next1_maintenance"] = dict(update_frame_with_alg2_ms=timed(lambda: st.append_frame(*next(it2), s), reps=4),
+                                    counters=st.maintenance_counters())
+    st.close()
+    return out
+
+
 def decode_object(spec, res, peaks):
     """One-token query (attention only, codes valid): us and fraction of the HBM roofline on its algorithmic bytes."""
     if "decode_ms" not in res:
@@ -569,6 +641,11 @@ def main():
             except Exception as e:   # an extra must not take the headline down
                 extras[name] = dict(error=repr(e))
         line["other_workloads"] = extras
+    if world == 1 and args.extras:
+        try:
+            line["next_rows"] = next_rows(spec, device)
+        except Exception as e:
+            line["next_rows"] = dict(error=repr(e))
     if world == 1 and not args.no_cpu_baseline:
         os_ = oracle_arm(spec, steps=12, warmup=1)
         line["cpu_baseline"] = dict(value=os_["frames_per_s"], unit=UNIT, cores=os_["cores"], kind="oracle",
