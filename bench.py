@@ -246,6 +246,7 @@ def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=Tr
             ts.append(e0.elapsed_time(e1))
         ts.sort()
         res["decode_ms"] = ts[len(ts) // 2]
+        res["decode_impl"] = st.stage_impl(2)
 
     if do_profile:   # per-kernel durations: same steps again with the library's stage events switched on
         st.profile_enable(True)
@@ -353,18 +354,26 @@ def next_rows(spec, device):
     return out
 
 
+def decode_bytes(spec, e_c):
+    """Algorithmic bytes of a one-token query (SURVEY 8(d) query formula with rows = the GQA group): near K, V rows, the
+    centres at e_c bytes per element (2 = the bf16 copies the decode kernel streams, 4 = the fp32 state), codes, masses."""
+    elt = 2 if spec.dtype == "bf16" else 4
+    W = spec.near_frames * spec.T
+    rows = spec.n_q_heads // spec.n_kv_heads
+    per_bank = 2 * W * spec.head_dim * elt + spec.k_max * (2 * spec.head_dim * e_c + 8 * spec.G + 4) + 2 * rows * spec.head_dim * elt
+    return per_bank * spec.n_banks
+
+
 def decode_object(spec, res, peaks):
     """One-token query (attention only, codes valid): us and fraction of the HBM roofline on its algorithmic bytes."""
     if "decode_ms" not in res:
         return None
-    elt = 2 if spec.dtype == "bf16" else 4
-    W = spec.near_frames * spec.T
-    rows = spec.n_q_heads // spec.n_kv_heads
-    per_bank = 2 * W * spec.head_dim * elt + spec.k_max * (2 * spec.head_dim * 4 + 8 * spec.G + 4) + 2 * rows * spec.head_dim * elt
-    b = per_bank * spec.n_banks
+    e_c = 2 if res.get("decode_impl", "").startswith("mma.sync register") else 4
+    b = decode_bytes(spec, e_c)
     gbs = b / (res["decode_ms"] * 1e-3) / 1e9
-    return dict(n_query_tokens=1, attention_us=res["decode_ms"] * 1e3, algorithmic_bytes=b, bound="hbm", achieved=gbs,
-                unit="GB/s", peak=peaks["hbm"], frac=gbs / peaks["hbm"])
+    return dict(n_query_tokens=1, attention_us=res["decode_ms"] * 1e3, algorithmic_bytes=b, centre_bytes_per_element=e_c,
+                bound="hbm", achieved=gbs, unit="GB/s", peak=peaks["hbm"], frac=gbs / peaks["hbm"],
+                impl=res.get("decode_impl"), roofline_us=b / peaks["hbm"] / 1e3)
 
 
 def tensor_peak(peaks, clocks):

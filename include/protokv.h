@@ -68,6 +68,8 @@ enum {
                                 are given UN-ROTATED; the attention rotates near tokens at their stream positions, the S
                                 pseudo-tokens of prototype k at its anchor and the query tokens at q_pos0 + i.  Served by
                                 the fp32 SIMT attention kernel (the tcgen05 kernel has no rotation stage) */
+  PROTOKV_NO_DECODE_KERNEL = 4096u, /* serve queries of <= 16 rows per bank with the 128-row tcgen05 kernel instead of
+                                the register-resident decode kernel (csrc/decode_attention2.cu, the default): cross-check */
   PROTOKV_WARMUP = 512u,     /* PQ codebook warm-up (readings 32-36): cfg.codebook_k/v are
                                 ignored; the residuals (r^K, r^V) of the tokens absorbed during the first t_warm steps go
                                 into a per-bank reservoir (Algorithm R, capacity warm_reservoir), no histogram is updated

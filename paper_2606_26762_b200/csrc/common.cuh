@@ -90,6 +90,8 @@ struct Dev {
   float* p;
   __nv_bfloat16* c_hi;  // [B][K][d] bf16 shadows (bf16 mode): c = c_hi + c_lo + O(2^-17 |c|)
   __nv_bfloat16* c_lo;
+  __nv_bfloat16* c_bf;  // [B][K][d] bf16(c), bf16(p): what the decode-style attention streams (bf16, d = 128 states);
+  __nv_bfloat16* p_bf;  // rewritten by whoever rewrites c / p
   int* n;        // [B][K]
   float* mu;     // [B][K][2]
   float* sigma;  // [B][K][3]
@@ -246,6 +248,12 @@ size_t decode_attention_part_bytes(const Dims& D);
 bool decode_attention_prepare();
 int launch_attention_decode(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
                             int* nsplit_out);
+// register-resident decode kernel (decode_attention2.cu): the default for n_q * group <= 16 rows per bank
+bool decode2_attention_supported(const Dims& D, int n_q);
+bool decode2_attention_prepare();
+int decode2_max_splits();
+int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
+                             int* nsplit_out);
 // merges A.nsplit partials per row ([rows][nsplit][d + 2] in Dev::part) into out / lse (bf16, d = 128)
 int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, cudaStream_t s);
 

@@ -1,0 +1,468 @@
+// Q2 fused attention for DECODE-STYLE queries, register-resident variant (bf16, d = 128, S = 8, G = 8, C = 16,
+// n_q * group <= 16 query rows per bank): Alg. 4 l.8-15 / Eq. 4 (L574: the bounded attention
+// over W + K_max S tokens is the only ProtoKV work on the latency of a query).  For a handful of rows that is ~2.7 MB per
+// bank streamed once, i.e. HBM time; the kernel is built so that nothing but those bytes moves:
+//
+//   * every warp is its own flash-decoding worker over a strided share of the bank's context, with NO shared-memory
+//     operand staging and no block barrier in the loop: mma.sync m16n8k16 B fragments are filled straight from global
+//     memory.  The contraction index of Q K^T may be permuted freely, so a lane's four 16-byte loads of a key row are
+//     contiguous 64-byte pieces (chunk q = j + 4c holds dims [8q, 8q + 8) = k-steps 2c and 2c + 1); Q's A fragments use
+//     the same permutation.  For P V the output dims are permuted instead (MMA column n of tile i = dim 16 n + i), so a
+//     lane reads the 32 contiguous bytes [16 g, 16 g + 16) of each of its four value rows and two PRMTs per tile pair
+//     the tokens up;
+//   * pseudo-tokens k~ = c_k + concat_g CK_g[z], v~ = p_k + concat_g CV_g[z] (Alg. 4 l.5-9) exist only as B fragments:
+//     the lane takes its chunks of bf16(c_k) / bf16(p_k) (copies kept by the update path), adds its 16-byte pieces of the selected codewords
+//     from a 4 KB bf16 codebook in shared memory (add.rn.bf16x2 -- the same rounding as the tcgen05 kernel's builders),
+//     and feeds the MMA.  With the value-side dim permutation a lane's dims [16 g, 16 g + 16) are exactly PQ subspace g;
+//   * online softmax in the accumulator fragments (exp2 domain, log-mass bias log2 n_k on pseudo columns, Eq. 2/4), P
+//     re-used from the accumulators as the A fragment of P V (FlashAttention-2 register reuse).
+// A CTA's four warps merge their (m, l, O) through shared memory and write one unnormalised partial per query row;
+// attention_combine_kernel (query_kernels.cu) merges the nsplit partials of a row.
+#include "common.cuh"
+
+namespace pkv {
+
+constexpr int kD2Threads = 128, kD2Warps = 4;
+constexpr int kD2Rows = 16;
+constexpr int kD2CtasPerSm = 2;
+constexpr float kD2Log2e = 1.4426950408889634f;
+constexpr float kD2Ln2 = 0.6931471805599453f;
+constexpr float kD2Slack = 8.f;
+
+struct D2Smem {
+  static constexpr uint32_t CBK = 0;                     // [G][C][16] bf16 = 128 rows x 32 B
+  static constexpr uint32_t CBV = 4096;                  // the same at a 48-byte pitch: a quarter warp gathers up to 8 different
+                                                         // value codewords, which then fall into different bank groups
+  static constexpr uint32_t O = 10240;                    // [4 warps][16 rows][128] fp32 (re-uses the operand ring)
+  static constexpr uint32_t ML = O + 4 * 16 * 128 * 4;   // [4][16][2] fp32
+  static constexpr uint32_t Total = ML + 4 * 16 * 2 * 4;
+};
+
+struct D2Args {
+  const __nv_bfloat16* Q;
+  float* part;              // [(bsel * R + row) * nsplit + split][130]
+  int n_q, layer_begin, layer_count;
+  int n_near, n_act;
+  int use_bias;
+  int nsplit;
+  int R;                    // n_q * group
+};
+
+__device__ __forceinline__ void d2_mma(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+               "{%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t d2_pack(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ uint32_t d2_add2(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("add.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+__device__ __forceinline__ float d2_ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t d2_prmt(uint32_t a, uint32_t b, uint32_t sel) {
+  uint32_t r;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+  return r;
+}
+__device__ __forceinline__ uint4 d2_ldg16(const void* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ uint4 d2_add2x4(uint4 a, uint4 b) {
+  return make_uint4(d2_add2(a.x, b.x), d2_add2(a.y, b.y), d2_add2(a.z, b.z), d2_add2(a.w, b.w));
+}
+// 8 consecutive fp32 -> 4 bf16x2
+__device__ __forceinline__ uint4 d2_cvt8(const float* p) {
+  const float4 f0 = __ldg(reinterpret_cast<const float4*>(p)), f1 = __ldg(reinterpret_cast<const float4*>(p) + 1);
+  return make_uint4(d2_pack(f0.x, f0.y), d2_pack(f0.z, f0.w), d2_pack(f1.x, f1.y), d2_pack(f1.z, f1.w));
+}
+
+// Per-warp flash-decoding state: rows g and g + 8 of the 16-row MMA tile.
+struct D2Soft {
+  float m0, m1, l0, l1;
+};
+
+// One step over 16 context columns.  x0 / x1: logits (log2 domain, bias and mask applied) of column groups 0 / 1 in
+// accumulator layout (c0, c1: row g; c2, c3: row g + 8).  Returns P as the A fragment of the P V MMAs.
+__device__ __forceinline__ void d2_softmax(D2Soft& s, float (&o)[16][4], const float (&x0)[4], const float (&x1)[4],
+                                           uint32_t (&pa)[4]) {
+  float mx0 = fmaxf(fmaxf(x0[0], x0[1]), fmaxf(x1[0], x1[1]));
+  float mx1 = fmaxf(fmaxf(x0[2], x0[3]), fmaxf(x1[2], x1[3]));
+  mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1)); mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+  mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1)); mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+  // The reference maximum of a row moves only when a step's maximum exceeds it by more than kD2Slack (P <= 2^kD2Slack is
+  // harmless in bf16 / fp32), so that the rescale of the 64 O accumulators is rare instead of once per early step.
+  const float mn0 = mx0 > s.m0 + kD2Slack ? mx0 : s.m0, mn1 = mx1 > s.m1 + kD2Slack ? mx1 : s.m1;   // m = -inf: moves on any finite
+  const float mu0 = mn0 == -INFINITY ? 0.f : mn0, mu1 = mn1 == -INFINITY ? 0.f : mn1;   // all masked so far
+  const float a0 = d2_ex2(s.m0 - mu0), a1 = d2_ex2(s.m1 - mu1);   // m = -inf: 0
+  s.m0 = mn0; s.m1 = mn1;
+  const float p00 = d2_ex2(x0[0] - mu0), p01 = d2_ex2(x0[1] - mu0), p02 = d2_ex2(x0[2] - mu1), p03 = d2_ex2(x0[3] - mu1);
+  const float p10 = d2_ex2(x1[0] - mu0), p11 = d2_ex2(x1[1] - mu0), p12 = d2_ex2(x1[2] - mu1), p13 = d2_ex2(x1[3] - mu1);
+  s.l0 = fmaf(s.l0, a0, (p00 + p01) + (p10 + p11));
+  s.l1 = fmaf(s.l1, a1, (p02 + p03) + (p12 + p13));
+  if (__any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f)) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
+  }
+  pa[0] = d2_pack(p00, p01); pa[1] = d2_pack(p02, p03);
+  pa[2] = d2_pack(p10, p11); pa[3] = d2_pack(p12, p13);
+}
+
+// O += P V for 16 context rows: v[t][0..7] = the lane's 16 dims [16 g, 16 g + 16) of value row t (t = 0, 1: columns
+// 2j, 2j + 1 of group 0; t = 2, 3: of group 1) as bf16 pairs; MMA tile i pairs dim 16 g + i of two rows.
+__device__ __forceinline__ void d2_pv(float (&o)[16][4], const uint32_t (&pa)[4], const uint32_t (&v)[4][8]) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const uint32_t sel = (i & 1) ? 0x7632u : 0x5410u;
+    const uint32_t b0 = d2_prmt(v[0][i >> 1], v[1][i >> 1], sel);
+    const uint32_t b1 = d2_prmt(v[2][i >> 1], v[3][i >> 1], sel);
+    d2_mma(o[i], pa, b0, b1);
+  }
+}
+
+// Per-warp operand ring: every warp streams its own units (16 ring rows, or 8 prototypes) through kD2Stages stages
+// with cp.async -- two units in flight while one is consumed, no block barrier.
+constexpr int kD2Stages = 3;
+constexpr uint32_t kD2StageBytes = 8768;
+struct D2Stage {   // byte offsets inside a stage
+  static constexpr uint32_t K = 0, Vv = 4096;                                           // near unit: 16 rows x 256 B each
+  static constexpr uint32_t C = 0, P = 4096, ZK = 8192, ZV = 8448, LN = 8704, KD = 8736;  // far unit: 8 prototypes
+};
+constexpr uint32_t kD2Ring = 10240;                                                      // after the two codebooks
+constexpr uint32_t kD2SmemTotal = kD2Ring + kD2Warps * kD2Stages * kD2StageBytes;        // 113,408 B: two CTAs per SM
+static_assert(kD2Warps * kD2Stages * kD2StageBytes >= D2Smem::Total - D2Smem::O, "merge buffer must fit in the ring");
+
+__device__ __forceinline__ void d2_cp16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void d2_cp8(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ uint4 d2_cvt8s(const unsigned char* p) {    // 8 fp32 in shared memory -> 4 bf16x2
+  const float4 f0 = *reinterpret_cast<const float4*>(p), f1 = *reinterpret_cast<const float4*>(p + 16);
+  return make_uint4(d2_pack(f0.x, f0.y), d2_pack(f0.z, f0.w), d2_pack(f1.x, f1.y), d2_pack(f1.z, f1.w));
+}
+
+__global__ void __launch_bounds__(kD2Threads, kD2CtasPerSm) attention_decode2_kernel(Dims D, Dev V, D2Args A) {
+  extern __shared__ __align__(16) unsigned char sm[];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, j = lane & 3;
+  const int bsel = blockIdx.y, split = blockIdx.x;
+  const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
+  const int b = (st * D.L + A.layer_begin + ll) * D.Hkv + hd;
+  const bool has_cb = V.cbk != nullptr;
+
+  // ---- this warp's unit list and its first two units in flight ----
+  const int wi = split * kD2Warps + warp, NW = A.nsplit * kD2Warps;
+  const int NUn = (A.n_near + 15) >> 4, NUf = (A.n_act + 7) >> 3;
+  const int nn = wi < NUn ? (NUn - wi + NW - 1) / NW : 0, nf = wi < NUf ? (NUf - wi + NW - 1) / NW : 0;
+  const int ntot = nn + nf;
+  const char* ringK = (const char*)V.ringK + (size_t)b * D.Wf * D.T * 256;
+  const char* ringV = (const char*)V.ringV + (size_t)b * D.Wf * D.T * 256;
+  unsigned char* ring = sm + kD2Ring + warp * kD2Stages * kD2StageBytes;
+  const uint32_t ring_u32 = (uint32_t)__cvta_generic_to_shared(ring);
+  auto issue = [&](int i) {
+    if (i < ntot) {
+      const uint32_t dst = ring_u32 + (uint32_t)(i % kD2Stages) * kD2StageBytes;
+      if (i < nn) {
+        const int base = (wi + i * NW) << 4, last = A.n_near - 1;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {                         // 256 16-byte pieces per operand: piece = r * 32 + lane
+          const int piece = r * 32 + lane, row = piece >> 4, ch = piece & 15;
+          const size_t src = (size_t)min(base + row, last) * 256 + ch * 16;   // ragged tail: clamp, masked by the consumer
+          // 16-byte chunks are XOR-swizzled so that the fragment reads below are bank-conflict free: a quarter warp reads
+          // key rows g, g + 1 at the same chunks, and value rows 2j (+1) at chunks 2g, 2g + 1
+          d2_cp16(dst + D2Stage::K + row * 256 + ((ch ^ ((row & 1) << 2)) << 4), ringK + src);
+          d2_cp16(dst + D2Stage::Vv + row * 256 + ((ch ^ (((row >> 2) & 1) << 2)) << 4), ringV + src);
+        }
+      } else {
+        const size_t pk0 = (size_t)b * D.K + (size_t)(wi + (i - nn) * NW) * 8;
+        const char* cs = (const char*)(V.c_bf + pk0 * 128);     // bf16 copies of the centres (Dev::c_bf / p_bf)
+        const char* ps = (const char*)(V.p_bf + pk0 * 128);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {                           // 8 prototypes x 256 B = 128 pieces per side
+          d2_cp16(dst + D2Stage::C + (r * 32 + lane) * 16, cs + (r * 32 + lane) * 16);
+          d2_cp16(dst + D2Stage::P + (r * 32 + lane) * 16, ps + (r * 32 + lane) * 16);
+        }
+        if (lane < 16) d2_cp16(dst + D2Stage::ZK + lane * 16, (const char*)(V.codesK + pk0 * 8) + lane * 16);
+        else d2_cp16(dst + D2Stage::ZV + (lane - 16) * 16, (const char*)(V.codesV + pk0 * 8) + (lane - 16) * 16);
+        if (lane < 2) d2_cp16(dst + D2Stage::LN + lane * 16, (const char*)(V.logn + pk0) + lane * 16);
+        else if (lane == 2) d2_cp8(dst + D2Stage::KD, V.kind + pk0);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  issue(0);
+  issue(1);
+
+  // ---- codebooks as bf16 [g][z][16] (32-byte rows) ----
+  if (has_cb && A.n_act > 0) {
+    const float4* srck = reinterpret_cast<const float4*>(V.cbk + (size_t)b * 2048);
+    const float4* srcv = reinterpret_cast<const float4*>(V.cbv + (size_t)b * 2048);
+    for (int e = tid; e < 512; e += kD2Threads) {               // float4 e = (g * 16 + z) * 4 + quarter
+      const float4 a = srck[e], c = srcv[e];
+      *reinterpret_cast<uint2*>(sm + D2Smem::CBK + e * 8) = make_uint2(d2_pack(a.x, a.y), d2_pack(a.z, a.w));
+      *reinterpret_cast<uint2*>(sm + D2Smem::CBV + (e >> 2) * 48 + (e & 3) * 8) = make_uint2(d2_pack(c.x, c.y), d2_pack(c.z, c.w));
+    }
+  }
+
+  // ---- Q as A fragments under the key-side permutation: k-steps 2c, 2c + 1 <- chunk q = j + 4c of rows g, g + 8 ----
+  uint32_t qa[8][4];
+  {
+    uint4 t[4], u[4];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int r = g + 8 * h;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint4 val = make_uint4(0u, 0u, 0u, 0u);
+        if (r < A.R) {
+          const int qi = r / D.group, hh = r % D.group;
+          const size_t off = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh) * 128 + (j + 4 * c) * 8;
+          val = d2_ldg16(A.Q + off);
+        }
+        if (h == 0) t[c] = val; else u[c] = val;
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      qa[2 * c][0] = t[c].x; qa[2 * c][2] = t[c].y; qa[2 * c][1] = u[c].x; qa[2 * c][3] = u[c].y;
+      qa[2 * c + 1][0] = t[c].z; qa[2 * c + 1][2] = t[c].w; qa[2 * c + 1][1] = u[c].z; qa[2 * c + 1][3] = u[c].w;
+    }
+  }
+  __syncthreads();                                              // codebooks visible
+
+  float o[16][4];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) { o[i][0] = 0.f; o[i][1] = 0.f; o[i][2] = 0.f; o[i][3] = 0.f; }
+  D2Soft S{-INFINITY, -INFINITY, 0.f, 0.f};
+  const float sc2 = kD2Log2e * rsqrtf(128.f);
+  const unsigned char* cbK = sm + D2Smem::CBK;
+  const unsigned char* cbV = sm + D2Smem::CBV;
+
+  for (int i = 0; i < ntot; ++i) {
+    asm volatile("cp.async.wait_group 1;" ::: "memory");        // this lane's pieces of unit i have landed
+    __syncwarp();                                               // ... every lane's; and unit i - 1 has been consumed
+    issue(i + 2);
+    const unsigned char* stg = ring + (i % kD2Stages) * kD2StageBytes;
+    if (i < nn) {
+      // ---- near window: 16 ring rows ----
+      const int base = (wi + i * NW) << 4;
+      uint4 k0[4], k1[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int ch = (j + 4 * c) ^ ((g & 1) << 2);            // rows g and 8 + g have the same parity
+        k0[c] = *reinterpret_cast<const uint4*>(stg + D2Stage::K + g * 256 + ch * 16);
+        k1[c] = *reinterpret_cast<const uint4*>(stg + D2Stage::K + (8 + g) * 256 + ch * 16);
+      }
+      float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+      float s0b[4] = {0.f, 0.f, 0.f, 0.f}, s1b[4] = {0.f, 0.f, 0.f, 0.f};   // two accumulation chains per column group
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        d2_mma(s0, qa[2 * c], k0[c].x, k0[c].y);
+        d2_mma(s0b, qa[2 * c + 1], k0[c].z, k0[c].w);
+        d2_mma(s1, qa[2 * c], k1[c].x, k1[c].y);
+        d2_mma(s1b, qa[2 * c + 1], k1[c].z, k1[c].w);
+      }
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { s0[e] += s0b[e]; s1[e] += s1b[e]; }
+      const int c0 = base + 2 * j;                              // accumulator columns 2j, 2j + 1 of a group
+      float x0[4], x1[4];
+      x0[0] = c0 < A.n_near ? s0[0] * sc2 : -INFINITY; x0[1] = c0 + 1 < A.n_near ? s0[1] * sc2 : -INFINITY;
+      x0[2] = c0 < A.n_near ? s0[2] * sc2 : -INFINITY; x0[3] = c0 + 1 < A.n_near ? s0[3] * sc2 : -INFINITY;
+      x1[0] = c0 + 8 < A.n_near ? s1[0] * sc2 : -INFINITY; x1[1] = c0 + 9 < A.n_near ? s1[1] * sc2 : -INFINITY;
+      x1[2] = c0 + 8 < A.n_near ? s1[2] * sc2 : -INFINITY; x1[3] = c0 + 9 < A.n_near ? s1[3] * sc2 : -INFINITY;
+      uint32_t pa[4];
+      d2_softmax(S, o, x0, x1, pa);
+      uint32_t v[4][8];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const int row = (t >> 1) * 8 + 2 * j + (t & 1), sw = ((row >> 2) & 1) << 2;
+        const unsigned char* src = stg + D2Stage::Vv + row * 256;
+        // odd j reads its high half first: the eight lanes of a quarter warp then touch eight distinct 16-byte bank groups
+        const uint4 first = *reinterpret_cast<const uint4*>(src + (((2 * g + (j & 1)) ^ sw) << 4));
+        const uint4 second = *reinterpret_cast<const uint4*>(src + (((2 * g + 1 - (j & 1)) ^ sw) << 4));
+        const uint4 lo = (j & 1) ? second : first, hi = (j & 1) ? first : second;
+        v[t][0] = lo.x; v[t][1] = lo.y; v[t][2] = lo.z; v[t][3] = lo.w;
+        v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
+      }
+      d2_pv(o, pa, v);
+    } else {
+      // ---- far bank: 8 prototypes = 4 steps of 2 prototypes = 16 pseudo-tokens (column group = prototype, column = mode) ----
+      const int k0 = (wi + (i - nn) * NW) * 8;
+      const float* lns = reinterpret_cast<const float*>(stg + D2Stage::LN);
+      const uint32_t* zks = reinterpret_cast<const uint32_t*>(stg + D2Stage::ZK);
+      const uint32_t* zvs = reinterpret_cast<const uint32_t*>(stg + D2Stage::ZV);
+#pragma unroll 1
+      for (int ss = 0; ss < 4; ++ss) {
+        if (k0 + 2 * ss >= A.n_act) break;
+        int kind[2];
+        float bias[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          kind[h] = k0 + kl < A.n_act ? (int)stg[D2Stage::KD + kl] : 2;
+          bias[h] = kind[h] == 2 ? -INFINITY : (A.use_bias ? lns[kl] * kD2Log2e : 0.f);
+        }
+        // key side: lane (s = g, j) builds chunks q = j + 4c of k~_{k, s}
+        float s01[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          const uint32_t code = zks[kl * 8 + g];
+          uint4 kr[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) kr[c] = *reinterpret_cast<const uint4*>(stg + D2Stage::C + kl * 256 + (j + 4 * c) * 16);
+          if (kind[h] == 0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const int gg = (j + 4 * c) >> 1;
+              const uint32_t z = (code >> (4 * gg)) & 15u;
+              kr[c] = d2_add2x4(kr[c], *reinterpret_cast<const uint4*>(cbK + (gg * 16 + z) * 32 + (j & 1) * 16));
+            }
+          }
+          float sb[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            d2_mma(s01[h], qa[2 * c], kr[c].x, kr[c].y);
+            d2_mma(sb, qa[2 * c + 1], kr[c].z, kr[c].w);
+          }
+#pragma unroll
+          for (int e = 0; e < 4; ++e) s01[h][e] += sb[e];
+        }
+        float x0[4], x1[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { x0[e] = fmaf(s01[0][e], sc2, bias[0]); x1[e] = fmaf(s01[1][e], sc2, bias[1]); }
+        uint32_t pa[4];
+        d2_softmax(S, o, x0, x1, pa);
+        // value side: rows t = 0, 1: modes 2j, 2j + 1 of prototype A; t = 2, 3: of prototype B; dims [16 g, 16 g + 16) = subspace g
+        uint32_t v[4][8];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          const uint4 plo = *reinterpret_cast<const uint4*>(stg + D2Stage::P + kl * 256 + g * 32);
+          const uint4 phi = *reinterpret_cast<const uint4*>(stg + D2Stage::P + kl * 256 + g * 32 + 16);
+          const uint2 zz = *reinterpret_cast<const uint2*>(zvs + kl * 8 + 2 * j);
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            uint4 lo = plo, hi = phi;
+            if (kind[h] == 0) {
+              const uint32_t z = ((e ? zz.y : zz.x) >> (4 * g)) & 15u;
+              const uint4* cw = reinterpret_cast<const uint4*>(cbV + (g * 16 + z) * 48);
+              lo = d2_add2x4(lo, cw[0]); hi = d2_add2x4(hi, cw[1]);
+            }
+            const int t = 2 * h + e;
+            v[t][0] = lo.x; v[t][1] = lo.y; v[t][2] = lo.z; v[t][3] = lo.w;
+            v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
+          }
+        }
+        d2_pv(o, pa, v);
+      }
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();                                              // every warp is done with its ring: reuse it for the merge
+
+  // ---- merge the four warps' (m, l, O) and write this CTA's partial ----
+  S.l0 += __shfl_xor_sync(0xffffffffu, S.l0, 1); S.l0 += __shfl_xor_sync(0xffffffffu, S.l0, 2);
+  S.l1 += __shfl_xor_sync(0xffffffffu, S.l1, 1); S.l1 += __shfl_xor_sync(0xffffffffu, S.l1, 2);
+  float* Om = reinterpret_cast<float*>(sm + D2Smem::O) + warp * 16 * 128;
+  float* ml = reinterpret_cast<float*>(sm + D2Smem::ML) + warp * 32;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {            // tile i, accumulator column n = 2j (+1)  <->  dim 16 n + i
+    Om[g * 128 + 16 * (2 * j) + i] = o[i][0];
+    Om[g * 128 + 16 * (2 * j + 1) + i] = o[i][1];
+    Om[(g + 8) * 128 + 16 * (2 * j) + i] = o[i][2];
+    Om[(g + 8) * 128 + 16 * (2 * j + 1) + i] = o[i][3];
+  }
+  if (j == 0) { ml[g * 2] = S.m0; ml[g * 2 + 1] = S.l0; ml[(g + 8) * 2] = S.m1; ml[(g + 8) * 2 + 1] = S.l1; }
+  __syncthreads();
+  {
+    const int r = tid >> 3, d0 = (tid & 7) * 16;          // 16 rows x 8 threads, 16 dims each
+    if (r < A.R) {
+      const float* mlb = reinterpret_cast<const float*>(sm + D2Smem::ML);
+      float M = -INFINITY;
+#pragma unroll
+      for (int w = 0; w < kD2Warps; ++w) M = fmaxf(M, mlb[w * 32 + r * 2]);
+      const float Mu = M == -INFINITY ? 0.f : M;
+      float wgt[kD2Warps], l = 0.f;
+#pragma unroll
+      for (int w = 0; w < kD2Warps; ++w) {
+        wgt[w] = d2_ex2(mlb[w * 32 + r * 2] - Mu);
+        l = fmaf(mlb[w * 32 + r * 2 + 1], wgt[w], l);
+      }
+      float* dst = A.part + (((size_t)bsel * A.R + r) * A.nsplit + split) * 130;
+      const float* Ob = reinterpret_cast<const float*>(sm + D2Smem::O);
+#pragma unroll
+      for (int e = 0; e < 16; e += 4) {
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int w = 0; w < kD2Warps; ++w) {
+          const float4 x = *reinterpret_cast<const float4*>(Ob + (w * 16 + r) * 128 + d0 + e);
+          acc.x = fmaf(x.x, wgt[w], acc.x); acc.y = fmaf(x.y, wgt[w], acc.y);
+          acc.z = fmaf(x.z, wgt[w], acc.z); acc.w = fmaf(x.w, wgt[w], acc.w);
+        }
+        dst[d0 + e] = acc.x; dst[d0 + e + 1] = acc.y; dst[d0 + e + 2] = acc.z; dst[d0 + e + 3] = acc.w;
+      }
+      if ((tid & 7) == 0) {
+        dst[128] = M == -INFINITY ? -INFINITY : M * kD2Ln2;
+        dst[129] = l;
+      }
+    }
+  }
+}
+
+bool decode2_attention_supported(const Dims& D, int n_q) {
+  return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && n_q * D.group <= kD2Rows && D.K % 8 == 0;   // (Dev::c_bf exists for exactly these shapes)
+}
+
+bool decode2_attention_prepare() {
+  if (cudaFuncSetAttribute(attention_decode2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD2SmemTotal) !=
+      cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return true;
+}
+
+// Partials per row the launch below writes at most (part buffer sizing in carve()).
+int decode2_max_splits() { return 16; }
+
+int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
+                             int* nsplit_out) {
+  D2Args a{};
+  a.Q = (const __nv_bfloat16*)A.Q;
+  a.part = V.part;
+  a.n_q = A.n_q; a.layer_begin = A.layer_begin; a.layer_count = A.layer_count;
+  a.n_near = (H.flags & PROTOKV_FAR_ONLY) ? 0 : A.n_near;
+  a.n_act = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : A.n_act;
+  a.use_bias = !(H.flags & PROTOKV_NO_MASS_BIAS);
+  a.R = A.n_q * D.group;
+  const int nb = D.NS * A.layer_count * D.Hkv;
+  // splits per bank: the kernel's time goes like waves / ns with waves = ceil(nb ns / resident CTAs) -- take the smallest
+  // ns within 3 % of the best, so that the last wave is nearly full
+  const int units = (a.n_near + 15) / 16 + (a.n_act + 7) / 8;
+  int cap = (units + kD2Warps - 1) / kD2Warps;
+  if (cap > decode2_max_splits()) cap = decode2_max_splits();
+  if (cap < 1) cap = 1;
+  const int slots = kD2CtasPerSm * sm_count;
+  int ns = 1;
+  double best = 1e30;
+  for (int c = 1; c <= cap; ++c) {
+    const double cost = (double)(((long long)nb * c + slots - 1) / slots) / c * (1.0 + 0.02 * c);   // + per-CTA fixed work
+    if (cost < best * 0.97) { best = cost; ns = c; }
+  }
+  a.nsplit = ns;
+  *nsplit_out = ns;
+  attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
+  return 1;
+}
+
+}  // namespace pkv

@@ -63,4 +63,18 @@ __device__ __forceinline__ void store_shadows(const Dev& V, size_t off, const fl
   }
 }
 
+// bf16 copies of a centre (key or value side) for the decode-style attention: dst = c_bf or p_bf
+template <int VEC>
+__device__ __forceinline__ void store_bf16_copy(__nv_bfloat16* dst, size_t off, const float (&x)[VEC]) {
+  if (!dst) return;
+  __nv_bfloat16 h[VEC];
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) h[v] = __float2bfloat16_rn(x[v]);
+  if (VEC == 4) *reinterpret_cast<uint2*>(dst + off) = *reinterpret_cast<const uint2*>(h);
+  else {
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) dst[off + v] = h[v];
+  }
+}
+
 }  // namespace pkv

@@ -261,6 +261,11 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
     float cc = 0.f;
     for (int v = 0; v < vec; ++v) { const float x = V.c[pk * d + lane * vec + v]; cc = fmaf(x, x, cc); }
     cc = warp_sum(cc);
+    if (V.c_bf)
+      for (int e = lane; e < d; e += 32) {
+        V.c_bf[pk * d + e] = __float2bfloat16_rn(V.c[pk * d + e]);
+        V.p_bf[pk * d + e] = __float2bfloat16_rn(V.p[pk * d + e]);
+      }
     if (V.c_hi) {
       const float invc = inv_norm(cc);
       for (int v = 0; v < vec; ++v) {
@@ -311,6 +316,7 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
       const float kf = to_f32(Ke[e]), vf = to_f32(Ve[e]);
       V.c[pk * d + e] = kf;
       V.p[pk * d + e] = vf;
+      if (V.c_bf) { V.c_bf[pk * d + e] = __float2bfloat16_rn(kf); V.p_bf[pk * d + e] = __float2bfloat16_rn(vf); }
       cc = fmaf(kf, kf, cc);
     }
     cc = warp_sum(cc);

@@ -39,6 +39,7 @@ struct protokv_state {
   bool use_tc_assign;
   bool use_tc_attn;
   bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
+  bool use_decode2;       // the register-resident decode kernel serves them (default where supported)
   TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
@@ -209,6 +210,10 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
   if (D.bf16) {
     v.c_hi = (__nv_bfloat16*)take(BK * D.d * 2);
     v.c_lo = (__nv_bfloat16*)take(BK * D.d * 2);
+    if (decode2_attention_supported(D, 1)) {
+      v.c_bf = (__nv_bfloat16*)take(BK * D.d * 2);
+      v.p_bf = (__nv_bfloat16*)take(BK * D.d * 2);
+    }
   }
   v.n = (int*)take(BK * 4); v.mu = (float*)take(BK * 8); v.sigma = (float*)take(BK * 12);
   v.tau = (int*)take(BK * 4); v.pos = (long long*)take(BK * 8); v.nres = (uint32_t*)take(BK * 4);
@@ -249,6 +254,10 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
   size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
   if (tc_attention_supported(D) && tc_attention_part_bytes(D) > part_bytes) part_bytes = tc_attention_part_bytes(D);
   if (decode_attention_supported(D, 1) && decode_attention_part_bytes(D) > part_bytes) part_bytes = decode_attention_part_bytes(D);
+  if (decode2_attention_supported(D, 1)) {
+    const size_t need = (size_t)D.B * 16 * decode2_max_splits() * 130 * 4;
+    if (need > part_bytes) part_bytes = need;
+  }
   v.part = (float*)take(part_bytes);
   const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * elt;
   const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * elt;
@@ -353,6 +362,8 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->use_tc_attn = want_tc && !rope && tc_attention_supported(st->D) && st->maps.ok && tc_attention_prepare();
   st->use_decode_attn = want_tc && !rope && (cfg->flags & PROTOKV_DECODE_SPLITKV) && decode_attention_supported(st->D, 1) &&
                         decode_attention_prepare();
+  st->use_decode2 = want_tc && !rope && !st->use_decode_attn && !(cfg->flags & PROTOKV_NO_DECODE_KERNEL) &&
+                    decode2_attention_supported(st->D, 1) && decode2_attention_prepare();
   return st;
 }
 
@@ -529,6 +540,11 @@ int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, in
       st->launches += launch_attention_decode(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
       st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+    } else if (st->use_decode2 && decode2_attention_supported(D, n_q) && (uintptr_t)Q % 16 == 0) {
+      int ns = 1;
+      st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
+      A.nsplit = ns;
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
     } else if (st->use_tc_attn && (uintptr_t)Q % 16 == 0 && (uintptr_t)out % 8 == 0) {
       const int nl = launch_attention_tc(D, st->H, st->V, A, st->maps, st->sm_count, st->stream);
       if (nl < 0) return fail(PROTOKV_ECUDA, "cuTensorMapEncodeTiled failed for Q");
@@ -595,7 +611,8 @@ const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
   if (!st) return "none";
   if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
   if (stage == 1) return st->use_tc_attn ? "tcgen05" : "simt";
-  if (stage == 2) return st->use_decode_attn ? "mma.sync split-KV" : (st->use_tc_attn ? "tcgen05" : "simt");
+  if (stage == 2)
+    return st->use_decode_attn ? "mma.sync split-KV" : (st->use_decode2 ? "mma.sync register-resident" : (st->use_tc_attn ? "tcgen05" : "simt"));
   return "none";
 }
 

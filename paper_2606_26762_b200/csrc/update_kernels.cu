@@ -100,6 +100,7 @@ __global__ void fill_kernel(Dims D, Hyper H, Dev V, FrameArgs F) {
     float kf = to_f32(Ke[i]), vf = to_f32(Ve[i]);
     V.c[pk * D.d + i] = kf;
     V.p[pk * D.d + i] = vf;
+    if (V.c_bf) { V.c_bf[pk * D.d + i] = __float2bfloat16_rn(kf); V.p_bf[pk * D.d + i] = __float2bfloat16_rn(vf); }
     cc = fmaf(kf, kf, cc);
   }
   cc = warp_sum(cc);
@@ -425,6 +426,8 @@ __global__ void __launch_bounds__(kUpdThreads) update_kernel(Dims D, Hyper H, De
     for (int v = 0; v < VEC; ++v) cc = fmaf(c[v], c[v], cc);
     cc = warp_sum(cc);
     store_shadows<VEC>(V, pk * DH + lane * VEC, c, inv_norm(cc));
+    store_bf16_copy<VEC>(V.c_bf, pk * DH + lane * VEC, c);
+    store_bf16_copy<VEC>(V.p_bf, pk * DH + lane * VEC, p);
     if (lane == 0) {
       V.n[pk] = n;
       V.tau[pk] = F.t;
@@ -660,6 +663,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
         }
       }
       *(float4*)(V.p + pk * DH + lane * 4) = make_float4(p[0], p[1], p[2], p[3]);
+      store_bf16_copy<4>(V.p_bf, pk * DH + lane * 4, p);
       continue;
     }
     // ---- key side: l.8, l.10-12, the K half of l.13 and everything derived from the prototype
@@ -723,6 +727,7 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
     for (int v = 0; v < 4; ++v) cc = fmaf(c[v], c[v], cc);
     cc = warp_sum(cc);
     store_shadows<4>(V, pk * DH + lane * 4, c, inv_norm(cc));
+    store_bf16_copy<4>(V.c_bf, pk * DH + lane * 4, c);
     if (lane == 0) {
       const int m = r1 - r0;
       const int n = n_old + m;                                       // l.10
@@ -834,6 +839,11 @@ __global__ void refresh_derived_kernel(Dims D, Hyper H, Dev V, int b, int epoch)
       V.c_hi[pk * D.d + i] = hi; V.c_lo[pk * D.d + i] = lo;
     }
   }
+  if (V.c_bf)
+    for (int i = lane; i < D.d; i += 32) {
+      V.c_bf[pk * D.d + i] = __float2bfloat16_rn(V.c[pk * D.d + i]);
+      V.p_bf[pk * D.d + i] = __float2bfloat16_rn(V.p[pk * D.d + i]);
+    }
   if (lane == 0) {
     store_rec(V.rec, pk, make_rec(cc, V.mu[pk * 2], V.mu[pk * 2 + 1], V.sigma[pk * 3], V.sigma[pk * 3 + 1],
                          V.sigma[pk * 3 + 2], V.tau[pk], H));

@@ -37,6 +37,13 @@ def test_query_bytes_count_fp32_centres_and_codes():
     assert bench.query_bytes(c3) == per_bank * 112
 
 
+def test_decode_bytes_count_the_centres_at_the_streamed_width():
+    c3 = gen.spec_for("c3")
+    per_bank = 2 * 3136 * 128 * 2 + 1024 * (2 * 128 * 2 + 8 * 8 + 4) + 2 * 7 * 128 * 2
+    assert bench.decode_bytes(c3, 2) == per_bank * 112
+    assert bench.decode_bytes(c3, 4) - bench.decode_bytes(c3, 2) == 1024 * 2 * 128 * 2 * 112
+
+
 def test_peaks_fall_back_when_the_driver_file_is_absent(tmp_path, monkeypatch):
     monkeypatch.setattr(bench, "ROOT", str(tmp_path))
     p = bench.load_peaks()

@@ -16,7 +16,7 @@ from gpu_helpers import (make_gpu, make_oracles, run_stream, compare_ring, compa
                          compare_state, new_stats, step_teacher_forced)
 from oracle import FLAG_NEAR_ONLY, FLAG_FAR_ONLY, FLAG_NO_MASS_BIAS, FLAG_MAH_SQUARED
 from paper_2606_26762_b200 import (ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT,
-                                   DECODE_SPLITKV)
+                                   DECODE_SPLITKV, NO_DECODE_KERNEL)
 
 pytestmark = pytest.mark.gpu
 
@@ -465,12 +465,18 @@ def test_synthesis_and_bias_with_counts_beyond_the_log_table():
 # two-token queries against the oracle at every stage of a stream -- partial window (ragged near tail), bank still
 # filling (ragged prototype tail, zero-residual prototypes), steady state -- and under the ablation flags
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flags,oflags", [(0, 0), (NEAR_ONLY, FLAG_NEAR_ONLY), (FAR_ONLY, FLAG_FAR_ONLY),
-                                          (NO_MASS_BIAS, FLAG_NO_MASS_BIAS)])
-def test_decode_query_kernel(flags, oflags):
+_ROUTES = {0: "mma.sync register-resident", DECODE_SPLITKV: "mma.sync split-KV", NO_DECODE_KERNEL: "tcgen05"}
+
+
+@pytest.mark.parametrize("flags,oflags,route", [(0, 0, 0), (NEAR_ONLY, FLAG_NEAR_ONLY, 0), (FAR_ONLY, FLAG_FAR_ONLY, 0),
+                                                (NO_MASS_BIAS, FLAG_NO_MASS_BIAS, 0), (0, 0, DECODE_SPLITKV),
+                                                (FAR_ONLY, FLAG_FAR_ONLY, DECODE_SPLITKV), (0, 0, NO_DECODE_KERNEL)])
+def test_decode_query_kernel(flags, oflags, route):
+    """Default route = the register-resident decode kernel (csrc/decode_attention2.cu); the opt-in split-KV kernel and the
+    128-row tcgen05 kernel serve the same queries as cross-checks."""
     spec = gen.spec_for("c2", n_frames=40)
-    gpu = make_gpu(spec, flags=flags | DECODE_SPLITKV)
-    assert gpu.stage_impl(2).startswith("mma.sync")
+    gpu = make_gpu(spec, flags=flags | route)
+    assert gpu.stage_impl(2) == _ROUTES[route]
     oracles = make_oracles(spec, [0, 3], flags=oflags)
     Q = gen.queries(spec, 5)
     checkpoints = {2: 1, 9: 2, 17: 1, 19: 2, 23: 1, 39: 2}      # frame -> query tokens (7 or 14 rows per bank)
@@ -494,11 +500,31 @@ def test_decode_query_kernel(flags, oflags):
 
 def test_decode_query_full_size_c3_sampled():
     spec = gen.spec_for("c3", n_frames=24)
-    for flags in (0, DECODE_SPLITKV):                # the default route (tcgen05 kernel) and the opt-in one
+    for flags in (0, DECODE_SPLITKV, NO_DECODE_KERNEL):   # default (register-resident decode kernel) and the two others
         gpu = make_gpu(spec, flags=flags)
+        assert gpu.stage_impl(2) == _ROUTES[flags]
         banks = [0, 57, 111]
         oracles = make_oracles(spec, banks)
         run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=0, on_device=True)
         Q = gen.queries(spec, 1)[:, :, :1].contiguous()
         compare_attention(spec, gpu, oracles, Q, run_synthesis=True)
         gpu.close()
+
+
+def test_decode_query_c5_shape():
+    """GQA group 4, T = 576, K_max = 2048 (config 5's bank shape, one stream): 1-, 3- and 4-token queries (4, 12, 16 rows)
+    through the register-resident decode kernel while the bank fills and in steady state."""
+    spec = gen.spec_for("c5", n_frames=16, n_streams=1)
+    gpu = make_gpu(spec)
+    assert gpu.stage_impl(2) == _ROUTES[0]
+    oracles = make_oracles(spec, [0, 5])
+    Q = gen.queries(spec, 2)
+    stats = new_stats()
+    s = gen.grid_positions(spec)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats)
+        if f in (3, 9, 11, 15):
+            nq = {3: 1, 9: 4, 11: 3, 15: 4}[f]
+            compare_attention(spec, gpu, oracles, Q[:, :, :nq].contiguous(), run_synthesis=True)
+    gpu.close()
