@@ -419,12 +419,315 @@ __global__ void __launch_bounds__(kD2Threads, kD2CtasPerSm) attention_decode2_ke
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// The same kernel for <= 8 query rows per bank (one decoded token of a GQA group of up to 8 -- the common case), with
+// the MMA roles swapped so that nothing is padded: the 16 context columns of a step are the M dimension and the query
+// rows the N = 8 dimension.
+//   S^T = K~ Q^T   A = key rows g, g + 8 (same chunk permutation as above), B = Q^T: 8 MMAs per 16 columns
+//   softmax        thread (g, j) holds (ctx g | g + 8) x (rows 2j, 2j + 1); row maxima reduce over the g lanes
+//   P^T            the PV B fragment wants (ctx 2j, 2j + 1; row g): an 8 x 8 transpose inside the warp -- movmatrix
+//   O^T += V~^T P^T   A = V~^T (M = dims [16 g, 16 g + 16) in pairs, K = ctx), 8 MMAs per 16 columns, 32 accumulators
+// Half the MMAs, half the accumulators and ~150 registers: three CTAs (12 warps) per SM instead of two.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kD8CtasPerSm = 3;
+constexpr int kD8Stages = 2;
+constexpr uint32_t kD8StageBytes = 8192;
+constexpr uint32_t kD8Ring = 8192;                                                     // two bf16 codebooks, 32-byte rows
+constexpr uint32_t kD8SmemTotal = kD8Ring + kD2Warps * kD8Stages * kD8StageBytes;      // 73,728 B
+
+__device__ __forceinline__ void d8_mma(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                       uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+               "{%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t d8_trans(uint32_t x) {     // 8 x 8 b16 transpose across the warp
+  uint32_t r;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(r) : "r"(x));
+  return r;
+}
+
+// x[0], x[1]: (ctx g; rows 2j, 2j + 1), x[2], x[3]: (ctx g + 8; rows 2j, 2j + 1).  Returns the PV B fragment (P^T).
+__device__ __forceinline__ void d8_softmax(D2Soft& s, float (&o)[8][4], const float (&x)[4], uint32_t& b0, uint32_t& b1) {
+  float mx0 = fmaxf(x[0], x[2]), mx1 = fmaxf(x[1], x[3]);
+#pragma unroll
+  for (int sh = 4; sh <= 16; sh <<= 1) {
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, sh));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, sh));
+  }
+  const float mn0 = mx0 > s.m0 + kD2Slack ? mx0 : s.m0, mn1 = mx1 > s.m1 + kD2Slack ? mx1 : s.m1;   // lazy reference maximum
+  const float mu0 = mn0 == -INFINITY ? 0.f : mn0, mu1 = mn1 == -INFINITY ? 0.f : mn1;
+  const float a0 = d2_ex2(s.m0 - mu0), a1 = d2_ex2(s.m1 - mu1);
+  s.m0 = mn0; s.m1 = mn1;
+  const float p0 = d2_ex2(x[0] - mu0), p1 = d2_ex2(x[1] - mu1), p2 = d2_ex2(x[2] - mu0), p3 = d2_ex2(x[3] - mu1);
+  s.l0 = fmaf(s.l0, a0, p0 + p2);
+  s.l1 = fmaf(s.l1, a1, p1 + p3);
+  if (__any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f)) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { o[i][0] *= a0; o[i][1] *= a1; o[i][2] *= a0; o[i][3] *= a1; }
+  }
+  b0 = d8_trans(d2_pack(p0, p1));
+  b1 = d8_trans(d2_pack(p2, p3));
+}
+
+// O^T += V~^T P^T: v[t][0..7] as in d2_pv; tile i holds dims 16 g + 2 i (M index g) and 16 g + 2 i + 1 (M index g + 8)
+__device__ __forceinline__ void d8_pv(float (&o)[8][4], uint32_t b0, uint32_t b1, const uint32_t (&v)[4][8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const uint32_t a0 = d2_prmt(v[0][i], v[1][i], 0x5410u), a1 = d2_prmt(v[0][i], v[1][i], 0x7632u);
+    const uint32_t a2 = d2_prmt(v[2][i], v[3][i], 0x5410u), a3 = d2_prmt(v[2][i], v[3][i], 0x7632u);
+    d8_mma(o[i], a0, a1, a2, a3, b0, b1);
+  }
+}
+
+__global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
+  extern __shared__ __align__(16) unsigned char sm[];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, j = lane & 3;
+  const int bsel = blockIdx.y, split = blockIdx.x;
+  const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
+  const int b = (st * D.L + A.layer_begin + ll) * D.Hkv + hd;
+  const bool has_cb = V.cbk != nullptr;
+
+  const int wi = split * kD2Warps + warp, NW = A.nsplit * kD2Warps;
+  const int NUn = (A.n_near + 15) >> 4, NUf = (A.n_act + 7) >> 3;
+  const int nn = wi < NUn ? (NUn - wi + NW - 1) / NW : 0, nf = wi < NUf ? (NUf - wi + NW - 1) / NW : 0;
+  const int ntot = nn + nf;
+  const char* ringK = (const char*)V.ringK + (size_t)b * D.Wf * D.T * 256;
+  const char* ringV = (const char*)V.ringV + (size_t)b * D.Wf * D.T * 256;
+  unsigned char* ring = sm + kD8Ring + warp * kD8Stages * kD8StageBytes;
+  const uint32_t ring_u32 = (uint32_t)__cvta_generic_to_shared(ring);
+  auto issue = [&](int i) {
+    if (i < ntot) {
+      const uint32_t dst = ring_u32 + (uint32_t)(i % kD8Stages) * kD8StageBytes;
+      if (i < nn) {
+        const int base = (wi + i * NW) << 4, last = A.n_near - 1;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const int piece = r * 32 + lane, row = piece >> 4, ch = piece & 15;
+          const size_t src = (size_t)min(base + row, last) * 256 + ch * 16;
+          d2_cp16(dst + D2Stage::K + row * 256 + ((ch ^ ((row & 1) << 2)) << 4), ringK + src);
+          d2_cp16(dst + D2Stage::Vv + row * 256 + ((ch ^ (((row >> 2) & 1) << 2)) << 4), ringV + src);
+        }
+      } else {
+        const size_t pk0 = (size_t)b * D.K + (size_t)(wi + (i - nn) * NW) * 8;
+        const char* cs = (const char*)(V.c_bf + pk0 * 128);
+        const char* ps = (const char*)(V.p_bf + pk0 * 128);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          d2_cp16(dst + D2Stage::C + (r * 32 + lane) * 16, cs + (r * 32 + lane) * 16);
+          d2_cp16(dst + D2Stage::C + 2048 + (r * 32 + lane) * 16, ps + (r * 32 + lane) * 16);
+        }
+        if (lane < 16) d2_cp16(dst + 4096 + lane * 16, (const char*)(V.codesK + pk0 * 8) + lane * 16);
+        else d2_cp16(dst + 4352 + (lane - 16) * 16, (const char*)(V.codesV + pk0 * 8) + (lane - 16) * 16);
+        if (lane < 2) d2_cp16(dst + 4608 + lane * 16, (const char*)(V.logn + pk0) + lane * 16);
+        else if (lane == 2) d2_cp8(dst + 4640, V.kind + pk0);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  issue(0);
+
+  if (has_cb && A.n_act > 0) {
+    const float4* srck = reinterpret_cast<const float4*>(V.cbk + (size_t)b * 2048);
+    const float4* srcv = reinterpret_cast<const float4*>(V.cbv + (size_t)b * 2048);
+    for (int e = tid; e < 512; e += kD2Threads) {
+      const float4 a = srck[e], c = srcv[e];
+      *reinterpret_cast<uint2*>(sm + e * 8) = make_uint2(d2_pack(a.x, a.y), d2_pack(a.z, a.w));
+      *reinterpret_cast<uint2*>(sm + 4096 + e * 8) = make_uint2(d2_pack(c.x, c.y), d2_pack(c.z, c.w));
+    }
+  }
+  // Q^T as B fragments: column n = g is query row g; k-steps 2c, 2c + 1 <- chunk q = j + 4c
+  uint32_t qb[8][2];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    uint4 val = make_uint4(0u, 0u, 0u, 0u);
+    if (g < A.R) {
+      const int qi = g / D.group, hh = g % D.group;
+      const size_t off = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh) * 128 + (j + 4 * c) * 8;
+      val = d2_ldg16(A.Q + off);
+    }
+    qb[2 * c][0] = val.x; qb[2 * c][1] = val.y; qb[2 * c + 1][0] = val.z; qb[2 * c + 1][1] = val.w;
+  }
+  __syncthreads();
+
+  float o[8][4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { o[i][0] = 0.f; o[i][1] = 0.f; o[i][2] = 0.f; o[i][3] = 0.f; }
+  D2Soft S{-INFINITY, -INFINITY, 0.f, 0.f};                     // rows 2j (m0, l0) and 2j + 1 (m1, l1)
+  const float sc2 = kD2Log2e * rsqrtf(128.f);
+  const unsigned char* cbK = sm;
+  const unsigned char* cbV = sm + 4096;
+
+  for (int i = 0; i < ntot; ++i) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+    issue(i + 1);
+    const unsigned char* stg = ring + (i % kD8Stages) * kD8StageBytes;
+    if (i < nn) {
+      const int base = (wi + i * NW) << 4;
+      float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int ch = (j + 4 * c) ^ ((g & 1) << 2);
+        const uint4 ka = *reinterpret_cast<const uint4*>(stg + D2Stage::K + g * 256 + ch * 16);
+        const uint4 kb = *reinterpret_cast<const uint4*>(stg + D2Stage::K + (8 + g) * 256 + ch * 16);
+        d8_mma(s0, ka.x, kb.x, ka.y, kb.y, qb[2 * c][0], qb[2 * c][1]);
+        d8_mma(s1, ka.z, kb.z, ka.w, kb.w, qb[2 * c + 1][0], qb[2 * c + 1][1]);
+      }
+      float x[4];
+      const bool in0 = base + g < A.n_near, in1 = base + 8 + g < A.n_near;
+      x[0] = in0 ? (s0[0] + s1[0]) * sc2 : -INFINITY; x[1] = in0 ? (s0[1] + s1[1]) * sc2 : -INFINITY;
+      x[2] = in1 ? (s0[2] + s1[2]) * sc2 : -INFINITY; x[3] = in1 ? (s0[3] + s1[3]) * sc2 : -INFINITY;
+      uint32_t b0, b1;
+      d8_softmax(S, o, x, b0, b1);
+      uint32_t v[4][8];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const int row = (t >> 1) * 8 + 2 * j + (t & 1), sw = ((row >> 2) & 1) << 2;
+        const unsigned char* src = stg + D2Stage::Vv + row * 256;
+        const uint4 first = *reinterpret_cast<const uint4*>(src + (((2 * g + (j & 1)) ^ sw) << 4));
+        const uint4 second = *reinterpret_cast<const uint4*>(src + (((2 * g + 1 - (j & 1)) ^ sw) << 4));
+        const uint4 lo = (j & 1) ? second : first, hi = (j & 1) ? first : second;
+        v[t][0] = lo.x; v[t][1] = lo.y; v[t][2] = lo.z; v[t][3] = lo.w;
+        v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
+      }
+      d8_pv(o, b0, b1, v);
+    } else {
+      const int k0 = (wi + (i - nn) * NW) * 8;
+      const float* lns = reinterpret_cast<const float*>(stg + 4608);
+      const uint32_t* zks = reinterpret_cast<const uint32_t*>(stg + 4096);
+      const uint32_t* zvs = reinterpret_cast<const uint32_t*>(stg + 4352);
+#pragma unroll 1
+      for (int ss = 0; ss < 4; ++ss) {
+        if (k0 + 2 * ss >= A.n_act) break;
+        int kind[2];
+        float bias[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          kind[h] = k0 + kl < A.n_act ? (int)stg[4640 + kl] : 2;
+          bias[h] = kind[h] == 2 ? -INFINITY : (A.use_bias ? lns[kl] * kD2Log2e : 0.f);
+        }
+        // key side: rows g (prototype A, mode g) and g + 8 (prototype B, mode g) of the 16-column step
+        uint4 kr[2][4];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          const uint32_t code = zks[kl * 8 + g];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) kr[h][c] = *reinterpret_cast<const uint4*>(stg + D2Stage::C + kl * 256 + (j + 4 * c) * 16);
+          if (kind[h] == 0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const int gg = (j + 4 * c) >> 1;
+              const uint32_t z = (code >> (4 * gg)) & 15u;
+              kr[h][c] = d2_add2x4(kr[h][c], *reinterpret_cast<const uint4*>(cbK + (gg * 16 + z) * 32 + (j & 1) * 16));
+            }
+          }
+        }
+        float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          d8_mma(s0, kr[0][c].x, kr[1][c].x, kr[0][c].y, kr[1][c].y, qb[2 * c][0], qb[2 * c][1]);
+          d8_mma(s1, kr[0][c].z, kr[1][c].z, kr[0][c].w, kr[1][c].w, qb[2 * c + 1][0], qb[2 * c + 1][1]);
+        }
+        float x[4];
+        x[0] = fmaf(s0[0] + s1[0], sc2, bias[0]); x[1] = fmaf(s0[1] + s1[1], sc2, bias[0]);
+        x[2] = fmaf(s0[2] + s1[2], sc2, bias[1]); x[3] = fmaf(s0[3] + s1[3], sc2, bias[1]);
+        uint32_t b0, b1;
+        d8_softmax(S, o, x, b0, b1);
+        uint32_t v[4][8];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int kl = 2 * ss + h;
+          const uint4 plo = *reinterpret_cast<const uint4*>(stg + D2Stage::C + 2048 + kl * 256 + g * 32);
+          const uint4 phi = *reinterpret_cast<const uint4*>(stg + D2Stage::C + 2048 + kl * 256 + g * 32 + 16);
+          const uint2 zz = *reinterpret_cast<const uint2*>(zvs + kl * 8 + 2 * j);
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            uint4 lo = plo, hi = phi;
+            if (kind[h] == 0) {
+              const uint32_t z = ((e ? zz.y : zz.x) >> (4 * g)) & 15u;
+              const uint4* cw = reinterpret_cast<const uint4*>(cbV + (g * 16 + z) * 32);
+              lo = d2_add2x4(lo, cw[0]); hi = d2_add2x4(hi, cw[1]);
+            }
+            const int t = 2 * h + e;
+            v[t][0] = lo.x; v[t][1] = lo.y; v[t][2] = lo.z; v[t][3] = lo.w;
+            v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
+          }
+        }
+        d8_pv(o, b0, b1, v);
+      }
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+
+  // ---- merge the four warps' (m, l, O^T) and write this CTA's partial ----
+#pragma unroll
+  for (int sh = 4; sh <= 16; sh <<= 1) {
+    S.l0 += __shfl_xor_sync(0xffffffffu, S.l0, sh);
+    S.l1 += __shfl_xor_sync(0xffffffffu, S.l1, sh);
+  }
+  float* Om = reinterpret_cast<float*>(sm + kD8Ring) + warp * 8 * 128;      // [4 warps][8 rows][128]
+  float* ml = reinterpret_cast<float*>(sm + kD8Ring + 4 * 8 * 128 * 4) + warp * 16;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {             // tile i: M index g -> dim 16 g + 2 i, M index g + 8 -> dim 16 g + 2 i + 1
+    Om[(2 * j) * 128 + 16 * g + 2 * i] = o[i][0];
+    Om[(2 * j + 1) * 128 + 16 * g + 2 * i] = o[i][1];
+    Om[(2 * j) * 128 + 16 * g + 2 * i + 1] = o[i][2];
+    Om[(2 * j + 1) * 128 + 16 * g + 2 * i + 1] = o[i][3];
+  }
+  if (g == 0) { ml[(2 * j) * 2] = S.m0; ml[(2 * j) * 2 + 1] = S.l0; ml[(2 * j + 1) * 2] = S.m1; ml[(2 * j + 1) * 2 + 1] = S.l1; }
+  __syncthreads();
+  {
+    const int r = tid >> 4, d0 = (tid & 15) * 8;          // 8 rows x 16 threads, 8 dims each
+    if (r < A.R) {
+      const float* mlb = reinterpret_cast<const float*>(sm + kD8Ring + 4 * 8 * 128 * 4);
+      float M = -INFINITY;
+#pragma unroll
+      for (int w = 0; w < kD2Warps; ++w) M = fmaxf(M, mlb[w * 16 + r * 2]);
+      const float Mu = M == -INFINITY ? 0.f : M;
+      float wgt[kD2Warps], l = 0.f;
+#pragma unroll
+      for (int w = 0; w < kD2Warps; ++w) {
+        wgt[w] = d2_ex2(mlb[w * 16 + r * 2] - Mu);
+        l = fmaf(mlb[w * 16 + r * 2 + 1], wgt[w], l);
+      }
+      float* dst = A.part + (((size_t)bsel * A.R + r) * A.nsplit + split) * 130;
+      const float* Ob = reinterpret_cast<const float*>(sm + kD8Ring);
+#pragma unroll
+      for (int e = 0; e < 8; e += 4) {
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int w = 0; w < kD2Warps; ++w) {
+          const float4 xx = *reinterpret_cast<const float4*>(Ob + (w * 8 + r) * 128 + d0 + e);
+          acc.x = fmaf(xx.x, wgt[w], acc.x); acc.y = fmaf(xx.y, wgt[w], acc.y);
+          acc.z = fmaf(xx.z, wgt[w], acc.z); acc.w = fmaf(xx.w, wgt[w], acc.w);
+        }
+        dst[d0 + e] = acc.x; dst[d0 + e + 1] = acc.y; dst[d0 + e + 2] = acc.z; dst[d0 + e + 3] = acc.w;
+      }
+      if ((tid & 15) == 0) {
+        dst[128] = M == -INFINITY ? -INFINITY : M * kD2Ln2;
+        dst[129] = l;
+      }
+    }
+  }
+}
+
 bool decode2_attention_supported(const Dims& D, int n_q) {
   return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && n_q * D.group <= kD2Rows && D.K % 8 == 0;   // (Dev::c_bf exists for exactly these shapes)
 }
 
 bool decode2_attention_prepare() {
   if (cudaFuncSetAttribute(attention_decode2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD2SmemTotal) !=
+      cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  if (cudaFuncSetAttribute(attention_decode8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
       cudaSuccess) {
     cudaGetLastError();
     return false;
@@ -452,7 +755,8 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   int cap = (units + kD2Warps - 1) / kD2Warps;
   if (cap > decode2_max_splits()) cap = decode2_max_splits();
   if (cap < 1) cap = 1;
-  const int slots = kD2CtasPerSm * sm_count;
+  const bool rows8 = a.R <= 8;                                 // the N = 8 variant: three CTAs per SM
+  const int slots = (rows8 ? kD8CtasPerSm : kD2CtasPerSm) * sm_count;
   int ns = 1;
   double best = 1e30;
   for (int c = 1; c <= cap; ++c) {
@@ -461,7 +765,8 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   }
   a.nsplit = ns;
   *nsplit_out = ns;
-  attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
+  if (rows8) attention_decode8_kernel<<<dim3(ns, nb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  else attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
   return 1;
 }
 
