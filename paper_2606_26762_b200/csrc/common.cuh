@@ -112,6 +112,7 @@ struct Dev {
   const double* logtab;  // [PKV_SYN_LOGTAB] log(h + pq_eps), h = 0, 1, ...: built on the host at create (synthesis, Eq. 3)
   float* cbk;      // [B][G][C][sub]  (NULL when the state has no residual statistics)
   float* cbv;
+  __nv_bfloat16* cb_bf;  // [B][2][G * C][sub] bf16 copies of cbk, cbv (decode-style attention), written when the codebooks are
   // synthesis result
   uint32_t* codesK;  // [B][K][S], code of subspace g in bits [4g, 4g+4)
   uint32_t* codesV;
@@ -204,6 +205,7 @@ int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& 
 int launch_refresh_derived(const Dims& D, const Hyper& H, const Dev& V, int bank, int epoch, cudaStream_t s);
 int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s);
 int launch_or_u32(uint32_t* dst, uint32_t bits, cudaStream_t s);
+int launch_codebook_copy(const Dims& D, const Dev& V, const float* cbk, const float* cbv, cudaStream_t s);   // fills Dev::cb_bf
 // One-time (per device) function attributes of every kernel that needs more than 48 KB of shared memory for some
 // admissible shape; returns false if the device refuses one of them.
 bool update_kernels_prepare(const Dims& D);

@@ -432,7 +432,8 @@ __global__ void __launch_bounds__(kD2Threads, kD2CtasPerSm) attention_decode2_ke
 constexpr int kD8CtasPerSm = 3;
 constexpr int kD8Stages = 2;
 constexpr uint32_t kD8StageBytes = 8192;
-constexpr uint32_t kD8Ring = 8192;                                                     // two bf16 codebooks, 32-byte rows
+constexpr uint32_t kD8CbV = 4096;                                                      // two bf16 codebooks, 128 rows x 32 B each
+constexpr uint32_t kD8Ring = 8192;
 constexpr uint32_t kD8SmemTotal = kD8Ring + kD2Warps * kD8Stages * kD8StageBytes;      // 73,728 B
 
 __device__ __forceinline__ void d8_mma(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
@@ -527,17 +528,18 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
-  issue(0);
-
+  // the bank's bf16 codebooks (Dev::cb_bf) ride in the first cp.async group; they are needed from the first far unit on
   if (has_cb && A.n_act > 0) {
-    const float4* srck = reinterpret_cast<const float4*>(V.cbk + (size_t)b * 2048);
-    const float4* srcv = reinterpret_cast<const float4*>(V.cbv + (size_t)b * 2048);
-    for (int e = tid; e < 512; e += kD2Threads) {
-      const float4 a = srck[e], c = srcv[e];
-      *reinterpret_cast<uint2*>(sm + e * 8) = make_uint2(d2_pack(a.x, a.y), d2_pack(a.z, a.w));
-      *reinterpret_cast<uint2*>(sm + 4096 + e * 8) = make_uint2(d2_pack(c.x, c.y), d2_pack(c.z, c.w));
+    const char* src = (const char*)(V.cb_bf + (size_t)b * 4096);
+    const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(sm);
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      d2_cp16(s0 + (r * 128 + tid) * 16, src + (r * 128 + tid) * 16);
+      d2_cp16(s0 + kD8CbV + (r * 128 + tid) * 16, src + 4096 + (r * 128 + tid) * 16);
     }
   }
+  issue(0);
+
   // Q^T as B fragments: column n = g is query row g; k-steps 2c, 2c + 1 <- chunk q = j + 4c
   uint32_t qb[8][2];
 #pragma unroll
@@ -550,7 +552,6 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
     }
     qb[2 * c][0] = val.x; qb[2 * c][1] = val.y; qb[2 * c + 1][0] = val.z; qb[2 * c + 1][1] = val.w;
   }
-  __syncthreads();
 
   float o[8][4];
 #pragma unroll
@@ -558,10 +559,12 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
   D2Soft S{-INFINITY, -INFINITY, 0.f, 0.f};                     // rows 2j (m0, l0) and 2j + 1 (m1, l1)
   const float sc2 = kD2Log2e * rsqrtf(128.f);
   const unsigned char* cbK = sm;
-  const unsigned char* cbV = sm + 4096;
+  const unsigned char* cbV = sm + kD8CbV;
 
+  bool cb_ready = false;                                        // exactly one block barrier per warp: codebooks visible
   for (int i = 0; i < ntot; ++i) {
     asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (i == nn) { __syncthreads(); cb_ready = true; }          // first far unit of this warp (warp-uniform)
     __syncwarp();
     issue(i + 1);
     const unsigned char* stg = ring + (i % kD8Stages) * kD8StageBytes;
@@ -599,7 +602,7 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
       const float* lns = reinterpret_cast<const float*>(stg + 4608);
       const uint32_t* zks = reinterpret_cast<const uint32_t*>(stg + 4096);
       const uint32_t* zvs = reinterpret_cast<const uint32_t*>(stg + 4352);
-#pragma unroll 1
+#pragma unroll
       for (int ss = 0; ss < 4; ++ss) {
         if (k0 + 2 * ss >= A.n_act) break;
         int kind[2];
@@ -663,6 +666,7 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
     }
   }
   asm volatile("cp.async.wait_group 0;" ::: "memory");
+  if (!cb_ready) __syncthreads();                               // a warp without far units still owes the codebook barrier
   __syncthreads();
 
   // ---- merge the four warps' (m, l, O^T) and write this CTA's partial ----

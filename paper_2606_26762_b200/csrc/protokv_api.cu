@@ -213,6 +213,7 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
     if (decode2_attention_supported(D, 1)) {
       v.c_bf = (__nv_bfloat16*)take(BK * D.d * 2);
       v.p_bf = (__nv_bfloat16*)take(BK * D.d * 2);
+      if (has_cb) v.cb_bf = (__nv_bfloat16*)take((size_t)D.B * 2 * D.G * D.C * D.sub * 2);
     }
   }
   v.n = (int*)take(BK * 4); v.mu = (float*)take(BK * 8); v.sigma = (float*)take(BK * 12);
@@ -330,6 +331,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
     const size_t cb = (size_t)st->D.B * st->D.G * st->D.C * st->D.sub * 4;
     e = cudaMemcpyAsync(st->V.cbk, cfg->codebook_k, cb, cudaMemcpyDeviceToDevice, st->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st->V.cbv, cfg->codebook_v, cb, cudaMemcpyDeviceToDevice, st->stream);
+    if (e == cudaSuccess) { st->launches += launch_codebook_copy(st->D, st->V, st->V.cbk, st->V.cbv, st->stream); e = cudaGetLastError(); }
   }
   if (e == cudaSuccess) {   // numerators of Eq. 3 in log form (the host's libm, like the definition reads)
     st->logtab.resize(PKV_SYN_LOGTAB);
@@ -473,6 +475,7 @@ int protokv_train_codebooks(protokv_state* st) {
     return PROTOKV_OK;
   }
   st->launches += launch_kmeans(st->D, st->H, st->V, st->cb_store_k, st->cb_store_v, (long long)fill, st->stream);
+  st->launches += launch_codebook_copy(st->D, st->V, st->cb_store_k, st->cb_store_v, st->stream);
   PKV_CUDA(cudaGetLastError());
   st->V.cbk = st->cb_store_k; st->V.cbv = st->cb_store_v;     // from now on Alg. 1 l.13 updates the histograms
   st->codes_valid = false;

@@ -863,6 +863,19 @@ int launch_fill_u32(uint32_t* dst, uint32_t value, size_t n, cudaStream_t s) {
   return 1;
 }
 
+__global__ void codebook_copy_kernel(__nv_bfloat16* dst, const float* cbk, const float* cbv, size_t per_bank, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t b = i / (2 * per_bank), r = i % (2 * per_bank);
+    dst[i] = __float2bfloat16_rn(r < per_bank ? cbk[b * per_bank + r] : cbv[b * per_bank + r - per_bank]);
+  }
+}
+int launch_codebook_copy(const Dims& D, const Dev& V, const float* cbk, const float* cbv, cudaStream_t s) {
+  if (!V.cb_bf || !cbk) return 0;
+  const size_t per_bank = (size_t)D.G * D.C * D.sub, n = (size_t)D.B * 2 * per_bank;
+  codebook_copy_kernel<<<(unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, s>>>(V.cb_bf, cbk, cbv, per_bank, n);
+  return 1;
+}
+
 __global__ void or_u32_kernel(uint32_t* dst, uint32_t bits) { atomicOr(dst, bits); }
 int launch_or_u32(uint32_t* dst, uint32_t bits, cudaStream_t s) {
   or_u32_kernel<<<1, 1, 0, s>>>(dst, bits);
