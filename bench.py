@@ -340,8 +340,12 @@ def next_rows(spec, device):
     for K, V in frames:
         st.append_frame(K, V, s)
     st.synthesize()
+    Q1 = Q[:, :, :1].contiguous()
+    o1 = torch.empty_like(Q1)
     out["next3_rope_anchoring"] = dict(attention_ms=timed(lambda: st.query_attention_ex(Q, out=o, run_synthesis=False)),
-                                       attention_impl=st.stage_impl(1))
+                                       attention_impl=st.stage_impl(1),
+                                       one_token_query_ms=timed(lambda: st.query_attention_ex(Q1, n_q=1, out=o1, run_synthesis=False)),
+                                       note="attention_ms / one_token_query_ms include the fp64 sincos tables rebuilt per query")
     st.close()
     # NEXT-1: Alg. 2 maintenance, Table 5 defaults, in steady state
     st = mk(flags=B.MAINTENANCE)

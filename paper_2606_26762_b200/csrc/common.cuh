@@ -105,6 +105,7 @@ struct Dev {
   float2* ropeF;         // [Wf][d/2]       first position of the frame held in each ring slot
   float2* ropeP;         // [B][K][d/2]     anchor of every prototype
   float2* ropeQ;         // [Nq][d/2]       query tokens
+  float2* ropeR;         // [Wf * T][d/2]   every ring row at its stream position (what the decode-style kernel reads)
   uint32_t* nres;  // [B][K]
   ScoreRec* rec;   // [B * K / 2] pairs, see rec_slot()
   float* logn;     // [B][K]  log n_k (Eq. 4 bias)
@@ -252,6 +253,7 @@ int launch_attention_decode(const Dims& D, const Hyper& H, const Dev& V, const A
                             int* nsplit_out);
 // register-resident decode kernel (decode_attention2.cu): the default for n_q * group <= 16 rows per bank
 bool decode2_attention_supported(const Dims& D, int n_q);
+bool decode2_rope_supported(const Dims& D);
 bool decode2_attention_prepare();
 int decode2_max_splits();
 int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,

@@ -482,11 +482,31 @@ __device__ __forceinline__ void d8_pv(float (&o)[8][4], uint32_t b0, uint32_t b1
   }
 }
 
-__global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
+// Rotary embedding (PROTOKV_ROPE, D.1; readings 28-31) of 8 rotation pairs held as two 16-byte chunks: x =
+// dims [8q, 8q + 8) with q < 8, y = the partner dims [8q + 64, 8q + 72) -- the key-side chunk permutation keeps both in
+// one lane (chunks c and c + 2).  tab: the 8 (cos, sin) pairs of pair indices 8q .. 8q + 7 at the row's position.
+__device__ __forceinline__ void d8_rope8(uint4& x, uint4& y, const float2* __restrict__ tab) {
+  uint32_t xs[4] = {x.x, x.y, x.z, x.w}, ys[4] = {y.x, y.y, y.z, y.w};
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const float4 cs = __ldg(reinterpret_cast<const float4*>(tab) + t);       // (cos, sin) of pairs 2t, 2t + 1
+    const float xl = __uint_as_float(xs[t] << 16), xh = __uint_as_float(xs[t] & 0xffff0000u);
+    const float yl = __uint_as_float(ys[t] << 16), yh = __uint_as_float(ys[t] & 0xffff0000u);
+    xs[t] = d2_pack(fmaf(xl, cs.x, -yl * cs.y), fmaf(xh, cs.z, -yh * cs.w));
+    ys[t] = d2_pack(fmaf(yl, cs.x, xl * cs.y), fmaf(yh, cs.z, xh * cs.w));
+  }
+  x = make_uint4(xs[0], xs[1], xs[2], xs[3]);
+  y = make_uint4(ys[0], ys[1], ys[2], ys[3]);
+}
+
+// ROPE: keys and queries are rotated in registers on their way into the fragments.  blockIdx.z = block of 8 query rows: a
+// query of more rows (the multi-token prefill of a PROTOKV_ROPE state) runs as independent 8-row blocks over the same bank.
+template <bool ROPE>
+__global__ void __launch_bounds__(kD2Threads, ROPE ? 2 : kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
   extern __shared__ __align__(16) unsigned char sm[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, j = lane & 3;
-  const int bsel = blockIdx.y, split = blockIdx.x;
+  const int bsel = blockIdx.y, split = blockIdx.x, r0 = blockIdx.z * 8;   // first query row of this block
   const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
   const int b = (st * D.L + A.layer_begin + ll) * D.Hkv + hd;
   const bool has_cb = V.cbk != nullptr;
@@ -542,15 +562,25 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
 
   // Q^T as B fragments: column n = g is query row g; k-steps 2c, 2c + 1 <- chunk q = j + 4c
   uint32_t qb[8][2];
+  uint4 qv[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     uint4 val = make_uint4(0u, 0u, 0u, 0u);
-    if (g < A.R) {
-      const int qi = g / D.group, hh = g % D.group;
+    if (r0 + g < A.R) {
+      const int qi = (r0 + g) / D.group, hh = (r0 + g) % D.group;
       const size_t off = ((((size_t)st * A.layer_count + ll) * A.n_q + qi) * D.Hq + hd * D.group + hh) * 128 + (j + 4 * c) * 8;
       val = d2_ldg16(A.Q + off);
     }
-    qb[2 * c][0] = val.x; qb[2 * c][1] = val.y; qb[2 * c + 1][0] = val.z; qb[2 * c + 1][1] = val.w;
+    qv[c] = val;
+  }
+  if (ROPE && r0 + g < A.R) {                                    // query token qi sits at q_pos0 + qi (reading 29)
+    const float2* tq = V.ropeQ + (size_t)((r0 + g) / D.group) * 64;
+    d8_rope8(qv[0], qv[2], tq + 8 * j);
+    d8_rope8(qv[1], qv[3], tq + 8 * (j + 4));
+  }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    qb[2 * c][0] = qv[c].x; qb[2 * c][1] = qv[c].y; qb[2 * c + 1][0] = qv[c].z; qb[2 * c + 1][1] = qv[c].w;
   }
 
   float o[8][4];
@@ -572,12 +602,21 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
       const int base = (wi + i * NW) << 4;
       float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int ch = (j + 4 * c) ^ ((g & 1) << 2);
-        const uint4 ka = *reinterpret_cast<const uint4*>(stg + D2Stage::K + g * 256 + ch * 16);
-        const uint4 kb = *reinterpret_cast<const uint4*>(stg + D2Stage::K + (8 + g) * 256 + ch * 16);
-        d8_mma(s0, ka.x, kb.x, ka.y, kb.y, qb[2 * c][0], qb[2 * c][1]);
-        d8_mma(s1, ka.z, kb.z, ka.w, kb.w, qb[2 * c + 1][0], qb[2 * c + 1][1]);
+      for (int cp = 0; cp < 2; ++cp) {                          // chunks cp and cp + 2 hold the two halves of 8 rotation pairs
+        const int cha = (j + 4 * cp) ^ ((g & 1) << 2), chb = (j + 4 * cp + 8) ^ ((g & 1) << 2);
+        uint4 ka = *reinterpret_cast<const uint4*>(stg + D2Stage::K + g * 256 + cha * 16);
+        uint4 ka2 = *reinterpret_cast<const uint4*>(stg + D2Stage::K + g * 256 + chb * 16);
+        uint4 kb = *reinterpret_cast<const uint4*>(stg + D2Stage::K + (8 + g) * 256 + cha * 16);
+        uint4 kb2 = *reinterpret_cast<const uint4*>(stg + D2Stage::K + (8 + g) * 256 + chb * 16);
+        if (ROPE) {                                             // near tokens keep their stream positions (L126)
+          const int last = A.n_near - 1;
+          d8_rope8(ka, ka2, V.ropeR + (size_t)min(base + g, last) * 64 + 8 * (j + 4 * cp));
+          d8_rope8(kb, kb2, V.ropeR + (size_t)min(base + 8 + g, last) * 64 + 8 * (j + 4 * cp));
+        }
+        d8_mma(s0, ka.x, kb.x, ka.y, kb.y, qb[2 * cp][0], qb[2 * cp][1]);
+        d8_mma(s1, ka.z, kb.z, ka.w, kb.w, qb[2 * cp + 1][0], qb[2 * cp + 1][1]);
+        d8_mma(s0, ka2.x, kb2.x, ka2.y, kb2.y, qb[2 * cp + 4][0], qb[2 * cp + 4][1]);
+        d8_mma(s1, ka2.z, kb2.z, ka2.w, kb2.w, qb[2 * cp + 5][0], qb[2 * cp + 5][1]);
       }
       float x[4];
       const bool in0 = base + g < A.n_near, in1 = base + 8 + g < A.n_near;
@@ -628,6 +667,14 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
               const uint32_t z = (code >> (4 * gg)) & 15u;
               kr[h][c] = d2_add2x4(kr[h][c], *reinterpret_cast<const uint4*>(cbK + (gg * 16 + z) * 32 + (j & 1) * 16));
             }
+          }
+        }
+        if (ROPE) {                                             // the S pseudo-tokens of a prototype sit at its anchor (L126, D.1)
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const float2* tp = V.ropeP + ((size_t)b * D.K + min(k0 + 2 * ss + h, D.K - 1)) * 64;
+            d8_rope8(kr[h][0], kr[h][2], tp + 8 * j);
+            d8_rope8(kr[h][1], kr[h][3], tp + 8 * (j + 4));
           }
         }
         float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
@@ -688,7 +735,7 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
   __syncthreads();
   {
     const int r = tid >> 4, d0 = (tid & 15) * 8;          // 8 rows x 16 threads, 8 dims each
-    if (r < A.R) {
+    if (r0 + r < A.R) {
       const float* mlb = reinterpret_cast<const float*>(sm + kD8Ring + 4 * 8 * 128 * 4);
       float M = -INFINITY;
 #pragma unroll
@@ -700,7 +747,7 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
         wgt[w] = d2_ex2(mlb[w * 16 + r * 2] - Mu);
         l = fmaf(mlb[w * 16 + r * 2 + 1], wgt[w], l);
       }
-      float* dst = A.part + (((size_t)bsel * A.R + r) * A.nsplit + split) * 130;
+      float* dst = A.part + (((size_t)bsel * A.R + r0 + r) * A.nsplit + split) * 130;
       const float* Ob = reinterpret_cast<const float*>(sm + kD8Ring);
 #pragma unroll
       for (int e = 0; e < 8; e += 4) {
@@ -721,6 +768,11 @@ __global__ void __launch_bounds__(kD2Threads, kD8CtasPerSm) attention_decode8_ke
   }
 }
 
+// PROTOKV_ROPE states: any number of query rows (8-row blocks)
+bool decode2_rope_supported(const Dims& D) {
+  return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && D.K % 8 == 0;
+}
+
 bool decode2_attention_supported(const Dims& D, int n_q) {
   return D.bf16 && D.d == 128 && D.S == 8 && D.G == 8 && D.C == 16 && n_q * D.group <= kD2Rows && D.K % 8 == 0;   // (Dev::c_bf exists for exactly these shapes)
 }
@@ -731,8 +783,10 @@ bool decode2_attention_prepare() {
     cudaGetLastError();
     return false;
   }
-  if (cudaFuncSetAttribute(attention_decode8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
-      cudaSuccess) {
+  if (cudaFuncSetAttribute(attention_decode8_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+          cudaSuccess ||
+      cudaFuncSetAttribute(attention_decode8_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+          cudaSuccess) {
     cudaGetLastError();
     return false;
   }
@@ -759,17 +813,22 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   int cap = (units + kD2Warps - 1) / kD2Warps;
   if (cap > decode2_max_splits()) cap = decode2_max_splits();
   if (cap < 1) cap = 1;
-  const bool rows8 = a.R <= 8;                                 // the N = 8 variant: three CTAs per SM
-  const int slots = (rows8 ? kD8CtasPerSm : kD2CtasPerSm) * sm_count;
+  const bool rope = (H.flags & PROTOKV_ROPE) != 0;
+  const bool rows8 = rope || a.R <= 8;                         // the N = 8 variant; with ROPE every query runs as 8-row blocks
+  const int nrb = rows8 ? (a.R + 7) / 8 : 1;
+  const int slots = (rope ? 2 : (rows8 ? kD8CtasPerSm : kD2CtasPerSm)) * sm_count;
+  const long long room = ((long long)D.B * 16 * decode2_max_splits()) / ((long long)nb * a.R);   // partials the buffer holds per row
+  if (cap > room) cap = room < 1 ? 1 : (int)room;
   int ns = 1;
   double best = 1e30;
   for (int c = 1; c <= cap; ++c) {
-    const double cost = (double)(((long long)nb * c + slots - 1) / slots) / c * (1.0 + 0.02 * c);   // + per-CTA fixed work
+    const double cost = (double)(((long long)nb * nrb * c + slots - 1) / slots) / c * (1.0 + 0.02 * c);   // + per-CTA fixed work
     if (cost < best * 0.97) { best = cost; ns = c; }
   }
   a.nsplit = ns;
   *nsplit_out = ns;
-  if (rows8) attention_decode8_kernel<<<dim3(ns, nb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  if (rope) attention_decode8_kernel<true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  else if (rows8) attention_decode8_kernel<false><<<dim3(ns, nb, 1), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
   else attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
   return 1;
 }

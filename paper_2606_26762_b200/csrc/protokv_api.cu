@@ -40,6 +40,7 @@ struct protokv_state {
   bool use_tc_attn;
   bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
   bool use_decode2;       // the register-resident decode kernel serves them (default where supported)
+  bool use_decode_rope;   // PROTOKV_ROPE state served by the rotating variant of that kernel (any number of query rows)
   TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
@@ -210,7 +211,7 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
   if (D.bf16) {
     v.c_hi = (__nv_bfloat16*)take(BK * D.d * 2);
     v.c_lo = (__nv_bfloat16*)take(BK * D.d * 2);
-    if (decode2_attention_supported(D, 1)) {
+    if (decode2_rope_supported(D)) {
       v.c_bf = (__nv_bfloat16*)take(BK * D.d * 2);
       v.p_bf = (__nv_bfloat16*)take(BK * D.d * 2);
       if (has_cb) v.cb_bf = (__nv_bfloat16*)take((size_t)D.B * 2 * D.G * D.C * D.sub * 2);
@@ -223,6 +224,7 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
     const size_t h = (size_t)D.d / 2;
     v.ropeJ = (float2*)take((size_t)D.T * h * 8); v.ropeF = (float2*)take((size_t)D.Wf * h * 8);
     v.ropeP = (float2*)take(BK * h * 8); v.ropeQ = (float2*)take((size_t)D.Nq * h * 8);
+    v.ropeR = (float2*)take((size_t)D.Wf * D.T * h * 8);
   }
   v.rec = (ScoreRec*)take((BK + 1) * sizeof(ScoreRec)); v.logn = (float*)take(BK * 4);
   v.hist = (uint32_t*)take(BK * 2 * D.G * D.C * 4);
@@ -255,7 +257,7 @@ static size_t carve(const Dims& D, const Hyper& H, bool has_cb, bool rope, int n
   size_t part_bytes = rows * nsplit * (D.d + 2) * 4;
   if (tc_attention_supported(D) && tc_attention_part_bytes(D) > part_bytes) part_bytes = tc_attention_part_bytes(D);
   if (decode_attention_supported(D, 1) && decode_attention_part_bytes(D) > part_bytes) part_bytes = decode_attention_part_bytes(D);
-  if (decode2_attention_supported(D, 1)) {
+  if (decode2_rope_supported(D)) {
     const size_t need = (size_t)D.B * 16 * decode2_max_splits() * 130 * 4;
     if (need > part_bytes) part_bytes = need;
   }
@@ -366,6 +368,8 @@ protokv_state* protokv_create(const protokv_config* cfg) {
                         decode_attention_prepare();
   st->use_decode2 = want_tc && !rope && !st->use_decode_attn && !(cfg->flags & PROTOKV_NO_DECODE_KERNEL) &&
                     decode2_attention_supported(st->D, 1) && decode2_attention_prepare();
+  st->use_decode_rope = want_tc && (cfg->flags & PROTOKV_ROPE) && !(cfg->flags & (PROTOKV_VAR_ALLOC | PROTOKV_NO_DECODE_KERNEL)) &&
+                        decode2_rope_supported(st->D) && decode2_attention_prepare();
   return st;
 }
 
@@ -543,6 +547,12 @@ int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, in
       st->launches += launch_attention_decode(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
       st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+    } else if (st->use_decode_rope && (uintptr_t)Q % 16 == 0) {
+      int ns = 1;
+      st->launches += launch_rope_tables(D, st->H, st->V, A, st->stream);
+      st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
+      A.nsplit = ns;
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
     } else if (st->use_decode2 && decode2_attention_supported(D, n_q) && (uintptr_t)Q % 16 == 0) {
       int ns = 1;
       st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
@@ -613,9 +623,11 @@ int protokv_error_flags(protokv_state* st, uint32_t* flags, int32_t clear) {
 const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
   if (!st) return "none";
   if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
-  if (stage == 1) return st->use_tc_attn ? "tcgen05" : "simt";
+  if (stage == 1) return st->use_tc_attn ? "tcgen05" : (st->use_decode_rope ? "mma.sync register-resident (rope)" : "simt");
   if (stage == 2)
-    return st->use_decode_attn ? "mma.sync split-KV" : (st->use_decode2 ? "mma.sync register-resident" : (st->use_tc_attn ? "tcgen05" : "simt"));
+    return st->use_decode_attn ? "mma.sync split-KV"
+           : (st->use_decode2 ? "mma.sync register-resident"
+              : (st->use_decode_rope ? "mma.sync register-resident (rope)" : (st->use_tc_attn ? "tcgen05" : "simt")));
   return "none";
 }
 

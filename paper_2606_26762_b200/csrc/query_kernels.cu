@@ -316,7 +316,7 @@ __global__ void rope_tables_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
   for (int i = threadIdx.x; i < h; i += blockDim.x) inv_freq[i] = pow(H.rope_theta, -2.0 * (double)i / (double)D.d);
   __syncthreads();
   const long long nJ = (long long)D.T * h, nF = (long long)D.Wf * h, nQ = (long long)A.n_q * h;
-  const long long nP = (long long)D.B * D.K * h, total = nJ + nF + nQ + nP;
+  const long long nP = (long long)D.B * D.K * h, nR = (long long)D.Wf * D.T * h, total = nJ + nF + nQ + nP + nR;
   for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
     double p;
     float2* dst;
@@ -334,6 +334,13 @@ __global__ void rope_tables_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
       i = (int)(x % h);
       p = (double)(A.q_pos0 + x / h);
       dst = V.ropeQ + x;
+    } else if (e >= nJ + nF + nQ + nP) {     // ring row (slot, j) at the position of the frame the slot holds
+      const long long x = e - nJ - nF - nQ - nP;
+      i = (int)(x % h);
+      const long long row = x / h, slot = row / D.T, last = A.frames - 1;
+      const long long f = last >= slot ? last - ((last - slot) % D.Wf) : 0;
+      p = (double)(H.pos0 + f * D.T + row % D.T);
+      dst = V.ropeR + x;
     } else {
       const long long x = e - nJ - nF - nQ;
       i = (int)(x % h);
@@ -352,7 +359,7 @@ __global__ void rope_tables_kernel(Dims D, Hyper H, Dev V, AttnArgs A) {
 
 int launch_rope_tables(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s) {
   const int h = D.d / 2;
-  const long long total = (long long)(D.T + D.Wf + A.n_q) * h + (long long)D.B * D.K * h;
+  const long long total = (long long)(D.T + D.Wf + A.n_q) * h + (long long)D.B * D.K * h + (long long)D.Wf * D.T * h;
   const unsigned grid = (unsigned)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
   rope_tables_kernel<<<grid, 256, (size_t)h * 8, s>>>(D, H, V, A);
   return 1;

@@ -40,7 +40,7 @@ def test_workspace_bytes_is_host_only_and_scales():
     b = pkv.protokv_workspace_bytes(_cfg(n_layers=2))
     assert a > 0 and 1.4 * a < b < 2.1 * a     # a constant split-KV scratch term does not scale
     # config 2: ring 2 * 4 * 16 * 196 * 128 * 2 B = 6.4 MB, bank fp32 centres 2 * 4 * 1024 * 128 * 4 = 4.2 MB, ...
-    assert 15e6 < a < 40e6
+    assert 15e6 < a < 45e6     # (+ 2 MB of bf16 centre copies for the decode-style kernel since round 2)
     assert a % 256 == 0
 
 

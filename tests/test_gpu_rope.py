@@ -10,7 +10,7 @@ import pytest
 import gen
 from gpu_helpers import make_gpu, make_oracles, run_stream, compare_codes, compare_attention
 from oracle import FLAG_ROPE, FLAG_MAINTENANCE
-from paper_2606_26762_b200 import ROPE, MAINTENANCE
+from paper_2606_26762_b200 import ROPE, MAINTENANCE, FORCE_SIMT
 
 pytestmark = pytest.mark.gpu
 
@@ -34,11 +34,14 @@ def test_rope_c1_all_anchor_variants(anchor):
     assert (a - b).abs().max() > 1e-3
 
 
-def test_rope_bf16_gqa_shape_long_positions():
-    # config-2 shape (bf16, d = 128, GQA 28/4), default base 1e6, positions beyond 10^6 (pos0): fp32 angles would be off
+@pytest.mark.parametrize("route,impl", [(0, "mma.sync register-resident (rope)"), (FORCE_SIMT, "simt")])
+def test_rope_bf16_gqa_shape_long_positions(route, impl):
+    # config-2 shape (bf16, d = 128, GQA 28/4), default base 1e6, positions beyond 10^6 (pos0): fp32 angles would be off.
+    # Default route: the rotating variant of the register-resident kernel (8-row blocks); cross-check: the fp32 SIMT kernel
     spec = gen.spec_for("c2", n_frames=26)
     hyper = dict(pos0=1_500_000)
-    gpu = make_gpu(spec, flags=ROPE, **hyper)
+    gpu = make_gpu(spec, flags=ROPE | route, **hyper)
+    assert gpu.stage_impl(1) == impl
     oracles = make_oracles(spec, [0, 3], flags=FLAG_ROPE, **hyper)
     run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=13)
     compare_codes(gpu, oracles, spec.G)
@@ -56,3 +59,26 @@ def test_rope_with_maintenance_merges_anchors():
     assert gpu.maintenance_counters()["merges"] > 0
     compare_codes(gpu, oracles, spec.G)
     compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=False)
+
+
+@pytest.mark.parametrize("anchor", [0, 1, 2])
+def test_rope_decode_query_anchor_variants(anchor):
+    """One- and three-token queries (7 / 21 rows per bank) of a bf16 state through the rotating decode kernel at every stage
+    of a stream (partial window, bank filling, steady state), all three D.1 anchors."""
+    spec = gen.spec_for("c2", n_frames=30)
+    hyper = dict(rope_anchor=anchor, pos0=250_000)
+    gpu = make_gpu(spec, flags=ROPE, **hyper)
+    assert gpu.stage_impl(2) == "mma.sync register-resident (rope)"
+    oracles = make_oracles(spec, [1, 2], flags=FLAG_ROPE, **hyper)
+    Q = gen.queries(spec, 3)
+    from gpu_helpers import step_teacher_forced, new_stats
+    stats = new_stats()
+    s = gen.grid_positions(spec)
+    for f in range(spec.n_frames):
+        K, V = gen.frame_kv(spec, f)
+        step_teacher_forced(spec, gpu, oracles, f, K, V, s, stats)
+        if f in (3, 18, 22, 29):
+            nq = 1 if f % 2 else 3
+            compare_attention(spec, gpu, oracles, Q[:, :, 2:2 + nq].contiguous(), run_synthesis=True)
+    compare_attention(spec, gpu, oracles, Q[:, :, :1].contiguous(), run_synthesis=False, q_pos0=7)
+    gpu.close()
