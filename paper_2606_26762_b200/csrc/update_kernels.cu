@@ -525,14 +525,14 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   uint32_t* sorted = keys + Tpad;                             // [Tpad]
   int* segstart = (int*)(sorted + Tpad);                      // [Tpad + 1]
   __shared__ int wtot[kUfWarps];
-  __shared__ int nseg_s, nmine_s;
+  __shared__ int nseg_s, nmine_s, next_task_s;
 
   const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int ntok_all = D.T - F.n_fill;
   const bool has_cb = V.cbk != nullptr;
   const size_t bt = (size_t)b * D.T;
   const size_t rrow = ((size_t)b * D.Wf + F.slot) * D.T;      // ring row of evicted token 0
-  if (tid == 0) nmine_s = 0;
+  if (tid == 0) { nmine_s = 0; next_task_s = 0; }
   __syncthreads();
   // CTA x of the bank's gridDim.x CTAs owns the prototypes k with k mod gridDim.x == x: it keeps only the tokens
   // assigned to those, so that the sort below is over ~T / gridDim.x keys instead of T in every CTA
@@ -623,7 +623,13 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
 
   // A task = (segment, side): the key side replays c, mu, Sigma and the K histogram, the value side p and the V
   // histogram -- two independent dependency chains, so a segment's latency is that of the longer one
-  for (int task = warp; task < 2 * nseg; task += kUfWarps) {
+  // tasks are handed out dynamically (one shared counter per CTA): segments differ in length and the key side is the
+  // heavier one, so a static round-robin leaves the CTA waiting for its unluckiest warp
+  for (;;) {
+    int task = 0;
+    if (lane == 0) task = atomicAdd(&next_task_s, 1);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task >= 2 * nseg) break;
     const int seg = task >> 1, side = task & 1;
     const int r0 = segstart[seg], r1 = segstart[seg + 1];
     const int k = (int)(sorted[r0] >> 12);
