@@ -61,13 +61,16 @@ enum {
   PROTOKV_NEAR_ONLY = 8u,    /* attention over the near window only (L176)                              */
   PROTOKV_FAR_ONLY = 16u,    /* attention over pseudo-tokens only   (L177)                              */
   PROTOKV_FORCE_SIMT = 32u,  /* use the fp32 SIMT kernels even where a tcgen05 kernel exists (cross-check) */
-  PROTOKV_DECODE_SPLITKV = 128u, /* serve queries of <= 16 rows per bank with the split-KV mma.sync kernel
-                                (csrc/decode_attention.cu) instead of the 128-row tcgen05 kernel.  Measured on C3 (one
-                                query token, 7 rows per bank): 167-183 us against 161 us -- not faster, hence opt-in */
+  PROTOKV_DECODE_SPLITKV = 128u, /* serve queries of <= 16 rows per bank with the shared-memory split-KV mma.sync kernel
+                                (csrc/decode_attention.cu): the first decode kernel, kept as a cross-check (167-183 us
+                                on the C3 one-token query).  The default route for such queries is the register-resident
+                                kernel of csrc/decode_attention2.cu (86 us); the 128-row tcgen05 kernel takes 161 us */
   PROTOKV_ROPE = 256u,       /* rotary position anchoring (D.1 L578-596; readings 28-31): K and Q
                                 are given UN-ROTATED; the attention rotates near tokens at their stream positions, the S
-                                pseudo-tokens of prototype k at its anchor and the query tokens at q_pos0 + i.  Served by
-                                the fp32 SIMT attention kernel (the tcgen05 kernel has no rotation stage) */
+                                pseudo-tokens of prototype k at its anchor and the query tokens at q_pos0 + i.  bf16 states
+                                with head_dim 128 are served by the rotating variant of the register-resident kernel
+                                (csrc/decode_attention2.cu; queries of any length run as 8-row blocks), other shapes by
+                                the fp32 SIMT kernel; the tcgen05 prefill kernel has no rotation stage */
   PROTOKV_NO_DECODE_KERNEL = 4096u, /* serve queries of <= 16 rows per bank with the 128-row tcgen05 kernel instead of
                                 the register-resident decode kernel (csrc/decode_attention2.cu, the default): cross-check */
   PROTOKV_WARMUP = 512u,     /* PQ codebook warm-up (readings 32-36): cfg.codebook_k/v are
@@ -280,8 +283,9 @@ enum {
 int protokv_profile_enable(protokv_state *st, int32_t on);
 int protokv_profile_read(protokv_state *st, double *ms_sum, int64_t *launches);
 
-/* Names the kernel variant each stage uses for this state ("simt" / "tcgen05"), for reports.
- * stage: 0 = assignment, 1 = attention.  Returns a static string, never NULL. */
+/* Names the kernel variant each stage uses for this state, for reports: "simt", "tcgen05", "mma.sync register-resident"
+ * (+ " (rope)"), "mma.sync split-KV".  stage: 0 = assignment, 1 = attention (multi-token queries), 2 = attention of
+ * decode-style queries (<= 16 rows per bank).  Returns a static string, never NULL. */
 const char *protokv_stage_impl(const protokv_state *st, int32_t stage);
 
 #ifdef __cplusplus
