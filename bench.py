@@ -140,8 +140,10 @@ def make_state(spec, device):
 
 
 def steady_state_frames(spec):
-    """Frames to stream before the ring and the bank are full (+2 so that every prototype has absorbed tokens)."""
-    return spec.near_frames + math.ceil(spec.k_max / spec.T) + 2
+    """Frames to stream before the timed region: ring and bank full, plus 12 frames of absorptions so that most prototypes
+    carry residual statistics (two frames after the bank fills two thirds of them still have n_res = 0 and their
+    pseudo-tokens need no codeword: an easier query than a long stream's)."""
+    return spec.near_frames + math.ceil(spec.k_max / spec.T) + 12
 
 
 def run_workload(spec, device, steps, warmup, rank=0, do_e2e=True, do_profile=True, sampler=None, barrier=None):

@@ -49,10 +49,23 @@ def test_workspace_bytes_is_host_only_and_scales():
     (dict(C=17), "C <= 16"), (dict(G=3), "G in"), (dict(beam=4), "beam"), (dict(tokens_per_frame=0), "shape"),
     (dict(tokens_per_frame=5000), "4096"), (dict(alpha=1.5), "alpha"), (dict(pq_eps=0.0), "pq_eps"),
     (dict(flags=pkv.NEAR_ONLY | pkv.FAR_ONLY), "exclusive"), (dict(G=1, C=2, S=8, beam=8), "C^G"),
+    (dict(flags=pkv.WARMUP, t_warm=0), "warm-up"), (dict(flags=pkv.WARMUP, t_warm=8, km_batch=4096), "warm-up"),
+    (dict(flags=pkv.WARMUP_MANUAL), "WARMUP_MANUAL"), (dict(flags=pkv.VAR_ALLOC, s_cap=33), "s_cap"),
+    (dict(flags=pkv.VAR_ALLOC, s_cap=0), "s_cap"), (dict(flags=pkv.ROPE, rope_anchor=3), "rope"),
 ])
 def test_invalid_configs_are_rejected_with_a_message(kw, code_substr):
     assert pkv.protokv_workspace_bytes(_cfg(**kw)) == 0
     assert code_substr in pkv.protokv_last_error()
+
+
+def test_optional_rows_change_the_workspace_only_by_their_own_arrays():
+    base = pkv.protokv_workspace_bytes(_cfg())
+    warm = pkv.protokv_workspace_bytes(_cfg(flags=pkv.WARMUP, t_warm=40, warm_reservoir=2048))
+    # two reservoirs of 2,048 x 128 fp32 rows per bank + claim words + the per-frame slot plan
+    assert warm - base >= 4 * (2 * 2048 * 128 * 4 + 2048 * 8 + 196 * 4)
+    assert warm - base < 4 * (2 * 2048 * 128 * 4 + 2048 * 8 + 196 * 4) + 4096
+    var = pkv.protokv_workspace_bytes(_cfg(flags=pkv.VAR_ALLOC))
+    assert 0 < var - base < 4 * 1024 * 32 + 4096
 
 
 def test_struct_size_is_checked():
