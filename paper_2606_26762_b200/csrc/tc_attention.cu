@@ -631,9 +631,14 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
 }
 
 // Merges the pieces of every item: one warp per output row, 4 dims per lane.
+// WIDE = false: one warp per query row (few pieces per item: the batched query).  WIDE = true: one CTA per row, the four
+// warps take every fourth piece and merge through shared memory (few items cut into many pieces: a per-layer call, where
+// a single warp walking 37 pieces with four loads in flight was a 17 us latency chain).
+template <bool WIDE>
 __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArgs A, AtPlan P, const float* part,
                                                                    __nv_bfloat16* out, float* lse, int rows_total) {
-  const int gr = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const int wq = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int gr = WIDE ? (int)blockIdx.x : (int)blockIdx.x * 4 + wq;
   if (gr >= rows_total) return;
   const int Rb = A.n_q * D.group;
   const int bsel = gr / Rb, rr = gr % Rb;
@@ -653,26 +658,49 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
   float M = -INFINITY, l = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   bool poisoned = false;   // a piece with a NaN row sum (non-finite logits): the row is NaN, like the SIMT path returns it
-  for (int sp0 = 0; sp0 < np; sp0 += 4) {
+  const int pstep = WIDE ? 4 : 1, pfirst = WIDE ? wq : 0;    // this warp's pieces: pfirst, pfirst + pstep, ...
+  for (int sp0 = 0; pfirst + sp0 * pstep < np; sp0 += 4) {
     float2 ml[4];
     float4 v[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      const int sp = sp0 + u < np ? sp0 + u : np - 1;        // clamp: a repeated piece is skipped below
+      const int want = pfirst + (sp0 + u) * pstep;
+      const int sp = want < np ? want : np - 1;              // clamp: a repeated piece is skipped below
       const float* ps = base + sp * pstride;
       ml[u] = *reinterpret_cast<const float2*>(ps + 128);
       v[u] = *reinterpret_cast<const float4*>(ps + lane * 4);
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      if (sp0 + u < np && ml[u].y != ml[u].y) poisoned = true;
-      if (sp0 + u >= np || !(ml[u].y > 0.f)) continue;
+      const bool have = pfirst + (sp0 + u) * pstep < np;
+      if (have && ml[u].y != ml[u].y) poisoned = true;
+      if (!have || !(ml[u].y > 0.f)) continue;
       const float Mn = fmaxf(M, ml[u].x);
       const float so = __expf(M - Mn), sn = __expf(ml[u].x - Mn);   // M = -inf: so = 0
       l = fmaf(l, so, ml[u].y * sn);
       acc.x = fmaf(acc.x, so, v[u].x * sn); acc.y = fmaf(acc.y, so, v[u].y * sn);
       acc.z = fmaf(acc.z, so, v[u].z * sn); acc.w = fmaf(acc.w, so, v[u].w * sn);
       M = Mn;
+    }
+  }
+  if (WIDE) {                                                 // merge the four warps' running (M, l, acc)
+    __shared__ float4 sacc[4][32];
+    __shared__ float sml[4][2];
+    __shared__ int spois[4];
+    sacc[wq][lane] = acc;
+    if (lane == 0) { sml[wq][0] = M; sml[wq][1] = l; spois[wq] = poisoned ? 1 : 0; }
+    __syncthreads();
+    if (wq != 0) return;
+    M = fmaxf(fmaxf(sml[0][0], sml[1][0]), fmaxf(sml[2][0], sml[3][0]));
+    l = 0.f; acc = make_float4(0.f, 0.f, 0.f, 0.f); poisoned = false;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      poisoned = poisoned || spois[w] != 0;
+      if (!(sml[w][1] > 0.f)) continue;
+      const float sn = __expf(sml[w][0] - M);
+      const float4 x = sacc[w][lane];
+      l = fmaf(sml[w][1], sn, l);
+      acc.x = fmaf(x.x, sn, acc.x); acc.y = fmaf(x.y, sn, acc.y); acc.z = fmaf(x.z, sn, acc.z); acc.w = fmaf(x.w, sn, acc.w);
     }
   }
   float inv = l > 0.f ? 1.f / l : 0.f;
@@ -743,7 +771,10 @@ int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnA
     ++launched;
   }
   const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
-  attention_tc_combine_kernel<<<(rows_total + 3) / 4, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+  if (P.nsplit > 8)
+    attention_tc_combine_kernel<true><<<rows_total, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+  else
+    attention_tc_combine_kernel<false><<<(rows_total + 3) / 4, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
   return launched + 1;
 }
 
