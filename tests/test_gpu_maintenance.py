@@ -43,6 +43,9 @@ def test_maintenance_all_three_passes(name, force_simt):
     assert sum(int(gpu.export_state(b)["n"].sum()) for b in banks) == absorbed - got["decayed"] + got["recycled"]
     compare_codes(gpu, oracles, spec.G)
     compare_attention(spec, gpu, oracles, gen.queries(spec, 0), run_synthesis=True)
+    # decode-style queries over a bank with merged-away (absent) slots in the middle of the active prefix
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 1)[:, :, :1].contiguous(), run_synthesis=False)
+    compare_attention(spec, gpu, oracles, gen.queries(spec, 1)[:, :, 1:3].contiguous(), run_synthesis=False)
 
 
 # neutral settings: Alg. 2 runs every frame and must leave the plain path untouched, bit for bit in the integers

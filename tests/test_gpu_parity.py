@@ -528,3 +528,16 @@ def test_decode_query_c5_shape():
             nq = {3: 1, 9: 4, 11: 3, 15: 4}[f]
             compare_attention(spec, gpu, oracles, Q[:, :, :nq].contiguous(), run_synthesis=True)
     gpu.close()
+
+
+def test_decode_query_without_codebooks():
+    """No residual statistics (Table 2 "w/o residual stats"): every prototype contributes S copies of (c_k, p_k); the decode
+    kernels must not touch a codebook."""
+    spec = gen.spec_for("c2", n_frames=30)
+    gpu = make_gpu(spec, with_codebooks=False)
+    oracles = make_oracles(spec, [0, 2], with_codebooks=False)
+    run_stream(spec, gpu, oracles, spec.n_frames, check_state_every=0, with_codebooks=False)
+    Q = gen.queries(spec, 4)
+    compare_attention(spec, gpu, oracles, Q[:, :, :1].contiguous(), run_synthesis=True)
+    compare_attention(spec, gpu, oracles, Q[:, :, :2].contiguous(), run_synthesis=False)
+    gpu.close()

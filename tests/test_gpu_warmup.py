@@ -63,6 +63,8 @@ def test_reservoir_kmeans_and_the_stream_after_the_warmup(name, t_warm, R, after
     compare_codes(gpu, orc, spec.G)
     compare_attention(spec, gpu, orc, gen.queries(spec, 0), run_synthesis=False, use_gpu_codes=True,
                       rows_sample=range(0, spec.n_query_tokens * (spec.n_q_heads // spec.n_kv_heads), 5))
+    # a decode-style query reads the bf16 copies of the TRAINED codebooks (Dev::cb_bf, rewritten by the training)
+    compare_attention(spec, gpu, orc, gen.queries(spec, 2)[:, :, :1].contiguous(), run_synthesis=False, use_gpu_codes=True)
     assert gpu.error_flags() == 0
     gpu.close()
 
