@@ -81,7 +81,8 @@ enum {
   PROTOKV_WARMUP_MANUAL = 1024u, /* with PROTOKV_WARMUP: the training is started by protokv_train_codebooks instead */
   PROTOKV_VAR_ALLOC = 2048u, /* D.3 (readings 37-40): variance-aware pseudo-token counts
                                 S_k = S_tot Var(H_k) / sum_j Var(H_j) under S_tot = k_max S, 1 <= S_k <= s_cap, recomputed by
-                                every synthesis; served by the fp32 SIMT attention kernel (ragged pseudo-token counts) */
+                                every synthesis; bf16 states with head_dim 128 are served by the ragged variant of the
+                                register-resident kernel (8-row blocks), other shapes by the fp32 SIMT kernel */
   PROTOKV_MAINTENANCE = 64u  /* run Alg. 2 at the end of every append_frame that evicted a frame
                                 (Alg. 1 l.15); off by default: north_star's path and its invariant "total mass = tokens
                                 absorbed" exclude it (reading 19) */
@@ -284,7 +285,7 @@ int protokv_profile_enable(protokv_state *st, int32_t on);
 int protokv_profile_read(protokv_state *st, double *ms_sum, int64_t *launches);
 
 /* Names the kernel variant each stage uses for this state, for reports: "simt", "tcgen05", "mma.sync register-resident"
- * (+ " (rope)"), "mma.sync split-KV".  stage: 0 = assignment, 1 = attention (multi-token queries), 2 = attention of
+ * (+ " (blocks)": the rotating / ragged 8-row-block variants), "mma.sync split-KV".  stage: 0 = assignment, 1 = attention (multi-token queries), 2 = attention of
  * decode-style queries (<= 16 rows per bank).  Returns a static string, never NULL. */
 const char *protokv_stage_impl(const protokv_state *st, int32_t stage);
 

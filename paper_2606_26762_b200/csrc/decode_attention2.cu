@@ -142,6 +142,9 @@ static_assert(kD2Warps * kD2Stages * kD2StageBytes >= D2Smem::Total - D2Smem::O,
 __device__ __forceinline__ void d2_cp16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
+__device__ __forceinline__ void d2_cp4(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
 __device__ __forceinline__ void d2_cp8(uint32_t dst, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
@@ -501,8 +504,11 @@ __device__ __forceinline__ void d8_rope8(uint4& x, uint4& y, const float2* __res
 
 // ROPE: keys and queries are rotated in registers on their way into the fragments.  blockIdx.z = block of 8 query rows: a
 // query of more rows (the multi-token prefill of a PROTOKV_ROPE state) runs as independent 8-row blocks over the same bank.
-template <bool ROPE>
-__global__ void __launch_bounds__(kD2Threads, ROPE ? 2 : kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
+// RAGGED: PROTOKV_VAR_ALLOC (D.3) -- prototype k owns S_k rows of the bank's code arrays from row
+// soff[k]; a far unit is still 8 prototypes, but its pseudo-tokens are walked 16 rows at a time and every row looks up
+// its own prototype among the unit's eight.
+template <bool ROPE, bool RAGGED>
+__global__ void __launch_bounds__(kD2Threads, (ROPE || RAGGED) ? 2 : kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
   extern __shared__ __align__(16) unsigned char sm[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, j = lane & 3;
@@ -540,10 +546,24 @@ __global__ void __launch_bounds__(kD2Threads, ROPE ? 2 : kD8CtasPerSm) attention
           d2_cp16(dst + D2Stage::C + (r * 32 + lane) * 16, cs + (r * 32 + lane) * 16);
           d2_cp16(dst + D2Stage::C + 2048 + (r * 32 + lane) * 16, ps + (r * 32 + lane) * 16);
         }
-        if (lane < 16) d2_cp16(dst + 4096 + lane * 16, (const char*)(V.codesK + pk0 * 8) + lane * 16);
-        else d2_cp16(dst + 4352 + (lane - 16) * 16, (const char*)(V.codesV + pk0 * 8) + (lane - 16) * 16);
-        if (lane < 2) d2_cp16(dst + 4608 + lane * 16, (const char*)(V.logn + pk0) + lane * 16);
-        else if (lane == 2) d2_cp8(dst + 4640, V.kind + pk0);
+        if (RAGGED) {   // this unit's code rows [soff[k0], soff[k0 + 8)) (<= 256), its 9 offsets, masses and kinds
+          const int* so = V.soff + (size_t)b * (D.K + 1) + (pk0 - (size_t)b * D.K);
+          const int r0 = __ldg(so), nrows = __ldg(so + 8) - r0;
+          const uint32_t* ck = V.codesK + (size_t)b * D.K * 8 + r0;
+          const uint32_t* cv = V.codesV + (size_t)b * D.K * 8 + r0;
+          for (int e = lane; e < nrows; e += 32) {
+            d2_cp4(dst + 4096 + e * 4, ck + e);
+            d2_cp4(dst + 5120 + e * 4, cv + e);
+          }
+          if (lane < 9) d2_cp4(dst + 6192 + lane * 4, so + lane);
+          if (lane < 2) d2_cp16(dst + 6144 + lane * 16, (const char*)(V.logn + pk0) + lane * 16);
+          else if (lane == 2) d2_cp8(dst + 6176, V.kind + pk0);
+        } else {
+          if (lane < 16) d2_cp16(dst + 4096 + lane * 16, (const char*)(V.codesK + pk0 * 8) + lane * 16);
+          else d2_cp16(dst + 4352 + (lane - 16) * 16, (const char*)(V.codesV + pk0 * 8) + (lane - 16) * 16);
+          if (lane < 2) d2_cp16(dst + 4608 + lane * 16, (const char*)(V.logn + pk0) + lane * 16);
+          else if (lane == 2) d2_cp8(dst + 4640, V.kind + pk0);
+        }
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -636,6 +656,80 @@ __global__ void __launch_bounds__(kD2Threads, ROPE ? 2 : kD8CtasPerSm) attention
         v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
       }
       d8_pv(o, b0, b1, v);
+    } else if (RAGGED) {
+      const int k0 = (wi + (i - nn) * NW) * 8;
+      const float* lns = reinterpret_cast<const float*>(stg + 6144);
+      const uint32_t* zks = reinterpret_cast<const uint32_t*>(stg + 4096);
+      const uint32_t* zvs = reinterpret_cast<const uint32_t*>(stg + 5120);
+      const int* offs = reinterpret_cast<const int*>(stg + 6192);
+      int rel[8];                                               // first row of each of the unit's prototypes
+#pragma unroll
+      for (int q = 0; q < 8; ++q) rel[q] = offs[q] - offs[0];
+      const int nrows = offs[8] - offs[0];
+      auto owner = [&](int r) {                                 // prototype (0..7) that owns local row r
+        int kl = 0;
+#pragma unroll
+        for (int q = 1; q < 8; ++q) kl += r >= rel[q] ? 1 : 0;
+        return kl;
+      };
+#pragma unroll 1
+      for (int t0 = 0; t0 < nrows; t0 += 16) {
+        int kl[2], kind[2];
+        float bias[2];
+        uint4 kr[2][4];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                           // key side: rows t0 + g and t0 + 8 + g
+          const int r = t0 + 8 * h + g;
+          const bool in = r < nrows;
+          kl[h] = in ? owner(r) : 0;
+          kind[h] = in ? (int)stg[6176 + kl[h]] : 2;
+          bias[h] = kind[h] == 2 ? -INFINITY : (A.use_bias ? lns[kl[h]] * kD2Log2e : 0.f);
+          const uint32_t code = in ? zks[r] : 0u;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) kr[h][c] = *reinterpret_cast<const uint4*>(stg + D2Stage::C + kl[h] * 256 + (j + 4 * c) * 16);
+          if (kind[h] == 0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const int gg = (j + 4 * c) >> 1;
+              const uint32_t z = (code >> (4 * gg)) & 15u;
+              kr[h][c] = d2_add2x4(kr[h][c], *reinterpret_cast<const uint4*>(cbK + (gg * 16 + z) * 32 + (j & 1) * 16));
+            }
+          }
+          if (ROPE) {
+            const float2* tp = V.ropeP + ((size_t)b * D.K + min(k0 + kl[h], D.K - 1)) * 64;
+            d8_rope8(kr[h][0], kr[h][2], tp + 8 * j);
+            d8_rope8(kr[h][1], kr[h][3], tp + 8 * (j + 4));
+          }
+        }
+        float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          d8_mma(s0, kr[0][c].x, kr[1][c].x, kr[0][c].y, kr[1][c].y, qb[2 * c][0], qb[2 * c][1]);
+          d8_mma(s1, kr[0][c].z, kr[1][c].z, kr[0][c].w, kr[1][c].w, qb[2 * c + 1][0], qb[2 * c + 1][1]);
+        }
+        float x[4];
+        x[0] = fmaf(s0[0] + s1[0], sc2, bias[0]); x[1] = fmaf(s0[1] + s1[1], sc2, bias[0]);
+        x[2] = fmaf(s0[2] + s1[2], sc2, bias[1]); x[3] = fmaf(s0[3] + s1[3], sc2, bias[1]);
+        uint32_t b0, b1;
+        d8_softmax(S, o, x, b0, b1);
+        uint32_t v[4][8];
+#pragma unroll
+        for (int tt = 0; tt < 4; ++tt) {                        // value side: rows t0 + 2j (+1) and t0 + 8 + 2j (+1)
+          const int r = t0 + (tt >> 1) * 8 + 2 * j + (tt & 1);
+          const bool in = r < nrows;
+          const int kv = in ? owner(r) : 0;
+          uint4 lo = *reinterpret_cast<const uint4*>(stg + D2Stage::C + 2048 + kv * 256 + g * 32);
+          uint4 hi = *reinterpret_cast<const uint4*>(stg + D2Stage::C + 2048 + kv * 256 + g * 32 + 16);
+          if (in && stg[6176 + kv] == 0) {
+            const uint32_t z = (zvs[r] >> (4 * g)) & 15u;
+            const uint4* cw = reinterpret_cast<const uint4*>(cbV + (g * 16 + z) * 32);
+            lo = d2_add2x4(lo, cw[0]); hi = d2_add2x4(hi, cw[1]);
+          }
+          v[tt][0] = lo.x; v[tt][1] = lo.y; v[tt][2] = lo.z; v[tt][3] = lo.w;
+          v[tt][4] = hi.x; v[tt][5] = hi.y; v[tt][6] = hi.z; v[tt][7] = hi.w;
+        }
+        d8_pv(o, b0, b1, v);
+      }
     } else {
       const int k0 = (wi + (i - nn) * NW) * 8;
       const float* lns = reinterpret_cast<const float*>(stg + 4608);
@@ -783,9 +877,13 @@ bool decode2_attention_prepare() {
     cudaGetLastError();
     return false;
   }
-  if (cudaFuncSetAttribute(attention_decode8_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+  if (cudaFuncSetAttribute(attention_decode8_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
           cudaSuccess ||
-      cudaFuncSetAttribute(attention_decode8_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+      cudaFuncSetAttribute(attention_decode8_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+          cudaSuccess ||
+      cudaFuncSetAttribute(attention_decode8_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
+          cudaSuccess ||
+      cudaFuncSetAttribute(attention_decode8_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kD8SmemTotal) !=
           cudaSuccess) {
     cudaGetLastError();
     return false;
@@ -813,10 +911,10 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   int cap = (units + kD2Warps - 1) / kD2Warps;
   if (cap > decode2_max_splits()) cap = decode2_max_splits();
   if (cap < 1) cap = 1;
-  const bool rope = (H.flags & PROTOKV_ROPE) != 0;
-  const bool rows8 = rope || a.R <= 8;                         // the N = 8 variant; with ROPE every query runs as 8-row blocks
+  const bool rope = (H.flags & PROTOKV_ROPE) != 0, ragged = V.soff != nullptr;
+  const bool rows8 = rope || ragged || a.R <= 8;               // the N = 8 variant; ROPE / VAR_ALLOC queries run as 8-row blocks
   const int nrb = rows8 ? (a.R + 7) / 8 : 1;
-  const int slots = (rope ? 2 : (rows8 ? kD8CtasPerSm : kD2CtasPerSm)) * sm_count;
+  const int slots = ((rope || ragged) ? 2 : (rows8 ? kD8CtasPerSm : kD2CtasPerSm)) * sm_count;
   const long long room = ((long long)D.B * 16 * decode2_max_splits()) / ((long long)nb * a.R);   // partials the buffer holds per row
   if (cap > room) cap = room < 1 ? 1 : (int)room;
   int ns = 1;
@@ -827,8 +925,10 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   }
   a.nsplit = ns;
   *nsplit_out = ns;
-  if (rope) attention_decode8_kernel<true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
-  else if (rows8) attention_decode8_kernel<false><<<dim3(ns, nb, 1), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  if (rope && ragged) attention_decode8_kernel<true, true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  else if (rope) attention_decode8_kernel<true, false><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  else if (ragged) attention_decode8_kernel<false, true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
+  else if (rows8) attention_decode8_kernel<false, false><<<dim3(ns, nb, 1), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
   else attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
   return 1;
 }

@@ -40,7 +40,8 @@ struct protokv_state {
   bool use_tc_attn;
   bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
   bool use_decode2;       // the register-resident decode kernel serves them (default where supported)
-  bool use_decode_rope;   // PROTOKV_ROPE state served by the rotating variant of that kernel (any number of query rows)
+  bool use_decode_rope;   // PROTOKV_ROPE / PROTOKV_VAR_ALLOC state served by the rotating / ragged variants of that kernel
+                          // (any number of query rows)
   TcMaps maps;
   int nsplit;
   // stage timing (protokv_profile_*)
@@ -368,7 +369,8 @@ protokv_state* protokv_create(const protokv_config* cfg) {
                         decode_attention_prepare();
   st->use_decode2 = want_tc && !rope && !st->use_decode_attn && !(cfg->flags & PROTOKV_NO_DECODE_KERNEL) &&
                     decode2_attention_supported(st->D, 1) && decode2_attention_prepare();
-  st->use_decode_rope = want_tc && (cfg->flags & PROTOKV_ROPE) && !(cfg->flags & (PROTOKV_VAR_ALLOC | PROTOKV_NO_DECODE_KERNEL)) &&
+  // PROTOKV_ROPE and / or PROTOKV_VAR_ALLOC states: the rotating / ragged variants of that kernel, 8-row blocks
+  st->use_decode_rope = want_tc && (cfg->flags & (PROTOKV_ROPE | PROTOKV_VAR_ALLOC)) && !(cfg->flags & PROTOKV_NO_DECODE_KERNEL) &&
                         decode2_rope_supported(st->D) && decode2_attention_prepare();
   return st;
 }
@@ -549,7 +551,7 @@ int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, in
       st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
     } else if (st->use_decode_rope && (uintptr_t)Q % 16 == 0) {
       int ns = 1;
-      st->launches += launch_rope_tables(D, st->H, st->V, A, st->stream);
+      if (st->H.flags & PROTOKV_ROPE) st->launches += launch_rope_tables(D, st->H, st->V, A, st->stream);
       st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
       st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
@@ -623,11 +625,11 @@ int protokv_error_flags(protokv_state* st, uint32_t* flags, int32_t clear) {
 const char* protokv_stage_impl(const protokv_state* st, int32_t stage) {
   if (!st) return "none";
   if (stage == 0) return st->use_tc_assign ? "tcgen05" : "simt";
-  if (stage == 1) return st->use_tc_attn ? "tcgen05" : (st->use_decode_rope ? "mma.sync register-resident (rope)" : "simt");
+  if (stage == 1) return st->use_tc_attn ? "tcgen05" : (st->use_decode_rope ? "mma.sync register-resident (blocks)" : "simt");
   if (stage == 2)
     return st->use_decode_attn ? "mma.sync split-KV"
            : (st->use_decode2 ? "mma.sync register-resident"
-              : (st->use_decode_rope ? "mma.sync register-resident (rope)" : (st->use_tc_attn ? "tcgen05" : "simt")));
+              : (st->use_decode_rope ? "mma.sync register-resident (blocks)" : (st->use_tc_attn ? "tcgen05" : "simt")));
   return "none";
 }
 

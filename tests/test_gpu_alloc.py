@@ -43,7 +43,8 @@ def test_allocation_synthesis_and_attention(name, frames, s_cap, kmax):
     gpu = make_gpu(spec, flags=B.VAR_ALLOC, s_cap=s_cap, beam=32)
     banks = list(range(spec.n_banks))
     orc = make_oracles(spec, banks, flags=FLAG_VAR_ALLOC, s_cap=s_cap, beam=32)
-    assert gpu.stage_impl(1) == "simt"
+    # production shape: the ragged variant of the register-resident kernel (8-row blocks); fp32 / d = 64: the SIMT kernel
+    assert gpu.stage_impl(1) == ("mma.sync register-resident (blocks)" if name == "c2" else "simt")
     run_stream(spec, gpu, orc, frames, check_state_every=10)
     gpu.synthesize()
     _compare_ragged_codes(gpu, orc, spec.G)
@@ -55,6 +56,38 @@ def test_allocation_synthesis_and_attention(name, frames, s_cap, kmax):
             assert sk.sum() == spec.k_max * 8                            # S_tot = K_max S: L_context unchanged (L616)
     compare_attention(spec, gpu, orc, gen.queries(spec, 0), run_synthesis=False, use_gpu_codes=True,
                       rows_sample=range(0, spec.n_query_tokens * (spec.n_q_heads // spec.n_kv_heads), 5))
+    compare_attention(spec, gpu, orc, gen.queries(spec, 1)[:, :, :1].contiguous(), run_synthesis=False, use_gpu_codes=True)
+    gpu.close()
+
+
+def test_ragged_attention_routes_agree():
+    """The same VAR_ALLOC state through the ragged register-resident kernel and through the SIMT kernel (FORCE_SIMT)."""
+    spec = gen.spec_for("c2", n_frames=36, k_max=256)
+    outs = []
+    for route in (0, B.FORCE_SIMT):
+        gpu = make_gpu(spec, flags=B.VAR_ALLOC | route, s_cap=24)
+        s = gen.grid_positions(spec, device="cuda")
+        for f in range(spec.n_frames):
+            K, V = gen.frame_kv(spec, f, device="cuda")
+            gpu.append_frame(K, V, s)
+        outs.append(gpu.query_attention(gen.queries(spec, 0).cuda()).float().cpu())
+        gpu.close()
+    import torch
+    assert torch.allclose(outs[0], outs[1], atol=1e-2, rtol=2e-2)
+
+
+def test_ragged_allocation_with_rotary_anchoring():
+    """PROTOKV_VAR_ALLOC | PROTOKV_ROPE: ragged pseudo-token counts, every prototype's rows rotated at its anchor."""
+    from oracle import FLAG_ROPE
+    spec = gen.spec_for("c2", n_frames=32, k_max=128)
+    hyper = dict(s_cap=20, pos0=40_000, rope_anchor=2)
+    gpu = make_gpu(spec, flags=B.VAR_ALLOC | B.ROPE, **hyper)
+    orc = make_oracles(spec, [0, 3], flags=FLAG_VAR_ALLOC | FLAG_ROPE, **hyper)
+    run_stream(spec, gpu, orc, spec.n_frames, check_state_every=16)
+    gpu.synthesize()
+    _compare_ragged_codes(gpu, orc, spec.G)
+    compare_attention(spec, gpu, orc, gen.queries(spec, 0)[:, :, :5].contiguous(), run_synthesis=False, use_gpu_codes=True)
+    compare_attention(spec, gpu, orc, gen.queries(spec, 0)[:, :, :1].contiguous(), run_synthesis=False, use_gpu_codes=True)
     gpu.close()
 
 

@@ -34,7 +34,7 @@ def test_rope_c1_all_anchor_variants(anchor):
     assert (a - b).abs().max() > 1e-3
 
 
-@pytest.mark.parametrize("route,impl", [(0, "mma.sync register-resident (rope)"), (FORCE_SIMT, "simt")])
+@pytest.mark.parametrize("route,impl", [(0, "mma.sync register-resident (blocks)"), (FORCE_SIMT, "simt")])
 def test_rope_bf16_gqa_shape_long_positions(route, impl):
     # config-2 shape (bf16, d = 128, GQA 28/4), default base 1e6, positions beyond 10^6 (pos0): fp32 angles would be off.
     # Default route: the rotating variant of the register-resident kernel (8-row blocks); cross-check: the fp32 SIMT kernel
@@ -68,7 +68,7 @@ def test_rope_decode_query_anchor_variants(anchor):
     spec = gen.spec_for("c2", n_frames=30)
     hyper = dict(rope_anchor=anchor, pos0=250_000)
     gpu = make_gpu(spec, flags=ROPE, **hyper)
-    assert gpu.stage_impl(2) == "mma.sync register-resident (rope)"
+    assert gpu.stage_impl(2) == "mma.sync register-resident (blocks)"
     oracles = make_oracles(spec, [1, 2], flags=FLAG_ROPE, **hyper)
     Q = gen.queries(spec, 3)
     from gpu_helpers import step_teacher_forced, new_stats
