@@ -3,21 +3,24 @@
 // over W + K_max S tokens is the only ProtoKV work on the latency of a query).  For a handful of rows that is ~2.7 MB per
 // bank streamed once, i.e. HBM time; the kernel is built so that nothing but those bytes moves:
 //
-//   * every warp is its own flash-decoding worker over a strided share of the bank's context, with NO shared-memory
-//     operand staging and no block barrier in the loop: mma.sync m16n8k16 B fragments are filled straight from global
-//     memory.  The contraction index of Q K^T may be permuted freely, so a lane's four 16-byte loads of a key row are
-//     contiguous 64-byte pieces (chunk q = j + 4c holds dims [8q, 8q + 8) = k-steps 2c and 2c + 1); Q's A fragments use
-//     the same permutation.  For P V the output dims are permuted instead (MMA column n of tile i = dim 16 n + i), so a
-//     lane reads the 32 contiguous bytes [16 g, 16 g + 16) of each of its four value rows and two PRMTs per tile pair
-//     the tokens up;
+//   * every warp is its own flash-decoding worker over a strided share of the bank's context: it streams its units (16
+//     ring rows, or 8 prototypes) through a private cp.async ring in shared memory -- no block barrier in the loop -- and
+//     fills the mma.sync m16n8k16 operand fragments from there with plain 16-byte loads (chunks are XOR-swizzled at
+//     staging so that these loads are bank-conflict free).  The contraction index of Q K^T may be permuted freely, so a
+//     lane's four pieces of a key row are whole 16-byte chunks (chunk q = j + 4c holds dims [8q, 8q + 8) = k-steps 2c and
+//     2c + 1); the query fragments use the same permutation.  For P V the output dims are permuted instead (a lane owns
+//     dims [16 g, 16 g + 16) of its four value rows), and PRMTs pair two rows per operand register;
 //   * pseudo-tokens k~ = c_k + concat_g CK_g[z], v~ = p_k + concat_g CV_g[z] (Alg. 4 l.5-9) exist only as B fragments:
-//     the lane takes its chunks of bf16(c_k) / bf16(p_k) (copies kept by the update path), adds its 16-byte pieces of the selected codewords
-//     from a 4 KB bf16 codebook in shared memory (add.rn.bf16x2 -- the same rounding as the tcgen05 kernel's builders),
-//     and feeds the MMA.  With the value-side dim permutation a lane's dims [16 g, 16 g + 16) are exactly PQ subspace g;
+//     the lane takes its chunks of bf16(c_k) / bf16(p_k) (copies kept by the update path), adds its 16-byte pieces of
+//     the selected codewords from a 4 KB bf16 codebook in shared memory (add.rn.bf16x2 -- the same rounding as the
+//     tcgen05 kernel's builders), and feeds the MMA.  With the value-side dim permutation a lane's dims [16 g, 16 g + 16) are exactly PQ subspace g;
 //   * online softmax in the accumulator fragments (exp2 domain, log-mass bias log2 n_k on pseudo columns, Eq. 2/4), P
 //     re-used from the accumulators as the A fragment of P V (FlashAttention-2 register reuse).
 // A CTA's four warps merge their (m, l, O) through shared memory and write one unnormalised partial per query row;
 // attention_combine_kernel (query_kernels.cu) merges the nsplit partials of a row.
+// Two kernels: attention_decode2_kernel (9-16 rows: query rows = MMA M, padded to 16) and attention_decode8_kernel
+// (<= 8 rows: context columns = MMA M, rows = N = 8; its ROPE / RAGGED variants serve PROTOKV_ROPE / PROTOKV_VAR_ALLOC
+// states for queries of any length as 8-row blocks).  Measured history: profiles/r02_decode.md.
 #include "common.cuh"
 
 namespace pkv {
