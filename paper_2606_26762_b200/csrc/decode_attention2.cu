@@ -438,8 +438,8 @@ __global__ void __launch_bounds__(kD2Threads, kD2CtasPerSm) attention_decode2_ke
 constexpr int kD8CtasPerSm = 3;
 constexpr int kD8Stages = 2;
 constexpr uint32_t kD8StageBytes = 8192;
-constexpr uint32_t kD8CbV = 4096;                                                      // two bf16 codebooks, 128 rows x 32 B each
-constexpr uint32_t kD8Ring = 8192;
+constexpr uint32_t kD8CbV = 4128;                                                      // two bf16 codebooks: 128 rows x 32 B + one zero row
+constexpr uint32_t kD8Ring = 8256;
 constexpr uint32_t kD8SmemTotal = kD8Ring + kD2Warps * kD8Stages * kD8StageBytes;      // 73,728 B
 
 __device__ __forceinline__ void d8_mma(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
@@ -581,6 +581,10 @@ __global__ void __launch_bounds__(kD2Threads, (ROPE || RAGGED) ? 2 : kD8CtasPerS
       d2_cp16(s0 + kD8CbV + (r * 128 + tid) * 16, src + 4096 + (r * 128 + tid) * 16);
     }
   }
+  // row 128 of either codebook is all zero: prototypes without decoded residuals (n_res = 0, Alg. 4 l.3-4) add it, so that
+  // the fragment build of the fixed-S path is branch-free
+  if (tid < 8) reinterpret_cast<uint32_t*>(sm + 4096)[tid] = 0u;
+  else if (tid < 16) reinterpret_cast<uint32_t*>(sm + kD8CbV + 4096)[tid - 8] = 0u;
   issue(0);
 
   // Q^T as B fragments: column n = g is query row g; k-steps 2c, 2c + 1 <- chunk q = j + 4c
@@ -756,14 +760,11 @@ __global__ void __launch_bounds__(kD2Threads, (ROPE || RAGGED) ? 2 : kD8CtasPerS
           const int kl = 2 * ss + h;
           const uint32_t code = zks[kl * 8 + g];
 #pragma unroll
-          for (int c = 0; c < 4; ++c) kr[h][c] = *reinterpret_cast<const uint4*>(stg + D2Stage::C + kl * 256 + (j + 4 * c) * 16);
-          if (kind[h] == 0) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              const int gg = (j + 4 * c) >> 1;
-              const uint32_t z = (code >> (4 * gg)) & 15u;
-              kr[h][c] = d2_add2x4(kr[h][c], *reinterpret_cast<const uint4*>(cbK + (gg * 16 + z) * 32 + (j & 1) * 16));
-            }
+          for (int c = 0; c < 4; ++c) {
+            const int gg = (j + 4 * c) >> 1;
+            const uint32_t row = kind[h] == 0 ? (uint32_t)(gg * 16) + ((code >> (4 * gg)) & 15u) : 128u;
+            kr[h][c] = d2_add2x4(*reinterpret_cast<const uint4*>(stg + D2Stage::C + kl * 256 + (j + 4 * c) * 16),
+                                 *reinterpret_cast<const uint4*>(cbK + row * 32 + (j & 1) * 16));
           }
         }
         if (ROPE) {                                             // the S pseudo-tokens of a prototype sit at its anchor (L126, D.1)
@@ -794,12 +795,9 @@ __global__ void __launch_bounds__(kD2Threads, (ROPE || RAGGED) ? 2 : kD8CtasPerS
           const uint2 zz = *reinterpret_cast<const uint2*>(zvs + kl * 8 + 2 * j);
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
-            uint4 lo = plo, hi = phi;
-            if (kind[h] == 0) {
-              const uint32_t z = ((e ? zz.y : zz.x) >> (4 * g)) & 15u;
-              const uint4* cw = reinterpret_cast<const uint4*>(cbV + (g * 16 + z) * 32);
-              lo = d2_add2x4(lo, cw[0]); hi = d2_add2x4(hi, cw[1]);
-            }
+            const uint32_t row = kind[h] == 0 ? (uint32_t)(g * 16) + (((e ? zz.y : zz.x) >> (4 * g)) & 15u) : 128u;
+            const uint4* cw = reinterpret_cast<const uint4*>(cbV + row * 32);
+            const uint4 lo = d2_add2x4(plo, cw[0]), hi = d2_add2x4(phi, cw[1]);
             const int t = 2 * h + e;
             v[t][0] = lo.x; v[t][1] = lo.y; v[t][2] = lo.z; v[t][3] = lo.w;
             v[t][4] = hi.x; v[t][5] = hi.y; v[t][6] = hi.z; v[t][7] = hi.w;
