@@ -163,8 +163,11 @@ int protokv_append_frame(protokv_state *st, const void *K, const void *V, const 
 int protokv_query_attention(protokv_state *st, const void *Q, void *out);
 
 /* The same two calls with HOST buffers (pinned memory recommended): inputs are copied to the device and, for
- * the query, the result copied back, on the state's stream.  append returns without synchronising; the query
- * variant synchronises the stream before returning so `out` is ready. */
+ * the query, the result copied back.  The host-to-device copies run on a copy stream the library owns, next to the work
+ * that does not need them (Eq. 1 scoring and the prototype update only read the evicted frame already in the ring; the
+ * synthesis does not read Q); the state's stream waits for them before the ring append / the attention, so synchronising
+ * cfg.cuda_stream still covers the whole call.  append returns without synchronising; the query variant synchronises
+ * the stream before returning so `out` is ready. */
 int protokv_append_frame_host(protokv_state *st, const void *K, const void *V, const float *grid_pos);
 int protokv_query_attention_host(protokv_state *st, const void *Q, void *out);
 

@@ -40,6 +40,11 @@ struct protokv_state {
   bool use_tc_attn;
   bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
   bool use_decode2;       // the register-resident decode kernel serves them (default where supported)
+  // host-buffer variants: the H2D copies of a frame run on a copy stream of the library's own, next to the scoring and
+  // update kernels (which only need the evicted frame that is already in the ring); the ring append waits for them
+  cudaStream_t copy_stream;
+  cudaEvent_t ev_copied, ev_appended;
+  bool appended_pending;  // ev_appended has been recorded: the staging buffers are in use until it completes
   bool use_decode_rope;   // PROTOKV_ROPE / PROTOKV_VAR_ALLOC state served by the rotating / ragged variants of that kernel
                           // (any number of query rows)
   TcMaps maps;
@@ -346,6 +351,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
     delete st;
     return nullptr;
   }
+  st->copy_stream = nullptr; st->ev_copied = nullptr; st->ev_appended = nullptr; st->appended_pending = false;
   st->frames = 0; st->n_act = 0; st->launches = 0; st->last_ev_frame = -1; st->last_n_fill = 0;
   st->codes_valid = false;
   st->epoch = 1;
@@ -380,6 +386,9 @@ void protokv_destroy(protokv_state* st) {
   DeviceGuard dg(st);
   for (auto& sp : st->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto e : st->ev_free) cudaEventDestroy(e);
+  if (st->ev_copied) cudaEventDestroy(st->ev_copied);
+  if (st->ev_appended) cudaEventDestroy(st->ev_appended);
+  if (st->copy_stream) cudaStreamDestroy(st->copy_stream);
   delete st;
 }
 
@@ -405,7 +414,8 @@ int protokv_profile_read(protokv_state* st, double* ms_sum, int64_t* launches) {
   return PROTOKV_OK;
 }
 
-int protokv_append_frame(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
+// before_append: an event the ring append (the only consumer of K, V, grid_pos) waits for, or NULL
+static int append_frame_impl(protokv_state* st, const void* K, const void* V, const float* grid_pos, cudaEvent_t before_append) {
   if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
   if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
   DeviceGuard dg(st);
@@ -439,6 +449,7 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
       nl += launch_update(D, st->H, st->V, F, st->sm_count, st->stream);                // U4-U6
     }
   }
+  if (before_append) PKV_CUDA(cudaStreamWaitEvent(st->stream, before_append, 0));
   {
     StageTimer tm(st, PROTOKV_STAGE_APPEND);
     nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                  // U1 (overwrites the slot)
@@ -466,6 +477,10 @@ int protokv_append_frame(protokv_state* st, const void* K, const void* V, const 
   if (st->warm && !st->trained && !(st->cfg.flags & PROTOKV_WARMUP_MANUAL) && st->frames == st->cfg.t_warm)
     return protokv_train_codebooks(st);                                                 // end of the warm-up (reading 33)
   return PROTOKV_OK;
+}
+
+int protokv_append_frame(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
+  return append_frame_impl(st, K, V, grid_pos, nullptr);
 }
 
 int protokv_train_codebooks(protokv_state* st) {
@@ -578,15 +593,36 @@ int protokv_query_attention(protokv_state* st, const void* Q, void* out) {
   return protokv_query_attention_ex(st, Q, st->D.Nq, 0, st->D.L, out, nullptr, 1);
 }
 
+static int ensure_copy_stream(protokv_state* st);
+
 int protokv_append_frame_host(protokv_state* st, const void* K, const void* V, const float* grid_pos) {
   if (!st || !K || !V || !grid_pos) return fail(PROTOKV_EINVAL, "NULL argument");
   DeviceGuard dg(st);
   const Dims& D = st->D;
   const size_t frame = (size_t)D.NS * D.L * D.T * D.Hkv * D.d * (D.bf16 ? 2 : 4);
-  PKV_CUDA(cudaMemcpyAsync(st->V.stageK, K, frame, cudaMemcpyHostToDevice, st->stream));
-  PKV_CUDA(cudaMemcpyAsync(st->V.stageV, V, frame, cudaMemcpyHostToDevice, st->stream));
-  PKV_CUDA(cudaMemcpyAsync(st->V.stageS, grid_pos, (size_t)D.NS * D.T * 8, cudaMemcpyHostToDevice, st->stream));
-  return protokv_append_frame(st, st->V.stageK, st->V.stageV, st->V.stageS);
+  {
+    const int rc0 = ensure_copy_stream(st);
+    if (rc0 != PROTOKV_OK) return rc0;
+  }
+  // the staging buffers are free once the previous host-variant append has consumed them
+  if (st->appended_pending) PKV_CUDA(cudaStreamWaitEvent(st->copy_stream, st->ev_appended, 0));
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageK, K, frame, cudaMemcpyHostToDevice, st->copy_stream));
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageV, V, frame, cudaMemcpyHostToDevice, st->copy_stream));
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageS, grid_pos, (size_t)D.NS * D.T * 8, cudaMemcpyHostToDevice, st->copy_stream));
+  PKV_CUDA(cudaEventRecord(st->ev_copied, st->copy_stream));
+  const int rc = append_frame_impl(st, st->V.stageK, st->V.stageV, st->V.stageS, st->ev_copied);
+  if (rc != PROTOKV_OK) return rc;
+  PKV_CUDA(cudaEventRecord(st->ev_appended, st->stream));
+  st->appended_pending = true;
+  return PROTOKV_OK;
+}
+
+static int ensure_copy_stream(protokv_state* st) {
+  if (st->copy_stream) return PROTOKV_OK;
+  PKV_CUDA(cudaStreamCreateWithFlags(&st->copy_stream, cudaStreamNonBlocking));
+  PKV_CUDA(cudaEventCreateWithFlags(&st->ev_copied, cudaEventDisableTiming));
+  PKV_CUDA(cudaEventCreateWithFlags(&st->ev_appended, cudaEventDisableTiming));
+  return PROTOKV_OK;
 }
 
 int protokv_query_attention_host(protokv_state* st, const void* Q, void* out) {
@@ -594,8 +630,18 @@ int protokv_query_attention_host(protokv_state* st, const void* Q, void* out) {
   DeviceGuard dg(st);
   const Dims& D = st->D;
   const size_t qbytes = (size_t)D.NS * D.L * D.Nq * D.Hq * D.d * (D.bf16 ? 2 : 4);
-  PKV_CUDA(cudaMemcpyAsync(st->V.stageQ, Q, qbytes, cudaMemcpyHostToDevice, st->stream));
-  const int rc = protokv_query_attention(st, st->V.stageQ, st->V.stageO);
+  int rc = ensure_copy_stream(st);
+  if (rc != PROTOKV_OK) return rc;
+  // Q travels on the copy stream while the synthesis (which does not need it) runs; the previous query's attention has
+  // finished with the staging buffer (this call synchronises before it returns)
+  PKV_CUDA(cudaMemcpyAsync(st->V.stageQ, Q, qbytes, cudaMemcpyHostToDevice, st->copy_stream));
+  PKV_CUDA(cudaEventRecord(st->ev_copied, st->copy_stream));
+  if (!(st->H.flags & PROTOKV_NEAR_ONLY) && !st->codes_valid) {
+    rc = protokv_synthesize(st);
+    if (rc != PROTOKV_OK) return rc;
+  }
+  PKV_CUDA(cudaStreamWaitEvent(st->stream, st->ev_copied, 0));
+  rc = protokv_query_attention(st, st->V.stageQ, st->V.stageO);
   if (rc != PROTOKV_OK) return rc;
   PKV_CUDA(cudaMemcpyAsync(out, st->V.stageO, qbytes, cudaMemcpyDeviceToHost, st->stream));
   PKV_CUDA(cudaStreamSynchronize(st->stream));

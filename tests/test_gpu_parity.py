@@ -265,14 +265,24 @@ def test_ragged_frame_size_and_bf16_d64():
 # ---------------------------------------------------------------------------------------------------------
 # boundary behaviour: host variants, state import/export, errors
 # ---------------------------------------------------------------------------------------------------------
-def test_host_variants_match_device_calls():
-    spec = gen.spec_for("c1", n_frames=12)
+@pytest.mark.parametrize("name,frames", [("c1", 12), ("c2", 30)])
+def test_host_variants_match_device_calls(name, frames):
+    """The host-buffer entry points (copies on the library's copy stream, overlapped with the scoring / update kernels and
+    the synthesis) produce exactly what the device-pointer calls produce."""
+    spec = gen.spec_for(name, n_frames=frames)
     a, b = make_gpu(spec), make_gpu(spec)
     s = gen.grid_positions(spec)
+    hs = s.pin_memory()
+    keep = []
     for f in range(spec.n_frames):
         K, V = gen.frame_kv(spec, f)
         a.append_frame(K.cuda(), V.cuda(), s.cuda())
-        b.append_frame_host(K.pin_memory(), V.pin_memory(), s.pin_memory())
+        keep.append((K.pin_memory(), V.pin_memory()))        # arguments stay valid until the stream has passed the call
+        b.append_frame_host(keep[-1][0], keep[-1][1], hs)
+        if f % 7 == 3:
+            torch.cuda.synchronize()
+            keep.clear()
+    torch.cuda.synchronize()
     Q = gen.queries(spec, 0)
     oa = a.query_attention(Q.cuda()).cpu()
     ob = torch.empty_like(Q).pin_memory()
