@@ -211,7 +211,8 @@ int launch_codebook_copy(const Dims& D, const Dev& V, const float* cbk, const fl
 // admissible shape; returns false if the device refuses one of them.
 bool update_kernels_prepare(const Dims& D);
 bool query_kernels_prepare(const Dims& D);
-int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s);
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int max_dirty, int sm_count,
+                     cudaStream_t s);
 
 __device__ __forceinline__ void mark_dirty(const Dims& D, const Dev& V, int b, int k, int epoch) {
   V.dirty[(size_t)b * D.K + k] = (uint32_t)epoch;

@@ -36,6 +36,7 @@ struct protokv_state {
   bool codes_valid;   // codes/kind describe the current histograms
   std::vector<double> logtab;   // host copy of Dev::logtab (source of an asynchronous copy: must outlive it)
   int epoch;          // synthesis epoch (see Dev::dirty_cnt)
+  int dirty_bound;    // upper bound of the prototypes per bank stamped dirty since the last synthesis (sizes its grid)
   bool use_tc_assign;
   bool use_tc_attn;
   bool use_decode_attn;   // the split-KV mma.sync kernel serves queries of <= 16 rows per bank
@@ -355,6 +356,7 @@ protokv_state* protokv_create(const protokv_config* cfg) {
   st->frames = 0; st->n_act = 0; st->launches = 0; st->last_ev_frame = -1; st->last_n_fill = 0;
   st->codes_valid = false;
   st->epoch = 1;
+  st->dirty_bound = st->D.K;
   st->profiling = false;
   for (int i = 0; i < PROTOKV_N_STAGES; ++i) { st->prof_ms[i] = 0.0; st->prof_n[i] = 0; }
   st->maps.ok = false;
@@ -471,7 +473,10 @@ static int append_frame_impl(protokv_state* st, const void* K, const void* V, co
   st->n_act = F.n_act;
   st->last_ev_frame = F.ev_frame;
   st->last_n_fill = F.n_fill;
-  if (F.evicted) st->codes_valid = false;
+  if (F.evicted) {
+    st->codes_valid = false;   // fills and absorptions stamp at most T prototypes per bank; Alg. 2 may stamp any
+    st->dirty_bound = (st->H.flags & PROTOKV_MAINTENANCE) ? D.K : (st->dirty_bound + D.T < D.K ? st->dirty_bound + D.T : D.K);
+  }
   if (F.warm && F.evicted) st->res_seen += D.T - F.n_fill;
   st->frames += 1;
   if (st->warm && !st->trained && !(st->cfg.flags & PROTOKV_WARMUP_MANUAL) && st->frames == st->cfg.t_warm)
@@ -513,11 +518,12 @@ int protokv_synthesize(protokv_state* st) {
       st->launches += launch_allocation(st->D, st->H, st->V, st->n_act, st->stream);
       st->launches += launch_synthesis_var(st->D, st->H, st->V, st->n_act, st->stream);
     } else {
-      st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->sm_count, st->stream);
+      st->launches += launch_synthesis(st->D, st->H, st->V, st->n_act, st->epoch, st->dirty_bound, st->sm_count, st->stream);
     }
   }
   PKV_CUDA(cudaGetLastError());
   st->epoch += 1;
+  st->dirty_bound = 0;
   st->codes_valid = true;
   return PROTOKV_OK;
 }
@@ -763,6 +769,7 @@ int protokv_import_state(protokv_state* st, int32_t bank, const protokv_bank_vie
   PKV_CUDA(cudaGetLastError());
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   st->codes_valid = false;
+  st->dirty_bound = D.K;
   st->maint_full = true;
   return PROTOKV_OK;
 }
@@ -864,6 +871,7 @@ int protokv_import_codes(protokv_state* st, int32_t bank, const uint8_t* codes_k
   // Forced codes last until the next synthesis: the whole bank is stamped with the epoch the next synthesis decodes,
   // so that it re-derives every tuple from the histograms instead of keeping forced ones on untouched prototypes.
   st->launches += launch_fill_u32(st->V.dirty + (size_t)bank * D.K, (uint32_t)st->epoch, (size_t)D.K, st->stream);
+  st->dirty_bound = D.K;
   PKV_CUDA(cudaGetLastError());
   PKV_CUDA(cudaStreamSynchronize(st->stream));
   return PROTOKV_OK;

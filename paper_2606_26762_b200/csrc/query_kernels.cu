@@ -252,9 +252,13 @@ bool query_kernels_prepare(const Dims&) {
   return false;
 }
 
-int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int sm_count, cudaStream_t s) {
-  // grid-stride over each bank's work list; its length is only known on the device
-  int per_bank = (2 * D.K + kSynTasks - 1) / kSynTasks;
+int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int epoch, int max_dirty, int sm_count,
+                     cudaStream_t s) {
+  // grid-stride over each bank's work list; its length is only known on the device, but the host knows a bound: at most
+  // max_dirty prototypes per bank were stamped since the last synthesis (<= T per appended frame) -- blocks beyond that
+  // would only run the list compaction and exit
+  const int bound = max_dirty < D.K ? (max_dirty > 0 ? max_dirty : 1) : D.K;
+  int per_bank = (2 * bound + kSynTasks - 1) / kSynTasks;
   const int cap = (8 * sm_count + D.B - 1) / D.B;
   if (per_bank > cap) per_bank = cap;
   if (per_bank < 1) per_bank = 1;
