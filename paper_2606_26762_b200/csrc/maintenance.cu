@@ -31,9 +31,13 @@ struct MtSmemLayout {   // dynamic shared memory, sizes depend on K
   uint16_t* list;              // [K] changed list, later the list of emptied slots
   unsigned long long* cand;    // [kMtMaxCand] (i << 32 | j)
 };
+// The first four coordinates of every key centre are kept in shared memory as a second exact-safe filter of the pair
+// scan (a partial squared distance never exceeds the full one) while the bank is small enough for them to fit.
+constexpr int kMtC4MaxK = 8192;
 __host__ __device__ inline size_t mt_smem_bytes(int K) {
   const size_t words = (size_t)K / 32 + 1;
-  return align_up((size_t)K * 4 + 2 * words * 4 + (size_t)K * 2, 16) + (size_t)kMtMaxCand * 8;
+  return align_up((size_t)K * 4 + 2 * words * 4 + (size_t)K * 2, 16) + (size_t)kMtMaxCand * 8 +
+         (K <= kMtC4MaxK ? (size_t)K * 16 : 0);
 }
 
 __device__ __forceinline__ bool mt_bit(const uint32_t* bits, int k) { return (bits[k >> 5] >> (k & 31)) & 1u; }
@@ -86,6 +90,7 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
   uint32_t* chgbits = alive + words;
   uint16_t* list = reinterpret_cast<uint16_t*>(chgbits + words);
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(mt_smem + align_up((size_t)K * 4 + 2 * (size_t)words * 4 + (size_t)K * 2, 16));
+  float4* c4 = K <= kMtC4MaxK ? reinterpret_cast<float4*>(cand + kMtMaxCand) : nullptr;
   __shared__ int nlist, ncand, nsurv;
   __shared__ unsigned long long cur_key, min_key;
   __shared__ double red[2][kMtWarps];
@@ -119,6 +124,7 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
       ch = A.full || V.mstamp[pk] == A.t;   // touched by this frame's fill / update, or left changed by the previous pass
       const float invc = reinterpret_cast<const float*>(V.rec)[rec_slot(pk, 6)];
       norm_s[k] = invc > 0.f ? 1.f / invc : 0.f;
+      if (c4) c4[k] = *reinterpret_cast<const float4*>(V.c + pk * d);
     }
     const uint32_t ba = __ballot_sync(0xffffffffu, al), bc = __ballot_sync(0xffffffffu, ch && al);
     if (lane == 0 && (k0 >> 5) + warp < words) {
@@ -147,7 +153,13 @@ __global__ void __launch_bounds__(kMtThreads) maintenance_kernel(Dims D, Hyper H
       const float na = norm_s[a];
       for (int b0 = 0; b0 < nu; b0 += 32) {
         const int bb = b0 + lane;
-        if (bb >= nu || bb == a || !mt_bit(alive, bb)) continue;
+        if (bb >= nu || bb == a) continue;
+        if (c4) {   // first four coordinates from shared memory, tested first: almost every pair of different clusters ends here
+          const float4 q = c4[bb];
+          const float e0 = ca16[0] - q.x, e1 = ca16[1] - q.y, e2 = ca16[2] - q.z, e3 = ca16[3] - q.w;
+          if (fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, e3 * e3))) > A.eps_k * A.eps_k * 1.001f) continue;
+        }
+        if (!mt_bit(alive, bb)) continue;
         if (mt_bit(chgbits, bb) && bb < a) continue;          // both changed: the pair is taken from its lower member
         const float* cb = V.c + (pk0 + bb) * d;
         if (!mt_maybe_close(ca16, cb, na, norm_s[bb], A.eps_k, d)) continue;
