@@ -81,6 +81,8 @@ struct AtPlan {
 __host__ __device__ inline long long at_span_begin(const AtPlan& P, int cta) { return ((long long)cta * P.ttot) / P.grid; }
 // CTA whose span contains global tile x.
 __host__ __device__ inline int at_cta_of(const AtPlan& P, long long x) {
+  if ((P.ttot + 1) * P.grid < (1ll << 31))   // the usual case: 32-bit division (the 64-bit one is a ~100-instruction routine)
+    return (int)(((uint32_t)(x + 1) * (uint32_t)P.grid + (uint32_t)P.ttot - 1u) / (uint32_t)P.ttot) - 1;
   return (int)(((x + 1) * P.grid + P.ttot - 1) / P.ttot - 1);
 }
 
