@@ -83,6 +83,11 @@ enum {
                                 S_k = S_tot Var(H_k) / sum_j Var(H_j) under S_tot = k_max S, 1 <= S_k <= s_cap, recomputed by
                                 every synthesis; bf16 states with head_dim 128 are served by the ragged variant of the
                                 register-resident kernel (8-row blocks), other shapes by the fp32 SIMT kernel */
+  PROTOKV_SERIAL_LAUNCH = 8192u, /* launch every kernel fully serialised.  By default the kernels of a call are chained
+                                with programmatic dependent launch (score -> update -> ring append; synthesis -> attention
+                                -> combine; decode kernel -> combine): each kernel's set-up and the loads of data that no
+                                kernel of the chain writes run under its predecessor's tail.  Results are bit-identical;
+                                the flag exists for measurement and as a cross-check */
   PROTOKV_MAINTENANCE = 64u  /* run Alg. 2 at the end of every append_frame that evicted a frame
                                 (Alg. 1 l.15); off by default: north_star's path and its invariant "total mass = tokens
                                 absorbed" exclude it (reading 19) */

@@ -6,7 +6,7 @@ creating a state without an sm_100 device raises ProtoKVError.
 from .binding import (  # noqa: F401
     ProtoKV, ProtoKVConfig, ProtoKVError, load_library, DEFAULTS,
     F32, BF16, MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV, ROPE,
-    WARMUP, WARMUP_MANUAL, VAR_ALLOC, NO_DECODE_KERNEL,
+    WARMUP, WARMUP_MANUAL, VAR_ALLOC, NO_DECODE_KERNEL, SERIAL_LAUNCH,
     protokv_workspace_bytes, protokv_last_error, EXPORTED_SYMBOLS,
 )
 from .build import build  # noqa: F401

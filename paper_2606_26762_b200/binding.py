@@ -11,7 +11,7 @@ from .build import build
 
 F32, BF16 = 0, 1
 MAH_SQUARED, NO_MASS_BIAS, NO_RESIDUAL, NEAR_ONLY, FAR_ONLY, FORCE_SIMT, MAINTENANCE, DECODE_SPLITKV, ROPE = 1, 2, 4, 8, 16, 32, 64, 128, 256
-WARMUP, WARMUP_MANUAL, VAR_ALLOC, NO_DECODE_KERNEL = 512, 1024, 2048, 4096
+WARMUP, WARMUP_MANUAL, VAR_ALLOC, NO_DECODE_KERNEL, SERIAL_LAUNCH = 512, 1024, 2048, 4096, 8192
 
 # Table 5 of the paper + the constants the paper leaves open (readings 4, 6, 12)
 DEFAULTS = dict(S=8, G=8, C=16, beam=32, lambda_sp=0.1, lambda_idle=0.01, t_idle=120, alpha=0.05, beta=0.05,

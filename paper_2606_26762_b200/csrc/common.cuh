@@ -195,7 +195,32 @@ struct FrameArgs {
   int keys;      // 1: the assignment of this frame is in Dev::akey (tcgen05 path), 0: in Dev::assign / best (SIMT)
   int warm;      // 1: warm-up step -- residuals go to the reservoir slots of Dev::rslot, no histogram update
   long long res_base;  // residuals offered to each bank's reservoir before this frame
+  int pdl;       // host side only: the frame's kernels are launched with programmatic stream serialisation (see pdl_wait)
 };
+
+// Programmatic dependent launch along the library's kernel chains (score -> update -> ring append; synthesis ->
+// attention -> combine -> the next call's attention; decode kernel -> combine): a kernel launched with the attribute may
+// start once every CTA of its predecessor has executed pdl_trigger() or exited; before pdl_wait() returns (= the
+// predecessor has completed and its writes are visible) it touches nothing that a kernel of the library writes or that the
+// caller passes in, with one exception, the ring append (see protokv_api.cu).  A kernel triggers only AFTER its own wait,
+// so "the predecessor of my predecessor has completed" holds by induction.  Kernels whose successor is a persistent
+// one-CTA-per-SM kernel (ring append, attention) do not trigger: measured, such a successor pending under their tail
+// slows them down; it then starts at their exit and still skips the launch latency.  Without the attribute (and under
+// PROTOKV_SERIAL_LAUNCH) both instructions are no-ops.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_chain(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl,
+                                Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 
 // Every launcher returns the number of kernels it launched (0 if there was nothing to do).
 int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const void* Kin, const void* Vin,
@@ -260,7 +285,7 @@ int decode2_max_splits();
 int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
                              int* nsplit_out);
 // merges A.nsplit partials per row ([rows][nsplit][d + 2] in Dev::part) into out / lse (bf16, d = 128)
-int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, cudaStream_t s);
+int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, bool pdl, cudaStream_t s);
 
 // tcgen05 paths (bf16, d = 128).  The TMA tensor maps are built once per state.
 struct TcMaps {

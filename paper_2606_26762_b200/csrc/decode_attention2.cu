@@ -158,6 +158,7 @@ __device__ __forceinline__ uint4 d2_cvt8s(const unsigned char* p) {    // 8 fp32
 
 __global__ void __launch_bounds__(kD2Threads, kD2CtasPerSm) attention_decode2_kernel(Dims D, Dev V, D2Args A) {
   extern __shared__ __align__(16) unsigned char sm[];
+  pdl_wait();   // launched under the tail of the previous kernel of the stream (see common.cuh); no early trigger of its own
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, j = lane & 3;
   const int bsel = blockIdx.y, split = blockIdx.x;
@@ -513,6 +514,7 @@ __device__ __forceinline__ void d8_rope8(uint4& x, uint4& y, const float2* __res
 template <bool ROPE, bool RAGGED>
 __global__ void __launch_bounds__(kD2Threads, (ROPE || RAGGED) ? 2 : kD8CtasPerSm) attention_decode8_kernel(Dims D, Dev V, D2Args A) {
   extern __shared__ __align__(16) unsigned char sm[];
+  pdl_wait();   // launched under the tail of the previous kernel of the stream (see common.cuh); no early trigger of its own
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, j = lane & 3;
   const int bsel = blockIdx.y, split = blockIdx.x, r0 = blockIdx.z * 8;   // first query row of this block
@@ -926,11 +928,12 @@ int launch_attention_decode2(const Dims& D, const Hyper& H, const Dev& V, const 
   }
   a.nsplit = ns;
   *nsplit_out = ns;
-  if (rope && ragged) attention_decode8_kernel<true, true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
-  else if (rope) attention_decode8_kernel<true, false><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
-  else if (ragged) attention_decode8_kernel<false, true><<<dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
-  else if (rows8) attention_decode8_kernel<false, false><<<dim3(ns, nb, 1), kD2Threads, kD8SmemTotal, s>>>(D, V, a);
-  else attention_decode2_kernel<<<dim3(ns, nb), kD2Threads, kD2SmemTotal, s>>>(D, V, a);
+  const bool pdl = !(H.flags & PROTOKV_SERIAL_LAUNCH);
+  if (rope && ragged) launch_chain(attention_decode8_kernel<true, true>, dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s, pdl, D, V, a);
+  else if (rope) launch_chain(attention_decode8_kernel<true, false>, dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s, pdl, D, V, a);
+  else if (ragged) launch_chain(attention_decode8_kernel<false, true>, dim3(ns, nb, nrb), kD2Threads, kD8SmemTotal, s, pdl, D, V, a);
+  else if (rows8) launch_chain(attention_decode8_kernel<false, false>, dim3(ns, nb, 1), kD2Threads, kD8SmemTotal, s, pdl, D, V, a);
+  else launch_chain(attention_decode2_kernel, dim3(ns, nb), kD2Threads, kD2SmemTotal, s, pdl, D, V, a);
   return 1;
 }
 

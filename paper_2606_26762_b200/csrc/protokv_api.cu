@@ -434,6 +434,8 @@ static int append_frame_impl(protokv_state* st, const void* K, const void* V, co
   F.epoch = st->epoch;
   F.warm = st->warm && !st->trained && st->frames < st->cfg.t_warm;
   F.res_base = st->res_seen;
+  F.pdl = (st->cfg.flags & PROTOKV_SERIAL_LAUNCH) ? 0 : 1;   // score and update touch nothing of the chain before pdl_wait()
+  bool after_update = false;
   int nl = 0;
   if (F.evicted) {
     if (F.n_fill > 0) {
@@ -449,9 +451,13 @@ static int append_frame_impl(protokv_state* st, const void* K, const void* V, co
       StageTimer tm(st, PROTOKV_STAGE_UPDATE);
       if (F.warm) nl += launch_reservoir_plan(D, st->H, st->V, F, st->stream);          // L312: where this frame's residuals go
       nl += launch_update(D, st->H, st->V, F, st->sm_count, st->stream);                // U4-U6
+      after_update = true;
     }
   }
   if (before_append) PKV_CUDA(cudaStreamWaitEvent(st->stream, before_append, 0));
+  // the append reads the caller's K / V ahead of its pdl_wait(): only directly behind the update kernel, whose own wait
+  // has then returned, i.e. everything the caller enqueued before this call has completed (common.cuh, pdl_wait)
+  if (!after_update || before_append) F.pdl = 0;
   {
     StageTimer tm(st, PROTOKV_STAGE_APPEND);
     nl += launch_ring_append(D, st->V, F, K, V, grid_pos, st->stream);                  // U1 (overwrites the slot)
@@ -569,18 +575,18 @@ int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, in
       int ns = 1;
       st->launches += launch_attention_decode(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
-      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, !(st->cfg.flags & PROTOKV_SERIAL_LAUNCH), st->stream);
     } else if (st->use_decode_rope && (uintptr_t)Q % 16 == 0) {
       int ns = 1;
       if (st->H.flags & PROTOKV_ROPE) st->launches += launch_rope_tables(D, st->H, st->V, A, st->stream);
       st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
-      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, !(st->cfg.flags & PROTOKV_SERIAL_LAUNCH), st->stream);
     } else if (st->use_decode2 && decode2_attention_supported(D, n_q) && (uintptr_t)Q % 16 == 0) {
       int ns = 1;
       st->launches += launch_attention_decode2(D, st->H, st->V, A, st->sm_count, st->stream, &ns);
       A.nsplit = ns;
-      st->launches += launch_attention_combine_bf16_128(D, st->V, A, st->stream);
+      st->launches += launch_attention_combine_bf16_128(D, st->V, A, !(st->cfg.flags & PROTOKV_SERIAL_LAUNCH), st->stream);
     } else if (st->use_tc_attn && (uintptr_t)Q % 16 == 0 && (uintptr_t)out % 8 == 0) {
       const int nl = launch_attention_tc(D, st->H, st->V, A, st->maps, st->sm_count, st->stream);
       if (nl < 0) return fail(PROTOKV_ECUDA, "cuTensorMapEncodeTiled failed for Q");

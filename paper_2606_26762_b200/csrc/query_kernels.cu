@@ -126,6 +126,8 @@ __device__ __forceinline__ void syn_prepare(const Dims& D, const Hyper& H, const
 // (2) one thread per task walks the beam recurrence over g = 0..G-1.  Phase 1 is the 8-wide part of the work; phase 2
 // is the dependent chain that sets the kernel's duration, kept short by the single-key candidates.
 __global__ void __launch_bounds__(kSynThreads) synthesis_kernel(Dims D, Hyper H, Dev V, int n_act, int epoch) {
+  pdl_wait();      // launched when the ring append exits (it has no trigger of its own)
+  pdl_trigger();   // the attention kernel sets up (barriers, TMEM) as SMs drain
   extern __shared__ uint16_t syn_list[];      // [K]
   __shared__ int wcnt[kSynThreads / 32];
   __shared__ uint32_t prep[8 * kSynWords * kSynTasks];
@@ -262,7 +264,7 @@ int launch_synthesis(const Dims& D, const Hyper& H, const Dev& V, int n_act, int
   const int cap = (8 * sm_count + D.B - 1) / D.B;
   if (per_bank > cap) per_bank = cap;
   if (per_bank < 1) per_bank = 1;
-  synthesis_kernel<<<dim3(per_bank, D.B), kSynThreads, (size_t)D.K * 2, s>>>(D, H, V, n_act, epoch);
+  launch_chain(synthesis_kernel, dim3(per_bank, D.B), kSynThreads, (size_t)D.K * 2, s, !(H.flags & PROTOKV_SERIAL_LAUNCH), D, H, V, n_act, epoch);
   return 1;
 }
 
@@ -541,6 +543,8 @@ template <typename T, int DH>
 __global__ void __launch_bounds__(128) attention_combine_kernel(Dims D, Dev V, AttnArgs A, int rows_total) {
   constexpr int VEC = DH / 32;
   const int gr = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  pdl_wait();
+  pdl_trigger();   // the next query's kernel may set up while the rows are merged
   if (gr >= rows_total) return;
   const int R = A.n_q * D.group;
   const int bsel = gr / R, row = gr % R;
@@ -602,9 +606,9 @@ static int attention_simt_launch(const Dims& D, const Hyper& H, const Dev& V, co
   return 2;
 }
 
-int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, cudaStream_t s) {
+int launch_attention_combine_bf16_128(const Dims& D, const Dev& V, const AttnArgs& A, bool pdl, cudaStream_t s) {
   const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
-  attention_combine_kernel<__nv_bfloat16, 128><<<(rows_total + 3) / 4, 128, 0, s>>>(D, V, A, rows_total);
+  launch_chain(attention_combine_kernel<__nv_bfloat16, 128>, (rows_total + 3) / 4, 128, 0, s, pdl, D, V, A, rows_total);
   return 1;
 }
 

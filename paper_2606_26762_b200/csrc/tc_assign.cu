@@ -171,6 +171,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();        // barriers, TMEM and descriptors are set up under the tail of the previous frame's ring append
+  pdl_trigger();     // the update kernel may load its codebooks as soon as an SM frees
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -389,9 +391,9 @@ int launch_score_tc(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs
   P.units = D.B * P.NP * P.NC;
   const int grid = P.units < sm_count ? P.units : sm_count;
   if (H.flags & PROTOKV_MAH_SQUARED)
-    score_tc_kernel<true><<<grid, kAsThreads, AsSmem::Total + 1024, s>>>(maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
+    launch_chain(score_tc_kernel<true>, grid, kAsThreads, AsSmem::Total + 1024, s, F.pdl != 0, maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
   else
-    score_tc_kernel<false><<<grid, kAsThreads, AsSmem::Total + 1024, s>>>(maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
+    launch_chain(score_tc_kernel<false>, grid, kAsThreads, AsSmem::Total + 1024, s, F.pdl != 0, maps.ringK, maps.c_hi, maps.c_lo, D, H, V, F, P);
   return 1;
 }
 

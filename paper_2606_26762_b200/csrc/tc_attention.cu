@@ -611,6 +611,10 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  // barriers, TMEM and the zeroed Q rows are set up under the tail of the previous kernel of the stream (synthesis, or the
+  // combine of the previous per-layer call).  No pdl_trigger(): a combine grid made pending under this persistent kernel
+  // cost 7 % on the per-layer calls; launched at this kernel's exit it still skips the launch latency
+  pdl_wait();
 
   if (warp < 8) {
     reg_inc<kRegsSoftmax>();
@@ -641,6 +645,8 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
                                                                    __nv_bfloat16* out, float* lse, int rows_total) {
   const int wq = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int gr = WIDE ? (int)blockIdx.x : (int)blockIdx.x * 4 + wq;
+  pdl_wait();
+  pdl_trigger();   // the next call's kernel may set up while the rows are merged
   if (gr >= rows_total) return;
   const int Rb = A.n_q * D.group;
   const int bsel = gr / Rb, rr = gr % Rb;
@@ -748,6 +754,7 @@ int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnA
   a.n_near = (H.flags & PROTOKV_FAR_ONLY) ? 0 : A.n_near;
   a.n_act = (H.flags & PROTOKV_NEAR_ONLY) ? 0 : A.n_act;
   a.use_bias = !(H.flags & PROTOKV_NO_MASS_BIAS);
+  const bool pdl = !(H.flags & PROTOKV_SERIAL_LAUNCH);
   AtPlan P{};
   P.tb = at_rows_tb(D, A.n_q);
   P.nrb = (A.n_q + P.tb - 1) / P.tb;
@@ -769,14 +776,14 @@ int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnA
     CUtensorMap tmQ;
     const uint64_t ntok = (uint64_t)D.NS * A.layer_count * A.n_q;
     if (!make_tmap_3d_bf16(&tmQ, A.Q, 128, (uint64_t)D.Hq, ntok, 64, (uint32_t)D.group, (uint32_t)P.tb)) return -1;
-    attention_tc_kernel<<<P.grid, kAtThreads, AtSmem::Total + 1024, s>>>(tmQ, maps.ringK, maps.ringV, D, V, a, P, V.part);
+    launch_chain(attention_tc_kernel, P.grid, kAtThreads, AtSmem::Total + 1024, s, pdl, tmQ, maps.ringK, maps.ringV, D, V, a, P, V.part);
     ++launched;
   }
   const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
   if (P.nsplit > 8)
-    attention_tc_combine_kernel<true><<<rows_total, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+    launch_chain(attention_tc_combine_kernel<true>, rows_total, 128, 0, s, pdl, D, a, P, (const float*)V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
   else
-    attention_tc_combine_kernel<false><<<(rows_total + 3) / 4, 128, 0, s>>>(D, a, P, V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+    launch_chain(attention_tc_combine_kernel<false>, (rows_total + 3) / 4, 128, 0, s, pdl, D, a, P, (const float*)V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
   return launched + 1;
 }
 

@@ -18,12 +18,6 @@ __global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slo
                                                           const uint4* __restrict__ Vin,
                                                           const float* __restrict__ grid_pos, int vpr) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
-  if (gtid < (uint32_t)(D.NS * D.T * 2)) {
-    const int st = (int)(gtid / (uint32_t)(D.T * 2)), e = (int)(gtid % (uint32_t)(D.T * 2));
-    V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = grid_pos[gtid];
-  }
-  for (uint32_t i = gtid; i < (uint32_t)(D.B * D.T); i += gridDim.x * blockDim.x)
-    V.akey[i] = ~0ull;                                     // next frame's assignment keys (see tc_assign.cu)
   const uint32_t rows = (uint32_t)(D.B * D.T);
   const uint32_t grp = gtid / (uint32_t)vpr, v = gtid % (uint32_t)vpr;
   const uint32_t ngrp = gridDim.x * blockDim.x / (uint32_t)vpr;
@@ -38,9 +32,21 @@ __global__ void __launch_bounds__(256) ring_append_kernel(Dims D, Dev V, int slo
     const uint32_t sl = b / (uint32_t)D.Hkv, hd = b - sl * (uint32_t)D.Hkv;   // sl = stream * L + layer
     const size_t src = (((size_t)sl * D.T + j) * D.Hkv + hd) * vpr + v;
     orow[i] = valid ? (b * (uint32_t)D.Wf + (uint32_t)slot) * (uint32_t)D.T + j : 0xffffffffu;
-    wk[i] = Kin[src];
-    wv[i] = Vin[src];
+    wk[i] = __ldcg(Kin + src);                             // read once, ahead of pdl_wait(): straight from L2
+    wv[i] = __ldcg(Vin + src);
   }
+  float gp = 0.f;
+  const bool has_gp = gtid < (uint32_t)(D.NS * D.T * 2);
+  if (has_gp) gp = __ldcg(grid_pos + gtid);
+  // everything above reads the caller's buffers only; the slot is overwritten once the update kernel has completed
+  pdl_wait();   // no pdl_trigger(): the next frame's score kernel (one CTA per SM) started under this kernel's stores made
+                // C5 frames 9 % slower; launched at this kernel's exit it still skips the launch latency
+  if (has_gp) {
+    const int st = (int)(gtid / (uint32_t)(D.T * 2)), e = (int)(gtid % (uint32_t)(D.T * 2));
+    V.ringS[((size_t)st * D.Wf + slot) * D.T * 2 + e] = gp;
+  }
+  for (uint32_t i = gtid; i < (uint32_t)(D.B * D.T); i += gridDim.x * blockDim.x)
+    V.akey[i] = ~0ull;                                     // next frame's assignment keys (see tc_assign.cu)
   uint4* outK = (uint4*)V.ringK;
   uint4* outV = (uint4*)V.ringV;
 #pragma unroll
@@ -76,8 +82,8 @@ int launch_ring_append(const Dims& D, const Dev& V, const FrameArgs& F, const vo
   const size_t need = (size_t)D.NS * D.T * 2;              // grid_pos copy
   if (threads < need) threads = need;
   const unsigned grid = (unsigned)((threads + 255) / 256);
-  if (D.bf16) ring_append_kernel<true><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
-  else ring_append_kernel<false><<<grid, 256, 0, s>>>(D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
+  if (D.bf16) launch_chain(ring_append_kernel<true>, grid, 256, 0, s, F.pdl != 0, D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
+  else launch_chain(ring_append_kernel<false>, grid, 256, 0, s, F.pdl != 0, D, V, F.slot, (const uint4*)Kin, (const uint4*)Vin, grid_pos, vpr);
   return 1;
 }
 
@@ -533,6 +539,17 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
   const size_t bt = (size_t)b * D.T;
   const size_t rrow = ((size_t)b * D.Wf + F.slot) * D.T;      // ring row of evicted token 0
   if (tid == 0) { nmine_s = 0; next_task_s = 0; }
+  if (has_cb) {   // codebooks: not written by any kernel of the frame chain, so loaded ahead of pdl_wait()
+    const float4* sk = (const float4*)(V.cbk + (size_t)b * 2048);
+    const float4* sv = (const float4*)(V.cbv + (size_t)b * 2048);
+    for (int e = tid; e < 512; e += kUfThreads) {             // e = (g * 16 + z) * 4 + q
+      const int q = e & 3, z = (e >> 2) & 15, g = e >> 6;
+      cbk4[g * kCbG + q * 16 + z] = sk[e];
+      cbv4[g * kCbG + q * 16 + z] = sv[e];
+    }
+  }
+  pdl_wait();      // the assignment of this frame (score kernel) is complete and visible
+  pdl_trigger();   // the ring append may fetch the new frame's rows while this kernel runs
   __syncthreads();
   // CTA x of the bank's gridDim.x CTAs owns the prototypes k with k mod gridDim.x == x: it keeps only the tokens
   // assigned to those, so that the sort below is over ~T / gridDim.x keys instead of T in every CTA
@@ -556,15 +573,6 @@ __global__ void __launch_bounds__(kUfThreads, 4) update_fast_kernel(Dims D, Hype
       if (blockIdx.x == 0) { V.assign[bt + j] = -2; atomicOr(V.err, PKV_ERR_UNASSIGNED); }
     } else if ((uint32_t)a % gridDim.x == blockIdx.x) {
       keys[atomicAdd(&nmine_s, 1)] = ((uint32_t)a << 12) | (uint32_t)j;   // any order: the keys are distinct
-    }
-  }
-  if (has_cb) {
-    const float4* sk = (const float4*)(V.cbk + (size_t)b * 2048);
-    const float4* sv = (const float4*)(V.cbv + (size_t)b * 2048);
-    for (int e = tid; e < 512; e += kUfThreads) {             // e = (g * 16 + z) * 4 + q
-      const int q = e & 3, z = (e >> 2) & 15, g = e >> 6;
-      cbk4[g * kCbG + q * 16 + z] = sk[e];
-      cbv4[g * kCbG + q * 16 + z] = sv[e];
     }
   }
   __syncthreads();
@@ -799,8 +807,8 @@ int launch_update(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& 
     if (nsplit > max_split) nsplit = max_split;
     if (nsplit < 1) nsplit = 1;
     dim3 grid(nsplit, D.B);
-    if (D.bf16) update_fast_kernel<__nv_bfloat16><<<grid, kUfThreads, sm, s>>>(D, H, V, F, Tpad);
-    else update_fast_kernel<float><<<grid, kUfThreads, sm, s>>>(D, H, V, F, Tpad);
+    if (D.bf16) launch_chain(update_fast_kernel<__nv_bfloat16>, grid, kUfThreads, sm, s, F.pdl != 0, D, H, V, F, Tpad);
+    else launch_chain(update_fast_kernel<float>, grid, kUfThreads, sm, s, F.pdl != 0, D, H, V, F, Tpad);
     return 1;
   }
   const int P = next_pow2(ntok);

@@ -16,7 +16,7 @@ from gpu_helpers import (make_gpu, make_oracles, run_stream, compare_ring, compa
                          compare_state, new_stats, step_teacher_forced)
 from oracle import FLAG_NEAR_ONLY, FLAG_FAR_ONLY, FLAG_NO_MASS_BIAS, FLAG_MAH_SQUARED
 from paper_2606_26762_b200 import (ProtoKV, ProtoKVError, NEAR_ONLY, FAR_ONLY, NO_MASS_BIAS, MAH_SQUARED, FORCE_SIMT,
-                                   DECODE_SPLITKV, NO_DECODE_KERNEL)
+                                   DECODE_SPLITKV, NO_DECODE_KERNEL, SERIAL_LAUNCH)
 
 pytestmark = pytest.mark.gpu
 
@@ -551,3 +551,42 @@ def test_decode_query_without_codebooks():
     compare_attention(spec, gpu, oracles, Q[:, :, :1].contiguous(), run_synthesis=True)
     compare_attention(spec, gpu, oracles, Q[:, :, :2].contiguous(), run_synthesis=False)
     gpu.close()
+
+
+@pytest.mark.parametrize("name,frames", [("c2", 40), ("c1", 24)])
+def test_dependent_launch_chain_equals_serial_launches(name, frames):
+    """The default launch mode overlaps each kernel's set-up with its predecessor's tail (programmatic dependent launch,
+    csrc/common.cuh pdl_wait); PROTOKV_SERIAL_LAUNCH serialises every launch.  Same inputs, ONE pair of K / V buffers that a
+    copy kernel of the caller refills right before every append and overwrites right after it (the ring append reads them
+    ahead of its wait): ring, bank state, pseudo-token codes and attention outputs must agree bit for bit."""
+    spec = gen.spec_for(name, n_frames=frames)
+    s = gen.grid_positions(spec, device="cuda")
+    src = [gen.frame_kv(spec, f, device="cuda") for f in range(frames)]
+    Q = gen.queries(spec, 0).cuda()
+    Q1 = Q[:, :, :1].contiguous()
+    got = []
+    for flags in (0, SERIAL_LAUNCH):
+        gpu = make_gpu(spec, flags=flags)
+        K, V = torch.empty_like(src[0][0]), torch.empty_like(src[0][1])
+        outs = []
+        for f in range(frames):
+            K.copy_(src[f][0]); V.copy_(src[f][1])
+            gpu.append_frame(K, V, s)
+            K.fill_(7.0); V.fill_(-3.0)                                  # the caller reuses its buffers at once
+            if f % 9 == 8:
+                outs.append(gpu.query_attention(Q).float().cpu())
+                outs.append(gpu.query_attention_ex(Q1, n_q=1, run_synthesis=False).float().cpu())
+        gpu.synthesize()
+        for la in range(spec.n_layers):                                  # back-to-back per-layer calls
+            outs.append(gpu.query_attention_ex(Q[:, la:la + 1].contiguous(), layer_begin=la, layer_count=1,
+                                               run_synthesis=False).float().cpu())
+        banks = [0, spec.n_banks - 1]
+        got.append((outs, [gpu.export_state(b) for b in banks], [gpu.export_ring(b) for b in banks],
+                    [gpu.export_codes(b) for b in banks]))
+        gpu.close()
+    (oa, sa, ra, ca), (ob, sb, rb, cb) = got
+    assert len(oa) == len(ob) and all(torch.equal(x, y) for x, y in zip(oa, ob))
+    for x, y in zip(sa, sb):
+        assert all(np.array_equal(x[k], y[k], equal_nan=True) for k in x), [k for k in x if not np.array_equal(x[k], y[k])]
+    for x, y in zip(ra + ca, rb + cb):
+        assert all(np.array_equal(u, v) for u, v in zip(x, y))
