@@ -195,6 +195,21 @@ int protokv_query_attention_ex(protokv_state *st, const void *Q, int32_t n_q, in
 int protokv_query_attention_at(protokv_state *st, const void *Q, int32_t n_q, int32_t layer_begin, int32_t layer_count,
                                void *out, float *lse, int32_t run_synthesis, int64_t q_pos0);
 
+/* protokv_query_attention_ex for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same arguments and the same result (Alg. 4; Eq. 4), computed by the fp32 SIMT
+ * attention kernel whatever the state's default route is, with the split-context partials in a file-scope device array of
+ * the library (csrc/static_scratch.cu) instead of the workspace.  The call and everything under it performs no cudaMalloc,
+ * cudaFree or other allocating call.  The array holds protokv_static_scratch_bytes() = 8 MiB; every GPU that loads the
+ * library holds it until the process exits.  A query needs n_streams * layer_count * n_kv_heads * n_q * (n_q_heads /
+ * n_kv_heads) * (head_dim + 2) * 4 bytes per context split: one that does not fit with a single split returns
+ * PROTOKV_EUNSUPPORTED and leaves the state unchanged (config 3's one-token query needs 0.4 MB, its 32-token query 13 MB).
+ * The array is shared by every state and call on the GPU and keeps the last call's contents; nothing in it has to start at
+ * zero (each call rewrites every partial it reads).  Calls that overlap on one GPU (different streams) RACE on it; calls
+ * on one stream are ordered.  Q, out, lse: device, as for protokv_query_attention_ex; the stream is cfg.cuda_stream. */
+int protokv_query_attention_static(protokv_state *st, const void *Q, int32_t n_q, int32_t layer_begin,
+                                   int32_t layer_count, void *out, float *lse, int32_t run_synthesis);
+size_t protokv_static_scratch_bytes(void);
+
 /* Alg. 3 for every bank without the attention (timing / parity of the synthesis kernel alone). */
 int protokv_synthesize(protokv_state *st);
 

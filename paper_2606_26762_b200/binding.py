@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = [
     "protokv_export_ring", "protokv_export_codes", "protokv_import_codes", "protokv_last_frame_trace",
     "protokv_frames_seen", "protokv_kernel_launches", "protokv_stage_impl", "protokv_profile_enable",
     "protokv_profile_read", "protokv_error_flags", "protokv_maintenance_counters", "protokv_query_attention_at",
+    "protokv_query_attention_static", "protokv_static_scratch_bytes",
     "protokv_train_codebooks", "protokv_export_reservoir", "protokv_import_reservoir", "protokv_export_codebooks",
     "protokv_export_allocation",
 ]
@@ -85,6 +86,9 @@ def load_library():
     lib.protokv_last_error.restype = C.c_char_p
     lib.protokv_query_attention_ex.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32]
     lib.protokv_query_attention_at.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32, C.c_int64]
+    lib.protokv_query_attention_static.argtypes = [vp, vp, i32, i32, i32, vp, vp, i32]
+    lib.protokv_static_scratch_bytes.argtypes = []
+    lib.protokv_static_scratch_bytes.restype = C.c_size_t
     lib.protokv_synthesize.argtypes = [vp]
     lib.protokv_export_state.argtypes = [vp, i32, C.POINTER(_BankView)]
     lib.protokv_import_state.argtypes = [vp, i32, C.POINTER(_BankView)]
@@ -260,6 +264,22 @@ class ProtoKV:
         else:
             self._check(self._lib.protokv_query_attention_at(*args, int(q_pos0)))
         return (out, lse) if return_lse else out
+
+    def query_attention_static(self, Q, out, n_q=None, layer_begin=0, layer_count=None, lse=None, run_synthesis=True):
+        """protokv_query_attention_static: the partials live in the library's static device array; nothing is allocated
+        (out, and lse if wanted, are the caller's)."""
+        c = self.cfg
+        n_q = c.n_query_tokens if n_q is None else n_q
+        layer_count = c.n_layers if layer_count is None else layer_count
+        n = self._q_numel(n_q, layer_count)
+        self._check(self._lib.protokv_query_attention_static(
+            self._h, self._dev(Q, self.torch_dtype, n), n_q, layer_begin, layer_count, self._dev(out, self.torch_dtype, n),
+            lse.data_ptr() if lse is not None else None, int(run_synthesis)))
+        return out
+
+    @property
+    def static_scratch_bytes(self):
+        return int(self._lib.protokv_static_scratch_bytes())
 
     def synthesize(self):
         self._check(self._lib.protokv_synthesize(self._h))

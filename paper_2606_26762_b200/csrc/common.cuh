@@ -255,6 +255,10 @@ struct AttnArgs {
 int attention_simt_splits(const Dims& D, int sm_count);   // nsplit the SIMT kernel uses (part buffer sizing)
 int launch_attention_simt(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
 int launch_rope_tables(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, cudaStream_t s);
+// static_scratch.cu: the SIMT attention with its partials in the library's file-scope device array (no allocation)
+size_t static_scratch_bytes();
+int launch_attention_static(const Dims& D, const Hyper& H, const Dev& V, const AttnArgs& A, int sm_count, cudaStream_t s,
+                            size_t* need_bytes, cudaError_t* cuda_err);
 
 // PQ codebook warm-up (warmup.cu)
 int launch_reservoir_plan(const Dims& D, const Hyper& H, const Dev& V, const FrameArgs& F, cudaStream_t s);

@@ -600,6 +600,54 @@ int protokv_query_attention_at(protokv_state* st, const void* Q, int32_t n_q, in
   return PROTOKV_OK;
 }
 
+size_t protokv_static_scratch_bytes(void) { return static_scratch_bytes(); }
+
+int protokv_query_attention_static(protokv_state* st, const void* Q, int32_t n_q, int32_t layer_begin, int32_t layer_count,
+                                   void* out, float* lse, int32_t run_synthesis) {
+  if (!st || !Q || !out) return fail(PROTOKV_EINVAL, "NULL argument");
+  if (st->poisoned) return fail(PROTOKV_ESTATE, "an earlier launch failure left this state inconsistent; destroy it");
+  DeviceGuard dg(st);
+  const Dims& D = st->D;
+  if (n_q < 1 || n_q > D.Nq) return fail(PROTOKV_EINVAL, "n_q %d outside [1, %d]", n_q, D.Nq);
+  if (layer_begin < 0 || layer_count < 1 || layer_begin + layer_count > D.L)
+    return fail(PROTOKV_EINVAL, "layer range [%d, %d) outside [0, %d)", layer_begin, layer_begin + layer_count, D.L);
+  // the size check comes first: a query that does not fit leaves the state (codes, epoch) untouched
+  const size_t need = (size_t)D.NS * layer_count * D.Hkv * n_q * D.group * (D.d + 2) * sizeof(float);
+  if (need > static_scratch_bytes())
+    return fail(PROTOKV_EUNSUPPORTED, "query of %d tokens x %d layers needs %zu bytes of partials; the static scratch holds "
+                "%zu (use protokv_query_attention_ex, whose partials live in the workspace)", n_q, layer_count, need,
+                static_scratch_bytes());
+  if (!(st->H.flags & PROTOKV_NEAR_ONLY)) {
+    if (run_synthesis) {
+      if (!st->codes_valid) {
+        const int rc = protokv_synthesize(st);
+        if (rc != PROTOKV_OK) return rc;
+      }
+    } else if (!st->codes_valid) {
+      return fail(PROTOKV_ESTATE, "run_synthesis = 0 but no synthesis result is valid for the current state");
+    }
+  }
+  AttnArgs A{};
+  A.Q = Q; A.out = out; A.lse = lse;
+  A.q_pos0 = (long long)st->H.pos0 + st->frames * D.T; A.frames = st->frames;
+  A.n_q = n_q; A.layer_begin = layer_begin; A.layer_count = layer_count;
+  const int64_t held = st->frames < D.Wf ? st->frames : D.Wf;
+  A.n_near = (int)(held * D.T);
+  A.n_act = st->n_act;
+  size_t nb = 0;
+  cudaError_t ce = cudaSuccess;
+  int nl;
+  {
+    StageTimer tm(st, PROTOKV_STAGE_ATTN);
+    nl = launch_attention_static(D, st->H, st->V, A, st->sm_count, st->stream, &nb, &ce);
+  }
+  if (nl == -1) return fail(PROTOKV_EUNSUPPORTED, "query needs %zu bytes of partials; the static scratch holds %zu", nb, static_scratch_bytes());
+  if (nl == -2) return fail(PROTOKV_ECUDA, "cudaGetSymbolAddress(static scratch): %s", cudaGetErrorString(ce));
+  st->launches += nl;
+  PKV_CUDA(cudaGetLastError());
+  return PROTOKV_OK;
+}
+
 int protokv_query_attention(protokv_state* st, const void* Q, void* out) {
   if (!st) return fail(PROTOKV_EINVAL, "NULL state");
   return protokv_query_attention_ex(st, Q, st->D.Nq, 0, st->D.L, out, nullptr, 1);
