@@ -637,7 +637,7 @@ attention_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
 }
 
 // Merges the pieces of every item: one warp per output row, 4 dims per lane.
-// WIDE = false: one warp per query row (few pieces per item: the batched query).  WIDE = true: one CTA per row, the four
+// WIDE = false: one warp per query row (superseded by attention_tc_combine4_kernel below, not launched).  WIDE = true: one CTA per row, the four
 // warps take every fourth piece and merge through shared memory (few items cut into many pieces: a per-layer call, where
 // a single warp walking 37 pieces with four loads in flight was a 17 us latency chain).
 template <bool WIDE>
@@ -662,16 +662,17 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
   }
   const float* base = part + ((size_t)item * P.nsplit * kAtRows + rin) * kPartStride;
   const size_t pstride = (size_t)kAtRows * kPartStride;
-  // online merge, four pieces' loads in flight at a time
+  // online merge, four pieces' loads in flight at a time (eight were slower on the per-layer calls: 786 vs 772 us)
+  constexpr int U = 4;
   float M = -INFINITY, l = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   bool poisoned = false;   // a piece with a NaN row sum (non-finite logits): the row is NaN, like the SIMT path returns it
   const int pstep = WIDE ? 4 : 1, pfirst = WIDE ? wq : 0;    // this warp's pieces: pfirst, pfirst + pstep, ...
-  for (int sp0 = 0; pfirst + sp0 * pstep < np; sp0 += 4) {
-    float2 ml[4];
-    float4 v[4];
+  for (int sp0 = 0; pfirst + sp0 * pstep < np; sp0 += U) {
+    float2 ml[U];
+    float4 v[U];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < U; ++u) {
       const int want = pfirst + (sp0 + u) * pstep;
       const int sp = want < np ? want : np - 1;              // clamp: a repeated piece is skipped below
       const float* ps = base + sp * pstride;
@@ -679,7 +680,7 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
       v[u] = *reinterpret_cast<const float4*>(ps + lane * 4);
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < U; ++u) {
       const bool have = pfirst + (sp0 + u) * pstep < np;
       if (have && ml[u].y != ml[u].y) poisoned = true;
       if (!have || !(ml[u].y > 0.f)) continue;
@@ -719,6 +720,78 @@ __global__ void __launch_bounds__(128) attention_tc_combine_kernel(Dims D, AtArg
   o.y = pack_bf16(acc.z * inv, acc.w * inv);
   *reinterpret_cast<uint2*>(out + ooff * 128 + lane * 4) = o;
   if (lse && lane == 0) lse[ooff] = poisoned ? inv : (l > 0.f ? M + logf(l) : -INFINITY);
+}
+
+// The merge for items with few pieces (the batched query: <= 8 pieces per item, usually 1-3).  One warp merges FOUR
+// consecutive rows of one item: the item-level index arithmetic (seven unsigned divisions: the one-row-per-warp form spent
+// two thirds of its ~470 instructions per row on eleven signed ones) is done once per warp, and the loads of the four rows
+// of a piece are in flight together.  Same arithmetic per row as attention_tc_combine_kernel.
+__global__ void __launch_bounds__(128) attention_tc_combine4_kernel(Dims D, AtArgs A, AtPlan P, const float* part,
+                                                                    __nv_bfloat16* out, float* lse, uint32_t nq4,
+                                                                    uint32_t nwarps) {
+  const uint32_t wq = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t gw = blockIdx.x * 4 + wq;
+  pdl_wait();
+  pdl_trigger();   // the next call's kernel may set up while the rows are merged
+  if (gw >= nwarps) return;
+  const uint32_t item = gw / nq4, quad = gw - item * nq4;
+  const uint32_t bsel = item / (uint32_t)P.nrb, rb = item - bsel * (uint32_t)P.nrb;
+  const uint32_t t1 = bsel / (uint32_t)D.Hkv, hd = bsel - t1 * (uint32_t)D.Hkv;          // t1 = st * layer_count + ll
+  const uint32_t ntok = min((uint32_t)P.tb, (uint32_t)A.n_q - rb * (uint32_t)P.tb);
+  const uint32_t R = ntok * (uint32_t)D.group;                                             // valid rows of the item
+  const uint32_t rin0 = quad * 4;
+  if (rin0 >= R) return;
+  uint32_t np = 0;
+  if (P.ntile > 0) {
+    const int cf = at_cta_of(P, (long long)item * P.ntile);
+    np = (uint32_t)(at_cta_of(P, (long long)(item + 1) * P.ntile - 1) - cf + 1);
+  }
+  const float* base = part + ((size_t)item * P.nsplit * kAtRows + rin0) * kPartStride;
+  const size_t pstride = (size_t)kAtRows * kPartStride;
+  float M[4], l[4];
+  float4 acc[4];
+  bool poisoned[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { M[i] = -INFINITY; l[i] = 0.f; acc[i] = make_float4(0.f, 0.f, 0.f, 0.f); poisoned[i] = false; }
+  for (uint32_t sp = 0; sp < np; ++sp) {
+    const float* ps = base + sp * pstride;
+    float2 ml[4];
+    float4 v[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const uint32_t ri = rin0 + i < R ? i : 0;                  // clamp: rows past the item's end repeat row 0, never stored
+      ml[i] = *reinterpret_cast<const float2*>(ps + ri * kPartStride + 128);
+      v[i] = *reinterpret_cast<const float4*>(ps + ri * kPartStride + lane * 4);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      if (ml[i].y != ml[i].y) poisoned[i] = true;
+      if (!(ml[i].y > 0.f)) continue;
+      const float Mn = fmaxf(M[i], ml[i].x);
+      const float so = __expf(M[i] - Mn), sn = __expf(ml[i].x - Mn);   // M = -inf: so = 0
+      l[i] = fmaf(l[i], so, ml[i].y * sn);
+      acc[i].x = fmaf(acc[i].x, so, v[i].x * sn); acc[i].y = fmaf(acc[i].y, so, v[i].y * sn);
+      acc[i].z = fmaf(acc[i].z, so, v[i].z * sn); acc[i].w = fmaf(acc[i].w, so, v[i].w * sn);
+      M[i] = Mn;
+    }
+  }
+  uint32_t ql = rin0 / (uint32_t)D.group, hh = rin0 - ql * (uint32_t)D.group;             // token within the block, head
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (rin0 + i < R) {
+      float inv = l[i] > 0.f ? 1.f / l[i] : 0.f;
+      float4 a = acc[i];
+      float li = l[i];
+      if (poisoned[i]) { inv = __int_as_float(0x7fc00000); a = make_float4(1.f, 1.f, 1.f, 1.f); li = inv; }
+      const size_t ooff = ((size_t)t1 * A.n_q + rb * (uint32_t)P.tb + ql) * D.Hq + hd * (uint32_t)D.group + hh;
+      uint2 o;
+      o.x = pack_bf16(a.x * inv, a.y * inv);
+      o.y = pack_bf16(a.z * inv, a.w * inv);
+      *reinterpret_cast<uint2*>(out + ooff * 128 + lane * 4) = o;
+      if (lse && lane == 0) lse[ooff] = poisoned[i] ? inv : (li > 0.f ? M[i] + logf(li) : -INFINITY);
+    }
+    if (++hh == (uint32_t)D.group) { hh = 0; ++ql; }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -780,10 +853,12 @@ int launch_attention_tc(const Dims& D, const Hyper& H, const Dev& V, const AttnA
     ++launched;
   }
   const int rows_total = D.NS * A.layer_count * D.Hkv * A.n_q * D.group;
-  if (P.nsplit > 8)
+  if (P.nsplit > 8) {
     launch_chain(attention_tc_combine_kernel<true>, rows_total, 128, 0, s, pdl, D, a, P, (const float*)V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
-  else
-    launch_chain(attention_tc_combine_kernel<false>, (rows_total + 3) / 4, 128, 0, s, pdl, D, a, P, (const float*)V.part, (__nv_bfloat16*)A.out, A.lse, rows_total);
+  } else {
+    const uint32_t nq4 = (uint32_t)(P.tb * D.group + 3) / 4, nwarps = (uint32_t)P.items * nq4;
+    launch_chain(attention_tc_combine4_kernel, (nwarps + 3) / 4, 128, 0, s, pdl, D, a, P, (const float*)V.part, (__nv_bfloat16*)A.out, A.lse, nq4, nwarps);
+  }
   return launched + 1;
 }
 
