@@ -551,23 +551,38 @@ __global__ void __launch_bounds__(128) attention_combine_kernel(Dims D, Dev V, A
   const int hd = bsel % D.Hkv, ll = (bsel / D.Hkv) % A.layer_count, st = bsel / (D.Hkv * A.layer_count);
   const int qi = row / D.group, h = hd * D.group + row % D.group;
   const float* part = V.part + (size_t)gr * A.nsplit * (DH + 2);
-  float M = -INFINITY;
+  // online (max, sum) merge of the splits, eight splits' loads in flight at a time (a two-pass merge over a runtime split
+  // count kept one load in flight per warp: 2 x nsplit dependent L2 round trips for a few hundred bytes per row)
+  float M = -INFINITY, l = 0.f, acc[VEC];
   bool poisoned = false;   // a partial with a NaN maximum or row sum (non-finite logits): the row is NaN
-  for (int sp = 0; sp < A.nsplit; ++sp) {
-    const float m = part[sp * (DH + 2) + DH], ls = part[sp * (DH + 2) + DH + 1];
-    poisoned = poisoned || m != m || ls != ls;
-    M = fmaxf(M, m);
-  }
-  float l = 0.f, acc[VEC];
 #pragma unroll
   for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
-  if (M > -INFINITY) {
-    for (int sp = 0; sp < A.nsplit; ++sp) {
-      const float* ps = part + sp * (DH + 2);
-      const float w = __expf(ps[DH] - M);   // exp(-inf) = 0 for empty splits
-      l = fmaf(ps[DH + 1], w, l);
+  for (int sp0 = 0; sp0 < A.nsplit; sp0 += 8) {
+    float2 ml[8];
+    float pv[8][VEC];
 #pragma unroll
-      for (int v = 0; v < VEC; ++v) acc[v] = fmaf(ps[lane * VEC + v], w, acc[v]);
+    for (int u = 0; u < 8; ++u) {
+      const int sp = sp0 + u < A.nsplit ? sp0 + u : A.nsplit - 1;   // clamp: a repeated split is skipped below
+      const float* ps = part + (size_t)sp * (DH + 2);
+      ml[u] = *reinterpret_cast<const float2*>(ps + DH);
+#pragma unroll
+      for (int v = 0; v < VEC; v += 2) {                            // rows are (DH + 2) floats apart: 8-byte aligned, not 16
+        const float2 t = *reinterpret_cast<const float2*>(ps + lane * VEC + v);
+        pv[u][v] = t.x; pv[u][v + 1] = t.y;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      if (sp0 + u >= A.nsplit) continue;
+      const float m = ml[u].x, ls = ml[u].y;
+      poisoned = poisoned || m != m || ls != ls;
+      if (!(m > -INFINITY)) continue;                                // empty split
+      const float Mn = fmaxf(M, m);
+      const float so = __expf(M - Mn), sn = __expf(m - Mn);          // M = -inf: so = 0
+      l = fmaf(l, so, ls * sn);
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) acc[v] = fmaf(acc[v], so, pv[u][v] * sn);
+      M = Mn;
     }
   }
   float inv = l > 0.f ? 1.f / l : 0.f;
